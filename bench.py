@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""bench.py — FR RHS throughput (GDOF/s) on B200, one JSON line.
+
+A "step" is one pass of the whole hot path: one fr_rhs evaluation (all seven parts of the north_star)
+over the whole synthetic mesh.  Default workload: C3 of BASELINE.json — 32^3 periodic CURVED hexahedra,
+p=4, 3-D Navier-Stokes, fp64, Taylor-Green + seeded noise (the configuration the metric's target
+"p=4 hexahedral Navier-Stokes FP64 RHS" is quoted on).  Inputs exceed L2 (state 164 MB, working set >1 GB).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C2|C1|C4|C5] [--precision f64|f32]
+  python bench.py --impl reference ...      # the oracle on the host cores, bounded sample
+
+Multi-GPU: the path is single-GPU by the north_star ("no sharding or collectives") => replicas only:
+every rank runs the same workload; value = N * DOF / max-over-ranks time; scaling "weak".
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+import workloads as W  # noqa: E402
+
+METRIC = "FR RHS GDOF/s"
+UNIT = "GDOF/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C3")
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--n", type=int, default=0, help="elements per direction (0 = the config's own size)")
+    ap.add_argument("--p", type=int, default=0)
+    ap.add_argument("--system", default="")
+    ap.add_argument("--generic", action="store_true", help="force the generic staged kernels")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload(args):
+    over = {}
+    if args.n:
+        over["n"] = args.n
+    if args.p:
+        over["p"] = args.p
+    if args.system:
+        over["system"] = args.system
+    mesh, disc = W.config(args.workload, **over)
+    desc = {
+        "workload": "%s: %s %s mesh %s, p=%d, %s, %s, p_g=%d" % (
+            args.workload, "x".join(str(s) for s in mesh["shape"]), mesh["etype"],
+            "curved periodic" if mesh["p_g"] > 1 else "affine periodic", disc["p"], disc["system"], args.precision, mesh["p_g"]),
+        "elements": int(mesh["nodes"].shape[0]),
+        "p": disc["p"],
+        "system": disc["system"],
+        "l2": "inputs larger than L2 (no flush)",
+    }
+    return mesh, disc, over, desc
+
+
+# ----------------------------------------------------------------------------------------------
+# byte model: SURVEY 8(d) fused lower bound for the whole RHS, and the
+# compulsory (read-once / write-once) words per element of each kernel
+# ----------------------------------------------------------------------------------------------
+def rhs_algorithmic_words(nd, NV, Nu, Nf, ns, affine):
+    if ns:
+        w = 5 * NV * Nu + 12 * NV * Nf
+    else:
+        w = 2 * NV * Nu + 4 * NV * Nf  # read U, write R; U^f write + two-sided read, D~ write + read
+    if not affine:
+        w += (nd * nd + 1) * Nu + (nd + 1) * Nf
+    return w
+
+
+def kernel_words(name, nd, NV, Nu, Nf, ns):
+    """compulsory words per element for one launch group (inputs once + outputs once)."""
+    met = (nd * nd + 1) * Nu
+    t = {
+        # generic staged path (App A sequence)
+        "apply_M0": (Nu + Nf) * NV,
+        "common_sol": 2 * Nf * NV + Nf,
+        "apply_M46_M6": (Nu + Nf + nd * Nu) * NV,
+        "grad_phys": 2 * nd * Nu * NV + met,
+        "apply_M5": nd * (Nu + Nf) * NV,
+        "tflux": Nu * NV + (2 if ns else 1) * nd * Nu * NV + nd * nd * Nu,
+        "common_flux": (2 + (nd if ns else 0)) * Nf * NV + (nd + 2 + 2) * Nf // 2,
+        "apply_M132_M3_negdivconf": (nd * Nu + Nf + Nu) * NV + Nu,
+        # tensor-product path (fr_tensor.cu)
+        "tp_interp": (Nu + Nf) * NV,
+        "tp_grad": (Nu + Nf) * NV + met + (nd + 1) * Nf + (NV - 1) * Nf + Nf,
+        "tp_div": (2 * Nu + Nf) * NV + met + (nd + 1) * Nf + ((NV - 1) * Nf if ns else 0) + Nf,
+    }
+    return t.get(name)
+
+
+class ClockSampler(threading.Thread):
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.rows = index, False, []
+
+    def run(self):
+        q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q, "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if r[1].replace(".", "").isdigit()]
+        reasons = set()
+        for r in self.rows:
+            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def time_oracle(args, sample_n, reps):
+    """The oracle as it stands on the host cores, on a bounded sample of the workload's shape."""
+    from oracle.fr_oracle import FROracle
+
+    a2 = argparse.Namespace(**vars(args))
+    a2.n = sample_n
+    mesh, disc, over, _ = workload(a2)
+    o = FROracle(mesh, disc)
+    U = W.config_state(args.workload, np.asarray(o.xu_phys, float), **over)
+    o.rhs(U)
+    ts = []
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        o.rhs(U)
+        ts.append(time.perf_counter() - t0)
+    try:
+        from threadpoolctl import threadpool_info
+
+        cores = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+    except Exception:
+        cores = os.cpu_count()
+    return U.size, ts, cores, "%s-shaped %s sub-problem (%d elements, %d DOF), %d oracle RHS evaluations, numpy float64" % (
+        args.workload, "x".join(str(s) for s in mesh["shape"]), mesh["nodes"].shape[0], U.size, reps)
+
+
+def sample_size(args):
+    if args.workload in ("C3", "C2", "C5"):
+        return 8
+    if args.workload == "C4":
+        return 64
+    return 0
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    dof, ts, cores, sample = time_oracle(args, sample_size(args), max(args.steps, 1) + args.warmup)
+    ts = ts[args.warmup:]
+    ms = 1e3 * float(np.mean(ts))
+    val = dof / (ms * 1e-3) / 1e9
+    _, _, _, desc = workload(args)
+    desc["sample"] = sample
+    out = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": len(ts), "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": desc,
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out))
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+
+    from paper_1312_1638_b200 import Context
+    from paper_1312_1638_b200.binding import FLAG_FORCE_GENERIC
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the FR library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    mesh, disc, over, desc = workload(args)
+    t0 = time.time()
+    ctx = Context(mesh).setup_operators(precision=args.precision, flags=FLAG_FORCE_GENERIC if args.generic else 0, **disc)
+    setup_s = time.time() - t0
+    X = ctx.solution_point_coords()
+    U = ctx.pad(W.config_state(args.workload, X, **over))
+    dof = ctx.Nu * ctx.NV * ctx.n_elems
+    u_host = torch.from_numpy(U).pin_memory()
+    r_host = torch.empty_like(u_host).pin_memory()
+    u = u_host.cuda()
+    r = torch.zeros_like(u)
+    work = torch.zeros(ctx.workspace_bytes, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream().cuda_stream
+    up, rp, wp = u.data_ptr(), r.data_ptr(), work.data_ptr()
+
+    # ---- device-resident timing ----
+    for _ in range(max(args.warmup, 3)):
+        ctx.rhs(up, rp, wp, stream)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        ctx.rhs(up, rp, wp, stream)
+    ev1.record()
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    # keep the GPU busy a little longer if the timed region was too short for a clock sample
+    t_end = time.time() + max(0.0, 0.6 - ms_total * 1e-3)
+    while time.time() < t_end:
+        ctx.rhs(up, rp, wp, stream)
+        torch.cuda.synchronize()
+    sampler.stop_flag = True
+    sampler.join()
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    value = world * dof / (ms_step * 1e-3) / 1e9
+
+    # ---- end to end through the C ABI with host buffers (H2D + RHS + D2H per step) ----
+    n_e2e = max(3, min(args.steps, 10))
+    for _ in range(2):
+        ctx.rhs_host(u_host.data_ptr(), r_host.data_ptr(), up, rp, wp, stream)
+    barrier()
+    ev0.record()
+    for _ in range(n_e2e):
+        ctx.rhs_host(u_host.data_ptr(), r_host.data_ptr(), up, rp, wp, stream)
+    ev1.record()
+    barrier()
+    t = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item()) / n_e2e
+    e2e_val = world * dof / (e2e_ms * 1e-3) / 1e9
+
+    # ---- per-kernel durations (events between kernels, same stream), dominant kernel roofline ----
+    acc = {}
+    n_prof = max(3, min(args.steps, 10))
+    for _ in range(n_prof):
+        for name, ms in ctx.rhs_profiled(up, rp, wp, stream):
+            acc[name] = acc.get(name, 0.0) + ms / n_prof
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    peaks = {}
+    pk_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(pk_path):
+        peaks = json.load(open(pk_path))
+    peak_gbs = float(peaks.get("hbm_gbs", 6650.0))
+    peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s"
+    esz = 8  # intermediates are fp64 in both precisions; state words counted at the storage size below
+    nd, NV, Nu, Nf, ns = ctx.ndims, ctx.NV, ctx.Nu, ctx.Nf, disc["system"] == "navier-stokes"
+    affine = mesh["p_g"] == 1
+    kern = []
+    for name, ms in acc.items():
+        wds = kernel_words(name, nd, NV, Nu, Nf, ns)
+        gbs = (wds * esz * ctx.n_elems / (ms * 1e-3) / 1e9) if (wds and ms > 0) else None
+        kern.append({"name": name, "ms": ms, "share": ms / sum(acc.values()), "algorithmic_GBps": gbs})
+    kern.sort(key=lambda k: -k["ms"])
+    top = kern[0]
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(args.workload + "-" + args.precision, {}).get(top["name"])
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": top["name"], "achieved": top["algorithmic_GBps"], "peak": peak_gbs, "unit": "GB/s",
+                "frac": (top["algorithmic_GBps"] / peak_gbs) if top["algorithmic_GBps"] else None, "traffic": traffic,
+                "peak_source": peak_src, "kernel_ms": top["ms"], "kernel_share_of_step": top["share"]}
+    words = rhs_algorithmic_words(nd, NV, Nu, Nf, ns, affine)
+    rhs_gbs = words * (8 if args.precision == "f64" else 4) * ctx.n_elems / (ms_step * 1e-3) / 1e9
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": args.precision, "data": "synthetic", "config": dict(desc, parallelism="replicas only (%d)" % world, setup_s=round(setup_s, 2)),
+        "clocks": sampler.summary(),
+        "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(u_host.numel() * u_host.element_size()),
+                "d2h_bytes_per_step": int(r_host.numel() * r_host.element_size())},
+        "gpu_launches": int(ctx.rhs_kernel_launches) * args.steps,
+        "roofline": roofline,
+        "rhs_roofline": {"bound": "hbm", "algorithmic_bytes_per_point": words * (8 if args.precision == "f64" else 4) / Nu,
+                         "achieved": rhs_gbs, "peak": peak_gbs, "unit": "GB/s", "frac": rhs_gbs / peak_gbs,
+                         "note": "SURVEY 8(d) fused lower-bound bytes of the WHOLE RHS / measured RHS time"},
+        "kernels": kern,
+        "s_per_rk4_step": None,
+    }
+    # RK4 step time
+    for _ in range(2):
+        ctx.rk4_step(up, 1e-6, wp, stream)
+    torch.cuda.synchronize()
+    ev0.record()
+    nrk = 5
+    for _ in range(nrk):
+        ctx.rk4_step(up, 1e-6, wp, stream)
+    ev1.record()
+    torch.cuda.synchronize()
+    out["s_per_rk4_step"] = ev0.elapsed_time(ev1) * 1e-3 / nrk
+    if not args.no_cpu_baseline and world == 1:
+        cdof, ts, cores, sample = time_oracle(args, sample_size(args), 5)
+        out["cpu_baseline"] = {"value": cdof / float(np.mean(ts)) / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+    else:
+        out["cpu_baseline"] = None
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

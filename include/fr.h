@@ -1,0 +1,153 @@
+/* fr.h — C ABI of the B200-native Flux Reconstruction right-hand-side library.
+ *
+ * One hot path of arxiv/paper_1312_1638 (PyFR): the per-stage RHS of the FR discretisation of the
+ * compressible Euler / Navier-Stokes equations on quadrilateral, triangular and hexahedral grids,
+ * driven by classical RK4.  Citations are PAPER.md:<line>; A-numbers are the readings in DESIGN.md.
+ *
+ * Conventions (DESIGN.md "Conventions" has the full statement):
+ *  - State matrices are SoA  [point][variable][element], element fastest, leading
+ *    dimension ld = fr_leading_dim() >= n_elems (padded so every row starts on a 128-byte boundary).
+ *    Variables: rho, rho*v_x, rho*v_y, (rho*v_z,) E   (Eq 20 :474);  N_V = ndims + 2.
+ *  - quad/hex reference element [-1,1]^ndims, Gauss-Legendre tensor solution points
+ *    rho = i + n*j (+ n^2*k), n = p+1, first coordinate fastest; face f = 2*d + s (d = reference
+ *    direction, s = 0 at -1 / 1 at +1); flux point sigma = f*nfp + idx, idx = tensor GL index over the
+ *    remaining directions, lowest fastest.  Triangle: reference (-1,-1),(1,-1),(-1,1); solution
+ *    points = barycentric lattice (i+1,j+1,k+1)/(p+3) (A6), j outer / i inner; face k = edge
+ *    vertex k -> k+1, GL flux points along the edge.
+ *  - Geometry nodes: degree-p_g Lagrange on the equispaced lattice of the reference element,
+ *    first coordinate fastest (triangle: rows j = 0..p_g, i = 0..p_g-j).
+ *  - Every entry point returns 0 on success or a negative FR_E* code; fr_last_error() gives text.
+ *    No exception or abort crosses this boundary.  A NULL context is an error, not a crash.
+ *  - "host" / "dev" say where a pointer must live.  The library never frees caller memory.
+ */
+#ifndef FR_B200_H
+#define FR_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fr_ctx fr_ctx;
+
+enum { FR_QUAD = 0, FR_TRI = 1, FR_HEX = 2 };                  /* element types */
+enum { FR_EULER = 0, FR_NAVIER_STOKES = 1 };                   /* governing systems */
+enum { FR_F32 = 0, FR_F64 = 1 };                               /* storage precision of u / rhs */
+enum { FR_BC_SUP_INFLOW = 0, FR_BC_SUB_OUTFLOW = 1, FR_BC_NOSLIP_WALL = 2 }; /* App C :799-825 */
+
+enum {
+  FR_OK = 0,
+  FR_EINVAL = -1,    /* bad argument / NULL pointer / call order */
+  FR_EMESH = -2,     /* J <= 0, unmatched flux points, face referenced twice or never */
+  FR_ECUDA = -3,     /* a CUDA runtime call failed (text in fr_last_error) */
+  FR_ENOMEM = -4,
+  FR_EUNSUPPORTED = -5
+};
+
+/* Boundary condition, Appendix C.  SUP_INFLOW uses rho,v,p (Eq 47); SUB_OUTFLOW uses p (Eq 49);
+ * NOSLIP_WALL uses cpTw = C_p*T_w and v = v_w (Eq 51-53). */
+typedef struct {
+  int32_t kind;
+  double rho, v[3], p, cpTw;
+} fr_bc_desc;
+
+/* Mesh of ONE element type (mixed meshes: DESIGN.md "next").  All pointers: host, read during the
+ * call only (the library copies what it needs). */
+typedef struct {
+  int32_t ndims;           /* 2 | 3 */
+  int32_t etype;           /* FR_QUAD | FR_TRI | FR_HEX */
+  int32_t p_g;             /* geometry degree >= 1 */
+  int32_t n_bcs;           /* entries in bcs; boundary faces index it by bc_id */
+  int64_t n_elems;
+  int64_t n_ifaces;        /* interior + periodic interfaces, each listed once */
+  int64_t n_bfaces;
+  const double *nodes;     /* [n_elems][n_nodes(p_g)][ndims] */
+  const int32_t *ifaces;   /* [n_ifaces][4] = elemL, faceL, elemR, faceR; L/R order is significant (A12) */
+  const double *shifts;    /* [n_ifaces][ndims]: x_L(flux point) = x_R(flux point) + shift (periodic image) */
+  const int32_t *bfaces;   /* [n_bfaces][3] = elem, face, bc_id */
+  const fr_bc_desc *bcs;   /* [n_bcs] */
+} fr_mesh_desc;
+
+/* Discretisation: order p, system (§4), storage precision, gas constants gamma (Eq 21),
+ * mu, Pr (Eq 22-23; mu constant, A9), LDG beta / tau (Eq 25-27 :506-516; tau enters with the dissipative
+ * sign, A7).  Point sets and the DG correction function are fixed (A5, A6). */
+typedef struct {
+  int32_t p;
+  int32_t system;
+  int32_t precision;
+  int32_t flags;           /* FR_FLAG_* bits */
+  double gamma, mu, Pr, ldg_beta, ldg_tau;
+} fr_disc_desc;
+
+#define FR_FLAG_FORCE_GENERIC 1
+#define FR_FLAG_HOST_ONLY 2      /* build the host tables only (no CUDA call): queries work, fr_rhs fails */
+
+/* Creates a context (owned by the library; release with fr_teardown).  Validates connectivity only;
+ * geometric checks happen in fr_setup_operators once the point sets are known. */
+int fr_setup_mesh(fr_ctx **out, const fr_mesh_desc *mesh);
+
+/* Builds M0..M6 (App A :737-768) on the host in extended precision, the metric terms S = J*J^-1, 1/J
+ * (Eq 10, 12, 19) at the solution points, the physical normals and J*n (Eq 14, 16) at the flux points,
+ * matches flux-point pairs by physical coordinates (:182, :194) and orders them for coalesced access
+ * (:693); uploads the constants to the current CUDA device.  May be called again to change p/system.
+ * Errors: FR_EMESH on J <= 0 or unmatched / uncovered flux points. */
+int fr_setup_operators(fr_ctx *ctx, const fr_disc_desc *disc);
+
+/* Sizes (valid after fr_setup_operators; negative error code otherwise). */
+int64_t fr_num_solution_points(const fr_ctx *ctx); /* N_u per element */
+int64_t fr_num_flux_points(const fr_ctx *ctx);     /* N_f per element */
+int64_t fr_num_vars(const fr_ctx *ctx);            /* N_V */
+int64_t fr_num_pairs(const fr_ctx *ctx);           /* interior+periodic flux-point pairs */
+int64_t fr_leading_dim(const fr_ctx *ctx);         /* ld of every state matrix */
+int64_t fr_state_bytes(const fr_ctx *ctx);         /* N_u*N_V*ld*sizeof(precision) */
+int64_t fr_workspace_bytes(const fr_ctx *ctx);     /* scratch for fr_rhs + RK registers for fr_rk4_step */
+int64_t fr_rhs_kernel_launches(const fr_ctx *ctx); /* kernels one fr_rhs call launches */
+
+/* Physical coordinates of the solution points, host buffer [N_u][n_elems][ndims] doubles. */
+int fr_solution_point_coords(const fr_ctx *ctx, double *xyz_host);
+
+/* Operator matrices for operator-level tests: id 0..6 = M0..M6 (row-major doubles, host).
+ * fr_operator_dims gives rows, cols. */
+int fr_operator_dims(const fr_ctx *ctx, int id, int64_t *rows, int64_t *cols);
+int fr_get_operator(const fr_ctx *ctx, int id, double *buf_host);
+
+/* Host copies of the setup tables, for tests.  pairs: int32 [npairs][4] = sigmaL, elemL, sigmaR, elemR in
+ * iteration order; normals: [npairs][ndims] unit normal of the L side; jn: [npairs][2] = (J n)_L, (J n)_R
+ * (Eq 14, 16-17).  metrics: smat [ndims*ndims][N_u][ld] (S = J*J^-1, Eq 12) and rcpj [N_u][ld] (1/J). */
+int fr_get_pairs(const fr_ctx *ctx, int32_t *pairs_host, double *normals_host, double *jn_host);
+int fr_get_metrics(const fr_ctx *ctx, double *smat_host, double *rcpj_host);
+
+/* rhs = -div f(u, grad u)  (Eq 19 :243; the seven parts of BASELINE.json north_star).
+ * u_dev, rhs_dev: [N_u][N_V][ld] in the context's precision, device; u is not modified; rhs must not
+ * alias u.  work_dev: >= fr_workspace_bytes() device bytes, 256-byte aligned, caller-owned.
+ * stream: a cudaStream_t (as void*).  Asynchronous; no host synchronisation.  Pad columns
+ * (element index >= n_elems) of rhs are left untouched.  Non-finite states are not detected (A19). */
+int fr_rhs(fr_ctx *ctx, const void *u_dev, void *rhs_dev, void *work_dev, void *stream);
+
+/* fr_rhs with a CUDA event recorded on `stream` before each kernel and after the last; synchronises the
+ * stream and returns, for each of the *n_kernels launch groups, its duration ms[i] and a name
+ * (names_host: max_kernels x 32 chars).  For measurement only. */
+int fr_rhs_profiled(fr_ctx *ctx, const void *u_dev, void *rhs_dev, void *work_dev, void *stream, int max_kernels,
+                    int *n_kernels, float *ms_host, char *names_host);
+
+/* One classical RK4 step, u advanced in place; four fr_rhs evaluations. */
+int fr_rk4_step(fr_ctx *ctx, void *u_dev, double dt, void *work_dev, void *stream);
+
+/* End-to-end variant with HOST buffers: copies u_host -> u_dev (H2D), evaluates fr_rhs, copies
+ * rhs_dev -> rhs_host (D2H), all asynchronously on `stream` (pinned host memory recommended).
+ * u_dev / rhs_dev / work_dev are caller-allocated device staging buffers as in fr_rhs. */
+int fr_rhs_host(fr_ctx *ctx, const void *u_host, void *rhs_host, void *u_dev, void *rhs_dev, void *work_dev,
+                void *stream);
+
+/* Frees host objects and the library's own constant uploads.  NULL is allowed. */
+void fr_teardown(fr_ctx *ctx);
+
+/* Text of the last error on this context (or of the last failed fr_setup_mesh if ctx == NULL).
+ * The pointer stays valid until the next failing call on the same context. */
+const char *fr_last_error(const fr_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -494,7 +494,7 @@ class FROracle:
     # ---- the steps ----
     def interpolate(self, u):
         """O5, Eq 6 / Eq 41: U^f = M0 U."""
-        return np.einsum("sr,rvn->svn", self.M0, u)
+        return np.einsum("sr,rvn->svn", self.M0, u, optimize=True)
 
     def common_solution(self, uf):
         """O6, Eq 7 + Eq 25; boundary: C(u_L, B_ldg u_L) (:797)."""
@@ -514,11 +514,11 @@ class FROracle:
     def gradient(self, u, uf, C):
         """O7: Eq 9 literally (unfused), Eq 10, Eq 11."""
         nd, Nu = self.nd, self.Nu
-        qt = np.einsum("ks,svn->kvn", self.M6, C - uf) + np.einsum("kr,rvn->kvn", self.M4, u)
+        qt = np.einsum("ks,svn->kvn", self.M6, C - uf, optimize=True) + np.einsum("kr,rvn->kvn", self.M4, u, optimize=True)
         qt = qt.reshape(nd, Nu, self.NV, self.Nel)
         # q_n = (1/J) sum_i S[i][n] q~_i   (J^-T = S^T / J)
         q = np.stack([sum(self.Su[:, None, :, i, n] * qt[i] for i in range(nd)) / self.Ju[:, None, :] for n in range(nd)])
-        qf = np.stack([np.einsum("sr,rvn->svn", self.M0, q[n]) for n in range(nd)])
+        qf = np.stack([np.einsum("sr,rvn->svn", self.M0, q[n], optimize=True) for n in range(nd)])
         return q, qf
 
     def transformed_flux(self, u, q):
@@ -556,7 +556,7 @@ class FROracle:
 
     def divergence(self, ft, D):
         """O10: Eq 18 literally (unfused) then Eq 19."""
-        Rt = np.einsum("rs,svn->rvn", self.M3, D - np.einsum("sk,kvn->svn", self.M2, ft)) + np.einsum("rk,kvn->rvn", self.M1, ft)
+        Rt = np.einsum("rs,svn->rvn", self.M3, D - np.einsum("sk,kvn->svn", self.M2, ft), optimize=True) + np.einsum("rk,kvn->rvn", self.M1, ft, optimize=True)
         return -Rt / self.Ju[:, None, :]
 
     def rhs(self, u, return_parts=False):

@@ -1,0 +1,212 @@
+"""Thin ctypes binding of libfr_b200.so (include/fr.h).  Argument marshalling only: every step of the
+FR right-hand side runs in the library's CUDA kernels.  There is no CPU fallback: if the shared
+library is missing, importing this module raises.
+
+PyTorch appears only in the callers (tests, bench.py) to allocate device memory and streams; this
+module takes raw device pointers (ints) so it works with any allocator.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfr_b200.so")
+
+QUAD, TRI, HEX = 0, 1, 2
+EULER, NAVIER_STOKES = 0, 1
+F32, F64 = 0, 1
+BC_SUP_INFLOW, BC_SUB_OUTFLOW, BC_NOSLIP_WALL = 0, 1, 2
+FLAG_FORCE_GENERIC, FLAG_HOST_ONLY = 1, 2
+ETYPES = {"quad": QUAD, "tri": TRI, "hex": HEX}
+SYSTEMS = {"euler": EULER, "navier-stokes": NAVIER_STOKES}
+BC_KINDS = {"sup-inflow": BC_SUP_INFLOW, "sub-outflow": BC_SUB_OUTFLOW, "noslip-wall": BC_NOSLIP_WALL}
+
+
+class FrError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("fr error %d: %s" % (code, text))
+        self.code = code
+
+
+class fr_bc_desc(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("rho", C.c_double), ("v", C.c_double * 3), ("p", C.c_double), ("cpTw", C.c_double)]
+
+
+class fr_mesh_desc(C.Structure):
+    _fields_ = [
+        ("ndims", C.c_int32), ("etype", C.c_int32), ("p_g", C.c_int32), ("n_bcs", C.c_int32),
+        ("n_elems", C.c_int64), ("n_ifaces", C.c_int64), ("n_bfaces", C.c_int64),
+        ("nodes", C.c_void_p), ("ifaces", C.c_void_p), ("shifts", C.c_void_p), ("bfaces", C.c_void_p), ("bcs", C.c_void_p),
+    ]
+
+
+class fr_disc_desc(C.Structure):
+    _fields_ = [
+        ("p", C.c_int32), ("system", C.c_int32), ("precision", C.c_int32), ("flags", C.c_int32),
+        ("gamma", C.c_double), ("mu", C.c_double), ("Pr", C.c_double), ("ldg_beta", C.c_double), ("ldg_tau", C.c_double),
+    ]
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "libfr_b200.so is missing (%s): build it with `python -m paper_1312_1638_b200.build`; there is no CPU fallback" % LIB_PATH
+        )
+    lib = C.CDLL(LIB_PATH)
+    P, I64 = C.c_void_p, C.c_int64
+    sig = {
+        "fr_setup_mesh": (C.c_int, [C.POINTER(P), C.POINTER(fr_mesh_desc)]),
+        "fr_setup_operators": (C.c_int, [P, C.POINTER(fr_disc_desc)]),
+        "fr_num_solution_points": (I64, [P]), "fr_num_flux_points": (I64, [P]), "fr_num_vars": (I64, [P]),
+        "fr_num_pairs": (I64, [P]), "fr_leading_dim": (I64, [P]), "fr_state_bytes": (I64, [P]),
+        "fr_workspace_bytes": (I64, [P]), "fr_rhs_kernel_launches": (I64, [P]),
+        "fr_solution_point_coords": (C.c_int, [P, P]),
+        "fr_operator_dims": (C.c_int, [P, C.c_int, C.POINTER(I64), C.POINTER(I64)]),
+        "fr_get_operator": (C.c_int, [P, C.c_int, P]),
+        "fr_get_pairs": (C.c_int, [P, P, P, P]),
+        "fr_get_metrics": (C.c_int, [P, P, P]),
+        "fr_rhs": (C.c_int, [P, P, P, P, P]),
+        "fr_rhs_profiled": (C.c_int, [P, P, P, P, P, C.c_int, C.POINTER(C.c_int), P, P]),
+        "fr_rk4_step": (C.c_int, [P, P, C.c_double, P, P]),
+        "fr_rhs_host": (C.c_int, [P, P, P, P, P, P, P]),
+        "fr_teardown": (None, [P]),
+        "fr_last_error": (C.c_char_p, [P]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    return lib
+
+
+lib = _load()
+EXPORTS = ["fr_setup_mesh", "fr_setup_operators", "fr_num_solution_points", "fr_num_flux_points", "fr_num_vars", "fr_num_pairs",
+           "fr_leading_dim", "fr_state_bytes", "fr_workspace_bytes", "fr_rhs_kernel_launches", "fr_solution_point_coords",
+           "fr_operator_dims", "fr_get_operator", "fr_get_pairs", "fr_get_metrics", "fr_rhs", "fr_rhs_profiled", "fr_rk4_step", "fr_rhs_host",
+           "fr_teardown", "fr_last_error"]
+
+
+def _ptr(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None and a.size else None
+
+
+class Context:
+    """Owns one fr_ctx.  Method names mirror the C entry points."""
+
+    def __init__(self, mesh, bcs=None):
+        """mesh: workloads.py mesh dict; bcs: {bc_id: (kind, params)} as the oracle takes them."""
+        self._h = C.c_void_p()
+        self._keep = []
+        nodes = np.ascontiguousarray(mesh["nodes"], dtype=np.float64)
+        ifaces = np.ascontiguousarray(mesh["ifaces"], dtype=np.int32)
+        shifts = np.ascontiguousarray(mesh["shifts"], dtype=np.float64)
+        bfaces = np.ascontiguousarray(mesh["bfaces"], dtype=np.int32)
+        bcs = bcs or {}
+        nb = (max(bcs) + 1) if bcs else 0
+        arr = (fr_bc_desc * max(nb, 1))()
+        for i, (kind, par) in bcs.items():
+            arr[i].kind = BC_KINDS[kind]
+            arr[i].rho = float(par.get("rho", 0.0))
+            v = list(par.get("v", ())) + [0.0] * 3
+            for d in range(3):
+                arr[i].v[d] = float(v[d])
+            arr[i].p = float(par.get("p", 0.0))
+            arr[i].cpTw = float(par.get("cpTw", 0.0))
+        for i in range(nb):
+            if i not in bcs:
+                arr[i].kind = BC_SUP_INFLOW
+        d = fr_mesh_desc(
+            ndims=mesh["ndims"], etype=ETYPES[mesh["etype"]], p_g=mesh["p_g"], n_bcs=nb,
+            n_elems=nodes.shape[0], n_ifaces=ifaces.shape[0], n_bfaces=bfaces.shape[0],
+            nodes=_ptr(nodes), ifaces=_ptr(ifaces), shifts=_ptr(shifts), bfaces=_ptr(bfaces),
+            bcs=C.cast(arr, C.c_void_p) if nb else None,
+        )
+        rc = lib.fr_setup_mesh(C.byref(self._h), C.byref(d))
+        if rc != 0:
+            raise FrError(rc, (lib.fr_last_error(None) or b"").decode())
+        self.ndims, self.n_elems = mesh["ndims"], nodes.shape[0]
+
+    def _check(self, rc):
+        if rc != 0:
+            raise FrError(rc, (lib.fr_last_error(self._h) or b"").decode())
+
+    def setup_operators(self, p, system, precision="f64", gamma=1.4, mu=0.0, Pr=0.71, beta=0.5, tau=0.1, flags=0, **_):
+        d = fr_disc_desc(p=p, system=SYSTEMS[system], precision=F64 if precision in ("f64", F64) else F32, flags=flags,
+                         gamma=gamma, mu=mu, Pr=Pr, ldg_beta=beta, ldg_tau=tau)
+        self._check(lib.fr_setup_operators(self._h, C.byref(d)))
+        self.Nu = lib.fr_num_solution_points(self._h)
+        self.Nf = lib.fr_num_flux_points(self._h)
+        self.NV = lib.fr_num_vars(self._h)
+        self.ld = lib.fr_leading_dim(self._h)
+        self.dtype = np.float64 if d.precision == F64 else np.float32
+        return self
+
+    num_pairs = property(lambda self: lib.fr_num_pairs(self._h))
+    state_bytes = property(lambda self: lib.fr_state_bytes(self._h))
+    workspace_bytes = property(lambda self: lib.fr_workspace_bytes(self._h))
+    rhs_kernel_launches = property(lambda self: lib.fr_rhs_kernel_launches(self._h))
+
+    def solution_point_coords(self):
+        x = np.empty((self.Nu, self.n_elems, self.ndims), dtype=np.float64)
+        self._check(lib.fr_solution_point_coords(self._h, _ptr(x)))
+        return x
+
+    def get_operator(self, i):
+        r, c = C.c_int64(), C.c_int64()
+        self._check(lib.fr_operator_dims(self._h, i, C.byref(r), C.byref(c)))
+        m = np.empty((r.value, c.value), dtype=np.float64)
+        self._check(lib.fr_get_operator(self._h, i, _ptr(m)))
+        return m
+
+    def get_pairs(self):
+        n = self.num_pairs
+        pairs = np.empty((n, 4), dtype=np.int32)
+        nrm = np.empty((n, self.ndims), dtype=np.float64)
+        jn = np.empty((n, 2), dtype=np.float64)
+        self._check(lib.fr_get_pairs(self._h, _ptr(pairs), _ptr(nrm), _ptr(jn)))
+        return pairs, nrm, jn
+
+    def get_metrics(self):
+        s = np.empty((self.ndims * self.ndims, self.Nu, self.ld), dtype=np.float64)
+        r = np.empty((self.Nu, self.ld), dtype=np.float64)
+        self._check(lib.fr_get_metrics(self._h, _ptr(s), _ptr(r)))
+        return s, r
+
+    # --- the hot path: raw device pointers (ints) in, nothing out ---
+    def rhs(self, u_ptr, rhs_ptr, work_ptr, stream=0):
+        self._check(lib.fr_rhs(self._h, u_ptr, rhs_ptr, work_ptr, stream))
+
+    def rhs_profiled(self, u_ptr, rhs_ptr, work_ptr, stream=0):
+        """-> [(kernel name, ms)] for one RHS (events between kernels; synchronises)."""
+        n = C.c_int()
+        ms = (C.c_float * 32)()
+        names = C.create_string_buffer(32 * 32)
+        self._check(lib.fr_rhs_profiled(self._h, u_ptr, rhs_ptr, work_ptr, stream, 32, C.byref(n), C.cast(ms, C.c_void_p), C.cast(names, C.c_void_p)))
+        return [(names.raw[32 * i : 32 * i + 32].split(b"\0")[0].decode(), float(ms[i])) for i in range(n.value)]
+
+    def rk4_step(self, u_ptr, dt, work_ptr, stream=0):
+        self._check(lib.fr_rk4_step(self._h, u_ptr, float(dt), work_ptr, stream))
+
+    def rhs_host(self, u_host_ptr, rhs_host_ptr, u_ptr, rhs_ptr, work_ptr, stream=0):
+        self._check(lib.fr_rhs_host(self._h, u_host_ptr, rhs_host_ptr, u_ptr, rhs_ptr, work_ptr, stream))
+
+    # --- layout helpers (host side, no arithmetic of the method) ---
+    def pad(self, u):
+        """[Nu, NV, n_elems] -> padded [Nu, NV, ld] in the context precision (pad columns zero)."""
+        out = np.zeros((self.Nu, self.NV, self.ld), dtype=self.dtype)
+        out[:, :, : self.n_elems] = u
+        return out
+
+    def unpad(self, u):
+        return np.asarray(u)[:, :, : self.n_elems]
+
+    def teardown(self):
+        if self._h:
+            lib.fr_teardown(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.teardown()
+        except Exception:
+            pass

@@ -1,0 +1,62 @@
+// Device-side constant tables of a context and the launch entry points of the two kernel families.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "fr_physics.cuh"
+
+namespace fr {
+
+struct DevConsts {
+  int nd, NV, Nu, Nf, n, nfp, etype;
+  int64_t Nel, ld, npairs, nbnd;
+  bool ns;       // Navier-Stokes (gradients, LDG) or Euler
+  bool f64;      // storage precision of u / rhs
+  Phys ph;
+  // dense operators (device, row-major doubles)
+  const double *M0, *M3, *M6, *M46, *M132;
+  // metrics at solution points
+  const double *smat;   // [nd*nd][Nu][ld]
+  const double *rcpj;   // [Nu][ld]
+  // flux-point pairs in iteration order
+  const int32_t *pLs, *pLe, *pRs, *pRe;
+  const double *pn, *pJnL, *pJnR;
+  // boundary flux points
+  const int32_t *bs, *be, *bbc;
+  const double *bn, *bJn;
+  const BcDev *bcs;
+  int nbcs;
+  // element-centric tables (tensor-product kernels)
+  const int32_t *fp_pe, *fp_ps;
+  const double *fp_n, *fp_Jn;
+};
+
+// Workspace layout (doubles unless noted); offsets in bytes from work_dev
+struct WorkLayout {
+  int64_t uf, cf, qu, qf;          // generic path: U^f (-> D~), C^f, Q~ -> Q -> F~, Q^f
+  int64_t rk_k, rk_tmp, rk_acc;    // RK4 registers in the storage precision
+  int64_t total;
+};
+
+// Optional per-kernel timing: an event is recorded before every kernel and after the last one.
+struct Prof {
+  static const int MAXK = 32;
+  cudaEvent_t ev[MAXK + 1];
+  const char *names[MAXK];
+  int n = 0;
+  cudaStream_t s = nullptr;
+  void mark(const char *name) { if (n < MAXK) { names[n] = name; cudaEventRecord(ev[n], s); ++n; } }
+  void end() { cudaEventRecord(ev[n], s); }
+};
+#define FR_MARK(prof, name) do { if (prof) (prof)->mark(name); } while (0)
+
+// generic (staged, dense-operator) path: any element type.  Returns cudaGetLastError().
+cudaError_t generic_rhs(const DevConsts &c, const WorkLayout &w, const void *u, void *rhs, char *work, cudaStream_t s, Prof *prof);
+int generic_rhs_launches(const DevConsts &c);
+
+// RK4 register updates (fr_rk.cu)
+cudaError_t rk_axpy2(bool f64, int64_t n, const void *u, const void *k, double a, void *out1, double b, void *out2,
+                     int mode, cudaStream_t s);
+
+}  // namespace fr

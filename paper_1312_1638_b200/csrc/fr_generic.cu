@@ -1,0 +1,267 @@
+// Generic FR right-hand side: the paper's staged kernel sequence (App A) with dense
+// operator matrices, for any element type.  This is the path triangles and quadrilaterals run and the
+// fallback for hexahedra (FR_FLAG_FORCE_GENERIC); the tensor-product kernels in fr_tensor.cu replace it
+// for hexahedra.  All arithmetic in double; u / rhs are stored in T (float or double).
+#include "fr_dev.hpp"
+
+namespace fr {
+namespace {
+
+constexpr int RT = 8;  // rows of the operator per thread
+
+// out[blk][r][col] = sum_k A[r][k] in1[blk][k][col] (+ sum_k B[r][k] in2[k][col]),  col = a*ld + e.
+// SCALE: multiply by -rcpj[r][e] (Eq 19 :243, the paper's negdivconf kernel).
+template <typename TIN, typename TOUT, bool SCALE>
+__global__ void __launch_bounds__(128) k_apply(int M, int K1, const double *__restrict__ A, const TIN *__restrict__ in1, int K2,
+                                               const double *__restrict__ B, const double *__restrict__ in2, TOUT *__restrict__ out,
+                                               int64_t ld, int64_t Nel, int NV, const double *__restrict__ rcpj,
+                                               int64_t in_blk, int64_t out_blk) {
+  extern __shared__ double sA[];  // [RT][K1] then [RT][K2]
+  const int r0 = blockIdx.y * RT;
+  const int nr = min(RT, M - r0);
+  for (int i = threadIdx.x; i < RT * K1; i += blockDim.x) { int j = i / K1, k = i % K1; sA[i] = j < nr ? A[(size_t)(r0 + j) * K1 + k] : 0.0; }
+  double *sB = sA + RT * K1;
+  for (int i = threadIdx.x; i < RT * K2; i += blockDim.x) { int j = i / K2, k = i % K2; sB[i] = j < nr ? B[(size_t)(r0 + j) * K2 + k] : 0.0; }
+  __syncthreads();
+  const int64_t ncols = (int64_t)NV * ld;
+  const int64_t col = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (col >= ncols) return;
+  const int64_t e = col % ld;
+  if (e >= Nel) return;
+  in1 += (size_t)blockIdx.z * in_blk;
+  out += (size_t)blockIdx.z * out_blk;
+  double acc[RT];
+#pragma unroll
+  for (int j = 0; j < RT; ++j) acc[j] = 0.0;
+  for (int k = 0; k < K1; ++k) {
+    const double x = (double)in1[(size_t)k * ncols + col];
+#pragma unroll
+    for (int j = 0; j < RT; ++j) acc[j] = fma(sA[j * K1 + k], x, acc[j]);
+  }
+  for (int k = 0; k < K2; ++k) {
+    const double x = in2[(size_t)k * ncols + col];
+#pragma unroll
+    for (int j = 0; j < RT; ++j) acc[j] = fma(sB[j * K2 + k], x, acc[j]);
+  }
+#pragma unroll
+  for (int j = 0; j < RT; ++j)
+    if (j < nr) {
+      double v = acc[j];
+      if (SCALE) v = -v * rcpj[(size_t)(r0 + j) * ld + e];
+      out[(size_t)(r0 + j) * ncols + col] = (TOUT)v;
+    }
+}
+
+// Common solution, Eq 7 + Eq 25 (:192, :506): each pair visited once, same value to both sides.
+template <int ND>
+__global__ void k_common_sol(DevConsts c, const double *__restrict__ uf, double *__restrict__ cf) {
+  constexpr int NV = ND + 2;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= c.npairs) return;
+  const size_t oL = (size_t)c.pLs[i] * NV * c.ld + c.pLe[i], oR = (size_t)c.pRs[i] * NV * c.ld + c.pRe[i];
+  const double wl = 0.5 - c.ph.beta, wr = 0.5 + c.ph.beta;
+#pragma unroll
+  for (int a = 0; a < NV; ++a) {
+    const double v = wl * uf[oL + (size_t)a * c.ld] + wr * uf[oR + (size_t)a * c.ld];
+    cf[oL + (size_t)a * c.ld] = v;
+    cf[oR + (size_t)a * c.ld] = v;
+  }
+}
+
+// Boundary common solution C(u_L, B_ldg u_L)  (:797)
+template <int ND>
+__global__ void k_common_sol_bnd(DevConsts c, const double *__restrict__ uf, double *__restrict__ cf) {
+  constexpr int NV = ND + 2;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= c.nbnd) return;
+  const size_t o = (size_t)c.bs[i] * NV * c.ld + c.be[i];
+  double u[NV], gi[NV], gl[NV];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) u[a] = uf[o + (size_t)a * c.ld];
+  ghost_states<ND>(c.bcs[c.bbc[i]], u, c.ph.gamma, gi, gl);
+#pragma unroll
+  for (int a = 0; a < NV; ++a) cf[o + (size_t)a * c.ld] = (0.5 - c.ph.beta) * u[a] + (0.5 + c.ph.beta) * gl[a];
+}
+
+// q = J^-T q~ = (1/J) S^T q~, Eq 10 (:206), in place
+template <int ND>
+__global__ void k_grad_phys(DevConsts c, double *__restrict__ qu) {
+  constexpr int NV = ND + 2;
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (int64_t)c.Nu * c.ld) return;
+  const int64_t e = idx % c.ld, r = idx / c.ld;
+  if (e >= c.Nel) return;
+  double S[ND][ND];
+#pragma unroll
+  for (int i = 0; i < ND; ++i)
+#pragma unroll
+    for (int n = 0; n < ND; ++n) S[i][n] = c.smat[((size_t)(i * ND + n) * c.Nu + r) * c.ld + e];
+  const double rj = c.rcpj[(size_t)r * c.ld + e];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) {
+    double qt[ND];
+#pragma unroll
+    for (int i = 0; i < ND; ++i) qt[i] = qu[(((size_t)i * c.Nu + r) * NV + a) * c.ld + e];
+#pragma unroll
+    for (int n = 0; n < ND; ++n) {
+      double s = 0;
+#pragma unroll
+      for (int i = 0; i < ND; ++i) s = fma(S[i][n], qt[i], s);
+      qu[(((size_t)n * c.Nu + r) * NV + a) * c.ld + e] = s * rj;
+    }
+  }
+}
+
+// F~ = S (f_inv - f_vis), Eq 12 (:214) with Eq 20-24; in place over Q^u
+template <int ND, bool NS, typename T>
+__global__ void k_tflux(DevConsts c, const T *__restrict__ u, double *__restrict__ qu) {
+  constexpr int NV = ND + 2;
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (int64_t)c.Nu * c.ld) return;
+  const int64_t e = idx % c.ld, r = idx / c.ld;
+  if (e >= c.Nel) return;
+  double uu[NV], f[ND][NV], v[ND], p;
+#pragma unroll
+  for (int a = 0; a < NV; ++a) uu[a] = (double)u[((size_t)r * NV + a) * c.ld + e];
+  inviscid_flux<ND>(uu, c.ph.gamma, f, v, p);
+  if (NS) {
+    double q[ND][NV];
+#pragma unroll
+    for (int n = 0; n < ND; ++n)
+#pragma unroll
+      for (int a = 0; a < NV; ++a) q[n][a] = qu[(((size_t)n * c.Nu + r) * NV + a) * c.ld + e];
+    subtract_viscous_flux<ND>(uu, q, v, c.ph, f);
+  }
+  double S[ND][ND];
+#pragma unroll
+  for (int i = 0; i < ND; ++i)
+#pragma unroll
+    for (int n = 0; n < ND; ++n) S[i][n] = c.smat[((size_t)(i * ND + n) * c.Nu + r) * c.ld + e];
+#pragma unroll
+  for (int i = 0; i < ND; ++i)
+#pragma unroll
+    for (int a = 0; a < NV; ++a) {
+      double s = 0;
+#pragma unroll
+      for (int n = 0; n < ND; ++n) s = fma(S[i][n], f[n][a], s);
+      qu[(((size_t)i * c.Nu + r) * NV + a) * c.ld + e] = s;
+    }
+}
+
+// Common normal flux over flux-point pairs, Eq 15-17 (:227-235); in place over U^f -> D~ (:300)
+template <int ND, bool NS>
+__global__ void k_common_flux(DevConsts c, double *__restrict__ uf, const double *__restrict__ qf) {
+  constexpr int NV = ND + 2;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= c.npairs) return;
+  const size_t oL = (size_t)c.pLs[i] * NV * c.ld + c.pLe[i], oR = (size_t)c.pRs[i] * NV * c.ld + c.pRe[i];
+  const size_t blk = (size_t)c.Nf * NV * c.ld;
+  double uL[NV], uR[NV], qL[ND][NV], qR[ND][NV], nrm[ND], F[NV];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) { uL[a] = uf[oL + (size_t)a * c.ld]; uR[a] = uf[oR + (size_t)a * c.ld]; }
+  if (NS) {
+#pragma unroll
+    for (int n = 0; n < ND; ++n)
+#pragma unroll
+      for (int a = 0; a < NV; ++a) { qL[n][a] = qf[n * blk + oL + (size_t)a * c.ld]; qR[n][a] = qf[n * blk + oR + (size_t)a * c.ld]; }
+  }
+#pragma unroll
+  for (int n = 0; n < ND; ++n) nrm[n] = c.pn[(size_t)n * c.npairs + i];
+  common_flux<ND, NS>(uL, uR, uR, qL, qR, nrm, c.ph, F);
+  const double jl = c.pJnL[i], jr = c.pJnR[i];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) { uf[oL + (size_t)a * c.ld] = jl * F[a]; uf[oR + (size_t)a * c.ld] = -jr * F[a]; }
+}
+
+template <int ND, bool NS>
+__global__ void k_common_flux_bnd(DevConsts c, double *__restrict__ uf, const double *__restrict__ qf) {
+  constexpr int NV = ND + 2;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= c.nbnd) return;
+  const size_t o = (size_t)c.bs[i] * NV * c.ld + c.be[i];
+  const size_t blk = (size_t)c.Nf * NV * c.ld;
+  double uL[NV], gi[NV], gl[NV], qL[ND][NV], qR[ND][NV], nrm[ND], F[NV];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) uL[a] = uf[o + (size_t)a * c.ld];
+  const double keep = ghost_states<ND>(c.bcs[c.bbc[i]], uL, c.ph.gamma, gi, gl);
+  if (NS) {
+#pragma unroll
+    for (int n = 0; n < ND; ++n)
+#pragma unroll
+      for (int a = 0; a < NV; ++a) { qL[n][a] = qf[n * blk + o + (size_t)a * c.ld]; qR[n][a] = keep * qL[n][a]; }
+  }
+#pragma unroll
+  for (int n = 0; n < ND; ++n) nrm[n] = c.bn[(size_t)n * c.nbnd + i];
+  common_flux<ND, NS>(uL, gl, gi, qL, qR, nrm, c.ph, F);
+  const double jn = c.bJn[i];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) uf[o + (size_t)a * c.ld] = jn * F[a];
+}
+
+template <typename TIN, typename TOUT, bool SCALE>
+void apply(cudaStream_t s, const DevConsts &c, int M, int K1, const double *A, const TIN *in1, int K2, const double *B,
+           const double *in2, TOUT *out, int nblk = 1, int64_t in_blk = 0, int64_t out_blk = 0) {
+  const int64_t ncols = (int64_t)c.NV * c.ld;
+  dim3 grid((unsigned)((ncols + 127) / 128), (unsigned)((M + RT - 1) / RT), (unsigned)nblk);
+  size_t smem = (size_t)RT * (K1 + K2) * sizeof(double);
+  if (smem > 48 * 1024) cudaFuncSetAttribute(k_apply<TIN, TOUT, SCALE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  k_apply<TIN, TOUT, SCALE><<<grid, 128, smem, s>>>(M, K1, A, in1, K2, B, in2, out, c.ld, c.Nel, c.NV, c.rcpj, in_blk, out_blk);
+}
+
+template <int ND, bool NS, typename T>
+cudaError_t run(const DevConsts &c, const WorkLayout &w, const T *u, T *rhs, char *work, cudaStream_t s, Prof *prof) {
+  double *uf = (double *)(work + w.uf), *cf = (double *)(work + w.cf), *qu = (double *)(work + w.qu), *qf = (double *)(work + w.qf);
+  const int Nu = c.Nu, Nf = c.Nf;
+  const int TB = 128;
+  auto blocks = [&](int64_t n) { return (unsigned)((n + TB - 1) / TB); };
+  const int64_t npts = (int64_t)Nu * c.ld;
+  // (1) U^f = M0 U                                                       Eq 41 :745
+  FR_MARK(prof, "apply_M0");
+  apply<T, double, false>(s, c, Nf, Nu, c.M0, u, 0, nullptr, nullptr, uf);
+  if (NS) {
+    // (2) C^f                                                            Eq 7, 25
+    FR_MARK(prof, "common_sol");
+    if (c.npairs) k_common_sol<ND><<<blocks(c.npairs), TB, 0, s>>>(c, uf, cf);
+    if (c.nbnd) k_common_sol_bnd<ND><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, cf);
+    // (2) Q~ = (M4 - M6 M0) U + M6 C                                     Eq 42 :756
+    FR_MARK(prof, "apply_M46_M6");
+    apply<T, double, false>(s, c, ND * Nu, Nu, c.M46, u, Nf, c.M6, cf, qu);
+    // (3) Q = J^-T Q~ ; Q^f = M5 Q                                       Eq 10, Eq 43
+    FR_MARK(prof, "grad_phys");
+    k_grad_phys<ND><<<blocks(npts), TB, 0, s>>>(c, qu);
+    FR_MARK(prof, "apply_M5");
+    apply<double, double, false>(s, c, Nf, Nu, c.M0, qu, 0, nullptr, nullptr, qf, ND, (int64_t)Nu * c.NV * c.ld, (int64_t)Nf * c.NV * c.ld);
+  }
+  // (4) F~ = S f(U, Q)                                                   Eq 12
+  FR_MARK(prof, "tflux");
+  k_tflux<ND, NS, T><<<blocks(npts), TB, 0, s>>>(c, u, qu);
+  // (5) D~ = J n F(...)  in place over U^f                               Eq 15-17
+  FR_MARK(prof, "common_flux");
+  if (c.npairs) k_common_flux<ND, NS><<<blocks(c.npairs), TB, 0, s>>>(c, uf, qf);
+  if (c.nbnd) k_common_flux_bnd<ND, NS><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, qf);
+  // (6,7) R = -(1/J) {(M1 - M3 M2) F~ + M3 D~}                           Eq 44, Eq 19
+  FR_MARK(prof, "apply_M132_M3_negdivconf");
+  apply<double, T, true>(s, c, Nu, ND * Nu, c.M132, qu, Nf, c.M3, uf, rhs);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+int generic_rhs_launches(const DevConsts &c) {
+  int n = 4;  // interp, tflux, common flux, divergence
+  if (c.ns) n += 4;  // common solution, gradient, transform, interp of gradient
+  if (c.nbnd) n += c.ns ? 2 : 1;
+  if (!c.npairs) n -= c.ns ? 2 : 1;
+  return n;
+}
+
+cudaError_t generic_rhs(const DevConsts &c, const WorkLayout &w, const void *u, void *rhs, char *work, cudaStream_t s, Prof *prof) {
+#define FR_RUN(ND, NS)                                                                              \
+  (c.f64 ? run<ND, NS, double>(c, w, (const double *)u, (double *)rhs, work, s, prof)                      \
+         : run<ND, NS, float>(c, w, (const float *)u, (float *)rhs, work, s, prof))
+  if (c.nd == 2) return c.ns ? FR_RUN(2, true) : FR_RUN(2, false);
+  return c.ns ? FR_RUN(3, true) : FR_RUN(3, false);
+#undef FR_RUN
+}
+
+}  // namespace fr

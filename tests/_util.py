@@ -1,0 +1,45 @@
+"""Shared helpers for the parity tests (host-side marshalling only)."""
+import numpy as np
+
+
+def rel_l2_per_field(a, b):
+    """||a-b||_2 / ||b||_2 per variable; arrays [Nu, NV, Nel]."""
+    a = np.asarray(a, dtype=np.longdouble)
+    b = np.asarray(b, dtype=np.longdouble)
+    num = np.sqrt(np.sum((a - b) ** 2, axis=(0, 2)))
+    den = np.sqrt(np.sum(b ** 2, axis=(0, 2)))
+    return np.asarray(num / den, dtype=np.float64)
+
+
+class GpuRunner:
+    """Allocates device buffers with torch and calls the C-ABI through the binding."""
+
+    def __init__(self, ctx):
+        import torch
+
+        self.torch = torch
+        self.ctx = ctx
+        self.tdtype = torch.float64 if ctx.dtype == np.float64 else torch.float32
+        shape = (ctx.Nu, ctx.NV, ctx.ld)
+        self.u = torch.zeros(shape, dtype=self.tdtype, device="cuda")
+        self.r = torch.zeros(shape, dtype=self.tdtype, device="cuda")
+        self.work = torch.zeros(max(ctx.workspace_bytes, 256), dtype=torch.uint8, device="cuda")
+        self.stream = torch.cuda.current_stream().cuda_stream
+
+    def set_state(self, U):
+        self.u.copy_(self.torch.from_numpy(self.ctx.pad(U)))
+
+    def rhs(self, U=None):
+        if U is not None:
+            self.set_state(U)
+        self.r.fill_(float("nan"))
+        self.ctx.rhs(self.u.data_ptr(), self.r.data_ptr(), self.work.data_ptr(), self.stream)
+        self.torch.cuda.synchronize()
+        return self.ctx.unpad(self.r.cpu().numpy())
+
+    def rk4(self, U, dt, steps):
+        self.set_state(U)
+        for _ in range(steps):
+            self.ctx.rk4_step(self.u.data_ptr(), dt, self.work.data_ptr(), self.stream)
+        self.torch.cuda.synchronize()
+        return self.ctx.unpad(self.u.cpu().numpy())

@@ -1,0 +1,158 @@
+"""GPU parity: the CUDA library (through the C ABI) against the oracle on identical seeded inputs.
+Bar (BASELINE.json north_star): relative L2 per field <= 1e-12 in fp64, <= 1e-5 in fp32.
+Where the problem's own rounding floor (double oracle vs long-double oracle) is above
+1e-12/3 the bar is 3x that floor, measured in the same test and printed."""
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle.fr_oracle import FROracle, flux_inviscid
+from _util import GpuRunner, rel_l2_per_field
+
+pytestmark = pytest.mark.gpu
+
+TOL64, TOL32 = 1e-12, 1e-5
+
+
+def _ctx(mesh, disc, precision="f64", bcs=None, flags=0):
+    from paper_1312_1638_b200 import Context
+
+    return Context(mesh, bcs).setup_operators(precision=precision, flags=flags, **disc)
+
+
+def _bar(o, U, R_ref, tol=TOL64):
+    """max(tol, 3 x rounding floor of the problem) per field."""
+    mesh, prm, bcs = o.mesh, o.prm, o.bcs
+    old = FROracle(mesh, prm, bcs, dtype=np.longdouble)
+    floor = rel_l2_per_field(R_ref, old.rhs(np.asarray(U, dtype=np.longdouble)))
+    return np.maximum(tol, 3 * floor), floor
+
+
+def _check(name, got, ref, bar):
+    err = rel_l2_per_field(got, ref)
+    print("%s rel-L2 per field: %s  (bar %s)" % (name, np.array2string(err, precision=2), np.array2string(np.asarray(bar), precision=2)))
+    assert np.all(np.isfinite(got))
+    assert np.all(err <= bar), (name, err, bar)
+    return err
+
+
+CASES = {
+    "C1": ("C1", {}),
+    "C2-6": ("C2", dict(n=6)),
+    "C3-4": ("C3", dict(n=4)),
+    "C4-24": ("C4", dict(n=24)),
+    "C5-p1": ("C5", dict(n=5, p=1)),
+    "C5-p2-euler": ("C5", dict(n=5, p=2, system="euler")),
+    "C5-p5": ("C5", dict(n=3, p=5)),
+    "C5-p6-euler": ("C5", dict(n=3, p=6, system="euler")),
+}
+
+
+@pytest.mark.parametrize("flags", [0, 1], ids=["default", "generic"])
+@pytest.mark.parametrize("case", list(CASES))
+def test_rhs_parity_fp64(case, flags):
+    name, over = CASES[case]
+    mesh, disc = W.config(name, **over)
+    o = FROracle(mesh, disc)
+    ctx = _ctx(mesh, disc, flags=flags)
+    X = ctx.solution_point_coords()
+    assert np.allclose(X, np.asarray(o.xu_phys, float), atol=1e-13)
+    U = W.config_state(name, np.asarray(o.xu_phys, float), **over)
+    R = o.rhs(U)
+    bar, floor = _bar(o, U, R)
+    got = GpuRunner(ctx).rhs(U)
+    print("floor", floor)
+    _check(case, got, R, bar)
+
+
+@pytest.mark.parametrize("case", ["C3-4", "C5-p2-euler", "C5-p5"])
+def test_rhs_parity_fp32(case):
+    name, over = CASES[case]
+    mesh, disc = W.config(name, **over)
+    o = FROracle(mesh, disc)
+    U32 = W.config_state(name, np.asarray(o.xu_phys, float), **over).astype(np.float32)
+    R = o.rhs(U32.astype(np.float64))  # the oracle consumes the rounded inputs in double
+    ctx = _ctx(mesh, disc, precision="f32")
+    got = GpuRunner(ctx).rhs(U32)
+    assert got.dtype == np.float32
+    _check(case + "-fp32", got, R, TOL32)
+
+
+@pytest.mark.parametrize("case,steps", [("C1", 10), ("C2-6", 3)])
+def test_rk4_parity(case, steps):
+    name, over = CASES[case]
+    mesh, disc = W.config(name, **over)
+    o = FROracle(mesh, disc)
+    U = W.config_state(name, np.asarray(o.xu_phys, float), **over)
+    ref = U
+    for _ in range(steps):
+        ref = o.rk4_step(ref, disc["dt"])
+    ctx = _ctx(mesh, disc)
+    got = GpuRunner(ctx).rk4(U, disc["dt"], steps)
+    _check(case + "-rk4", got, ref, TOL64)
+    # the step did something
+    assert np.max(np.abs(ref - U)) > 1e-6
+
+
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_freestream_and_conservation_curved_hex(precision):
+    """north_star pins 3 and 4 on the GPU path, C3-shaped mesh (curved, p_g = p = 4)."""
+    mesh, disc = W.config("C3", n=4)
+    ctx = _ctx(mesh, disc, precision=precision)
+    o = FROracle(mesh, disc)
+    X = np.asarray(o.xu_phys, float)
+    run = GpuRunner(ctx)
+    U0 = np.moveaxis(W.uniform_state(X, rho=1.0, vel=(1.0, 1.0, 1.0), p=1.0), -1, 1)
+    R0 = run.rhs(U0.astype(ctx.dtype))
+    h = 2 * np.pi / 4
+    fmax = np.max(np.abs(flux_inviscid(np.moveaxis(U0, 1, 0), 1.4)))
+    tol = 1e-12 if precision == "f64" else 2e-6
+    assert np.max(np.abs(R0)) <= tol * fmax * 2 / h
+    U = W.config_state("C3", X).astype(ctx.dtype)
+    R = run.rhs(U).astype(np.float64)
+    tot, mag = o.integrate(R), o.integrate(np.abs(R))
+    assert np.all(np.abs(tot) <= (1e-12 if precision == "f64" else 1e-6) * mag), (tot, mag)
+
+
+def test_boundary_conditions_parity():
+    """Appendix C ghost-state boundaries on the GPU path (2-D quads and 3-D hexes, tiny cases)."""
+    free = dict(rho=1.2, v=(2.5, 0.4, 0.1), p=1.0)
+    for nd in (2, 3):
+        mesh = W.box_mesh((4,) * nd, (1.0,) * nd, periodic=(False,) * (nd - 1) + (True,))
+        bcs = {0: ("sup-inflow", free), 1: ("sub-outflow", dict(p=0.9)), 2: ("noslip-wall", dict(cpTw=3.0, v=(0.3, 0.0, 0.0))),
+               3: ("noslip-wall", dict(cpTw=3.2, v=(0.0, 0.0, 0.0)))}
+        if nd == 2:
+            bcs = {0: bcs[0], 1: bcs[1]}
+            mesh = W.box_mesh((4, 4), (1.0, 1.0), periodic=(False, True))
+        disc = dict(p=2, system="navier-stokes", gamma=1.4, mu=0.02, Pr=0.71, beta=0.5, tau=0.1)
+        o = FROracle(mesh, disc, bcs)
+        X = np.asarray(o.xu_phys, float)
+        U = np.moveaxis(W.add_relative_noise(W.uniform_state(X, rho=1.2, vel=(2.5, 0.4, 0.1)[:nd], p=1.0), 2e-2, 5), -1, 1)
+        R = o.rhs(U)
+        for flags in (0, 1):
+            got = GpuRunner(_ctx(mesh, disc, bcs=bcs, flags=flags)).rhs(U)
+            _check("bc-%dd-flags%d" % (nd, flags), got, R, TOL64)
+
+
+def test_beta_tau_variants():
+    """LDG parameters other than the paper's beta=1/2 (Eq 25-27): beta=0, beta=-1/2, tau=0."""
+    mesh, disc = W.config("C2", n=3)
+    for beta, tau in ((0.0, 0.1), (-0.5, 0.0), (0.25, 1.0)):
+        d = dict(disc, beta=beta, tau=tau)
+        o = FROracle(mesh, d)
+        U = W.config_state("C3", np.asarray(o.xu_phys, float))
+        R = o.rhs(U)
+        got = GpuRunner(_ctx(mesh, d)).rhs(U)
+        _check("beta%g-tau%g" % (beta, tau), got, R, TOL64)
+
+
+def test_error_paths_on_device():
+    from paper_1312_1638_b200 import FrError
+
+    mesh, disc = W.config("C1")
+    ctx = _ctx(mesh, disc)
+    run = GpuRunner(ctx)
+    with pytest.raises(FrError):
+        ctx.rhs(run.u.data_ptr(), run.u.data_ptr(), run.work.data_ptr(), run.stream)  # aliasing
+    with pytest.raises(FrError):
+        ctx.rhs(0, run.r.data_ptr(), run.work.data_ptr(), run.stream)  # NULL
