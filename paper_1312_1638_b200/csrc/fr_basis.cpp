@@ -175,7 +175,7 @@ void build_ref_ops(int etype, int p, int p_g, RefOps &o) {
       legendre(p, -g[i], a, da); legendre(p + 1, -g[i], b, db); gm[i] = (da + db) / 2;
     }
     std::vector<real> Dh(n * n);
-    for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) Dh[i * n + j] = D[i * n + j] - gm[i] * lm[j] - gp[i] * lp[j];
+    for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) Dh[i * n + j] = D[i * n + j] + gm[i] * lm[j] - gp[i] * lp[j];  // M2 carries the reference normal: -1 on the -1 face
     o.D1 = round_to_double(D); o.lm = round_to_double(lm); o.lp = round_to_double(lp);
     o.gm = round_to_double(gm); o.gp = round_to_double(gp); o.Dhat = round_to_double(Dh);
     // point sets

@@ -54,6 +54,10 @@ struct Prof {
 // generic (staged, dense-operator) path: any element type.  Returns cudaGetLastError().
 cudaError_t generic_rhs(const DevConsts &c, const WorkLayout &w, const void *u, void *rhs, char *work, cudaStream_t s, Prof *prof);
 int generic_rhs_launches(const DevConsts &c);
+// point-wise / pair kernels of the generic path reused by the tensor-product path
+void launch_common_jump(const DevConsts &c, const double *uf, double *cf, cudaStream_t s);  // {C - u^f} of Eq 9
+void launch_tflux(const DevConsts &c, const void *u, double *qu, cudaStream_t s);           // Eq 12, in place over Q^u
+void launch_common_flux(const DevConsts &c, double *uf, const double *qf, cudaStream_t s);  // Eq 15-17, in place over U^f
 
 // RK4 register updates (fr_rk.cu)
 cudaError_t rk_axpy2(bool f64, int64_t n, const void *u, const void *k, double a, void *out1, double b, void *out2,

@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(128) k_apply(int M, int K1, const double *__re
 }
 
 // Common solution, Eq 7 + Eq 25 (:192, :506): each pair visited once, same value to both sides.
-template <int ND>
+template <int ND, bool JUMP>
 __global__ void k_common_sol(DevConsts c, const double *__restrict__ uf, double *__restrict__ cf) {
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -62,14 +62,15 @@ __global__ void k_common_sol(DevConsts c, const double *__restrict__ uf, double 
   const double wl = 0.5 - c.ph.beta, wr = 0.5 + c.ph.beta;
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
-    const double v = wl * uf[oL + (size_t)a * c.ld] + wr * uf[oR + (size_t)a * c.ld];
-    cf[oL + (size_t)a * c.ld] = v;
-    cf[oR + (size_t)a * c.ld] = v;
+    const double ul = uf[oL + (size_t)a * c.ld], ur = uf[oR + (size_t)a * c.ld];
+    const double v = wl * ul + wr * ur;
+    cf[oL + (size_t)a * c.ld] = JUMP ? v - ul : v;   // JUMP: the {C - u^f} of Eq 9 directly
+    cf[oR + (size_t)a * c.ld] = JUMP ? v - ur : v;
   }
 }
 
 // Boundary common solution C(u_L, B_ldg u_L)  (:797)
-template <int ND>
+template <int ND, bool JUMP>
 __global__ void k_common_sol_bnd(DevConsts c, const double *__restrict__ uf, double *__restrict__ cf) {
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -80,7 +81,7 @@ __global__ void k_common_sol_bnd(DevConsts c, const double *__restrict__ uf, dou
   for (int a = 0; a < NV; ++a) u[a] = uf[o + (size_t)a * c.ld];
   ghost_states<ND>(c.bcs[c.bbc[i]], u, c.ph.gamma, gi, gl);
 #pragma unroll
-  for (int a = 0; a < NV; ++a) cf[o + (size_t)a * c.ld] = (0.5 - c.ph.beta) * u[a] + (0.5 + c.ph.beta) * gl[a];
+  for (int a = 0; a < NV; ++a) cf[o + (size_t)a * c.ld] = (0.5 - c.ph.beta) * u[a] + (0.5 + c.ph.beta) * gl[a] - (JUMP ? u[a] : 0.0);
 }
 
 // q = J^-T q~ = (1/J) S^T q~, Eq 10 (:206), in place
@@ -221,8 +222,8 @@ cudaError_t run(const DevConsts &c, const WorkLayout &w, const T *u, T *rhs, cha
   if (NS) {
     // (2) C^f                                                            Eq 7, 25
     FR_MARK(prof, "common_sol");
-    if (c.npairs) k_common_sol<ND><<<blocks(c.npairs), TB, 0, s>>>(c, uf, cf);
-    if (c.nbnd) k_common_sol_bnd<ND><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, cf);
+    if (c.npairs) k_common_sol<ND, false><<<blocks(c.npairs), TB, 0, s>>>(c, uf, cf);
+    if (c.nbnd) k_common_sol_bnd<ND, false><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, cf);
     // (2) Q~ = (M4 - M6 M0) U + M6 C                                     Eq 42 :756
     FR_MARK(prof, "apply_M46_M6");
     apply<T, double, false>(s, c, ND * Nu, Nu, c.M46, u, Nf, c.M6, cf, qu);
@@ -246,6 +247,42 @@ cudaError_t run(const DevConsts &c, const WorkLayout &w, const T *u, T *rhs, cha
 }
 
 }  // namespace
+
+// launchers shared with the tensor-product path (fr_tensor.cu)
+void launch_common_jump(const DevConsts &c, const double *uf, double *cf, cudaStream_t s) {
+  const int TB = 128;
+  if (c.nd == 2) {
+    if (c.npairs) k_common_sol<2, true><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, uf, cf);
+    if (c.nbnd) k_common_sol_bnd<2, true><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, uf, cf);
+  } else {
+    if (c.npairs) k_common_sol<3, true><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, uf, cf);
+    if (c.nbnd) k_common_sol_bnd<3, true><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, uf, cf);
+  }
+}
+
+template <int ND, bool NS>
+static void launch_flux_t(const DevConsts &c, const void *u, double *qu, double *uf, const double *qf, bool do_tflux, bool do_common, cudaStream_t s) {
+  const int TB = 128;
+  const int64_t npts = (int64_t)c.Nu * c.ld;
+  if (do_tflux) {
+    if (c.f64) k_tflux<ND, NS, double><<<(unsigned)((npts + TB - 1) / TB), TB, 0, s>>>(c, (const double *)u, qu);
+    else k_tflux<ND, NS, float><<<(unsigned)((npts + TB - 1) / TB), TB, 0, s>>>(c, (const float *)u, qu);
+  }
+  if (do_common) {
+    if (c.npairs) k_common_flux<ND, NS><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, uf, qf);
+    if (c.nbnd) k_common_flux_bnd<ND, NS><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, uf, qf);
+  }
+}
+
+void launch_tflux(const DevConsts &c, const void *u, double *qu, cudaStream_t s) {
+  if (c.nd == 2) { if (c.ns) launch_flux_t<2, true>(c, u, qu, nullptr, nullptr, true, false, s); else launch_flux_t<2, false>(c, u, qu, nullptr, nullptr, true, false, s); }
+  else { if (c.ns) launch_flux_t<3, true>(c, u, qu, nullptr, nullptr, true, false, s); else launch_flux_t<3, false>(c, u, qu, nullptr, nullptr, true, false, s); }
+}
+
+void launch_common_flux(const DevConsts &c, double *uf, const double *qf, cudaStream_t s) {
+  if (c.nd == 2) { if (c.ns) launch_flux_t<2, true>(c, nullptr, nullptr, uf, qf, false, true, s); else launch_flux_t<2, false>(c, nullptr, nullptr, uf, qf, false, true, s); }
+  else { if (c.ns) launch_flux_t<3, true>(c, nullptr, nullptr, uf, qf, false, true, s); else launch_flux_t<3, false>(c, nullptr, nullptr, uf, qf, false, true, s); }
+}
 
 int generic_rhs_launches(const DevConsts &c) {
   int n = 4;  // interp, tflux, common flux, divergence

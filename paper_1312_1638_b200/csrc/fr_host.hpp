@@ -23,7 +23,7 @@ struct RefOps {
   std::vector<double> D1;               // D1[i][j] = l_j'(xi_i)
   std::vector<double> lm, lp;           // l_j(-1), l_j(+1)
   std::vector<double> gm, gp;           // lifting coefficients: (div g) of the -1 / +1 face point at node i
-  std::vector<double> Dhat;             // D1 - gm lm^T - gp lp^T   (1-D form of M1 - M3 M2)
+  std::vector<double> Dhat;             // D1 + gm lm^T - gp lp^T   (1-D form of M1 - M3 M2; reference normal -1 on the -1 face)
   // geometry basis (degree p_g) at the solution / flux points
   int p_g = 0, Nn = 0;
   std::vector<long double> Gu, dGu, Gf, dGf;  // [Nu][Nn], [nd][Nu][Nn], [Nf][Nn], [nd][Nf][Nn]

@@ -1,9 +1,234 @@
-// Tensor-product kernels (placeholder until the sum-factorised hexahedral path lands).
+// Tensor-product (sum-factorised) kernels for quadrilateral / hexahedral elements.
+//
+// On tensor-product elements every row of M0, M4, M1, M3, M6 touches one line of
+// n = p+1 solution points (plus the two flux points at its ends), so the dense App-A GEMMs of the paper
+// (2*N_V*(8 N_f N_u + 6 N_u^2) flop per element) collapse to N_V*(12 n^4 + 72 n^3): the path becomes
+// HBM-bound.  The paper anticipates "bespoke matrix multiply kernels" (:282).
+//
+// Layout: every state matrix is [row][variable][ld], element fastest; a warp covers 32
+// consecutive columns (variable, element) of one row, so every global access is a fully used 256-byte row
+// segment.  Threads own output points and gather the n values of each line through L1 (a CTA covers all
+// rows of its 32 columns, so each input is fetched from L2/HBM once per CTA).
+// The 1-D operators travel as a kernel parameter (constant bank, uniform broadcast reads).
 #include "fr_tensor.hpp"
 
 namespace fr {
-bool tensor_supported(const DevConsts &) { return false; }
-cudaError_t tensor_plan(const DevConsts &, const RefOps &, const MeshConsts &, TensorPlan &, std::vector<void *> &) { return cudaErrorNotSupported; }
-cudaError_t tensor_rhs(const DevConsts &, const TensorPlan &, const void *, void *, char *, cudaStream_t, Prof *) { return cudaErrorNotSupported; }
-int tensor_rhs_launches(const DevConsts &) { return 0; }
+namespace {
+
+template <int N>
+struct Ops1D {
+  double D[N * N];    // D[i][m] = l_m'(xi_i)
+  double Dh[N * N];   // D + gm lm^T - gp lp^T  (1-D form of M1 - M3 M2, Eq 44 :773; M2 holds n~ = -1 on the -1 face)
+  double lm[N], lp[N];  // l_m(-1), l_m(+1)                    (M0, Eq 41)
+  double gm[N], gp[N];  // div g of the -1 / +1 face point at node i (M3, M6)
+};
+
+__host__ __device__ constexpr int ipow(int b, int e) { return e == 0 ? 1 : b * ipow(b, e - 1); }
+
+// rho of point m on the line through (direction d, face-point index idx)
+template <int N, int ND>
+__device__ __forceinline__ int line_base(int d, int idx, int &stride) {
+  if (ND == 2) {
+    stride = d == 0 ? 1 : N;
+    return d == 0 ? N * idx : idx;
+  }
+  const int a = idx % N, b = idx / N;
+  if (d == 0) { stride = 1; return N * a + N * N * b; }
+  if (d == 1) { stride = N; return a + N * N * b; }
+  stride = N * N;
+  return a + N * b;
+}
+
+// U^f = M0 U (Eq 6 / Eq 41) and, with nblk = ND, Q^f = M5 Q (Eq 11 / Eq 43).
+template <int N, int ND, typename TIN>
+__global__ void __launch_bounds__(1024) k_tp_interp(Ops1D<N> op, const TIN *__restrict__ in, double *__restrict__ out, int64_t ncols,
+                                                    int64_t ld, int64_t Nel, int64_t in_blk, int64_t out_blk) {
+  constexpr int NFP = ipow(N, ND - 1);
+  const int64_t col = (int64_t)blockIdx.x * 32 + threadIdx.x;
+  if (col >= ncols || (col % ld) >= Nel) return;
+  in += (size_t)blockIdx.z * in_blk + col;
+  out += (size_t)blockIdx.z * out_blk + col;
+  for (int idx = threadIdx.y; idx < NFP; idx += blockDim.y) {
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+      int stride;
+      const int base = line_base<N, ND>(d, idx, stride);
+      double sm = 0, sp = 0;
+#pragma unroll
+      for (int m = 0; m < N; ++m) {
+        const double v = (double)in[(size_t)(base + m * stride) * ncols];
+        sm = fma(op.lm[m], v, sm);
+        sp = fma(op.lp[m], v, sp);
+      }
+      out[(size_t)((2 * d) * NFP + idx) * ncols] = sm;
+      out[(size_t)((2 * d + 1) * NFP + idx) * ncols] = sp;
+    }
+  }
+}
+
+// Q = J^-T {M4 U + M6 (C - U^f)}  (Eq 9-10 / Eq 42): thread per solution point and column.
+// jump = C - U^f at the flux points (written by the common-solution kernel).
+template <int N, int ND, typename TIN>
+__global__ void __launch_bounds__(1024) k_tp_grad(Ops1D<N> op, const TIN *__restrict__ u, const double *__restrict__ jump,
+                                                  const double *__restrict__ smat, const double *__restrict__ rcpj,
+                                                  double *__restrict__ q, int64_t ncols, int64_t ld, int64_t Nel) {
+  constexpr int NU = ipow(N, ND), NFP = ipow(N, ND - 1);
+  const int64_t col = (int64_t)blockIdx.x * 32 + threadIdx.x;
+  if (col >= ncols) return;
+  const int64_t e = col % ld;
+  if (e >= Nel) return;
+  u += col; jump += col; q += col;
+  for (int r = threadIdx.y; r < NU; r += blockDim.y) {
+    int ii[3];
+    ii[0] = r % N; ii[1] = (r / N) % N; ii[2] = ND == 3 ? r / (N * N) : 0;
+    double qt[ND];
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+      const int stride = d == 0 ? 1 : (d == 1 ? N : N * N);
+      const int base = r - ii[d] * stride;
+      // face-point index of this line: the remaining tensor indices, lowest fastest
+      int idx;
+      if (ND == 2) idx = d == 0 ? ii[1] : ii[0];
+      else idx = d == 0 ? ii[1] + N * ii[2] : (d == 1 ? ii[0] + N * ii[2] : ii[0] + N * ii[1]);
+      double s = 0;
+#pragma unroll
+      for (int m = 0; m < N; ++m) s = fma(op.D[ii[d] * N + m], (double)u[(size_t)(base + m * stride) * ncols], s);
+      // M6 = n~ (x) M3 (A1): the reference normal is -1 on the -1 face
+      s = fma(-op.gm[ii[d]], jump[(size_t)((2 * d) * NFP + idx) * ncols], s);
+      s = fma(op.gp[ii[d]], jump[(size_t)((2 * d + 1) * NFP + idx) * ncols], s);
+      qt[d] = s;
+    }
+    const double rj = rcpj[(size_t)r * ld + e];
+#pragma unroll
+    for (int n = 0; n < ND; ++n) {
+      double s = 0;
+#pragma unroll
+      for (int i = 0; i < ND; ++i) s = fma(smat[((size_t)(i * ND + n) * NU + r) * ld + e], qt[i], s);
+      q[(size_t)(n * NU + r) * ncols] = s * rj;
+    }
+  }
+}
+
+// R = -(1/J) {(M1 - M3 M2) F~ + M3 D~}  (Eq 18-19 / Eq 44): thread per solution point and column.
+template <int N, int ND, typename TOUT>
+__global__ void __launch_bounds__(1024) k_tp_div(Ops1D<N> op, const double *__restrict__ ft, const double *__restrict__ dt,
+                                                 const double *__restrict__ rcpj, TOUT *__restrict__ rhs, int64_t ncols, int64_t ld,
+                                                 int64_t Nel) {
+  constexpr int NU = ipow(N, ND), NFP = ipow(N, ND - 1);
+  const int64_t col = (int64_t)blockIdx.x * 32 + threadIdx.x;
+  if (col >= ncols) return;
+  const int64_t e = col % ld;
+  if (e >= Nel) return;
+  ft += col; dt += col; rhs += col;
+  for (int r = threadIdx.y; r < NU; r += blockDim.y) {
+    int ii[3];
+    ii[0] = r % N; ii[1] = (r / N) % N; ii[2] = ND == 3 ? r / (N * N) : 0;
+    double acc = 0;
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+      const int stride = d == 0 ? 1 : (d == 1 ? N : N * N);
+      const int base = r - ii[d] * stride;
+      int idx;
+      if (ND == 2) idx = d == 0 ? ii[1] : ii[0];
+      else idx = d == 0 ? ii[1] + N * ii[2] : (d == 1 ? ii[0] + N * ii[2] : ii[0] + N * ii[1]);
+      const double *f = ft + (size_t)d * NU * ncols;
+#pragma unroll
+      for (int m = 0; m < N; ++m) acc = fma(op.Dh[ii[d] * N + m], f[(size_t)(base + m * stride) * ncols], acc);
+      acc = fma(op.gm[ii[d]], dt[(size_t)((2 * d) * NFP + idx) * ncols], acc);
+      acc = fma(op.gp[ii[d]], dt[(size_t)((2 * d + 1) * NFP + idx) * ncols], acc);
+    }
+    rhs[(size_t)r * ncols] = (TOUT)(-acc * rcpj[(size_t)r * ld + e]);
+  }
+}
+
+template <int N>
+Ops1D<N> make_ops(const double *h) {  // h: D, Dh, lm, lp, gm, gp packed
+  Ops1D<N> o;
+  const double *p = h;
+  for (int i = 0; i < N * N; ++i) o.D[i] = *p++;
+  for (int i = 0; i < N * N; ++i) o.Dh[i] = *p++;
+  for (int i = 0; i < N; ++i) o.lm[i] = *p++;
+  for (int i = 0; i < N; ++i) o.lp[i] = *p++;
+  for (int i = 0; i < N; ++i) o.gm[i] = *p++;
+  for (int i = 0; i < N; ++i) o.gp[i] = *p++;
+  return o;
+}
+
+template <int N, int ND, typename T>
+cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, char *work, cudaStream_t s, Prof *prof) {
+  constexpr int NU = ipow(N, ND), NFP = ipow(N, ND - 1), NF = 2 * ND * NFP;
+  const Ops1D<N> op = make_ops<N>(tp.h_ops);
+  const int64_t ncols = (int64_t)c.NV * c.ld;
+  double *uf = (double *)(work + tp.off_uf), *cf = (double *)(work + tp.off_cf), *qu = (double *)(work + tp.off_qu),
+         *qf = (double *)(work + tp.off_qf);
+  const unsigned gx = (unsigned)((ncols + 31) / 32);
+  const dim3 bf(32, NFP < 32 ? NFP : 32), bu(32, NU < 32 ? NU : 32);
+  FR_MARK(prof, "tp_interp");
+  k_tp_interp<N, ND, T><<<dim3(gx, 1, 1), bf, 0, s>>>(op, u, uf, ncols, c.ld, c.Nel, 0, 0);
+  if (c.ns) {
+    FR_MARK(prof, "common_sol");
+    launch_common_jump(c, uf, cf, s);
+    FR_MARK(prof, "tp_grad");
+    k_tp_grad<N, ND, T><<<dim3(gx, 1, 1), bu, 0, s>>>(op, u, cf, c.smat, c.rcpj, qu, ncols, c.ld, c.Nel);
+    FR_MARK(prof, "tp_interp_q");
+    k_tp_interp<N, ND, double><<<dim3(gx, 1, ND), bf, 0, s>>>(op, qu, qf, ncols, c.ld, c.Nel, (int64_t)NU * ncols, (int64_t)NF * ncols);
+  }
+  FR_MARK(prof, "tflux");
+  launch_tflux(c, u, qu, s);
+  FR_MARK(prof, "common_flux");
+  launch_common_flux(c, uf, qf, s);
+  FR_MARK(prof, "tp_div");
+  k_tp_div<N, ND, T><<<dim3(gx, 1, 1), bu, 0, s>>>(op, qu, uf, c.rcpj, rhs, ncols, c.ld, c.Nel);
+  return cudaGetLastError();
+}
+
+template <int ND>
+cudaError_t dispatch_n(const DevConsts &c, const TensorPlan &tp, const void *u, void *rhs, char *work, cudaStream_t s, Prof *prof) {
+#define FR_CASE(NN)                                                                                              \
+  case NN:                                                                                                       \
+    return c.f64 ? run<NN, ND, double>(c, tp, (const double *)u, (double *)rhs, work, s, prof)                    \
+                 : run<NN, ND, float>(c, tp, (const float *)u, (float *)rhs, work, s, prof);
+  switch (c.n) {
+    FR_CASE(1) FR_CASE(2) FR_CASE(3) FR_CASE(4) FR_CASE(5) FR_CASE(6) FR_CASE(7) FR_CASE(8)
+    default: return cudaErrorNotSupported;
+  }
+#undef FR_CASE
+}
+
+}  // namespace
+
+bool tensor_supported(const DevConsts &c) { return (c.etype == FR_QUAD || c.etype == FR_HEX) && c.n >= 1 && c.n <= 8; }
+
+cudaError_t tensor_plan(const DevConsts &c, const RefOps &o, const MeshConsts &, TensorPlan &tp, std::vector<void *> &) {
+  tp = TensorPlan();
+  const int n = o.n;
+  double *p = tp.h_ops;
+  for (int i = 0; i < n * n; ++i) *p++ = o.D1[i];
+  for (int i = 0; i < n * n; ++i) *p++ = o.Dhat[i];
+  for (int i = 0; i < n; ++i) *p++ = o.lm[i];
+  for (int i = 0; i < n; ++i) *p++ = o.lp[i];
+  for (int i = 0; i < n; ++i) *p++ = o.gm[i];
+  for (int i = 0; i < n; ++i) *p++ = o.gp[i];
+  auto al = [](int64_t x) { return (x + 255) / 256 * 256; };
+  const int64_t ncols = (int64_t)c.NV * c.ld;
+  int64_t off = 0;
+  tp.off_uf = off; off = al(off + (int64_t)o.Nf * ncols * 8);
+  tp.off_cf = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
+  tp.off_qu = off; off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
+  tp.off_qf = off; if (c.ns) off = al(off + (int64_t)o.nd * o.Nf * ncols * 8);
+  tp.work_bytes = off;
+  return cudaSuccess;
+}
+
+cudaError_t tensor_rhs(const DevConsts &c, const TensorPlan &tp, const void *u, void *rhs, char *work, cudaStream_t s, Prof *prof) {
+  return c.nd == 2 ? dispatch_n<2>(c, tp, u, rhs, work, s, prof) : dispatch_n<3>(c, tp, u, rhs, work, s, prof);
+}
+
+int tensor_rhs_launches(const DevConsts &c) {
+  int n = 4 + (c.ns ? 3 : 0);  // interp, tflux, common flux, div (+ common sol, grad, interp q)
+  if (c.nbnd) n += c.ns ? 2 : 1;
+  if (!c.npairs) n -= c.ns ? 2 : 1;
+  return n;
+}
+
 }  // namespace fr

@@ -9,10 +9,9 @@ namespace fr {
 
 struct TensorPlan {
   int64_t work_bytes = 0;
-  // workspace offsets (bytes) of the flux-point intermediates
-  int64_t off_uf = 0, off_gf = 0;
-  const double *ops1d = nullptr;  // device: D1, lm, lp, gm, gp, Dhat
-  int variant = 0;
+  // workspace offsets (bytes): U^f (-> D~), jump C - U^f, Q~ -> Q -> F~, Q^f
+  int64_t off_uf = 0, off_cf = 0, off_qu = 0, off_qf = 0;
+  double h_ops[2 * 64 + 4 * 8];   // host copy of the 1-D operators: D, Dhat, lm, lp, gm, gp (n <= 8)
 };
 
 bool tensor_supported(const DevConsts &c);
