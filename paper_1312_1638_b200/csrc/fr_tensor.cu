@@ -12,6 +12,8 @@
 // The 1-D operators travel as a kernel parameter (constant bank, uniform broadcast reads).
 #include "fr_tensor.hpp"
 
+#include <cstdlib>
+
 namespace fr {
 namespace {
 
@@ -44,7 +46,7 @@ template <int N, int ND, typename TIN>
 __global__ void __launch_bounds__(1024) k_tp_interp(Ops1D<N> op, const TIN *__restrict__ in, double *__restrict__ out, int64_t ncols,
                                                     int64_t ld, int64_t Nel, int64_t in_blk, int64_t out_blk) {
   constexpr int NFP = ipow(N, ND - 1);
-  const int64_t col = (int64_t)blockIdx.x * 32 + threadIdx.x;
+  const int64_t col = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (col >= ncols || (col % ld) >= Nel) return;
   in += (size_t)blockIdx.z * in_blk + col;
   out += (size_t)blockIdx.z * out_blk + col;
@@ -66,45 +68,51 @@ __global__ void __launch_bounds__(1024) k_tp_interp(Ops1D<N> op, const TIN *__re
   }
 }
 
-// Q = J^-T {M4 U + M6 (C - U^f)}  (Eq 9-10 / Eq 42): thread per solution point and column.
-// jump = C - U^f at the flux points (written by the common-solution kernel).
+// Q = J^-T {M4 U + M6 (C - U^f)}  (Eq 9-10 / Eq 42): thread per solution point and element, looping over
+// the variables so that S and 1/J are loaded once.  jump = C - U^f at the flux points.
 template <int N, int ND, typename TIN>
-__global__ void __launch_bounds__(1024) k_tp_grad(Ops1D<N> op, const TIN *__restrict__ u, const double *__restrict__ jump,
+__global__ void __launch_bounds__(256) k_tp_grad(Ops1D<N> op, const TIN *__restrict__ u, const double *__restrict__ jump,
                                                   const double *__restrict__ smat, const double *__restrict__ rcpj,
                                                   double *__restrict__ q, int64_t ncols, int64_t ld, int64_t Nel) {
-  constexpr int NU = ipow(N, ND), NFP = ipow(N, ND - 1);
-  const int64_t col = (int64_t)blockIdx.x * 32 + threadIdx.x;
-  if (col >= ncols) return;
-  const int64_t e = col % ld;
+  constexpr int NU = ipow(N, ND), NFP = ipow(N, ND - 1), NV = ND + 2;
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= Nel) return;
-  u += col; jump += col; q += col;
+  u += e; jump += e; q += e;
   for (int r = threadIdx.y; r < NU; r += blockDim.y) {
     int ii[3];
     ii[0] = r % N; ii[1] = (r / N) % N; ii[2] = ND == 3 ? r / (N * N) : 0;
-    double qt[ND];
+    double S[ND][ND];
 #pragma unroll
-    for (int d = 0; d < ND; ++d) {
-      const int stride = d == 0 ? 1 : (d == 1 ? N : N * N);
-      const int base = r - ii[d] * stride;
-      // face-point index of this line: the remaining tensor indices, lowest fastest
-      int idx;
-      if (ND == 2) idx = d == 0 ? ii[1] : ii[0];
-      else idx = d == 0 ? ii[1] + N * ii[2] : (d == 1 ? ii[0] + N * ii[2] : ii[0] + N * ii[1]);
-      double s = 0;
+    for (int i = 0; i < ND; ++i)
 #pragma unroll
-      for (int m = 0; m < N; ++m) s = fma(op.D[ii[d] * N + m], (double)u[(size_t)(base + m * stride) * ncols], s);
-      // M6 = n~ (x) M3 (A1): the reference normal is -1 on the -1 face
-      s = fma(-op.gm[ii[d]], jump[(size_t)((2 * d) * NFP + idx) * ncols], s);
-      s = fma(op.gp[ii[d]], jump[(size_t)((2 * d + 1) * NFP + idx) * ncols], s);
-      qt[d] = s;
-    }
+      for (int n = 0; n < ND; ++n) S[i][n] = smat[((size_t)(i * ND + n) * NU + r) * ld + e];
     const double rj = rcpj[(size_t)r * ld + e];
+#pragma unroll 1
+    for (int a = 0; a < NV; ++a) {
+      double qt[ND];
 #pragma unroll
-    for (int n = 0; n < ND; ++n) {
-      double s = 0;
+      for (int d = 0; d < ND; ++d) {
+        const int stride = d == 0 ? 1 : (d == 1 ? N : N * N);
+        const int base = r - ii[d] * stride;
+        // face-point index of this line: the remaining tensor indices, lowest fastest
+        int idx;
+        if (ND == 2) idx = d == 0 ? ii[1] : ii[0];
+        else idx = d == 0 ? ii[1] + N * ii[2] : (d == 1 ? ii[0] + N * ii[2] : ii[0] + N * ii[1]);
+        double s = 0;
 #pragma unroll
-      for (int i = 0; i < ND; ++i) s = fma(smat[((size_t)(i * ND + n) * NU + r) * ld + e], qt[i], s);
-      q[(size_t)(n * NU + r) * ncols] = s * rj;
+        for (int m = 0; m < N; ++m) s = fma(op.D[ii[d] * N + m], (double)u[(size_t)(base + m * stride) * ncols + a * ld], s);
+        // M6 = n~ (x) M3 (A1): the reference normal is -1 on the -1 face
+        s = fma(-op.gm[ii[d]], jump[(size_t)((2 * d) * NFP + idx) * ncols + a * ld], s);
+        s = fma(op.gp[ii[d]], jump[(size_t)((2 * d + 1) * NFP + idx) * ncols + a * ld], s);
+        qt[d] = s;
+      }
+#pragma unroll
+      for (int n = 0; n < ND; ++n) {
+        double s = 0;
+#pragma unroll
+        for (int i = 0; i < ND; ++i) s = fma(S[i][n], qt[i], s);
+        q[(size_t)(n * NU + r) * ncols + a * ld] = s * rj;
+      }
     }
   }
 }
@@ -115,7 +123,7 @@ __global__ void __launch_bounds__(1024) k_tp_div(Ops1D<N> op, const double *__re
                                                  const double *__restrict__ rcpj, TOUT *__restrict__ rhs, int64_t ncols, int64_t ld,
                                                  int64_t Nel) {
   constexpr int NU = ipow(N, ND), NFP = ipow(N, ND - 1);
-  const int64_t col = (int64_t)blockIdx.x * 32 + threadIdx.x;
+  const int64_t col = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (col >= ncols) return;
   const int64_t e = col % ld;
   if (e >= Nel) return;
@@ -161,15 +169,17 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
   const int64_t ncols = (int64_t)c.NV * c.ld;
   double *uf = (double *)(work + tp.off_uf), *cf = (double *)(work + tp.off_cf), *qu = (double *)(work + tp.off_qu),
          *qf = (double *)(work + tp.off_qf);
-  const unsigned gx = (unsigned)((ncols + 31) / 32);
-  const dim3 bf(32, NFP < 32 ? NFP : 32), bu(32, NU < 32 ? NU : 32);
+  static const int LW = getenv("FR_LW") ? atoi(getenv("FR_LW")) : 32;   // lanes (columns) per CTA row
+  const int rows = 1024 / LW;
+  const unsigned gx = (unsigned)((ncols + LW - 1) / LW), ge = (unsigned)((c.Nel + LW - 1) / LW);
+  const dim3 bf(LW, NFP < rows ? NFP : rows), bu(LW, NU < rows ? NU : rows);
   FR_MARK(prof, "tp_interp");
   k_tp_interp<N, ND, T><<<dim3(gx, 1, 1), bf, 0, s>>>(op, u, uf, ncols, c.ld, c.Nel, 0, 0);
   if (c.ns) {
     FR_MARK(prof, "common_sol");
     launch_common_jump(c, uf, cf, s);
     FR_MARK(prof, "tp_grad");
-    k_tp_grad<N, ND, T><<<dim3(gx, 1, 1), bu, 0, s>>>(op, u, cf, c.smat, c.rcpj, qu, ncols, c.ld, c.Nel);
+    k_tp_grad<N, ND, T><<<dim3(ge, 1, 1), dim3(LW, 256 / LW), 0, s>>>(op, u, cf, c.smat, c.rcpj, qu, ncols, c.ld, c.Nel);
     FR_MARK(prof, "tp_interp_q");
     k_tp_interp<N, ND, double><<<dim3(gx, 1, ND), bf, 0, s>>>(op, qu, qf, ncols, c.ld, c.Nel, (int64_t)NU * ncols, (int64_t)NF * ncols);
   }
