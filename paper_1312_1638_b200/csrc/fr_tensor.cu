@@ -149,6 +149,28 @@ __global__ void __launch_bounds__(1024) k_tp_div(Ops1D<N> op, const double *__re
   }
 }
 
+#include "fr_hex.cuh"
+
+template <int N, bool NS, typename T>
+void launch_hex_fluxdiv(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *qu, const double *dt, T *rhs, cudaStream_t s) {
+  constexpr int E = N <= 3 ? 32 : (N <= 5 ? 16 : 8);
+  const size_t smem = (size_t)(N * N + 2 * 2 * 5 * N * N * E) * sizeof(double);
+  auto kern = k_hex_fluxdiv<N, E, NS, T>;
+  static bool attr_done = false;
+  if (!attr_done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
+  kern<<<(unsigned)((c.Nel + E - 1) / E), dim3(E, N * N), smem, s>>>(op, c.ph, u, qu, c.smat, c.rcpj, dt, rhs, c.ld, c.Nel);
+}
+
+template <int N, typename T>
+void launch_hex_grad(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *jump, double *qu, cudaStream_t s) {
+  constexpr int E = N <= 3 ? 32 : (N <= 5 ? 16 : 8);
+  const size_t smem = (size_t)(N * N + 2 * 5 * N * N * E) * sizeof(double);
+  auto kern = k_hex_grad<N, E, T>;
+  static bool attr_done = false;
+  if (!attr_done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
+  kern<<<(unsigned)((c.Nel + E - 1) / E), dim3(E, N * N), smem, s>>>(op, u, jump, c.smat, c.rcpj, qu, c.ld, c.Nel);
+}
+
 template <int N>
 Ops1D<N> make_ops(const double *h) {  // h: D, Dh, lm, lp, gm, gp packed
   Ops1D<N> o;
@@ -178,10 +200,25 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
   if (c.ns) {
     FR_MARK(prof, "common_sol");
     launch_common_jump(c, uf, cf, s);
-    FR_MARK(prof, "tp_grad");
-    k_tp_grad<N, ND, T><<<dim3(ge, 1, 1), dim3(LW, 256 / LW), 0, s>>>(op, u, cf, c.smat, c.rcpj, qu, ncols, c.ld, c.Nel);
+    static const bool fuse_g = !getenv("FR_NOFUSE");
+    if (ND == 3 && fuse_g) {
+      FR_MARK(prof, "hex_grad");
+      launch_hex_grad<N, T>(op, c, u, cf, qu, s);
+    } else {
+      FR_MARK(prof, "tp_grad");
+      k_tp_grad<N, ND, T><<<dim3(ge, 1, 1), dim3(LW, 256 / LW), 0, s>>>(op, u, cf, c.smat, c.rcpj, qu, ncols, c.ld, c.Nel);
+    }
     FR_MARK(prof, "tp_interp_q");
     k_tp_interp<N, ND, double><<<dim3(gx, 1, ND), bf, 0, s>>>(op, qu, qf, ncols, c.ld, c.Nel, (int64_t)NU * ncols, (int64_t)NF * ncols);
+  }
+  static const bool fuse = !getenv("FR_NOFUSE");
+  if (ND == 3 && fuse) {
+    FR_MARK(prof, "common_flux");
+    launch_common_flux(c, uf, qf, s);
+    FR_MARK(prof, "hex_fluxdiv");
+    if (c.ns) launch_hex_fluxdiv<N, true, T>(op, c, u, qu, uf, rhs, s);
+    else launch_hex_fluxdiv<N, false, T>(op, c, u, qu, uf, rhs, s);
+    return cudaGetLastError();
   }
   FR_MARK(prof, "tflux");
   launch_tflux(c, u, qu, s);
