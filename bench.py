@@ -96,10 +96,31 @@ def kernel_words(name, nd, NV, Nu, Nf, ns):
         "apply_M132_M3_negdivconf": (nd * Nu + Nf + Nu) * NV + Nu,
         # tensor-product path (fr_tensor.cu)
         "tp_interp": (Nu + Nf) * NV,
+        "tp_interp_q": nd * (Nu + Nf) * NV,
+        "hex_grad": (Nu + Nf) * NV + met + nd * Nu * NV,
+        "hex_fluxdiv": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
+        "hex_rhs": (2 * Nu + 2 * Nf) * NV + met,
         "tp_grad": (Nu + Nf) * NV + met + (nd + 1) * Nf + (NV - 1) * Nf + Nf,
         "tp_div": (2 * Nu + Nf) * NV + met + (nd + 1) * Nf + ((NV - 1) * Nf if ns else 0) + Nf,
     }
     return t.get(name)
+
+
+def max_over_ranks(ms, world, device="cuda"):
+    """Timed-region duration = max over ranks (the only cross-rank exchange of the replicas-only N>1 path)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(dof, ms_step, world):
+    """Whole-job GDOF/s: every rank processed `dof` per step (weak scaling, replicas)."""
+    return world * dof / (ms_step * 1e-3) / 1e9
 
 
 class ClockSampler(threading.Thread):
@@ -244,11 +265,8 @@ def main():
         torch.cuda.synchronize()
     sampler.stop_flag = True
     sampler.join()
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
-    value = world * dof / (ms_step * 1e-3) / 1e9
+    ms_step = max_over_ranks(ms_total, world) / args.steps
+    value = aggregate_value(dof, ms_step, world)
 
     # ---- end to end through the C ABI with host buffers (H2D + RHS + D2H per step) ----
     n_e2e = max(3, min(args.steps, 10))
@@ -260,11 +278,8 @@ def main():
         ctx.rhs_host(u_host.data_ptr(), r_host.data_ptr(), up, rp, wp, stream)
     ev1.record()
     barrier()
-    t = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_ms = float(t.item()) / n_e2e
-    e2e_val = world * dof / (e2e_ms * 1e-3) / 1e9
+    e2e_ms = max_over_ranks(ev0.elapsed_time(ev1), world) / n_e2e
+    e2e_val = aggregate_value(dof, e2e_ms, world)
 
     # ---- per-kernel durations (events between kernels, same stream), dominant kernel roofline ----
     acc = {}

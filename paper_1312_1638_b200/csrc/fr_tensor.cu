@@ -151,24 +151,49 @@ __global__ void __launch_bounds__(1024) k_tp_div(Ops1D<N> op, const double *__re
 
 #include "fr_hex.cuh"
 
-template <int N, bool NS, typename T>
-void launch_hex_fluxdiv(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *qu, const double *dt, T *rhs, cudaStream_t s) {
-  constexpr int E = N <= 3 ? 32 : (N <= 5 ? 16 : 8);
+template <int N, int E, bool NS, typename T>
+void launch_hex_fluxdiv_e(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *qu, const double *dt, T *rhs, cudaStream_t s) {
   const size_t smem = (size_t)(N * N + 2 * 2 * 5 * N * N * E) * sizeof(double);
   auto kern = k_hex_fluxdiv<N, E, NS, T>;
   static bool attr_done = false;
   if (!attr_done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
   kern<<<(unsigned)((c.Nel + E - 1) / E), dim3(E, N * N), smem, s>>>(op, c.ph, u, qu, c.smat, c.rcpj, dt, rhs, c.ld, c.Nel);
 }
+template <int N, bool NS, typename T>
+void launch_hex_fluxdiv(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *qu, const double *dt, T *rhs, cudaStream_t s) {
+  constexpr int E = N <= 3 ? 32 : (N <= 5 ? 16 : 8);
+  static const int e_env = getenv("FR_E") ? atoi(getenv("FR_E")) : 0;
+  if (e_env == 8 && E > 8) return launch_hex_fluxdiv_e<N, 8, NS, T>(op, c, u, qu, dt, rhs, s);
+  launch_hex_fluxdiv_e<N, E, NS, T>(op, c, u, qu, dt, rhs, s);
+}
 
 template <int N, typename T>
-void launch_hex_grad(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *jump, double *qu, cudaStream_t s) {
+void launch_hex_rhs(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *jump, const double *dt, T *rhs, cudaStream_t s) {
   constexpr int E = N <= 3 ? 32 : (N <= 5 ? 16 : 8);
+  constexpr size_t base = (size_t)(2 * N * N + 5 * N * N * N * E) * sizeof(double);
+  constexpr size_t slice = (size_t)(2 * 5 * N * N * E) * sizeof(double);
+  constexpr int NB = (base + 2 * slice <= 200 * 1024) ? 2 : 1;
+  const size_t smem = base + NB * slice;
+  auto kern = k_hex_rhs<N, E, NB, T>;
+  static bool attr_done = false;
+  if (!attr_done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
+  kern<<<(unsigned)((c.Nel + E - 1) / E), dim3(E, N * N), smem, s>>>(op, c.ph, u, jump, c.smat, c.rcpj, dt, rhs, c.ld, c.Nel);
+}
+
+template <int N, int E, typename T>
+void launch_hex_grad_e(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *jump, double *qu, cudaStream_t s) {
   const size_t smem = (size_t)(N * N + 2 * 5 * N * N * E) * sizeof(double);
   auto kern = k_hex_grad<N, E, T>;
   static bool attr_done = false;
   if (!attr_done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
   kern<<<(unsigned)((c.Nel + E - 1) / E), dim3(E, N * N), smem, s>>>(op, u, jump, c.smat, c.rcpj, qu, c.ld, c.Nel);
+}
+template <int N, typename T>
+void launch_hex_grad(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *jump, double *qu, cudaStream_t s) {
+  constexpr int E = N <= 3 ? 32 : (N <= 5 ? 16 : 8);
+  static const int e_env = getenv("FR_E") ? atoi(getenv("FR_E")) : 0;
+  if (e_env == 8 && E > 8) return launch_hex_grad_e<N, 8, T>(op, c, u, jump, qu, s);
+  launch_hex_grad_e<N, E, T>(op, c, u, jump, qu, s);
 }
 
 template <int N>
@@ -215,6 +240,12 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
   if (ND == 3 && fuse) {
     FR_MARK(prof, "common_flux");
     launch_common_flux(c, uf, qf, s);
+    static const bool recompute = getenv("FR_RECOMPUTE") != nullptr;  // experimental: recompute Q instead of reading it
+    if (c.ns && recompute) {
+      FR_MARK(prof, "hex_rhs");
+      launch_hex_rhs<N, T>(op, c, u, cf, uf, rhs, s);
+      return cudaGetLastError();
+    }
     FR_MARK(prof, "hex_fluxdiv");
     if (c.ns) launch_hex_fluxdiv<N, true, T>(op, c, u, qu, uf, rhs, s);
     else launch_hex_fluxdiv<N, false, T>(op, c, u, qu, uf, rhs, s);

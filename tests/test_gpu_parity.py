@@ -156,3 +156,95 @@ def test_error_paths_on_device():
         ctx.rhs(run.u.data_ptr(), run.u.data_ptr(), run.work.data_ptr(), run.stream)  # aliasing
     with pytest.raises(FrError):
         ctx.rhs(0, run.r.data_ptr(), run.work.data_ptr(), run.stream)  # NULL
+
+
+# ------------------------------------------------------------------------------------------
+# BASELINE.json full sizes, in the launch configuration bench.py times
+# ------------------------------------------------------------------------------------------
+DUMMY_BC = {0: ("sup-inflow", dict(rho=1.0, v=(0.1, 0.2, 0.3), p=50.0))}
+
+
+def _sampled_parity(name, precision, n_seeds=10, seed=99):
+    """Full-size run on the GPU; the oracle recomputes the RHS of sampled elements on the patch of
+    their neighbours' neighbours (workloads.patch_around), where it equals the full-mesh RHS."""
+    mesh, disc = W.config(name)
+    ctx = _ctx(mesh, disc, precision=precision)
+    X = ctx.solution_point_coords()
+    U = W.config_state(name, X).astype(ctx.dtype)
+    got = GpuRunner(ctx).rhs(U)
+    assert np.all(np.isfinite(got))
+    n_el = mesh["nodes"].shape[0]
+    rng = np.random.default_rng(seed)
+    seeds = np.unique(np.concatenate([[0, n_el - 1, n_el // 2], rng.integers(0, n_el, n_seeds)]))
+    sub, ids, pos = W.patch_around(mesh, seeds)
+    bcs = {0: (DUMMY_BC[0][0], dict(DUMMY_BC[0][1], v=DUMMY_BC[0][1]["v"][: mesh["ndims"]]))}
+    o = FROracle(sub, disc, bcs)
+    assert np.allclose(X[:, ids], np.asarray(o.xu_phys, float), atol=1e-12)
+    ref = o.rhs(U[:, :, ids].astype(np.float64))[:, :, pos]
+    return got[:, :, seeds], ref, o, U[:, :, ids], pos
+
+
+def test_full_size_C3_fp64_sampled():
+    got, ref, o, Usub, pos = _sampled_parity("C3", "f64")
+    old = FROracle(o.mesh, o.prm, o.bcs, dtype=np.longdouble)
+    floor = rel_l2_per_field(ref, old.rhs(np.asarray(Usub, dtype=np.longdouble))[:, :, pos])
+    print("floor", floor)
+    _check("C3-full-fp64", got, ref, np.maximum(TOL64, 3 * floor))
+
+
+def test_full_size_C3_fp32_sampled():
+    got, ref, *_ = _sampled_parity("C3", "f32")
+    _check("C3-full-fp32", got, ref, TOL32)
+
+
+def test_full_size_C2_rhs_and_20_steps():
+    """C2 as BASELINE.json states it: one RHS (full comparison) plus 20 RK4 steps.  The 20-step state is
+    checked through invariants that hold at any size (conservation of the quadrature-weighted integrals of
+    every conserved variable on the periodic mesh) and against the oracle on the 8^3 version of the case."""
+    mesh, disc = W.config("C2")
+    o = FROracle(mesh, disc)
+    ctx = _ctx(mesh, disc)
+    U = W.config_state("C2", np.asarray(o.xu_phys, float))
+    R = o.rhs(U)
+    bar, floor = _bar(o, U, R)
+    print("floor", floor)
+    run = GpuRunner(ctx)
+    _check("C2-full", run.rhs(U), R, bar)
+    U20 = run.rk4(U, disc["dt"], disc["steps"])
+    assert np.all(np.isfinite(U20)) and np.max(np.abs(U20 - U)) > 1e-4
+    i0, i1 = o.integrate(U), o.integrate(U20)
+    scale = o.integrate(np.abs(U)) + 1.0
+    assert np.all(np.abs(i1 - i0) <= 1e-12 * scale), (i0, i1)
+    # oracle comparison of the 20-step state at 8^3
+    mesh8, _ = W.config("C2", n=8)
+    o8 = FROracle(mesh8, disc)
+    U8 = W.config_state("C2", np.asarray(o8.xu_phys, float))
+    ref = U8
+    for _ in range(disc["steps"]):
+        ref = o8.rk4_step(ref, disc["dt"])
+    got = GpuRunner(_ctx(mesh8, disc)).rk4(U8, disc["dt"], disc["steps"])
+    _check("C2-8-rk4x20", got, ref, TOL64)
+
+
+def test_full_size_C4_triangles():
+    mesh, disc = W.config("C4")
+    o = FROracle(mesh, disc)
+    ctx = _ctx(mesh, disc)
+    U = W.config_state("C4", np.asarray(o.xu_phys, float))
+    R = o.rhs(U)
+    bar, floor = _bar(o, U, R)
+    print("floor", floor)
+    _check("C4-full", GpuRunner(ctx).rhs(U), R, bar)
+
+
+def test_empty_and_ragged_sizes():
+    """Element counts that are not multiples of the CTA tile / lane padding (1, 3, 17 elements per
+    direction ...) and a single element periodic onto itself."""
+    for shape, p in (((1, 1, 1), 2), ((3, 1, 2), 4), ((17, 1, 1), 3), ((5, 7), 2), ((1, 1), 3)):
+        nd = len(shape)
+        mesh = W.box_mesh(shape, (2 * np.pi,) * nd)
+        disc = dict(p=p, system="navier-stokes", gamma=1.4, mu=0.01, Pr=0.71, beta=0.5, tau=0.1)
+        o = FROracle(mesh, disc)
+        X = np.asarray(o.xu_phys, float)
+        U = W.config_state("C5", X, p=p) if nd == 3 else np.ascontiguousarray(np.moveaxis(W.fourier_state(X, 7), -1, 1))
+        _check("ragged-%s" % (shape,), GpuRunner(_ctx(mesh, disc)).rhs(U), o.rhs(U), TOL64)

@@ -333,3 +333,48 @@ def config_state(name, X, **over):
     else:
         raise KeyError(name)
     return np.ascontiguousarray(np.moveaxis(U, -1, 1))
+
+
+# ----------------------------------------------------------------------------
+# sampling helper for full-size parity: a patch of the mesh around seed elements
+# ----------------------------------------------------------------------------
+def patch_around(mesh, seeds, hops=2):
+    """Sub-mesh made of `seeds` and every element within `hops` face-neighbour steps.
+
+    The RHS of a Navier-Stokes FR element depends on its neighbours' neighbours (compact LDG stencil),
+    so on the returned patch the RHS of the SEED elements equals the RHS on the full mesh, whatever the
+    boundary condition put on the cut faces (bc_id 0).  Returns (sub_mesh, element ids [n_sub] into the
+    full mesh, positions of the seeds inside the patch).  No arithmetic of the method here: topology only.
+    """
+    ifc = mesh["ifaces"]
+    n_el = mesh["nodes"].shape[0]
+    inside = np.zeros(n_el, dtype=bool)
+    inside[np.asarray(seeds)] = True
+    for _ in range(hops):
+        touch = inside[ifc[:, 0]] | inside[ifc[:, 2]]
+        inside[ifc[touch, 0]] = True
+        inside[ifc[touch, 2]] = True
+    ids = np.flatnonzero(inside)
+    remap = -np.ones(n_el, dtype=np.int64)
+    remap[ids] = np.arange(ids.size)
+    inL, inR = inside[ifc[:, 0]], inside[ifc[:, 2]]
+    both = inL & inR
+    sub_if = ifc[both].copy()
+    sub_if[:, 0] = remap[sub_if[:, 0]]
+    sub_if[:, 2] = remap[sub_if[:, 2]]
+    cutL = ifc[inL & ~inR]
+    cutR = ifc[inR & ~inL]
+    bf = [np.stack([remap[cutL[:, 0]], cutL[:, 1], np.zeros(len(cutL), dtype=np.int64)], -1),
+          np.stack([remap[cutR[:, 2]], cutR[:, 3], np.zeros(len(cutR), dtype=np.int64)], -1)]
+    old_b = mesh["bfaces"]
+    if len(old_b):
+        keep = inside[old_b[:, 0]]
+        ob = old_b[keep].copy().astype(np.int64)
+        ob[:, 0] = remap[ob[:, 0]]
+        bf.append(ob)
+    sub = dict(mesh)
+    sub["nodes"] = np.ascontiguousarray(mesh["nodes"][ids])
+    sub["ifaces"] = sub_if.astype(np.int32)
+    sub["shifts"] = np.ascontiguousarray(mesh["shifts"][both])
+    sub["bfaces"] = np.concatenate(bf).astype(np.int32)
+    return sub, ids, remap[np.asarray(seeds)]
