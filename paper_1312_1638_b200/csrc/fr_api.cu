@@ -8,6 +8,7 @@
 
 #include "fr_dev.hpp"
 #include "fr_host.hpp"
+#include "fr_hex_tma.hpp"
 #include "fr_tensor.hpp"
 
 using namespace fr;
@@ -129,6 +130,9 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     UP(mc.pLs, pLs); UP(mc.pLe, pLe); UP(mc.pRs, pRs); UP(mc.pRe, pRe);
     UP(mc.pn, pn); UP(mc.pJnL, pJnL); UP(mc.pJnR, pJnR);
     UP(mc.bs, bs); UP(mc.be, be); UP(mc.bbc, bbc); UP(mc.bn, bn); UP(mc.bJn, bJn);
+    // element-centric flux-point tables of the fused hexahedral gradient kernel (own normals, boundary ids)
+    const bool want_tma = !(d->flags & FR_FLAG_FORCE_GENERIC) && o.etype == FR_HEX && dc.ns && hex_tma_supported(o.n, dc.f64);
+    if (want_tma) { UP(mc.fp_n, fp_n); if (mc.nbnd) { UP(mc.fp_pe, fp_pe); } }
 #undef UP
     std::vector<BcDev> bcs(c->mesh.bcs.size());
     for (size_t i = 0; i < bcs.size(); ++i) {

@@ -3,6 +3,7 @@
 // fallback for hexahedra (FR_FLAG_FORCE_GENERIC); the tensor-product kernels in fr_tensor.cu replace it
 // for hexahedra.  All arithmetic in double; u / rhs are stored in T (float or double).
 #include "fr_dev.hpp"
+#include "fr_hex_tma.hpp"
 
 namespace fr {
 namespace {
@@ -199,6 +200,52 @@ __global__ void k_common_flux_bnd(DevConsts c, double *__restrict__ uf, const do
   for (int a = 0; a < NV; ++a) uf[o + (size_t)a * c.ld] = jn * F[a];
 }
 
+// Common normal flux with the viscous part pre-contracted by the element kernels (fr_hex_tma.cu):
+// gf = n_own . f_vis(u^f, q^f) at every flux point with the element's OWN outward normal, so that
+// n_L . f_R^vis = -gf_R.   F = Rusanov + tau (u_L - u_R) - {(1/2+beta) gf_L - (1/2-beta) gf_R}   (Eq 26-27, A7)
+template <int ND>
+__global__ void k_common_flux_g(DevConsts c, double *__restrict__ uf, const double *__restrict__ gf) {
+  constexpr int NV = ND + 2;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= c.npairs) return;
+  const size_t oL = (size_t)c.pLs[i] * NV * c.ld + c.pLe[i], oR = (size_t)c.pRs[i] * NV * c.ld + c.pRe[i];
+  const double wl = 0.5 + c.ph.beta, wr = 0.5 - c.ph.beta;
+  double uL[NV], uR[NV], gL[NV], gR[NV], nrm[ND], F[NV];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) { uL[a] = uf[oL + (size_t)a * c.ld]; uR[a] = uf[oR + (size_t)a * c.ld]; }
+#pragma unroll
+  for (int a = 0; a < NV; ++a) { gL[a] = wl != 0.0 ? gf[oL + (size_t)a * c.ld] : 0.0; gR[a] = wr != 0.0 ? gf[oR + (size_t)a * c.ld] : 0.0; }
+#pragma unroll
+  for (int n = 0; n < ND; ++n) nrm[n] = c.pn[(size_t)n * c.npairs + i];
+  rusanov<ND>(uL, uR, nrm, c.ph.gamma, F);
+  const double jl = c.pJnL[i], jr = c.pJnR[i];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) {
+    const double f = F[a] + c.ph.tau * (uL[a] - uR[a]) - (wl * gL[a] - wr * gR[a]);
+    uf[oL + (size_t)a * c.ld] = jl * f;
+    uf[oR + (size_t)a * c.ld] = -jr * f;
+  }
+}
+
+// boundary flux points: gf already holds the complete LDG viscous flux with the ghost state (App C)
+template <int ND>
+__global__ void k_common_flux_bnd_g(DevConsts c, double *__restrict__ uf, const double *__restrict__ gf) {
+  constexpr int NV = ND + 2;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= c.nbnd) return;
+  const size_t o = (size_t)c.bs[i] * NV * c.ld + c.be[i];
+  double uL[NV], gi[NV], gl[NV], nrm[ND], F[NV];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) uL[a] = uf[o + (size_t)a * c.ld];
+  ghost_states<ND>(c.bcs[c.bbc[i]], uL, c.ph.gamma, gi, gl);
+#pragma unroll
+  for (int n = 0; n < ND; ++n) nrm[n] = c.bn[(size_t)n * c.nbnd + i];
+  rusanov<ND>(uL, gi, nrm, c.ph.gamma, F);
+  const double jn = c.bJn[i];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) uf[o + (size_t)a * c.ld] = jn * (F[a] + c.ph.tau * (uL[a] - gl[a]) - gf[o + (size_t)a * c.ld]);
+}
+
 template <typename TIN, typename TOUT, bool SCALE>
 void apply(cudaStream_t s, const DevConsts &c, int M, int K1, const double *A, const TIN *in1, int K2, const double *B,
            const double *in2, TOUT *out, int nblk = 1, int64_t in_blk = 0, int64_t out_blk = 0) {
@@ -282,6 +329,12 @@ void launch_tflux(const DevConsts &c, const void *u, double *qu, cudaStream_t s)
 void launch_common_flux(const DevConsts &c, double *uf, const double *qf, cudaStream_t s) {
   if (c.nd == 2) { if (c.ns) launch_flux_t<2, true>(c, nullptr, nullptr, uf, qf, false, true, s); else launch_flux_t<2, false>(c, nullptr, nullptr, uf, qf, false, true, s); }
   else { if (c.ns) launch_flux_t<3, true>(c, nullptr, nullptr, uf, qf, false, true, s); else launch_flux_t<3, false>(c, nullptr, nullptr, uf, qf, false, true, s); }
+}
+
+void launch_common_flux_g(const DevConsts &c, double *uf, const double *gf, cudaStream_t s) {
+  const int TB = 128;
+  if (c.npairs) k_common_flux_g<3><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
+  if (c.nbnd) k_common_flux_bnd_g<3><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
 }
 
 int generic_rhs_launches(const DevConsts &c) {

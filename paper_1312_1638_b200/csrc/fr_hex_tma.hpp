@@ -1,0 +1,20 @@
+// TMA-pipelined hexahedral kernels (fr_hex_tma.cu): launch entry points used by the tensor-product driver.
+#pragma once
+#include "fr_dev.hpp"
+
+namespace fr {
+
+// true when the sm_100a TMA kernels can run this n = p+1 / precision (shared memory fits, driver exposes the encoder)
+bool hex_tma_supported(int n, bool f64);
+
+// G^f = n . f_vis(U^f, Q^f) at every flux point, Q recomputed from u and jump = C - U^f  (parts 2b, 3 of the north_star)
+cudaError_t hex_tma_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, cudaStream_t s);
+
+// rhs = -(1/J) {(M1 - M3 M2) S f(U, Q) + M3 D~}  (parts 4, 6, 7; Q recomputed for Navier-Stokes)
+cudaError_t hex_tma_rhs(const DevConsts &c, const double *h_ops, const void *u, const double *jump, const double *dt, void *rhs,
+                        cudaStream_t s);
+
+// Eq 15-17 over flux-point pairs with the viscous part taken from G^f; in place over U^f -> D~ (fr_generic.cu)
+void launch_common_flux_g(const DevConsts &c, double *uf, const double *gf, cudaStream_t s);
+
+}  // namespace fr

@@ -11,21 +11,14 @@
 // rows of its 32 columns, so each input is fetched from L2/HBM once per CTA).
 // The 1-D operators travel as a kernel parameter (constant bank, uniform broadcast reads).
 #include "fr_tensor.hpp"
+#include "fr_hex_tma.hpp"
+#include "fr_ops1d.cuh"
 
 #include <cstdlib>
 
 namespace fr {
 namespace {
 
-template <int N>
-struct Ops1D {
-  double D[N * N];    // D[i][m] = l_m'(xi_i)
-  double Dh[N * N];   // D + gm lm^T - gp lp^T  (1-D form of M1 - M3 M2, Eq 44 :773; M2 holds n~ = -1 on the -1 face)
-  double lm[N], lp[N];  // l_m(-1), l_m(+1)                    (M0, Eq 41)
-  double gm[N], gp[N];  // div g of the -1 / +1 face point at node i (M3, M6)
-};
-
-__host__ __device__ constexpr int ipow(int b, int e) { return e == 0 ? 1 : b * ipow(b, e - 1); }
 
 // rho of point m on the line through (direction d, face-point index idx)
 template <int N, int ND>
@@ -196,19 +189,6 @@ void launch_hex_grad(const Ops1D<N> &op, const DevConsts &c, const T *u, const d
   launch_hex_grad_e<N, E, T>(op, c, u, jump, qu, s);
 }
 
-template <int N>
-Ops1D<N> make_ops(const double *h) {  // h: D, Dh, lm, lp, gm, gp packed
-  Ops1D<N> o;
-  const double *p = h;
-  for (int i = 0; i < N * N; ++i) o.D[i] = *p++;
-  for (int i = 0; i < N * N; ++i) o.Dh[i] = *p++;
-  for (int i = 0; i < N; ++i) o.lm[i] = *p++;
-  for (int i = 0; i < N; ++i) o.lp[i] = *p++;
-  for (int i = 0; i < N; ++i) o.gm[i] = *p++;
-  for (int i = 0; i < N; ++i) o.gp[i] = *p++;
-  return o;
-}
-
 template <int N, int ND, typename T>
 cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, char *work, cudaStream_t s, Prof *prof) {
   constexpr int NU = ipow(N, ND), NFP = ipow(N, ND - 1), NF = 2 * ND * NFP;
@@ -222,6 +202,25 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
   const dim3 bf(LW, NFP < rows ? NFP : rows), bu(LW, NU < rows ? NU : rows);
   FR_MARK(prof, "tp_interp");
   k_tp_interp<N, ND, T><<<dim3(gx, 1, 1), bf, 0, s>>>(op, u, uf, ncols, c.ld, c.Nel, 0, 0);
+  if (ND == 3 && tp.use_tma) {
+    // sm_100a path: 5 launches for Navier-Stokes (3 for Euler); neither Q nor Q^f nor F~ is stored
+    cudaError_t e = cudaSuccess;
+    if (c.ns) {
+      FR_MARK(prof, "common_sol");
+      launch_common_jump(c, uf, cf, s);
+      FR_MARK(prof, "hex_gradface");
+      e = hex_tma_gradface(c, tp.h_ops, u, cf, qu, s);
+      if (e != cudaSuccess) return e;
+      FR_MARK(prof, "common_flux_g");
+      launch_common_flux_g(c, uf, qu, s);
+    } else {
+      FR_MARK(prof, "common_flux");
+      launch_common_flux(c, uf, qf, s);
+    }
+    FR_MARK(prof, "hex_rhs_tma");
+    e = hex_tma_rhs(c, tp.h_ops, u, cf, uf, rhs, s);
+    return e != cudaSuccess ? e : cudaGetLastError();
+  }
   if (c.ns) {
     FR_MARK(prof, "common_sol");
     launch_common_jump(c, uf, cf, s);
@@ -292,8 +291,14 @@ cudaError_t tensor_plan(const DevConsts &c, const RefOps &o, const MeshConsts &,
   int64_t off = 0;
   tp.off_uf = off; off = al(off + (int64_t)o.Nf * ncols * 8);
   tp.off_cf = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
-  tp.off_qu = off; off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
-  tp.off_qf = off; if (c.ns) off = al(off + (int64_t)o.nd * o.Nf * ncols * 8);
+  tp.use_tma = c.etype == FR_HEX && hex_tma_supported(c.n, c.f64);
+  if (tp.use_tma) {  // only G^f besides U^f and the jumps
+    tp.off_qu = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
+    tp.off_qf = off;
+  } else {
+    tp.off_qu = off; off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
+    tp.off_qf = off; if (c.ns) off = al(off + (int64_t)o.nd * o.Nf * ncols * 8);
+  }
   tp.work_bytes = off;
   return cudaSuccess;
 }
@@ -303,6 +308,12 @@ cudaError_t tensor_rhs(const DevConsts &c, const TensorPlan &tp, const void *u, 
 }
 
 int tensor_rhs_launches(const DevConsts &c) {
+  if (c.etype == FR_HEX && hex_tma_supported(c.n, c.f64)) {
+    int n = c.ns ? 5 : 3;  // interp, (common sol, gradface,) common flux, rhs
+    if (c.nbnd) n += c.ns ? 2 : 1;
+    if (!c.npairs) n -= c.ns ? 2 : 1;
+    return n;
+  }
   int n = 4 + (c.ns ? 3 : 0);  // interp, tflux, common flux, div (+ common sol, grad, interp q)
   if (c.nbnd) n += c.ns ? 2 : 1;
   if (!c.npairs) n -= c.ns ? 2 : 1;
