@@ -148,8 +148,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
                   const double *__restrict__ jump, const double *__restrict__ dt, T *__restrict__ rhs, int64_t ld, int64_t Nel) {
   using L = RhsLay<N, E, NS, T, NB>;
   constexpr int NFP = N * N;
-  extern __shared__ unsigned char smem_raw[];
-  unsigned char *sm = (unsigned char *)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  unsigned char *sm = smem_raw + ((128u - (smem_addr(smem_raw) & 127u)) & 127u);  // stays in the shared address space
   uint64_t *bar = (uint64_t *)(sm + L::BAR);  // [0]: U block + 1/J block, [1], [2]: stages
   double *sD = (double *)(sm + L::OPS), *sDh = sD + N * N;
   const T *sU = (const T *)(sm + L::U);            // [NU*NV][E], row = (NFP k + ij) NV + a
@@ -318,8 +318,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
                    const BcDev *__restrict__ bcs, double *__restrict__ gf, int64_t ld, int64_t Nel) {
   using L = GfLay<N, E, T>;
   constexpr int NFP = N * N, NF = 6 * NFP;
-  extern __shared__ unsigned char smem_raw[];
-  unsigned char *sm = (unsigned char *)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  unsigned char *sm = smem_raw + ((128u - (smem_addr(smem_raw) & 127u)) & 127u);  // stays in the shared address space
   uint64_t *bar = (uint64_t *)(sm + L::BAR);
   double *sD = (double *)(sm + L::OPS), *sL = sD + N * N;  // sL[0][m] = l_m(-1), sL[1][m] = l_m(+1)
   const T *sU = (const T *)(sm + L::U);
@@ -520,7 +520,7 @@ cudaError_t set_smem(K kern, size_t smem, bool &done) {
   return e;
 }
 
-template <int N, int E, bool NS, typename T>
+template <int N, int E, bool NS, typename T, int CAP = 8>
 cudaError_t launch_rhs(const DevConsts &c, const double *h_ops, const void *u, const double *jump, const double *dt, void *rhs,
                        cudaStream_t s) {
   constexpr int NB1 = 1;
@@ -530,7 +530,7 @@ cudaError_t launch_rhs(const DevConsts &c, const double *h_ops, const void *u, c
   constexpr int NB = (L2::TOTAL <= SMEM_MAX && min_blocks(L2::TOTAL, N * N * E) == min_blocks(L1::TOTAL, N * N * E)) ? 2 : 1;
   using L = RhsLay<N, E, NS, T, NB>;
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
-  constexpr int MINB = min_blocks(L::TOTAL, N * N * E);
+  constexpr int MINB = min_blocks(L::TOTAL, N * N * E) < CAP ? min_blocks(L::TOTAL, N * N * E) : CAP;
   Maps<N, E> m;
   if (!make_maps<N, E, T>(c, u, jump, m, NS)) return cudaErrorNotSupported;
   auto kern = k_hex_rhs_tma<N, E, NS, T, NB, MINB>;
@@ -542,11 +542,11 @@ cudaError_t launch_rhs(const DevConsts &c, const double *h_ops, const void *u, c
   return cudaGetLastError();
 }
 
-template <int N, int E, typename T>
+template <int N, int E, typename T, int CAP = 8>
 cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, cudaStream_t s) {
   using L = GfLay<N, E, T>;
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
-  constexpr int MINB = min_blocks(L::TOTAL, N * N * E);
+  constexpr int MINB = min_blocks(L::TOTAL, N * N * E) < CAP ? min_blocks(L::TOTAL, N * N * E) : CAP;
   Maps<N, E> m;
   if (!make_maps<N, E, T>(c, u, jump, m, true)) return cudaErrorNotSupported;
   const Ops1D<N> op = make_ops<N>(h_ops);
@@ -585,8 +585,10 @@ int env_e() {
 template <int N, typename T>
 cudaError_t rhs_n(const DevConsts &c, const double *h_ops, const void *u, const double *jump, const double *dt, void *rhs, cudaStream_t s) {
   if constexpr (fits<N, T>()) {
-    if constexpr (N == 4 || N == 5) {
+    if constexpr (N == 5 && sizeof(T) == 8) {  // tuning variants (FR_TMA_E = 16 | 12 | 81 (E = 8, one CTA per SM))
       if (env_e() == 16) return c.ns ? launch_rhs<N, 16, true, T>(c, h_ops, u, jump, dt, rhs, s) : launch_rhs<N, 16, false, T>(c, h_ops, u, jump, dt, rhs, s);
+      if (env_e() == 12) return c.ns ? launch_rhs<N, 12, true, T>(c, h_ops, u, jump, dt, rhs, s) : launch_rhs<N, 12, false, T>(c, h_ops, u, jump, dt, rhs, s);
+      if (env_e() == 81) return c.ns ? launch_rhs<N, 8, true, T, 1>(c, h_ops, u, jump, dt, rhs, s) : launch_rhs<N, 8, false, T, 1>(c, h_ops, u, jump, dt, rhs, s);
     }
     constexpr int E = Cfg<N>::E;
     return c.ns ? launch_rhs<N, E, true, T>(c, h_ops, u, jump, dt, rhs, s) : launch_rhs<N, E, false, T>(c, h_ops, u, jump, dt, rhs, s);
@@ -598,8 +600,10 @@ cudaError_t rhs_n(const DevConsts &c, const double *h_ops, const void *u, const 
 template <int N, typename T>
 cudaError_t gradface_n(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, cudaStream_t s) {
   if constexpr (fits<N, T>()) {
-    if constexpr (N == 4 || N == 5) {
+    if constexpr (N == 5 && sizeof(T) == 8) {
       if (env_e() == 16) return launch_gradface<N, 16, T>(c, h_ops, u, jump, gf, s);
+      if (env_e() == 12) return launch_gradface<N, 12, T>(c, h_ops, u, jump, gf, s);
+      if (env_e() == 81) return launch_gradface<N, 8, T, 1>(c, h_ops, u, jump, gf, s);
     }
     return launch_gradface<N, Cfg<N>::E, T>(c, h_ops, u, jump, gf, s);
   } else {
