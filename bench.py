@@ -100,6 +100,11 @@ def kernel_words(name, nd, NV, Nu, Nf, ns):
         "hex_grad": (Nu + Nf) * NV + met + nd * Nu * NV,
         "hex_fluxdiv": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
         "hex_rhs": (2 * Nu + 2 * Nf) * NV + met,
+        # TMA-pipelined hexahedral path (fr_hex_tma.cu, fr_hex_fluxdiv_tma.cu)
+        "hex_gradface": (Nu + 2 * Nf) * NV + met + nd * Nf + nd * Nu * NV,  # U, jump, S, 1/J, normals -> G^f, Q
+        "common_flux_g": 3 * Nf * NV + (nd + 2 + 2) * Nf // 2,              # U^f, G^f -> D~ (in place), normals, J n
+        "hex_rhs_tma": (2 * Nu + 2 * Nf) * NV + met,                        # U, jump, S, 1/J, D~ -> R
+        "hex_fluxdiv_tma": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
         "tp_grad": (Nu + Nf) * NV + met + (nd + 1) * Nf + (NV - 1) * Nf + Nf,
         "tp_div": (2 * Nu + Nf) * NV + met + (nd + 1) * Nf + ((NV - 1) * Nf if ns else 0) + Nf,
     }

@@ -1,0 +1,247 @@
+// k_hex_fluxdiv_tma: parts (4), (6), (7) of the right-hand side on hexahedra in one TMA-pipelined kernel (sm_100a):
+//   F~ = S f(U, Q)  (Eq 12 :214 with Eq 20-24),  R = -(1/J) {(M1 - M3 M2) F~ + M3 D~}  (Eq 18-19 / Eq 44 :772).
+// A CTA owns E consecutive elements and walks them slice by slice (z = k).  Everything a slice needs -- the metric
+// terms S (9 rows per point), the U slice and, for Navier-Stokes, the Q slice written by k_hex_gradface -- arrives
+// in a two-stage ring of TMA box loads completing on mbarriers, issued two slices ahead by one thread.  F~ never
+// leaves the SM: its x/y parts go through one shared-memory slice, its z part straight into the column accumulators.
+#include "fr_tma.cuh"
+
+namespace fr {
+namespace {
+
+template <int N, int E, bool NS, typename T, int NB>
+struct FdLay {
+  static constexpr int NFP = N * N, NU = N * NFP;
+  static constexpr size_t BAR = 0;
+  static constexpr size_t OPS = 128;  // sDh [N*N], sGm [N], sGp [N]
+  static constexpr size_t ST = OPS + al128((N * N + 2 * N) * 8);
+  static constexpr uint32_t S_TX = 9 * NFP * E * 8, U_TX = NFP * NV * E * sizeof(T), Q_TX = NS ? 3 * NV * NFP * E * 8 : 0;
+  static constexpr size_t ST_U = al128(S_TX);
+  static constexpr size_t ST_Q = ST_U + al128(U_TX);
+  static constexpr size_t ST_BYTES = ST_Q + al128(Q_TX);
+  static constexpr size_t F = ST + 2 * ST_BYTES;
+  static constexpr size_t F_BYTES = 2 * NV * NFP * E * 8;
+  static constexpr size_t TOTAL = F + NB * F_BYTES + 128;  // + slack for the manual 128-byte alignment
+};
+
+// tmS: smat as (ld, NU, 9), box (E, NFP, 9);  tmU: u as (ld, NFP*NV, N), box (E, NFP*NV, 1);
+// tmQ: Q workspace as (ld, NV*NFP, 3N), box (E, NV*NFP, 3)  (slice-major layout written by k_hex_gradface).
+template <int N, int E, bool NS, typename T, int NB, int MINB>
+__global__ void __launch_bounds__(N *N *E, MINB)
+    k_hex_fluxdiv_tma(const __grid_constant__ CUtensorMap tmS, const __grid_constant__ CUtensorMap tmU,
+                      const __grid_constant__ CUtensorMap tmQ, Ops1D<N> op, Phys ph, const double *__restrict__ rcpj,
+                      const double *__restrict__ dt, T *__restrict__ rhs, int64_t ld, int64_t Nel) {
+  using L = FdLay<N, E, NS, T, NB>;
+  constexpr int NFP = N * N;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  unsigned char *sm = smem_raw + ((128u - (smem_addr(smem_raw) & 127u)) & 127u);  // stays in the shared address space
+  uint64_t *bar = (uint64_t *)(sm + L::BAR);
+  double *sDh = (double *)(sm + L::OPS), *sGm = sDh + N * N, *sGp = sGm + N;
+  unsigned char *sSt = sm + L::ST;
+  double *sF = (double *)(sm + L::F);  // [NB][2][NV][NFP][E]
+  const int tid = threadIdx.x, el = tid % E, ij = tid / E, i = ij % N, j = ij / N;
+  const int e0 = blockIdx.x * E;
+  const int64_t e = (int64_t)e0 + el;
+  const bool act = e < Nel;
+
+  if (tid == 0) {
+    mbar_init(&bar[0], 1); mbar_init(&bar[1], 1);
+    fence_barrier_init();
+    fence_proxy_async();
+  }
+  for (int t = tid; t < N * N; t += NFP * E) sDh[t] = op.Dh[t];
+  for (int t = tid; t < N; t += NFP * E) { sGm[t] = op.gm[t]; sGp[t] = op.gp[t]; }
+  __syncthreads();
+  auto issue_stage = [&](int s, int k) {
+    mbar_expect_tx(&bar[s], L::S_TX + L::U_TX + L::Q_TX);
+    tma_load_3d(sSt + s * L::ST_BYTES, &tmS, e0, NFP * k, 0, &bar[s]);
+    tma_load_3d(sSt + s * L::ST_BYTES + L::ST_U, &tmU, e0, 0, k, &bar[s]);
+    if (NS) tma_load_3d(sSt + s * L::ST_BYTES + L::ST_Q, &tmQ, e0, 0, 3 * k, &bar[s]);
+  };
+  if (tid == 0) {
+    issue_stage(0, 0);
+    if (N > 1) issue_stage(1, 1);
+  }
+  double acc[N][NV];
+#pragma unroll
+  for (int k = 0; k < N; ++k)
+#pragma unroll
+    for (int a = 0; a < NV; ++a) acc[k][a] = 0.0;
+
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    mbar_wait(&bar[k & 1], (k >> 1) & 1);
+    const double *stS = (const double *)(sSt + (k & 1) * L::ST_BYTES);
+    const T *stU = (const T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_U);
+    const double *stQ = (const double *)(sSt + (k & 1) * L::ST_BYTES + L::ST_Q);
+    double *buf = sF + (NB == 2 ? (k & 1) : 0) * (2 * NV * NFP * E);
+    {
+      double S[3][3], uu[NV];
+#pragma unroll
+      for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) S[a][b] = stS[((a * 3 + b) * NFP + ij) * E + el];
+#pragma unroll
+      for (int a = 0; a < NV; ++a) uu[a] = (double)stU[(ij * NV + a) * E + el];
+      // primitive variables (Eq 20-21)
+      const double rrho = 1.0 / uu[0], En = uu[4];
+      double v[3], ke = 0;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) { v[d] = uu[1 + d] * rrho; ke += uu[1 + d] * v[d]; }
+      const double p = (ph.gamma - 1.0) * (En - 0.5 * ke);
+      // viscous stress Tm and energy flux w = v.Tm + (mu gamma / Pr) grad e  (Eq 22-24, A8), built variable by variable
+      double Tm[3][3], w[3];
+      if (NS) {
+        double g0[3], dv[3][3], de[3];
+#pragma unroll
+        for (int a = 0; a < NV; ++a)
+#pragma unroll
+          for (int n = 0; n < 3; ++n) {
+            const double g = stQ[((n * NV + a) * NFP + ij) * E + el];
+            if (a == 0) g0[n] = g;
+            else if (a < 4) dv[n][a - 1] = (g - v[a - 1] * g0[n]) * rrho;  // d_n v_j by the quotient rule
+            else de[n] = (g - (En * rrho) * g0[n]) * rrho;
+          }
+        const double lam = -2.0 / 3.0 * ph.mu * (dv[0][0] + dv[1][1] + dv[2][2]);
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+          for (int b = 0; b < 3; ++b) Tm[a][b] = ph.mu * (dv[a][b] + dv[b][a]) + (a == b ? lam : 0.0);
+        const double kap = ph.mu * ph.gamma / ph.Pr;
+#pragma unroll
+        for (int n = 0; n < 3; ++n) {
+          double d = de[n], vt = 0;
+#pragma unroll
+          for (int b = 0; b < 3; ++b) { d -= v[b] * dv[n][b]; vt += v[b] * Tm[b][n]; }
+          w[n] = vt + kap * d;
+        }
+      }
+      if (NB == 1 && k > 0) __syncthreads();  // the previous slice's contraction has finished reading sF
+      // F~_i = sum_n S[i][n] (f_inv - f_vis)_n  (Eq 12), one variable at a time
+#pragma unroll
+      for (int a = 0; a < NV; ++a) {
+        double f[3];
+#pragma unroll
+        for (int n = 0; n < 3; ++n) {
+          if (a == 0) f[n] = uu[1 + n];
+          else if (a < 4) { f[n] = uu[1 + n] * v[a - 1] + (a - 1 == n ? p : 0.0); if (NS) f[n] -= Tm[n][a - 1]; }
+          else { f[n] = v[n] * (En + p); if (NS) f[n] -= w[n]; }
+        }
+        buf[((0 * NV + a) * NFP + ij) * E + el] = fma(S[0][0], f[0], fma(S[0][1], f[1], S[0][2] * f[2]));
+        buf[((1 * NV + a) * NFP + ij) * E + el] = fma(S[1][0], f[0], fma(S[1][1], f[1], S[1][2] * f[2]));
+        const double fz = fma(S[2][0], f[0], fma(S[2][1], f[1], S[2][2] * f[2]));
+#pragma unroll
+        for (int kk = 0; kk < N; ++kk) acc[kk][a] = fma(op.Dh[kk * N + k], fz, acc[kk][a]);
+      }
+    }
+    __syncthreads();
+    // every thread has consumed stage k&1: refill it with slice k+2
+    if (tid == 0 && k + 2 < N) issue_stage(k & 1, k + 2);
+    // x and y contractions within the slice
+#pragma unroll
+    for (int m = 0; m < N; ++m) {
+      const double dx = sDh[i * N + m], dy = sDh[j * N + m];
+#pragma unroll
+      for (int a = 0; a < NV; ++a) {
+        acc[k][a] = fma(dx, buf[((0 * NV + a) * NFP + j * N + m) * E + el], acc[k][a]);
+        acc[k][a] = fma(dy, buf[((1 * NV + a) * NFP + m * N + i) * E + el], acc[k][a]);
+      }
+    }
+  }
+  if (!act) return;
+  // lifting M3 D~ and the -1/J scale (Eq 19); faces: 0,1 = x-,x+ (idx j + N k); 2,3 = y (i + N k); 4,5 = z (i + N j)
+  const double gmi = sGm[i], gpi = sGp[i], gmj = sGm[j], gpj = sGp[j];
+  double dzm[NV], dzp[NV];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) {
+    dzm[a] = dt[((size_t)(4 * NFP + ij) * NV + a) * ld + e];
+    dzp[a] = dt[((size_t)(5 * NFP + ij) * NV + a) * ld + e];
+  }
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    const int r = ij + NFP * k;
+    const double rj = rcpj[(size_t)r * ld + e];
+    const int fx = j + N * k, fy = i + N * k;
+#pragma unroll
+    for (int a = 0; a < NV; ++a) {
+      double v = acc[k][a];
+      v = fma(op.gm[k], dzm[a], v);
+      v = fma(op.gp[k], dzp[a], v);
+      v = fma(gmi, dt[((size_t)(0 * NFP + fx) * NV + a) * ld + e], v);
+      v = fma(gpi, dt[((size_t)(1 * NFP + fx) * NV + a) * ld + e], v);
+      v = fma(gmj, dt[((size_t)(2 * NFP + fy) * NV + a) * ld + e], v);
+      v = fma(gpj, dt[((size_t)(3 * NFP + fy) * NV + a) * ld + e], v);
+      rhs[((size_t)r * NV + a) * ld + e] = (T)(-v * rj);
+    }
+  }
+}
+
+template <int N, int E, bool NS, typename T, int CAP = 8>
+cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *u, const double *q, const double *dt, void *rhs,
+                           cudaStream_t s) {
+  constexpr int NFP = N * N, NU = N * NFP;
+  using L2 = FdLay<N, E, NS, T, 2>;
+  using L1 = FdLay<N, E, NS, T, 1>;
+  // double-buffer F~ when that does not cost a resident CTA
+  constexpr int NB = (L2::TOTAL <= SMEM_MAX && min_blocks(L2::TOTAL, N * N * E) == min_blocks(L1::TOTAL, N * N * E)) ? 2 : 1;
+  using L = FdLay<N, E, NS, T, NB>;
+  static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
+  constexpr int MINB = min_blocks(L::TOTAL, N * N * E) < CAP ? min_blocks(L::TOTAL, N * N * E) : CAP;
+  const uint64_t ld = (uint64_t)c.ld;
+  CUtensorMap mS, mU, mQ;
+  bool ok = encode3(&mS, true, c.smat, ld, NU, 9, ld, (uint64_t)NU * ld, E, NFP, 9);
+  ok = ok && encode3(&mU, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 1);
+  if (NS) ok = ok && encode3(&mQ, true, q, ld, NV * NFP, 3 * N, ld, (uint64_t)NV * NFP * ld, E, NV * NFP, 3);
+  else mQ = mS;
+  if (!ok) return cudaErrorNotSupported;
+  auto kern = k_hex_fluxdiv_tma<N, E, NS, T, NB, MINB>;
+  static bool done = false;
+  cudaError_t err = set_smem(kern, L::TOTAL, done);
+  if (err != cudaSuccess) return err;
+  const Ops1D<N> op = make_ops<N>(h_ops);
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(mS, mU, mQ, op, c.ph, c.rcpj, dt, (T *)rhs, c.ld, c.Nel);
+  return cudaGetLastError();
+}
+
+template <int N, typename T>
+constexpr bool fd_fits() {
+  return FdLay<N, Cfg<N>::E, true, T, 1>::TOTAL <= SMEM_MAX && N * N * Cfg<N>::E <= 1024 && N * N * NV <= 256;
+}
+
+template <int N, typename T>
+cudaError_t fluxdiv_n(const DevConsts &c, const double *h_ops, const void *u, const double *q, const double *dt, void *rhs, cudaStream_t s) {
+  if constexpr (fd_fits<N, T>()) {
+    if constexpr (N == 5 && sizeof(T) == 8) {  // tuning variants (FR_TMA_E = 16 | 81 (E = 8, one CTA per SM))
+      if (env_e() == 16) return c.ns ? launch_fluxdiv<N, 16, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, 16, false, T>(c, h_ops, u, q, dt, rhs, s);
+      if (env_e() == 81) return c.ns ? launch_fluxdiv<N, 8, true, T, 1>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, 8, false, T, 1>(c, h_ops, u, q, dt, rhs, s);
+    }
+    constexpr int E = Cfg<N>::E;
+    return c.ns ? launch_fluxdiv<N, E, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, E, false, T>(c, h_ops, u, q, dt, rhs, s);
+  } else {
+    return cudaErrorNotSupported;
+  }
+}
+
+}  // namespace
+
+bool hex_tma_fluxdiv_supported(int n, bool f64) {
+  if (getenv("FR_NO_TMA") || !encoder()) return false;
+  switch (n) {
+#define FR_CASE(NN) case NN: return f64 ? fd_fits<NN, double>() : fd_fits<NN, float>();
+    FR_CASE(2) FR_CASE(3) FR_CASE(4) FR_CASE(5) FR_CASE(6) FR_CASE(7)
+#undef FR_CASE
+    default: return false;
+  }
+}
+
+cudaError_t hex_tma_fluxdiv(const DevConsts &c, const double *h_ops, const void *u, const double *q, const double *dt, void *rhs,
+                            cudaStream_t s) {
+  switch (c.n) {
+#define FR_CASE(NN) case NN: return c.f64 ? fluxdiv_n<NN, double>(c, h_ops, u, q, dt, rhs, s) : fluxdiv_n<NN, float>(c, h_ops, u, q, dt, rhs, s);
+    FR_CASE(2) FR_CASE(3) FR_CASE(4) FR_CASE(5) FR_CASE(6) FR_CASE(7)
+#undef FR_CASE
+    default: return cudaErrorNotSupported;
+  }
+}
+
+}  // namespace fr

@@ -17,56 +17,10 @@
 // mbarriers, issued two slices ahead by one thread, so HBM latency is covered without registers or occupancy.
 // Thread (e, i, j) owns the column of points (i, j, .); contractions along x and y read shared memory,
 // contractions along z use operator entries from the constant bank.
-#include <cuda.h>  // CUtensorMap and its enums (types only: the encoder is fetched through the runtime)
-
-#include <cstdint>
-#include <cstdlib>
-
-#include "fr_hex_tma.hpp"
-#include "fr_ops1d.cuh"
+#include "fr_tma.cuh"
 
 namespace fr {
 namespace {
-
-constexpr int NV = 5;
-constexpr size_t SMEM_MAX = 227 * 1024;
-
-__host__ __device__ constexpr size_t al128(size_t x) { return (x + 127) / 128 * 128; }
-
-// ---------------------------------------------------------------------------------------------
-// PTX wrappers: mbarrier + bulk tensor copies
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-  const uint32_t a = smem_addr(bar);
-  uint32_t ok;
-  do {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n"
-        : "=r"(ok)
-        : "r"(a), "r"(parity)
-        : "memory");
-  } while (!ok);
-}
-__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, uint64_t *bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
-          smem_addr(dst)),
-      "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_addr(bar))
-      : "memory");
-}
 
 // ---------------------------------------------------------------------------------------------
 // shared-memory layouts (byte offsets from a 128-byte aligned base)
@@ -75,8 +29,8 @@ template <int N, int E, bool NS, typename T, int NB>
 struct RhsLay {
   static constexpr int NFP = N * N, NU = N * NFP;
   static constexpr size_t BAR = 0;
-  static constexpr size_t OPS = 128;  // sD, sDh
-  static constexpr size_t U = OPS + al128(2 * N * N * 8);
+  static constexpr size_t OPS = 128;  // sD, sDh, sGm, sGp
+  static constexpr size_t U = OPS + al128((2 * N * N + 2 * N) * 8);
   static constexpr uint32_t U_TX = NU * NV * E * sizeof(T);
   static constexpr size_t RJ = U + al128(U_TX);
   static constexpr uint32_t RJ_TX = NU * E * 8;
@@ -93,8 +47,8 @@ template <int N, int E, typename T>
 struct GfLay {
   static constexpr int NFP = N * N, NU = N * NFP;
   static constexpr size_t BAR = 0;
-  static constexpr size_t OPS = 128;  // sD [N*N], sL [2][N]
-  static constexpr size_t U = OPS + al128((N * N + 2 * N) * 8);
+  static constexpr size_t OPS = 128;  // sD [N*N], sL [2][N], sGm [N], sGp [N]
+  static constexpr size_t U = OPS + al128((N * N + 4 * N) * 8);
   static constexpr uint32_t U_TX = NU * NV * E * sizeof(T);
   static constexpr size_t ST = U + al128(U_TX);
   static constexpr uint32_t S_TX = 9 * NFP * E * 8, R_TX = NFP * E * 8, J_TX = 4 * N * NV * E * 8;
@@ -105,23 +59,6 @@ struct GfLay {
   static constexpr size_t Q_BYTES = 3 * NV * NFP * E * 8;
   static constexpr size_t TOTAL = Q + Q_BYTES + 128;
 };
-
-// resident CTAs per SM the kernel is compiled for: limited by shared memory, by >= 128 registers per thread
-constexpr int min_blocks(size_t smem, int threads) {
-  int by_smem = (int)((SMEM_MAX + 1024) / (smem + 1024));
-  int warps = (threads + 31) / 32;
-  int by_regs = 65536 / (128 * 32 * warps);
-  int by_thr = 2048 / (32 * warps);
-  int m = by_smem < by_regs ? by_smem : by_regs;
-  m = m < by_thr ? m : by_thr;
-  return m < 1 ? 1 : (m > 8 ? 8 : m);
-}
-
-// Q~ -> Q at one solution point for variable a:  q_n = (1/J) sum_i S[i][n] q~_i   (Eq 10 :206)
-__device__ __forceinline__ void to_physical(const double (*S)[3], double rj, double qx, double qy, double qz, double *q) {
-#pragma unroll
-  for (int n = 0; n < 3; ++n) q[n] = rj * fma(S[0][n], qx, fma(S[1][n], qy, S[2][n] * qz));
-}
 
 // F~ = S f(u, q) at one point (Eq 12 :214 with Eq 20-24)
 template <bool NS>
@@ -151,7 +88,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char *sm = smem_raw + ((128u - (smem_addr(smem_raw) & 127u)) & 127u);  // stays in the shared address space
   uint64_t *bar = (uint64_t *)(sm + L::BAR);  // [0]: U block + 1/J block, [1], [2]: stages
-  double *sD = (double *)(sm + L::OPS), *sDh = sD + N * N;
+  double *sD = (double *)(sm + L::OPS), *sDh = sD + N * N, *sGm = sDh + N * N, *sGp = sGm + N;
   const T *sU = (const T *)(sm + L::U);            // [NU*NV][E], row = (NFP k + ij) NV + a
   const double *sRJ = (const double *)(sm + L::RJ);  // [NU][E]
   unsigned char *sSt = sm + L::ST;
@@ -167,6 +104,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     fence_proxy_async();
   }
   for (int t = tid; t < N * N; t += NFP * E) { sD[t] = op.D[t]; sDh[t] = op.Dh[t]; }
+  for (int t = tid; t < N; t += NFP * E) { sGm[t] = op.gm[t]; sGp[t] = op.gp[t]; }
   __syncthreads();
   auto issue_stage = [&](int s, int k) {
     mbar_expect_tx(&bar[1 + s], L::S_TX + L::J_TX);
@@ -180,15 +118,15 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     issue_stage(0, 0);
     if (N > 1) issue_stage(1, 1);
   }
+  // z-face jumps of this column: re-read from L2 in every slice, one variable ahead of their use, instead of
+  // staying in registers (10 values) across the whole kernel.
+  auto ldj = [&](int face, int a) { return ld_nc_once(jump + ((size_t)(face * NFP + ij) * NV + a) * ld + e); };
   double jzm[NV], jzp[NV];
-  if (NS) {
+  auto load_jz = [&]() {
 #pragma unroll
-    for (int a = 0; a < NV; ++a) {
-      jzm[a] = jump[((size_t)(4 * NFP + ij) * NV + a) * ld + e];
-      jzp[a] = jump[((size_t)(5 * NFP + ij) * NV + a) * ld + e];
-    }
-  }
-  const double gmi = op.gm[i], gpi = op.gp[i], gmj = op.gm[j], gpj = op.gp[j];
+    for (int a = 0; a < NV; ++a) { jzm[a] = ldj(4, a); jzp[a] = ldj(5, a); }
+  };
+  if (NS) load_jz();
   double acc[N][NV];
 #pragma unroll
   for (int k = 0; k < N; ++k)
@@ -201,9 +139,9 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     mbar_wait(&bar[1 + (k & 1)], (k >> 1) & 1);
     const double *stS = (const double *)(sSt + (k & 1) * L::ST_BYTES);
     const double *stJ = (const double *)(sSt + (k & 1) * L::ST_BYTES + L::ST_J);
-    double F[3][NV];
+    double *buf = sF + (NB == 2 ? (k & 1) : 0) * (2 * NV * NFP * E);
     {
-      double S[3][3], uu[NV], qq[3][NV];
+      double S[3][3], uu[NV];
 #pragma unroll
       for (int a = 0; a < 3; ++a)
 #pragma unroll
@@ -211,8 +149,19 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       const T *su = sU + (size_t)(NFP * k) * NV * E + el;  // slice k
 #pragma unroll
       for (int a = 0; a < NV; ++a) uu[a] = (double)su[(ij * NV + a) * E];
+      // primitive variables (Eq 20-21)
+      const double rrho = 1.0 / uu[0], En = uu[4];
+      double v[3], ke = 0;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) { v[d] = uu[1 + d] * rrho; ke += uu[1 + d] * v[d]; }
+      const double p = (ph.gamma - 1.0) * (En - 0.5 * ke);
+      // viscous stress Tm and the energy flux w = v.Tm + (mu gamma / Pr) grad e  (Eq 22-24, A8), built variable by
+      // variable from the corrected physical gradients so that the 15 gradient values are never all live
+      double Tm[3][3], w[3];
       if (NS) {
         const double rj = sRJ[(NFP * k + ij) * E + el];
+        const double gmi = sGm[i], gpi = sGp[i], gmj = sGm[j], gpj = sGp[j];
+        double g0[3], dv[3][3], de[3];
 #pragma unroll
         for (int a = 0; a < NV; ++a) {
           // M6 = n~ (x) M3 (A1): the reference normal is -1 on the -1 faces
@@ -225,28 +174,52 @@ __global__ void __launch_bounds__(N *N *E, MINB)
             qy = fma(sD[j * N + m], (double)su[((m * N + i) * NV + a) * E], qy);
             qz = fma(op.D[k * N + m], (double)sU[((size_t)(NFP * m + ij) * NV + a) * E + el], qz);
           }
-          double q3[3];
-          to_physical(S, rj, qx, qy, qz, q3);
-          qq[0][a] = q3[0]; qq[1][a] = q3[1]; qq[2][a] = q3[2];
+          double g[3];
+          to_physical(S, rj, qx, qy, qz, g);
+#pragma unroll
+          for (int n = 0; n < 3; ++n) {
+            if (a == 0) g0[n] = g[n];
+            else if (a < 4) dv[n][a - 1] = (g[n] - v[a - 1] * g0[n]) * rrho;   // d_n v_j by the quotient rule
+            else de[n] = (g[n] - (En * rrho) * g0[n]) * rrho;
+          }
+        }
+        const double lam = -2.0 / 3.0 * ph.mu * (dv[0][0] + dv[1][1] + dv[2][2]);
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+          for (int b = 0; b < 3; ++b) Tm[a][b] = ph.mu * (dv[a][b] + dv[b][a]) + (a == b ? lam : 0.0);
+        const double kap = ph.mu * ph.gamma / ph.Pr;
+#pragma unroll
+        for (int n = 0; n < 3; ++n) {
+          double d = de[n], vt = 0;
+#pragma unroll
+          for (int b = 0; b < 3; ++b) { d -= v[b] * dv[n][b]; vt += v[b] * Tm[b][n]; }
+          w[n] = vt + kap * d;
         }
       }
-      point_tflux<NS>(uu, qq, S, ph, F);
+      if (NB == 1 && k > 0) __syncthreads();  // the previous slice's contraction has finished reading sF
+      // F~_i = sum_n S[i][n] (f_inv - f_vis)_n  (Eq 12), one variable at a time: x/y parts to shared memory,
+      // z part straight into the column accumulators
+#pragma unroll
+      for (int a = 0; a < NV; ++a) {
+        double f[3];
+#pragma unroll
+        for (int n = 0; n < 3; ++n) {
+          if (a == 0) f[n] = uu[1 + n];
+          else if (a < 4) { f[n] = uu[1 + n] * v[a - 1] + (a - 1 == n ? p : 0.0); if (NS) f[n] -= Tm[n][a - 1]; }
+          else { f[n] = v[n] * (En + p); if (NS) f[n] -= w[n]; }
+        }
+        buf[((0 * NV + a) * NFP + ij) * E + el] = fma(S[0][0], f[0], fma(S[0][1], f[1], S[0][2] * f[2]));
+        buf[((1 * NV + a) * NFP + ij) * E + el] = fma(S[1][0], f[0], fma(S[1][1], f[1], S[1][2] * f[2]));
+        const double fz = fma(S[2][0], f[0], fma(S[2][1], f[1], S[2][2] * f[2]));
+#pragma unroll
+        for (int kk = 0; kk < N; ++kk) acc[kk][a] = fma(op.Dh[kk * N + k], fz, acc[kk][a]);
+      }
     }
-    double *buf = sF + (NB == 2 ? (k & 1) : 0) * (2 * NV * NFP * E);
-    if (NB == 1 && k > 0) __syncthreads();  // the previous slice's contraction has finished reading sF
-#pragma unroll
-    for (int a = 0; a < NV; ++a) {
-      buf[((0 * NV + a) * NFP + ij) * E + el] = F[0][a];
-      buf[((1 * NV + a) * NFP + ij) * E + el] = F[1][a];
-    }
-    // z contraction: this point contributes to every point of its column
-#pragma unroll
-    for (int kk = 0; kk < N; ++kk)
-#pragma unroll
-      for (int a = 0; a < NV; ++a) acc[kk][a] = fma(op.Dh[kk * N + k], F[2][a], acc[kk][a]);
     __syncthreads();
     // every thread has consumed stage k&1: refill it with slice k+2
     if (tid == 0 && k + 2 < N) issue_stage(k & 1, k + 2);
+    if (NS && k + 1 < N) load_jz();
     // x and y contractions within the slice
 #pragma unroll
     for (int m = 0; m < N; ++m) {
@@ -260,6 +233,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   }
   if (!act) return;
   // lifting M3 D~ and the -1/J scale (Eq 19); faces: 0,1 = x-,x+ (idx j + N k); 2,3 = y (i + N k); 4,5 = z (i + N j)
+  const double gmi = sGm[i], gpi = sGp[i], gmj = sGm[j], gpj = sGp[j];
   double dzm[NV], dzp[NV];
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
@@ -288,6 +262,46 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 // ---------------------------------------------------------------------------------------------
 // k_hex_gradface
 // ---------------------------------------------------------------------------------------------
+// n . f_vis(u, q) (Eq 22-24) with the gradient fed one conserved variable at a time (getg(a, g) -> d_n u_a), so that
+// at most the velocity-gradient tensor is live: d_i v_j by the quotient rule, Delta dT = (mu gamma / Pr) d e (A8).
+template <typename GetG>
+__device__ __forceinline__ void visc_normal_stream(const double *u, const double *nrm, const Phys &ph, GetG getg, double *G) {
+  const double rrho = 1.0 / u[0], En = u[4];
+  double v[3], g0[3], dv[3][3], de[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) v[d] = u[1 + d] * rrho;
+#pragma unroll
+  for (int a = 0; a < NV; ++a) {
+    double g[3];
+    getg(a, g);
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+      if (a == 0) g0[n] = g[n];
+      else if (a < 4) dv[n][a - 1] = (g[n] - v[a - 1] * g0[n]) * rrho;
+      else de[n] = (g[n] - (En * rrho) * g0[n]) * rrho;
+    }
+  }
+  const double lam = -2.0 / 3.0 * ph.mu * (dv[0][0] + dv[1][1] + dv[2][2]);
+  const double kap = ph.mu * ph.gamma / ph.Pr;
+  double Tm[3][3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = 0; b < 3; ++b) Tm[a][b] = ph.mu * (dv[a][b] + dv[b][a]) + (a == b ? lam : 0.0);
+  G[0] = 0.0;
+#pragma unroll
+  for (int b = 0; b < 3; ++b) G[1 + b] = fma(nrm[0], Tm[0][b], fma(nrm[1], Tm[1][b], nrm[2] * Tm[2][b]));
+  double s = 0;
+#pragma unroll
+  for (int n = 0; n < 3; ++n) {
+    double d = de[n], vt = 0;
+#pragma unroll
+    for (int b = 0; b < 3; ++b) { d -= v[b] * dv[n][b]; vt += v[b] * Tm[b][n]; }
+    s = fma(nrm[n], vt + kap * d, s);
+  }
+  G[4] = s;
+}
+
 // G at one flux point from the interpolated state and gradient.  Interior: n . f_vis(u^f, q^f) with the
 // element's own outward normal (the pair kernel applies the LDG weights 1/2 +- beta, Eq 27).  Boundary:
 // the complete (1/2+beta) n.f_vis(u_L, q_L) + (1/2-beta) n.f_vis(B_ldg u_L, B_ldg q_L)  (App C, A20).
@@ -310,10 +324,13 @@ __device__ __forceinline__ void face_visc(const double *uf, const double (*qf)[N
 }
 
 // tmU, tmS, tmJ as above; tmR: rcpj as (ld, NFP, N), box (E, NFP, 1).
-template <int N, int E, bool BND, typename T, int MINB>
+// SQ: also store Q slice by slice (bulk tensor store of the shared-memory slice) for k_hex_fluxdiv_tma;
+// tmQ: Q workspace as (ld, NV*NFP, 3N), box (E, NV*NFP, 3): slice k, component n, variable a, point ij.
+template <int N, int E, bool BND, bool SQ, typename T, int MINB>
 __global__ void __launch_bounds__(N *N *E, MINB)
     k_hex_gradface(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS,
-                   const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmJ, Ops1D<N> op, Phys ph,
+                   const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmJ,
+                   const __grid_constant__ CUtensorMap tmQ, Ops1D<N> op, Phys ph,
                    const double *__restrict__ jump, const double *__restrict__ fp_n, const int32_t *__restrict__ fp_pe,
                    const BcDev *__restrict__ bcs, double *__restrict__ gf, int64_t ld, int64_t Nel) {
   using L = GfLay<N, E, T>;
@@ -322,6 +339,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   unsigned char *sm = smem_raw + ((128u - (smem_addr(smem_raw) & 127u)) & 127u);  // stays in the shared address space
   uint64_t *bar = (uint64_t *)(sm + L::BAR);
   double *sD = (double *)(sm + L::OPS), *sL = sD + N * N;  // sL[0][m] = l_m(-1), sL[1][m] = l_m(+1)
+  double *sGm = sL + 2 * N, *sGp = sGm + N;
   const T *sU = (const T *)(sm + L::U);
   unsigned char *sSt = sm + L::ST;
   double *sQ = (double *)(sm + L::Q);  // [3*NV][NFP][E]
@@ -336,7 +354,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     fence_proxy_async();
   }
   for (int t = tid; t < N * N; t += NFP * E) sD[t] = op.D[t];
-  for (int t = tid; t < N; t += NFP * E) { sL[t] = op.lm[t]; sL[N + t] = op.lp[t]; }
+  for (int t = tid; t < N; t += NFP * E) { sL[t] = op.lm[t]; sL[N + t] = op.lp[t]; sGm[t] = op.gm[t]; sGp[t] = op.gp[t]; }
   __syncthreads();
   auto issue_stage = [&](int s, int k) {
     mbar_expect_tx(&bar[1 + s], L::S_TX + L::R_TX + L::J_TX);
@@ -350,13 +368,9 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     issue_stage(0, 0);
     if (N > 1) issue_stage(1, 1);
   }
-  double jzm[NV], jzp[NV];
-#pragma unroll
-  for (int a = 0; a < NV; ++a) {
-    jzm[a] = jump[((size_t)(4 * NFP + ij) * NV + a) * ld + e];
-    jzp[a] = jump[((size_t)(5 * NFP + ij) * NV + a) * ld + e];
-  }
-  const double gmi = op.gm[i], gpi = op.gp[i], gmj = op.gm[j], gpj = op.gp[j];
+  // z-face jumps of this column: re-read from L2 in every slice, one variable ahead of their use
+  auto ldj = [&](int face, int a) { return ld_nc_once(jump + ((size_t)(face * NFP + ij) * NV + a) * ld + e); };
+  double jm_nx = ldj(4, 0), jp_nx = ldj(5, 0);
   double zm[3][NV], zp[3][NV];  // Q interpolated to the two z faces of this column
 #pragma unroll
   for (int n = 0; n < 3; ++n)
@@ -378,11 +392,14 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
         for (int b = 0; b < 3; ++b) S[a][b] = stS[((a * 3 + b) * NFP + ij) * E + el];
       const double rj = stR[ij * E + el];
+      const double gmi = sGm[i], gpi = sGp[i], gmj = sGm[j], gpj = sGp[j];
 #pragma unroll
       for (int a = 0; a < NV; ++a) {
         double qx = fma(gpi, stJ[((1 * N + j) * NV + a) * E + el], -gmi * stJ[((0 * N + j) * NV + a) * E + el]);
         double qy = fma(gpj, stJ[((3 * N + i) * NV + a) * E + el], -gmj * stJ[((2 * N + i) * NV + a) * E + el]);
-        double qz = fma(op.gp[k], jzp[a], -op.gm[k] * jzm[a]);
+        const double jm = jm_nx, jp = jp_nx;
+        if (a + 1 < NV) { jm_nx = ldj(4, a + 1); jp_nx = ldj(5, a + 1); }
+        double qz = fma(op.gp[k], jp, -op.gm[k] * jm);
 #pragma unroll
         for (int m = 0; m < N; ++m) {
           qx = fma(sD[i * N + m], (double)su[((j * N + m) * NV + a) * E], qx);
@@ -399,42 +416,61 @@ __global__ void __launch_bounds__(N *N *E, MINB)
         }
       }
     }
+    if (SQ) fence_proxy_async();  // make the sQ writes visible to the bulk store
     __syncthreads();  // Q of the slice is complete; stage k&1 has been consumed
     if (tid == 0 && k + 2 < N) issue_stage(k & 1, k + 2);
+    if (SQ && tid == 0) { tma_store_3d(&tmQ, e0, 0, 3 * k, sQ); tma_store_commit(); }
     // x / y faces of the slice: 4 N flux points per element, one thread each
     for (int t = ij; t < 4 * N; t += NFP) {
       const int f = t / N, m = t % N;
       const int base = f < 2 ? m * N : m, stride = f < 2 ? 1 : N;
       const double *lc = sL + (f & 1) * N;
       const int fp = f * NFP + m + N * k;
-      double nrm[3], uf[NV], qf[3][NV], G[NV];
+      double nrm[3], uf[NV], G[NV];
 #pragma unroll
       for (int n = 0; n < 3; ++n) nrm[n] = fp_n[((size_t)n * NF + fp) * ld + e];
-      const int pe = BND ? fp_pe[(size_t)fp * ld + e] : 0;
 #pragma unroll
       for (int a = 0; a < NV; ++a) uf[a] = 0.0;
 #pragma unroll
-      for (int n = 0; n < 3; ++n)
-#pragma unroll
-        for (int a = 0; a < NV; ++a) qf[n][a] = 0.0;
-#pragma unroll
       for (int mm = 0; mm < N; ++mm) {
         const double l = lc[mm];
-        const int pt = base + mm * stride;
 #pragma unroll
-        for (int a = 0; a < NV; ++a) uf[a] = fma(l, (double)su[(pt * NV + a) * E], uf[a]);
+        for (int a = 0; a < NV; ++a) uf[a] = fma(l, (double)su[((base + mm * stride) * NV + a) * E], uf[a]);
+      }
+      if constexpr (BND) {
+        const int pe = fp_pe[(size_t)fp * ld + e];
+        double qf[3][NV];
 #pragma unroll
         for (int n = 0; n < 3; ++n)
 #pragma unroll
-          for (int a = 0; a < NV; ++a) qf[n][a] = fma(l, sQ[((n * NV + a) * NFP + pt) * E + el], qf[n][a]);
+          for (int a = 0; a < NV; ++a) {
+            double q = 0;
+#pragma unroll
+            for (int mm = 0; mm < N; ++mm) q = fma(lc[mm], sQ[((n * NV + a) * NFP + base + mm * stride) * E + el], q);
+            qf[n][a] = q;
+          }
+        face_visc<BND>(uf, qf, nrm, ph, pe, bcs, G);
+      } else {
+        visc_normal_stream(uf, nrm, ph, [&](int a, double *g) {
+#pragma unroll
+          for (int n = 0; n < 3; ++n) {
+            double q = 0;
+#pragma unroll
+            for (int mm = 0; mm < N; ++mm) q = fma(lc[mm], sQ[((n * NV + a) * NFP + base + mm * stride) * E + el], q);
+            g[n] = q;
+          }
+        }, G);
       }
-      face_visc<BND>(uf, qf, nrm, ph, pe, bcs, G);
       if (act) {
 #pragma unroll
         for (int a = 0; a < NV; ++a) gf[((size_t)fp * NV + a) * ld + e] = G[a];
       }
     }
-    if (k + 1 < N) __syncthreads();  // before the next slice overwrites sQ
+    if (SQ && tid == 0) tma_store_wait_read();  // the bulk store has read sQ
+    if (k + 1 < N) {
+      jm_nx = ldj(4, 0); jp_nx = ldj(5, 0);
+      __syncthreads();  // before the next slice overwrites sQ
+    }
   }
   // z faces of the column
 #pragma unroll
@@ -451,7 +487,11 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
       for (int a = 0; a < NV; ++a)
         uf[a] = fma(s ? op.lp[m] : op.lm[m], (double)sU[((size_t)(NFP * m + ij) * NV + a) * E + el], uf[a]);
-    face_visc<BND>(uf, s ? zp : zm, nrm, ph, pe, bcs, G);
+    if constexpr (BND) face_visc<BND>(uf, s ? zp : zm, nrm, ph, pe, bcs, G);
+    else visc_normal_stream(uf, nrm, ph, [&](int a, double *g) {
+#pragma unroll
+      for (int n = 0; n < 3; ++n) g[n] = s ? zp[n][a] : zm[n][a];
+    }, G);
     if (act) {
 #pragma unroll
       for (int a = 0; a < NV; ++a) gf[((size_t)fp * NV + a) * ld + e] = G[a];
@@ -462,44 +502,13 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 // ---------------------------------------------------------------------------------------------
 // host side: tensor maps and launches
 // ---------------------------------------------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
-                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encoder() {
-  static EncodeTiledFn fn = [] {
-    void *p = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
-      p = nullptr;
-    return (EncodeTiledFn)p;
-  }();
-  return fn;
-}
-
-// 3-D view (d0 = elements (contiguous), d1 = rows, d2 = blocks of rows); strides in elements
-bool encode3(CUtensorMap *m, bool f64, const void *base, uint64_t d0, uint64_t d1, uint64_t d2, uint64_t s1, uint64_t s2, uint32_t b0,
-             uint32_t b1, uint32_t b2) {
-  EncodeTiledFn fn = encoder();
-  if (!fn) return false;
-  const uint64_t esz = f64 ? 8 : 4;
-  cuuint64_t dims[3] = {d0, d1, d2};
-  cuuint64_t strides[2] = {s1 * esz, s2 * esz};
-  cuuint32_t box[3] = {b0, b1, b2};
-  cuuint32_t estr[3] = {1, 1, 1};
-  CUresult r = fn(m, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void *>(base), dims, strides,
-                  box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  return r == CUDA_SUCCESS;
-}
-
 template <int N, int E>
 struct Maps {
-  CUtensorMap U, S, R, R1, J;
+  CUtensorMap U, S, R, R1, J, Q;
 };
 
 template <int N, int E, typename T>
-bool make_maps(const DevConsts &c, const void *u, const double *jump, Maps<N, E> &m, bool need_j) {
+bool make_maps(const DevConsts &c, const void *u, const double *jump, Maps<N, E> &m, bool need_j, const double *q = nullptr) {
   constexpr int NFP = N * N, NU = N * NFP;
   const uint64_t ld = (uint64_t)c.ld;
   bool ok = encode3(&m.U, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, N);
@@ -508,16 +517,9 @@ bool make_maps(const DevConsts &c, const void *u, const double *jump, Maps<N, E>
   ok = ok && encode3(&m.R1, true, c.rcpj, ld, NFP, N, ld, (uint64_t)NFP * ld, E, NFP, 1);
   if (need_j) ok = ok && encode3(&m.J, true, jump, ld, NFP * NV, 6, ld, (uint64_t)NFP * NV * ld, E, N * NV, 4);
   else m.J = m.R;
+  if (q) ok = ok && encode3(&m.Q, true, q, ld, NV * NFP, 3 * N, ld, (uint64_t)NV * NFP * ld, E, NV * NFP, 3);
+  else m.Q = m.R;
   return ok;
-}
-
-template <typename K>
-cudaError_t set_smem(K kern, size_t smem, bool &done) {
-  if (done) return cudaSuccess;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-  done = e == cudaSuccess;
-  return e;
 }
 
 template <int N, int E, bool NS, typename T, int CAP = 8>
@@ -542,44 +544,34 @@ cudaError_t launch_rhs(const DevConsts &c, const double *h_ops, const void *u, c
   return cudaGetLastError();
 }
 
+template <int N, int E, bool BND, bool SQ, typename T, int MINB>
+cudaError_t launch_gradface_k(const DevConsts &c, const Maps<N, E> &m, const Ops1D<N> &op, const double *jump, double *gf, cudaStream_t s) {
+  using L = GfLay<N, E, T>;
+  auto kern = k_hex_gradface<N, E, BND, SQ, T, MINB>;
+  static bool done = false;
+  cudaError_t err = set_smem(kern, L::TOTAL, done);
+  if (err != cudaSuccess) return err;
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.J, m.Q, op, c.ph, jump, c.fp_n, c.fp_pe, c.bcs, gf, c.ld,
+                                                                  c.Nel);
+  return cudaGetLastError();
+}
+
 template <int N, int E, typename T, int CAP = 8>
-cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, cudaStream_t s) {
+cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, double *q,
+                            cudaStream_t s) {
   using L = GfLay<N, E, T>;
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
   constexpr int MINB = min_blocks(L::TOTAL, N * N * E) < CAP ? min_blocks(L::TOTAL, N * N * E) : CAP;
   Maps<N, E> m;
-  if (!make_maps<N, E, T>(c, u, jump, m, true)) return cudaErrorNotSupported;
+  if (!make_maps<N, E, T>(c, u, jump, m, true, q)) return cudaErrorNotSupported;
   const Ops1D<N> op = make_ops<N>(h_ops);
-  const unsigned grid = (unsigned)((c.Nel + E - 1) / E);
-  cudaError_t err;
-  if (c.nbnd) {
-    auto kern = k_hex_gradface<N, E, true, T, MINB>;
-    static bool done = false;
-    if ((err = set_smem(kern, L::TOTAL, done)) != cudaSuccess) return err;
-    kern<<<grid, N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.J, op, c.ph, jump, c.fp_n, c.fp_pe, c.bcs, gf, c.ld, c.Nel);
-  } else {
-    auto kern = k_hex_gradface<N, E, false, T, MINB>;
-    static bool done = false;
-    if ((err = set_smem(kern, L::TOTAL, done)) != cudaSuccess) return err;
-    kern<<<grid, N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.J, op, c.ph, jump, c.fp_n, c.fp_pe, c.bcs, gf, c.ld, c.Nel);
-  }
-  return cudaGetLastError();
+  if (c.nbnd) return q ? launch_gradface_k<N, E, true, true, T, MINB>(c, m, op, jump, gf, s) : launch_gradface_k<N, E, true, false, T, MINB>(c, m, op, jump, gf, s);
+  return q ? launch_gradface_k<N, E, false, true, T, MINB>(c, m, op, jump, gf, s) : launch_gradface_k<N, E, false, false, T, MINB>(c, m, op, jump, gf, s);
 }
-
-// elements per CTA for each n = p + 1 (row segments of E*8 bytes)
-template <int N>
-struct Cfg {
-  static constexpr int E = N <= 2 ? 32 : (N == 3 ? 16 : 8);
-};
 
 template <int N, typename T>
 constexpr bool fits() {
   return GfLay<N, Cfg<N>::E, T>::TOTAL <= SMEM_MAX && RhsLay<N, Cfg<N>::E, true, T, 1>::TOTAL <= SMEM_MAX && N * N * Cfg<N>::E <= 1024;
-}
-
-int env_e() {
-  static const int v = getenv("FR_TMA_E") ? atoi(getenv("FR_TMA_E")) : 0;
-  return v;
 }
 
 template <int N, typename T>
@@ -598,14 +590,14 @@ cudaError_t rhs_n(const DevConsts &c, const double *h_ops, const void *u, const 
 }
 
 template <int N, typename T>
-cudaError_t gradface_n(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, cudaStream_t s) {
+cudaError_t gradface_n(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, double *q, cudaStream_t s) {
   if constexpr (fits<N, T>()) {
     if constexpr (N == 5 && sizeof(T) == 8) {
-      if (env_e() == 16) return launch_gradface<N, 16, T>(c, h_ops, u, jump, gf, s);
-      if (env_e() == 12) return launch_gradface<N, 12, T>(c, h_ops, u, jump, gf, s);
-      if (env_e() == 81) return launch_gradface<N, 8, T, 1>(c, h_ops, u, jump, gf, s);
+      if (env_e() == 16) return launch_gradface<N, 16, T>(c, h_ops, u, jump, gf, q, s);
+      if (env_e() == 12) return launch_gradface<N, 12, T>(c, h_ops, u, jump, gf, q, s);
+      if (env_e() == 81) return launch_gradface<N, 8, T, 1>(c, h_ops, u, jump, gf, q, s);
     }
-    return launch_gradface<N, Cfg<N>::E, T>(c, h_ops, u, jump, gf, s);
+    return launch_gradface<N, Cfg<N>::E, T>(c, h_ops, u, jump, gf, q, s);
   } else {
     return cudaErrorNotSupported;
   }
@@ -634,9 +626,10 @@ cudaError_t hex_tma_rhs(const DevConsts &c, const double *h_ops, const void *u, 
   }
 }
 
-cudaError_t hex_tma_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, cudaStream_t s) {
+cudaError_t hex_tma_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, double *q,
+                             cudaStream_t s) {
   switch (c.n) {
-#define FR_CASE(NN) case NN: return c.f64 ? gradface_n<NN, double>(c, h_ops, u, jump, gf, s) : gradface_n<NN, float>(c, h_ops, u, jump, gf, s);
+#define FR_CASE(NN) case NN: return c.f64 ? gradface_n<NN, double>(c, h_ops, u, jump, gf, q, s) : gradface_n<NN, float>(c, h_ops, u, jump, gf, q, s);
     FR_CASE(2) FR_CASE(3) FR_CASE(4) FR_CASE(5) FR_CASE(6) FR_CASE(7)
 #undef FR_CASE
     default: return cudaErrorNotSupported;

@@ -7,8 +7,15 @@ namespace fr {
 // true when the sm_100a TMA kernels can run this n = p+1 / precision (shared memory fits, driver exposes the encoder)
 bool hex_tma_supported(int n, bool f64);
 
-// G^f = n . f_vis(U^f, Q^f) at every flux point, Q recomputed from u and jump = C - U^f  (parts 2b, 3 of the north_star)
-cudaError_t hex_tma_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, cudaStream_t s);
+// G^f = n . f_vis(U^f, Q^f) at every flux point, Q computed from u and jump = C - U^f  (parts 2b, 3 of the north_star);
+// q != NULL: Q is also stored, slice-major [N][3][NV][NFP][ld], for hex_tma_fluxdiv
+cudaError_t hex_tma_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, double *q,
+                             cudaStream_t s);
+
+// rhs = -(1/J) {(M1 - M3 M2) S f(U, Q) + M3 D~} with Q read back (fr_hex_fluxdiv_tma.cu); Euler: q unused
+cudaError_t hex_tma_fluxdiv(const DevConsts &c, const double *h_ops, const void *u, const double *q, const double *dt, void *rhs,
+                            cudaStream_t s);
+bool hex_tma_fluxdiv_supported(int n, bool f64);
 
 // rhs = -(1/J) {(M1 - M3 M2) S f(U, Q) + M3 D~}  (parts 4, 6, 7; Q recomputed for Navier-Stokes)
 cudaError_t hex_tma_rhs(const DevConsts &c, const double *h_ops, const void *u, const double *jump, const double *dt, void *rhs,

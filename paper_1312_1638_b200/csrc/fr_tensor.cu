@@ -203,13 +203,13 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
   FR_MARK(prof, "tp_interp");
   k_tp_interp<N, ND, T><<<dim3(gx, 1, 1), bf, 0, s>>>(op, u, uf, ncols, c.ld, c.Nel, 0, 0);
   if (ND == 3 && tp.use_tma) {
-    // sm_100a path: 5 launches for Navier-Stokes (3 for Euler); neither Q nor Q^f nor F~ is stored
+    // sm_100a path: 5 launches for Navier-Stokes (3 for Euler); neither Q^f nor F~ is stored
     cudaError_t e = cudaSuccess;
     if (c.ns) {
       FR_MARK(prof, "common_sol");
       launch_common_jump(c, uf, cf, s);
       FR_MARK(prof, "hex_gradface");
-      e = hex_tma_gradface(c, tp.h_ops, u, cf, qu, s);
+      e = hex_tma_gradface(c, tp.h_ops, u, cf, qu, tp.tma_q ? qf : nullptr, s);
       if (e != cudaSuccess) return e;
       FR_MARK(prof, "common_flux_g");
       launch_common_flux_g(c, uf, qu, s);
@@ -217,8 +217,13 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
       FR_MARK(prof, "common_flux");
       launch_common_flux(c, uf, qf, s);
     }
-    FR_MARK(prof, "hex_rhs_tma");
-    e = hex_tma_rhs(c, tp.h_ops, u, cf, uf, rhs, s);
+    if (tp.tma_q) {
+      FR_MARK(prof, "hex_fluxdiv_tma");
+      e = hex_tma_fluxdiv(c, tp.h_ops, u, qf, uf, rhs, s);
+    } else {  // Q recomputed from the jumps instead of being read back
+      FR_MARK(prof, "hex_rhs_tma");
+      e = hex_tma_rhs(c, tp.h_ops, u, cf, uf, rhs, s);
+    }
     return e != cudaSuccess ? e : cudaGetLastError();
   }
   if (c.ns) {
@@ -292,9 +297,10 @@ cudaError_t tensor_plan(const DevConsts &c, const RefOps &o, const MeshConsts &,
   tp.off_uf = off; off = al(off + (int64_t)o.Nf * ncols * 8);
   tp.off_cf = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
   tp.use_tma = c.etype == FR_HEX && hex_tma_supported(c.n, c.f64);
-  if (tp.use_tma) {  // only G^f besides U^f and the jumps
+  tp.tma_q = tp.use_tma && hex_tma_fluxdiv_supported(c.n, c.f64) && !getenv("FR_TMA_RECOMPUTE");
+  if (tp.use_tma) {  // G^f (and Q, slice-major) besides U^f and the jumps
     tp.off_qu = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
-    tp.off_qf = off;
+    tp.off_qf = off; if (c.ns && tp.tma_q) off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
   } else {
     tp.off_qu = off; off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
     tp.off_qf = off; if (c.ns) off = al(off + (int64_t)o.nd * o.Nf * ncols * 8);

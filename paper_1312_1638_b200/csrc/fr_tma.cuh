@@ -1,0 +1,139 @@
+// Shared pieces of the TMA-pipelined hexahedral kernels (fr_hex_tma.cu, fr_hex_fluxdiv_tma.cu): PTX wrappers for
+// mbarriers and bulk tensor copies (sm_100a), the tensor-map encoder fetched through the runtime, launch helpers.
+#pragma once
+#include <cuda.h>  // CUtensorMap and its enums (types only: the encoder is fetched through the runtime)
+
+#include <cstdint>
+#include <cstdlib>
+
+#include "fr_hex_tma.hpp"
+#include "fr_ops1d.cuh"
+
+namespace fr {
+namespace {
+
+constexpr int NV = 5;
+constexpr size_t SMEM_MAX = 227 * 1024;
+
+__host__ __device__ constexpr size_t al128(size_t x) { return (x + 127) / 128 * 128; }
+
+// ---------------------------------------------------------------------------------------------
+// PTX wrappers: mbarrier + bulk tensor copies
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  const uint32_t a = smem_addr(bar);
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(a), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+// global load that the compiler may neither merge with an earlier load of the same address nor hoist
+__device__ __forceinline__ double ld_nc_once(const double *p) {
+  double v;
+  asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, uint64_t *bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+          smem_addr(dst)),
+      "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_addr(bar))
+      : "memory");
+}
+
+// bulk tensor store shared -> global (bulk async-group completion)
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap *tm, int c0, int c1, int c2, const void *src) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(tm), "r"(c0), "r"(c1), "r"(c2),
+               "r"(smem_addr(src))
+               : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+
+// resident CTAs per SM the kernel is compiled for: limited by shared memory, by >= 128 registers per thread
+constexpr int min_blocks(size_t smem, int threads) {
+  int by_smem = (int)((SMEM_MAX + 1024) / (smem + 1024));
+  int warps = (threads + 31) / 32;
+  int by_regs = 65536 / (128 * 32 * warps);
+  int by_thr = 2048 / (32 * warps);
+  int m = by_smem < by_regs ? by_smem : by_regs;
+  m = m < by_thr ? m : by_thr;
+  return m < 1 ? 1 : (m > 8 ? 8 : m);
+}
+
+// Q~ -> Q at one solution point for variable a:  q_n = (1/J) sum_i S[i][n] q~_i   (Eq 10 :206)
+__device__ __forceinline__ void to_physical(const double (*S)[3], double rj, double qx, double qy, double qz, double *q) {
+#pragma unroll
+  for (int n = 0; n < 3; ++n) q[n] = rj * fma(S[0][n], qx, fma(S[1][n], qy, S[2][n] * qz));
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encoder() {
+  static EncodeTiledFn fn = [] {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return (EncodeTiledFn)p;
+  }();
+  return fn;
+}
+
+// 3-D view (d0 = elements (contiguous), d1 = rows, d2 = blocks of rows); strides in elements
+bool encode3(CUtensorMap *m, bool f64, const void *base, uint64_t d0, uint64_t d1, uint64_t d2, uint64_t s1, uint64_t s2, uint32_t b0,
+             uint32_t b1, uint32_t b2) {
+  EncodeTiledFn fn = encoder();
+  if (!fn) return false;
+  const uint64_t esz = f64 ? 8 : 4;
+  cuuint64_t dims[3] = {d0, d1, d2};
+  cuuint64_t strides[2] = {s1 * esz, s2 * esz};
+  cuuint32_t box[3] = {b0, b1, b2};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = fn(m, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void *>(base), dims, strides,
+                  box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
+template <typename K>
+cudaError_t set_smem(K kern, size_t smem, bool &done) {
+  if (done) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  done = e == cudaSuccess;
+  return e;
+}
+
+// elements per CTA for each n = p + 1 (row segments of E*8 bytes)
+template <int N>
+struct Cfg {
+  static constexpr int E = N <= 2 ? 32 : (N == 3 ? 16 : 8);
+};
+
+int env_e() {
+  static const int v = getenv("FR_TMA_E") ? atoi(getenv("FR_TMA_E")) : 0;
+  return v;
+}
+
+}  // namespace
+}  // namespace fr
