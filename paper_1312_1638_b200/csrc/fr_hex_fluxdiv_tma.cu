@@ -22,14 +22,22 @@ struct FdLay {
   static constexpr size_t F = ST + 2 * ST_BYTES;
   static constexpr size_t F_BYTES = 2 * NV * NFP * E * 8;
   static constexpr size_t TOTAL = F + NB * F_BYTES + 128;  // + slack for the manual 128-byte alignment
+  // epilogue operands by TMA into the stage buffers once they are free: D~ of the x/y faces + 1/J, D~ of the z faces
+  static constexpr uint32_t DXY_TX = 4 * NFP * NV * E * 8, RJ_TX = NU * E * 8, DZ_TX = 2 * NFP * NV * E * 8;
+  static constexpr size_t EP_RJ = al128(DXY_TX);
+  static constexpr bool EPI_TMA = N >= 2 && EP_RJ + RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
 };
 
 // tmS: smat as (ld, NU, 9), box (E, NFP, 9);  tmU: u as (ld, NFP*NV, N), box (E, NFP*NV, 1);
 // tmQ: Q workspace as (ld, NV*NFP, 3N), box (E, NV*NFP, 3)  (slice-major layout written by k_hex_gradface).
+// Epilogue operands (when they fit the stage buffers): tmD4 / tmD2: D~ as (ld, NFP*NV, 6), boxes (E, NFP*NV, 4) / (E, NFP*NV, 2);
+// tmR: rcpj as (ld, NFP, N), box (E, NFP, N).
 template <int N, int E, bool NS, typename T, int NB, int MINB>
 __global__ void __launch_bounds__(N *N *E, MINB)
     k_hex_fluxdiv_tma(const __grid_constant__ CUtensorMap tmS, const __grid_constant__ CUtensorMap tmU,
-                      const __grid_constant__ CUtensorMap tmQ, Ops1D<N> op, Phys ph, const double *__restrict__ rcpj,
+                      const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmD4,
+                      const __grid_constant__ CUtensorMap tmD2, const __grid_constant__ CUtensorMap tmR, Ops1D<N> op, Phys ph,
+                      const double *__restrict__ rcpj,
                       const double *__restrict__ dt, T *__restrict__ rhs, int64_t ld, int64_t Nel) {
   using L = FdLay<N, E, NS, T, NB>;
   constexpr int NFP = N * N;
@@ -45,7 +53,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   const bool act = e < Nel;
 
   if (tid == 0) {
-    mbar_init(&bar[0], 1); mbar_init(&bar[1], 1);
+    mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); mbar_init(&bar[2], 1); mbar_init(&bar[3], 1);
     fence_barrier_init();
     fence_proxy_async();
   }
@@ -137,6 +145,15 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     __syncthreads();
     // every thread has consumed stage k&1: refill it with slice k+2
     if (tid == 0 && k + 2 < N) issue_stage(k & 1, k + 2);
+    if (L::EPI_TMA && tid == 0 && k == N - 2) {  // this stage is not refilled any more: bring D~ (x/y faces) and 1/J
+      mbar_expect_tx(&bar[2], L::DXY_TX + L::RJ_TX);
+      tma_load_3d(sSt + (k & 1) * L::ST_BYTES, &tmD4, e0, 0, 0, &bar[2]);
+      tma_load_3d(sSt + (k & 1) * L::ST_BYTES + L::EP_RJ, &tmR, e0, 0, 0, &bar[2]);
+    }
+    if (L::EPI_TMA && tid == 0 && k == N - 1) {  // D~ of the z faces
+      mbar_expect_tx(&bar[3], L::DZ_TX);
+      tma_load_3d(sSt + (k & 1) * L::ST_BYTES, &tmD2, e0, 0, 4, &bar[3]);
+    }
     // x and y contractions within the slice
 #pragma unroll
     for (int m = 0; m < N; ++m) {
@@ -148,9 +165,35 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       }
     }
   }
-  if (!act) return;
   // lifting M3 D~ and the -1/J scale (Eq 19); faces: 0,1 = x-,x+ (idx j + N k); 2,3 = y (i + N k); 4,5 = z (i + N j)
   const double gmi = sGm[i], gpi = sGp[i], gmj = sGm[j], gpj = sGp[j];
+  if (L::EPI_TMA) {
+    const double *sDxy = (const double *)(sSt + ((N - 2) & 1) * L::ST_BYTES);           // [4][NFP*NV][E]
+    const double *sRJ = (const double *)(sSt + ((N - 2) & 1) * L::ST_BYTES + L::EP_RJ);  // [NU][E]
+    const double *sDz = (const double *)(sSt + ((N - 1) & 1) * L::ST_BYTES);           // [2][NFP*NV][E]
+    mbar_wait(&bar[2], 0);
+    mbar_wait(&bar[3], 0);
+    if (!act) return;
+#pragma unroll
+    for (int k = 0; k < N; ++k) {
+      const int r = ij + NFP * k;
+      const double rj = sRJ[r * E + el];
+      const int fx = j + N * k, fy = i + N * k;
+#pragma unroll
+      for (int a = 0; a < NV; ++a) {
+        double v = acc[k][a];
+        v = fma(op.gm[k], sDz[((0 * NFP + ij) * NV + a) * E + el], v);
+        v = fma(op.gp[k], sDz[((1 * NFP + ij) * NV + a) * E + el], v);
+        v = fma(gmi, sDxy[((0 * NFP + fx) * NV + a) * E + el], v);
+        v = fma(gpi, sDxy[((1 * NFP + fx) * NV + a) * E + el], v);
+        v = fma(gmj, sDxy[((2 * NFP + fy) * NV + a) * E + el], v);
+        v = fma(gpj, sDxy[((3 * NFP + fy) * NV + a) * E + el], v);
+        rhs[((size_t)r * NV + a) * ld + e] = (T)(-v * rj);
+      }
+    }
+    return;
+  }
+  if (!act) return;
   double dzm[NV], dzp[NV];
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
@@ -188,18 +231,22 @@ cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
   constexpr int MINB = min_blocks(L::TOTAL, N * N * E) < CAP ? min_blocks(L::TOTAL, N * N * E) : CAP;
   const uint64_t ld = (uint64_t)c.ld;
-  CUtensorMap mS, mU, mQ;
+  CUtensorMap mS, mU, mQ, mD4, mD2, mR;
   bool ok = encode3(&mS, true, c.smat, ld, NU, 9, ld, (uint64_t)NU * ld, E, NFP, 9);
   ok = ok && encode3(&mU, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 1);
   if (NS) ok = ok && encode3(&mQ, true, q, ld, NV * NFP, 3 * N, ld, (uint64_t)NV * NFP * ld, E, NV * NFP, 3);
   else mQ = mS;
+  ok = ok && encode3(&mD4, true, dt, ld, NFP * NV, 6, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 4);
+  ok = ok && encode3(&mD2, true, dt, ld, NFP * NV, 6, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 2);
+  ok = ok && encode3(&mR, true, c.rcpj, ld, NFP, N, ld, (uint64_t)NFP * ld, E, NFP, N);
   if (!ok) return cudaErrorNotSupported;
   auto kern = k_hex_fluxdiv_tma<N, E, NS, T, NB, MINB>;
   static bool done = false;
   cudaError_t err = set_smem(kern, L::TOTAL, done);
   if (err != cudaSuccess) return err;
   const Ops1D<N> op = make_ops<N>(h_ops);
-  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(mS, mU, mQ, op, c.ph, c.rcpj, dt, (T *)rhs, c.ld, c.Nel);
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(mS, mU, mQ, mD4, mD2, mR, op, c.ph, c.rcpj, dt, (T *)rhs, c.ld,
+                                                                  c.Nel);
   return cudaGetLastError();
 }
 
