@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
         for (int a = 0; a < NV; ++a)
 #pragma unroll
           for (int n = 0; n < 3; ++n) {
-            const double g = stQ[((n * NV + a) * NFP + ij) * E + el];
+            const double g = stQ[((n * NFP + ij) * NV + a) * E + el];
             if (a == 0) g0[n] = g;
             else if (a < 4) dv[n][a - 1] = (g - v[a - 1] * g0[n]) * rrho;  // d_n v_j by the quotient rule
             else de[n] = (g - (En * rrho) * g0[n]) * rrho;
@@ -260,6 +260,7 @@ cudaError_t fluxdiv_n(const DevConsts &c, const double *h_ops, const void *u, co
   if constexpr (fd_fits<N, T>()) {
     if constexpr (N == 5 && sizeof(T) == 8) {  // tuning variants (FR_TMA_E = 16 | 81 (E = 8, one CTA per SM))
       if (env_e() == 16) return c.ns ? launch_fluxdiv<N, 16, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, 16, false, T>(c, h_ops, u, q, dt, rhs, s);
+      if (env_e() == 4) return c.ns ? launch_fluxdiv<N, 4, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, 4, false, T>(c, h_ops, u, q, dt, rhs, s);
       if (env_e() == 81) return c.ns ? launch_fluxdiv<N, 8, true, T, 1>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, 8, false, T, 1>(c, h_ops, u, q, dt, rhs, s);
     }
     constexpr int E = Cfg<N>::E;

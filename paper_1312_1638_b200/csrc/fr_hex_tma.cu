@@ -262,67 +262,6 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 // ---------------------------------------------------------------------------------------------
 // k_hex_gradface
 // ---------------------------------------------------------------------------------------------
-// n . f_vis(u, q) (Eq 22-24) with the gradient fed one conserved variable at a time (getg(a, g) -> d_n u_a), so that
-// at most the velocity-gradient tensor is live: d_i v_j by the quotient rule, Delta dT = (mu gamma / Pr) d e (A8).
-template <typename GetG>
-__device__ __forceinline__ void visc_normal_stream(const double *u, const double *nrm, const Phys &ph, GetG getg, double *G) {
-  const double rrho = 1.0 / u[0], En = u[4];
-  double v[3], g0[3], dv[3][3], de[3];
-#pragma unroll
-  for (int d = 0; d < 3; ++d) v[d] = u[1 + d] * rrho;
-#pragma unroll
-  for (int a = 0; a < NV; ++a) {
-    double g[3];
-    getg(a, g);
-#pragma unroll
-    for (int n = 0; n < 3; ++n) {
-      if (a == 0) g0[n] = g[n];
-      else if (a < 4) dv[n][a - 1] = (g[n] - v[a - 1] * g0[n]) * rrho;
-      else de[n] = (g[n] - (En * rrho) * g0[n]) * rrho;
-    }
-  }
-  const double lam = -2.0 / 3.0 * ph.mu * (dv[0][0] + dv[1][1] + dv[2][2]);
-  const double kap = ph.mu * ph.gamma / ph.Pr;
-  double Tm[3][3];
-#pragma unroll
-  for (int a = 0; a < 3; ++a)
-#pragma unroll
-    for (int b = 0; b < 3; ++b) Tm[a][b] = ph.mu * (dv[a][b] + dv[b][a]) + (a == b ? lam : 0.0);
-  G[0] = 0.0;
-#pragma unroll
-  for (int b = 0; b < 3; ++b) G[1 + b] = fma(nrm[0], Tm[0][b], fma(nrm[1], Tm[1][b], nrm[2] * Tm[2][b]));
-  double s = 0;
-#pragma unroll
-  for (int n = 0; n < 3; ++n) {
-    double d = de[n], vt = 0;
-#pragma unroll
-    for (int b = 0; b < 3; ++b) { d -= v[b] * dv[n][b]; vt += v[b] * Tm[b][n]; }
-    s = fma(nrm[n], vt + kap * d, s);
-  }
-  G[4] = s;
-}
-
-// G at one flux point from the interpolated state and gradient.  Interior: n . f_vis(u^f, q^f) with the
-// element's own outward normal (the pair kernel applies the LDG weights 1/2 +- beta, Eq 27).  Boundary:
-// the complete (1/2+beta) n.f_vis(u_L, q_L) + (1/2-beta) n.f_vis(B_ldg u_L, B_ldg q_L)  (App C, A20).
-template <bool BND>
-__device__ __forceinline__ void face_visc(const double *uf, const double (*qf)[NV], const double *nrm, const Phys &ph, int pe,
-                                          const BcDev *__restrict__ bcs, double *G) {
-  normal_viscous_flux<3>(uf, qf, nrm, ph, G);
-  if (BND && pe < 0) {
-    double gi[NV], gl[NV], qg[3][NV], GR[NV];
-    const double keep = ghost_states<3>(bcs[-1 - pe], uf, ph.gamma, gi, gl);
-#pragma unroll
-    for (int n = 0; n < 3; ++n)
-#pragma unroll
-      for (int a = 0; a < NV; ++a) qg[n][a] = keep * qf[n][a];
-    normal_viscous_flux<3>(gl, qg, nrm, ph, GR);
-    const double wl = 0.5 + ph.beta, wr = 0.5 - ph.beta;
-#pragma unroll
-    for (int a = 0; a < NV; ++a) G[a] = (wl != 0.0 ? wl * G[a] : 0.0) + (wr != 0.0 ? wr * GR[a] : 0.0);
-  }
-}
-
 // tmU, tmS, tmJ as above; tmR: rcpj as (ld, NFP, N), box (E, NFP, 1).
 // SQ: also store Q slice by slice (bulk tensor store of the shared-memory slice) for k_hex_fluxdiv_tma;
 // tmQ: Q workspace as (ld, NV*NFP, 3N), box (E, NV*NFP, 3): slice k, component n, variable a, point ij.
@@ -342,7 +281,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   double *sGm = sL + 2 * N, *sGp = sGm + N;
   const T *sU = (const T *)(sm + L::U);
   unsigned char *sSt = sm + L::ST;
-  double *sQ = (double *)(sm + L::Q);  // [3*NV][NFP][E]
+  double *sQ = (double *)(sm + L::Q);  // [3][NFP][NV][E]
   const int tid = threadIdx.x, el = tid % E, ij = tid / E, i = ij % N, j = ij / N;
   const int e0 = blockIdx.x * E;
   const int64_t e = (int64_t)e0 + el;
@@ -410,7 +349,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
         to_physical(S, rj, qx, qy, qz, q3);
 #pragma unroll
         for (int n = 0; n < 3; ++n) {
-          sQ[((n * NV + a) * NFP + ij) * E + el] = q3[n];
+          sQ[((n * NFP + ij) * NV + a) * E + el] = q3[n];
           zm[n][a] = fma(op.lm[k], q3[n], zm[n][a]);
           zp[n][a] = fma(op.lp[k], q3[n], zp[n][a]);
         }
@@ -446,7 +385,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
           for (int a = 0; a < NV; ++a) {
             double q = 0;
 #pragma unroll
-            for (int mm = 0; mm < N; ++mm) q = fma(lc[mm], sQ[((n * NV + a) * NFP + base + mm * stride) * E + el], q);
+            for (int mm = 0; mm < N; ++mm) q = fma(lc[mm], sQ[((n * NFP + base + mm * stride) * NV + a) * E + el], q);
             qf[n][a] = q;
           }
         face_visc<BND>(uf, qf, nrm, ph, pe, bcs, G);
@@ -456,7 +395,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
           for (int n = 0; n < 3; ++n) {
             double q = 0;
 #pragma unroll
-            for (int mm = 0; mm < N; ++mm) q = fma(lc[mm], sQ[((n * NV + a) * NFP + base + mm * stride) * E + el], q);
+            for (int mm = 0; mm < N; ++mm) q = fma(lc[mm], sQ[((n * NFP + base + mm * stride) * NV + a) * E + el], q);
             g[n] = q;
           }
         }, G);
@@ -596,6 +535,7 @@ cudaError_t gradface_n(const DevConsts &c, const double *h_ops, const void *u, c
       if (env_e() == 16) return launch_gradface<N, 16, T>(c, h_ops, u, jump, gf, q, s);
       if (env_e() == 12) return launch_gradface<N, 12, T>(c, h_ops, u, jump, gf, q, s);
       if (env_e() == 81) return launch_gradface<N, 8, T, 1>(c, h_ops, u, jump, gf, q, s);
+      if (env_e() == 4) return launch_gradface<N, 4, T>(c, h_ops, u, jump, gf, q, s);
     }
     return launch_gradface<N, Cfg<N>::E, T>(c, h_ops, u, jump, gf, q, s);
   } else {
