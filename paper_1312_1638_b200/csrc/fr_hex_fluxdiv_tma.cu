@@ -21,11 +21,16 @@ struct FdLay {
   static constexpr size_t ST_BYTES = ST_Q + al128(Q_TX);
   static constexpr size_t F = ST + 2 * ST_BYTES;
   static constexpr size_t F_BYTES = 2 * NV * NFP * E * 8;
-  static constexpr size_t TOTAL = F + NB * F_BYTES + 128;  // + slack for the manual 128-byte alignment
-  // epilogue operands by TMA into the stage buffers once they are free: D~ of the x/y faces + 1/J, D~ of the z faces
+  // epilogue operands by TMA: D~ of the x/y faces, 1/J, D~ of the z faces.  EPI_ST: all into the stage buffers once they
+  // are free (Navier-Stokes: the stages are large).  EPI_DED: the stages are too small for D~ of the x/y faces (Euler), which
+  // gets a buffer of its own, loaded at kernel start; 1/J and the z faces still reuse the freed stages.
   static constexpr uint32_t DXY_TX = 4 * NFP * NV * E * 8, RJ_TX = NU * E * 8, DZ_TX = 2 * NFP * NV * E * 8;
   static constexpr size_t EP_RJ = al128(DXY_TX);
-  static constexpr bool EPI_TMA = N >= 2 && EP_RJ + RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
+  static constexpr bool EPI_ST = N >= 2 && EP_RJ + RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
+  static constexpr bool EPI_DED = N >= 2 && !EPI_ST && RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
+  static constexpr bool EPI_TMA = EPI_ST || EPI_DED;
+  static constexpr size_t DED = F + NB * F_BYTES;
+  static constexpr size_t TOTAL = DED + (EPI_DED ? al128(DXY_TX) : 0) + 128;  // + slack for the manual 128-byte alignment
 };
 
 // tmS: smat as (ld, NU, 9), box (E, NFP, 9);  tmU: u as (ld, NFP*NV, N), box (E, NFP*NV, 1);
@@ -53,7 +58,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   const bool act = e < Nel;
 
   if (tid == 0) {
-    mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); mbar_init(&bar[2], 1); mbar_init(&bar[3], 1);
+    mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); mbar_init(&bar[2], 1); mbar_init(&bar[3], 1); mbar_init(&bar[4], 1);
     fence_barrier_init();
     fence_proxy_async();
   }
@@ -69,6 +74,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   if (tid == 0) {
     issue_stage(0, 0);
     if (N > 1) issue_stage(1, 1);
+    if (L::EPI_DED) { mbar_expect_tx(&bar[2], L::DXY_TX); tma_load_3d(sm + L::DED, &tmD4, e0, 0, 0, &bar[2]); }
   }
   double acc[N][NV];
 #pragma unroll
@@ -145,10 +151,15 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     __syncthreads();
     // every thread has consumed stage k&1: refill it with slice k+2
     if (tid == 0 && k + 2 < N) issue_stage(k & 1, k + 2);
-    if (L::EPI_TMA && tid == 0 && k == N - 2) {  // this stage is not refilled any more: bring D~ (x/y faces) and 1/J
-      mbar_expect_tx(&bar[2], L::DXY_TX + L::RJ_TX);
+    if (L::EPI_ST && tid == 0 && k == N - 2) {  // this stage is not refilled any more: bring D~ (x/y faces) and 1/J
+      mbar_expect_tx(&bar[2], L::DXY_TX);
       tma_load_3d(sSt + (k & 1) * L::ST_BYTES, &tmD4, e0, 0, 0, &bar[2]);
-      tma_load_3d(sSt + (k & 1) * L::ST_BYTES + L::EP_RJ, &tmR, e0, 0, 0, &bar[2]);
+      mbar_expect_tx(&bar[4], L::RJ_TX);
+      tma_load_3d(sSt + (k & 1) * L::ST_BYTES + L::EP_RJ, &tmR, e0, 0, 0, &bar[4]);
+    }
+    if (L::EPI_DED && tid == 0 && k == N - 2) {
+      mbar_expect_tx(&bar[4], L::RJ_TX);
+      tma_load_3d(sSt + (k & 1) * L::ST_BYTES, &tmR, e0, 0, 0, &bar[4]);
     }
     if (L::EPI_TMA && tid == 0 && k == N - 1) {  // D~ of the z faces
       mbar_expect_tx(&bar[3], L::DZ_TX);
@@ -168,11 +179,12 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   // lifting M3 D~ and the -1/J scale (Eq 19); faces: 0,1 = x-,x+ (idx j + N k); 2,3 = y (i + N k); 4,5 = z (i + N j)
   const double gmi = sGm[i], gpi = sGp[i], gmj = sGm[j], gpj = sGp[j];
   if (L::EPI_TMA) {
-    const double *sDxy = (const double *)(sSt + ((N - 2) & 1) * L::ST_BYTES);           // [4][NFP*NV][E]
-    const double *sRJ = (const double *)(sSt + ((N - 2) & 1) * L::ST_BYTES + L::EP_RJ);  // [NU][E]
-    const double *sDz = (const double *)(sSt + ((N - 1) & 1) * L::ST_BYTES);           // [2][NFP*NV][E]
+    const double *sDxy = (const double *)(L::EPI_DED ? sm + L::DED : sSt + ((N - 2) & 1) * L::ST_BYTES);  // [4][NFP*NV][E]
+    const double *sRJ = (const double *)(sSt + ((N - 2) & 1) * L::ST_BYTES + (L::EPI_DED ? 0 : L::EP_RJ));  // [NU][E]
+    const double *sDz = (const double *)(sSt + ((N - 1) & 1) * L::ST_BYTES);                               // [2][NFP*NV][E]
     mbar_wait(&bar[2], 0);
     mbar_wait(&bar[3], 0);
+    mbar_wait(&bar[4], 0);
     if (!act) return;
 #pragma unroll
     for (int k = 0; k < N; ++k) {

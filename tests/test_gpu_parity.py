@@ -248,3 +248,54 @@ def test_empty_and_ragged_sizes():
         X = np.asarray(o.xu_phys, float)
         U = W.config_state("C5", X, p=p) if nd == 3 else np.ascontiguousarray(np.moveaxis(W.fourier_state(X, 7), -1, 1))
         _check("ragged-%s" % (shape,), GpuRunner(_ctx(mesh, disc)).rhs(U), o.rhs(U), TOL64)
+
+
+# ------------------------------------------------------------------------------------------
+# sm_100a TMA-pipelined hexahedral path (fr_hex_tma.cu, fr_hex_fluxdiv_tma.cu)
+# ------------------------------------------------------------------------------------------
+def test_tma_path_is_the_default_on_hexes():
+    """Hexahedra, 1 <= p <= 5 (fp64): 5 launches per Navier-Stokes RHS, 3 per Euler RHS."""
+    for system, want in (("navier-stokes", 5), ("euler", 3)):
+        mesh, disc = W.config("C5", n=3, p=3, system=system)
+        ctx = _ctx(mesh, disc)
+        assert ctx.rhs_kernel_launches == want, (system, ctx.rhs_kernel_launches)
+        names = [n for n, _ in ctx.rhs_profiled(*_ptrs(GpuRunner(ctx)))]
+        assert any("tma" in n for n in names), names
+
+
+def _ptrs(run):
+    return run.u.data_ptr(), run.r.data_ptr(), run.work.data_ptr(), run.stream
+
+
+@pytest.mark.parametrize("p", [1, 2, 3, 4, 5])
+def test_tma_recompute_variant(p, monkeypatch):
+    """The alternative last kernel (k_hex_rhs_tma: Q recomputed from U and the jumps instead of read back)."""
+    monkeypatch.setenv("FR_TMA_RECOMPUTE", "1")
+    mesh, disc = W.config("C3", n=3, p=p)
+    o = FROracle(mesh, disc)
+    U = W.config_state("C3", np.asarray(o.xu_phys, float), n=3, p=p)
+    R = o.rhs(U)
+    bar, _ = _bar(o, U, R)
+    ctx = _ctx(mesh, disc)
+    run = GpuRunner(ctx)
+    got = run.rhs(U)
+    assert "hex_rhs_tma" in [n for n, _ in ctx.rhs_profiled(*_ptrs(run))]
+    _check("recompute-p%d" % p, got, R, bar)
+
+
+def test_tma_curved_all_orders_and_ragged_blocks():
+    """Curved hexes at every order the TMA kernels are built for, element counts that are not multiples of the CTA tile
+    (E = 32, 16, 8 elements), Euler and Navier-Stokes, fp64 and fp32."""
+    for p, shape in ((1, (5, 3, 3)), (2, (3, 3, 2)), (3, (3, 2, 2)), (4, (3, 3, 1)), (5, (3, 1, 1))):
+        for system in ("navier-stokes", "euler"):
+            _, disc = W.config("C3", n=3, p=p)
+            disc = dict(disc, system=system)
+            mesh = W.box_mesh(shape, (2 * np.pi,) * 3, p_g=p, warp=W.sine_warp(0.05))
+            o = FROracle(mesh, disc)
+            U = W.config_state("C3", np.asarray(o.xu_phys, float), n=3, p=p)
+            R = o.rhs(U)
+            bar, _ = _bar(o, U, R)
+            _check("tma-p%d-%s" % (p, system), GpuRunner(_ctx(mesh, disc)).rhs(U), R, bar)
+            U32 = U.astype(np.float32)
+            R32 = o.rhs(U32.astype(np.float64))
+            _check("tma-p%d-%s-fp32" % (p, system), GpuRunner(_ctx(mesh, disc, precision="f32")).rhs(U32), R32, TOL32)
