@@ -50,10 +50,12 @@ struct GfLay {
   static constexpr size_t OPS = 128;  // sD [N*N], sL [2][N], sGm [N], sGp [N]
   static constexpr size_t U = OPS + al128((N * N + 4 * N) * 8);
   static constexpr uint32_t U_TX = NU * NV * E * sizeof(T);
-  static constexpr size_t ST = U + al128(U_TX);
+  static constexpr size_t JZ = U + al128(U_TX);                   // jumps of the two z faces [2][NFP*NV][E], loaded once
+  static constexpr uint32_t JZ_TX = 2 * NFP * NV * E * 8;
+  static constexpr size_t SS = JZ + al128(JZ_TX);                 // S of the current slice: ONE buffer, refilled during the face phase
   static constexpr uint32_t S_TX = 9 * NFP * E * 8, R_TX = NFP * E * 8, J_TX = 4 * N * NV * E * 8;
-  static constexpr size_t ST_R = al128(S_TX);
-  static constexpr size_t ST_J = ST_R + al128(R_TX);
+  static constexpr size_t ST = SS + al128(S_TX);                  // two stages of {1/J, x/y-face jumps}
+  static constexpr size_t ST_J = al128(R_TX);
   static constexpr size_t ST_BYTES = ST_J + al128(J_TX);
   static constexpr size_t Q = ST + 2 * ST_BYTES;
   static constexpr size_t Q_BYTES = 3 * NV * NFP * E * 8;
@@ -269,7 +271,7 @@ template <int N, int E, bool BND, bool SQ, typename T, int MINB>
 __global__ void __launch_bounds__(N *N *E, MINB)
     k_hex_gradface(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS,
                    const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmJ,
-                   const __grid_constant__ CUtensorMap tmQ, Ops1D<N> op, Phys ph,
+                   const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmJz, Ops1D<N> op, Phys ph,
                    const double *__restrict__ jump, const double *__restrict__ fp_n, const int32_t *__restrict__ fp_pe,
                    const BcDev *__restrict__ bcs, double *__restrict__ gf, int64_t ld, int64_t Nel) {
   using L = GfLay<N, E, T>;
@@ -280,6 +282,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   double *sD = (double *)(sm + L::OPS), *sL = sD + N * N;  // sL[0][m] = l_m(-1), sL[1][m] = l_m(+1)
   double *sGm = sL + 2 * N, *sGp = sGm + N;
   const T *sU = (const T *)(sm + L::U);
+  const double *sJz = (const double *)(sm + L::JZ);
+  const double *stS = (const double *)(sm + L::SS);
   unsigned char *sSt = sm + L::ST;
   double *sQ = (double *)(sm + L::Q);  // [3][NFP][NV][E]
   const int tid = threadIdx.x, el = tid % E, ij = tid / E, i = ij % N, j = ij / N;
@@ -288,7 +292,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   const bool act = e < Nel;
 
   if (tid == 0) {
-    mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); mbar_init(&bar[2], 1);
+    mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); mbar_init(&bar[2], 1); mbar_init(&bar[3], 1);
     fence_barrier_init();
     fence_proxy_async();
   }
@@ -296,20 +300,22 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   for (int t = tid; t < N; t += NFP * E) { sL[t] = op.lm[t]; sL[N + t] = op.lp[t]; sGm[t] = op.gm[t]; sGp[t] = op.gp[t]; }
   __syncthreads();
   auto issue_stage = [&](int s, int k) {
-    mbar_expect_tx(&bar[1 + s], L::S_TX + L::R_TX + L::J_TX);
-    tma_load_3d(sSt + s * L::ST_BYTES, &tmS, e0, NFP * k, 0, &bar[1 + s]);
-    tma_load_3d(sSt + s * L::ST_BYTES + L::ST_R, &tmR, e0, 0, k, &bar[1 + s]);
+    mbar_expect_tx(&bar[1 + s], L::R_TX + L::J_TX);
+    tma_load_3d(sSt + s * L::ST_BYTES, &tmR, e0, 0, k, &bar[1 + s]);
     tma_load_3d(sSt + s * L::ST_BYTES + L::ST_J, &tmJ, e0, N * k * NV, 0, &bar[1 + s]);
   };
+  auto issue_S = [&](int k) {
+    mbar_expect_tx(&bar[3], L::S_TX);
+    tma_load_3d(sm + L::SS, &tmS, e0, NFP * k, 0, &bar[3]);
+  };
   if (tid == 0) {
-    mbar_expect_tx(&bar[0], L::U_TX);
+    mbar_expect_tx(&bar[0], L::U_TX + L::JZ_TX);
     tma_load_3d(sm + L::U, &tmU, e0, 0, 0, &bar[0]);
+    tma_load_3d(sm + L::JZ, &tmJz, e0, 0, 4, &bar[0]);
+    issue_S(0);
     issue_stage(0, 0);
     if (N > 1) issue_stage(1, 1);
   }
-  // z-face jumps of this column: re-read from L2 in every slice, one variable ahead of their use
-  auto ldj = [&](int face, int a) { return ld_nc_once(jump + ((size_t)(face * NFP + ij) * NV + a) * ld + e); };
-  double jm_nx = ldj(4, 0), jp_nx = ldj(5, 0);
   double zm[3][NV], zp[3][NV];  // Q interpolated to the two z faces of this column
 #pragma unroll
   for (int n = 0; n < 3; ++n)
@@ -320,8 +326,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
   for (int k = 0; k < N; ++k) {
     mbar_wait(&bar[1 + (k & 1)], (k >> 1) & 1);
-    const double *stS = (const double *)(sSt + (k & 1) * L::ST_BYTES);
-    const double *stR = (const double *)(sSt + (k & 1) * L::ST_BYTES + L::ST_R);
+    mbar_wait(&bar[3], k & 1);
+    const double *stR = (const double *)(sSt + (k & 1) * L::ST_BYTES);
     const double *stJ = (const double *)(sSt + (k & 1) * L::ST_BYTES + L::ST_J);
     const T *su = sU + (size_t)(NFP * k) * NV * E + el;  // slice k
     {
@@ -336,9 +342,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       for (int a = 0; a < NV; ++a) {
         double qx = fma(gpi, stJ[((1 * N + j) * NV + a) * E + el], -gmi * stJ[((0 * N + j) * NV + a) * E + el]);
         double qy = fma(gpj, stJ[((3 * N + i) * NV + a) * E + el], -gmj * stJ[((2 * N + i) * NV + a) * E + el]);
-        const double jm = jm_nx, jp = jp_nx;
-        if (a + 1 < NV) { jm_nx = ldj(4, a + 1); jp_nx = ldj(5, a + 1); }
-        double qz = fma(op.gp[k], jp, -op.gm[k] * jm);
+        double qz = fma(op.gp[k], sJz[((1 * NFP + ij) * NV + a) * E + el], -op.gm[k] * sJz[((0 * NFP + ij) * NV + a) * E + el]);
 #pragma unroll
         for (int m = 0; m < N; ++m) {
           qx = fma(sD[i * N + m], (double)su[((j * N + m) * NV + a) * E], qx);
@@ -357,6 +361,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     }
     if (SQ) fence_proxy_async();  // make the sQ writes visible to the bulk store
     __syncthreads();  // Q of the slice is complete; stage k&1 has been consumed
+    if (tid == 0 && k + 1 < N) issue_S(k + 1);
     if (tid == 0 && k + 2 < N) issue_stage(k & 1, k + 2);
     if (SQ && tid == 0) { tma_store_3d(&tmQ, e0, 0, 3 * k, sQ); tma_store_commit(); }
     // x / y faces of the slice: 4 N flux points per element, one thread each
@@ -406,10 +411,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       }
     }
     if (SQ && tid == 0) tma_store_wait_read();  // the bulk store has read sQ
-    if (k + 1 < N) {
-      jm_nx = ldj(4, 0); jp_nx = ldj(5, 0);
-      __syncthreads();  // before the next slice overwrites sQ
-    }
+    if (k + 1 < N) __syncthreads();  // before the next slice overwrites sQ
   }
   // z faces of the column
 #pragma unroll
@@ -443,7 +445,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 // ---------------------------------------------------------------------------------------------
 template <int N, int E>
 struct Maps {
-  CUtensorMap U, S, R, R1, J, Q;
+  CUtensorMap U, S, R, R1, J, Jz, Q;
 };
 
 template <int N, int E, typename T>
@@ -454,8 +456,12 @@ bool make_maps(const DevConsts &c, const void *u, const double *jump, Maps<N, E>
   ok = ok && encode3(&m.S, true, c.smat, ld, NU, 9, ld, (uint64_t)NU * ld, E, NFP, 9);
   ok = ok && encode3(&m.R, true, c.rcpj, ld, NFP, N, ld, (uint64_t)NFP * ld, E, NFP, N);
   ok = ok && encode3(&m.R1, true, c.rcpj, ld, NFP, N, ld, (uint64_t)NFP * ld, E, NFP, 1);
-  if (need_j) ok = ok && encode3(&m.J, true, jump, ld, NFP * NV, 6, ld, (uint64_t)NFP * NV * ld, E, N * NV, 4);
-  else m.J = m.R;
+  if (need_j) {
+    ok = ok && encode3(&m.J, true, jump, ld, NFP * NV, 6, ld, (uint64_t)NFP * NV * ld, E, N * NV, 4);
+    ok = ok && encode3(&m.Jz, true, jump, ld, NFP * NV, 6, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 2);
+  } else {
+    m.J = m.R; m.Jz = m.R;
+  }
   if (q) ok = ok && encode3(&m.Q, true, q, ld, NV * NFP, 3 * N, ld, (uint64_t)NV * NFP * ld, E, NV * NFP, 3);
   else m.Q = m.R;
   return ok;
@@ -490,7 +496,8 @@ cudaError_t launch_gradface_k(const DevConsts &c, const Maps<N, E> &m, const Ops
   static bool done = false;
   cudaError_t err = set_smem(kern, L::TOTAL, done);
   if (err != cudaSuccess) return err;
-  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.J, m.Q, op, c.ph, jump, c.fp_n, c.fp_pe, c.bcs, gf, c.ld,
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.J, m.Q, m.Jz, op, c.ph, jump, c.fp_n, c.fp_pe, c.bcs, gf,
+                                                                  c.ld,
                                                                   c.Nel);
   return cudaGetLastError();
 }
