@@ -299,3 +299,44 @@ def test_tma_curved_all_orders_and_ragged_blocks():
             U32 = U.astype(np.float32)
             R32 = o.rhs(U32.astype(np.float64))
             _check("tma-p%d-%s-fp32" % (p, system), GpuRunner(_ctx(mesh, disc, precision="f32")).rhs(U32), R32, TOL32)
+
+
+# ------------------------------------------------------------------------------------------
+# the paper's Couette case (Eq 34-36, constants at PAPER.md:589) with the App C.4 walls
+# ------------------------------------------------------------------------------------------
+def _couette(X, gamma=1.4, Pr=0.72, cp=1005.0, Tw=300.0, pc=1e5, vw=69.445, H=1.0):
+    phi = X[..., 1] / H
+    rho = gamma / (gamma - 1) * 2 * pc / (2 * cp * Tw + Pr * vw * vw * phi * (1 - phi))
+    comps = [rho, rho * vw * phi, 0 * rho] + ([0 * rho] if X.shape[-1] == 3 else []) + [pc / (gamma - 1) + 0.5 * rho * (vw * phi) ** 2]
+    return np.ascontiguousarray(np.moveaxis(np.stack(comps, -1), -1, 1))
+
+
+@pytest.mark.parametrize("nd", [2, 3])
+def test_couette_steady_state_on_gpu(nd):
+    """The analytic Couette profile is a steady state of the discrete operator up to spectrally small truncation error
+    (walls at y = 0 at rest and y = 1 moving, periodic elsewhere); the GPU residual equals the oracle's and the state
+    does not drift over RK4 steps.  Hexes run the TMA path with boundary flux points."""
+    cp, Tw, vw, Pr, mu = 1005.0, 300.0, 69.445, 0.72, 0.417
+    wall0, wall1 = ("noslip-wall", dict(cpTw=cp * Tw, v=(0.0,) * nd)), ("noslip-wall", dict(cpTw=cp * Tw, v=(vw,) + (0.0,) * (nd - 1)))
+    shape, per = ((2, 2), (True, False)) if nd == 2 else ((2, 2, 2), (True, False, True))
+    mesh = W.box_mesh(shape, (1.0,) * nd, periodic=per)
+    bcs = {2: wall0, 3: wall1}
+    res = []
+    for p in (1, 2, 4):
+        disc = dict(p=p, system="navier-stokes", gamma=1.4, mu=mu, Pr=Pr, beta=0.5, tau=0.1)
+        o = FROracle(mesh, disc, bcs)
+        U = _couette(np.asarray(o.xu_phys, float))
+        R = o.rhs(U)
+        run = GpuRunner(_ctx(mesh, disc, bcs=bcs))
+        got = run.rhs(U)
+        scale = 1e5 * 2 / 0.5
+        assert np.max(np.abs(got - R)) <= 1e-10 * scale, (p, np.max(np.abs(got - R)))
+        res.append(np.max(np.abs(got[:, 1:3])) / scale)
+        if p == 4:
+            dt = 2e-6
+            U1 = run.rk4(U, dt, 20)
+            sc = np.max(np.abs(U), axis=(0, 2), keepdims=True)
+            sc[:, 1:-1] = np.max(sc[:, 1:-1])  # all momentum components on the scale of rho * v_w
+            drift = np.max(np.abs(U1 - U) / sc)
+            assert drift < 1e-8, drift
+    assert res[0] > 10 * res[1] > 100 * res[2] and res[2] < 1e-7, res
