@@ -340,3 +340,20 @@ def test_couette_steady_state_on_gpu(nd):
             drift = np.max(np.abs(U1 - U) / sc)
             assert drift < 1e-8, drift
     assert res[0] > 10 * res[1] > 100 * res[2] and res[2] < 1e-7, res
+
+
+def test_pre_tma_hex_kernels_still_match(monkeypatch):
+    """The register/L1 z-slab kernels of fr_hex.cuh (the path p = 6 fp64 takes for lack of shared memory, and any
+    device without a tensor-map encoder) stay covered: FR_NO_TMA=1 forces them at p = 3."""
+    monkeypatch.setenv("FR_NO_TMA", "1")
+    mesh, disc = W.config("C3", n=3, p=3)
+    o = FROracle(mesh, disc)
+    U = W.config_state("C3", np.asarray(o.xu_phys, float), n=3, p=3)
+    R = o.rhs(U)
+    bar, _ = _bar(o, U, R)
+    ctx = _ctx(mesh, disc)
+    run = GpuRunner(ctx)
+    got = run.rhs(U)
+    names = [n for n, _ in ctx.rhs_profiled(*_ptrs(run))]
+    assert "hex_grad" in names and "hex_fluxdiv" in names, names
+    _check("pre-tma-p3", got, R, bar)
