@@ -4,6 +4,7 @@
 #include <exception>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "fr_dev.hpp"
@@ -107,10 +108,14 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     c->ready = false;
     free_dev(c);
     build_ref_ops(c->mesh.etype, d->p, c->mesh.p_g, c->ops);
-    const int64_t lane = (d->precision == FR_F64) ? 16 : 32;  // 128-byte rows (north_star: padded for 128-byte coalescing)
+    const int64_t lane = FR_BLK;  // rows start on 128-byte boundaries (north_star) and hold whole element blocks (fp_row)
     const int64_t ld = align_up(c->mesh.Nel, lane);
     std::string err;
-    int rc = build_mesh_consts(c->mesh, c->ops, ld, c->mc, err);
+    c->host_only = (d->flags & FR_FLAG_HOST_ONLY) != 0;
+    // hexahedra on the TMA-pipelined kernels keep every internal array element-blocked (fr_dev.hpp: fp_row)
+    const bool blk = !c->host_only && !(d->flags & FR_FLAG_FORCE_GENERIC) && c->ops.etype == FR_HEX &&
+                     hex_tma_supported(c->ops.n, d->precision == FR_F64);
+    int rc = build_mesh_consts(c->mesh, c->ops, ld, blk ? FR_BLK : 0, c->mc, err);
     if (rc != FR_OK) return fail(c, rc, err);
     c->disc = *d;
     const RefOps &o = c->ops;
@@ -124,15 +129,24 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     c->host_only = (d->flags & FR_FLAG_HOST_ONLY) != 0;
     if (c->host_only) { c->use_tensor = false; c->wl = WorkLayout(); c->ready = true; return FR_OK; }
     cudaError_t e = cudaSuccess;
+    dc.blk = blk;
+    auto reblock = [&](const auto &src, int rows) {  // [rows][ld] -> [ld / FR_BLK][rows][FR_BLK]
+      typename std::decay<decltype(src)>::type dst(src.size());
+      for (int64_t b = 0; b < ld / FR_BLK; ++b)
+        for (int r = 0; r < rows; ++r)
+          std::memcpy(&dst[((size_t)b * rows + r) * FR_BLK], &src[(size_t)r * ld + (size_t)b * FR_BLK], FR_BLK * sizeof(src[0]));
+      return dst;
+    };
 #define UP(vec, field) if (e == cudaSuccess) e = upload(c, vec, &dc.field)
     UP(o.M[0], M0); UP(o.M[3], M3); UP(o.M[6], M6); UP(o.M46, M46); UP(o.M132, M132);
-    UP(mc.smat, smat); UP(mc.rcpj, rcpj);
+    if (dc.blk) { UP(reblock(mc.smat, o.nd * o.nd * o.Nu), smat); UP(reblock(mc.rcpj, o.Nu), rcpj); }
+    else { UP(mc.smat, smat); UP(mc.rcpj, rcpj); }
     UP(mc.pLs, pLs); UP(mc.pLe, pLe); UP(mc.pRs, pRs); UP(mc.pRe, pRe);
     UP(mc.pn, pn); UP(mc.pJnL, pJnL); UP(mc.pJnR, pJnR);
     UP(mc.bs, bs); UP(mc.be, be); UP(mc.bbc, bbc); UP(mc.bn, bn); UP(mc.bJn, bJn);
     // element-centric flux-point tables of the fused hexahedral gradient kernel (own normals, boundary ids)
     const bool want_tma = !(d->flags & FR_FLAG_FORCE_GENERIC) && o.etype == FR_HEX && dc.ns && hex_tma_supported(o.n, dc.f64);
-    if (want_tma) { UP(mc.fp_n, fp_n); if (mc.nbnd) { UP(mc.fp_pe, fp_pe); } }
+    if (want_tma) { UP(reblock(mc.fp_n, o.nd * o.Nf), fp_n); if (mc.nbnd) { UP(reblock(mc.fp_pe, o.Nf), fp_pe); } }
 #undef UP
     std::vector<BcDev> bcs(c->mesh.bcs.size());
     for (size_t i = 0; i < bcs.size(); ++i) {

@@ -13,6 +13,7 @@ struct DevConsts {
   int64_t Nel, ld, npairs, nbnd;
   bool ns;       // Navier-Stokes (gradients, LDG) or Euler
   bool f64;      // storage precision of u / rhs
+  bool blk;      // library-internal arrays are element-blocked (FR_BLK elements per block), see fp_row()
   Phys ph;
   // dense operators (device, row-major doubles)
   const double *M0, *M3, *M6, *M46, *M132;
@@ -31,6 +32,19 @@ struct DevConsts {
   const int32_t *fp_pe, *fp_ps;
   const double *fp_n, *fp_Jn;
 };
+
+// Element-blocked layout of library-internal arrays (flux-point arrays U^f / D~, jumps, G^f, Q, and the metric / normal
+// tables of the hexahedral TMA path).  The caller-visible layout [row][ld] puts consecutive rows ld*8 bytes apart: at
+// 10^6 elements every row of a CTA's working set lies in a page of its own and the TMA kernels run at less than half
+// speed (measured).  Internal arrays therefore use [element block][row][FR_BLK]: all rows that belong
+// to FR_BLK consecutive elements are contiguous.  u and rhs keep the ABI layout.
+constexpr int FR_BLK = 32;
+
+// start of row `row` (of `rows` per element) for element e, and the distance between consecutive rows of one element
+__host__ __device__ inline size_t fp_row(bool blk, int64_t ld, int rows, int row, int64_t e) {
+  return blk ? ((size_t)(e / FR_BLK) * rows + row) * FR_BLK + (size_t)(e % FR_BLK) : (size_t)row * ld + e;
+}
+__host__ __device__ inline size_t fp_rstride(bool blk, int64_t ld) { return blk ? (size_t)FR_BLK : (size_t)ld; }
 
 // Workspace layout (doubles unless noted); offsets in bytes from work_dev
 struct WorkLayout {

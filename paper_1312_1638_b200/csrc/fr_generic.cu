@@ -59,14 +59,15 @@ __global__ void k_common_sol(DevConsts c, const double *__restrict__ uf, double 
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.npairs) return;
-  const size_t oL = (size_t)c.pLs[i] * NV * c.ld + c.pLe[i], oR = (size_t)c.pRs[i] * NV * c.ld + c.pRe[i];
+  const size_t oL = fp_row(c.blk, c.ld, c.Nf * NV, c.pLs[i] * NV, c.pLe[i]), oR = fp_row(c.blk, c.ld, c.Nf * NV, c.pRs[i] * NV, c.pRe[i]);
+  const size_t vs = fp_rstride(c.blk, c.ld);  // distance between the variables of one flux point
   const double wl = 0.5 - c.ph.beta, wr = 0.5 + c.ph.beta;
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
-    const double ul = uf[oL + (size_t)a * c.ld], ur = uf[oR + (size_t)a * c.ld];
+    const double ul = uf[oL + (size_t)a * vs], ur = uf[oR + (size_t)a * vs];
     const double v = wl * ul + wr * ur;
-    cf[oL + (size_t)a * c.ld] = JUMP ? v - ul : v;   // JUMP: the {C - u^f} of Eq 9 directly
-    cf[oR + (size_t)a * c.ld] = JUMP ? v - ur : v;
+    cf[oL + (size_t)a * vs] = JUMP ? v - ul : v;   // JUMP: the {C - u^f} of Eq 9 directly
+    cf[oR + (size_t)a * vs] = JUMP ? v - ur : v;
   }
 }
 
@@ -76,13 +77,14 @@ __global__ void k_common_sol_bnd(DevConsts c, const double *__restrict__ uf, dou
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.nbnd) return;
-  const size_t o = (size_t)c.bs[i] * NV * c.ld + c.be[i];
+  const size_t o = fp_row(c.blk, c.ld, c.Nf * NV, c.bs[i] * NV, c.be[i]);
+  const size_t vs = fp_rstride(c.blk, c.ld);
   double u[NV], gi[NV], gl[NV];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) u[a] = uf[o + (size_t)a * c.ld];
+  for (int a = 0; a < NV; ++a) u[a] = uf[o + (size_t)a * vs];
   ghost_states<ND>(c.bcs[c.bbc[i]], u, c.ph.gamma, gi, gl);
 #pragma unroll
-  for (int a = 0; a < NV; ++a) cf[o + (size_t)a * c.ld] = (0.5 - c.ph.beta) * u[a] + (0.5 + c.ph.beta) * gl[a] - (JUMP ? u[a] : 0.0);
+  for (int a = 0; a < NV; ++a) cf[o + (size_t)a * vs] = (0.5 - c.ph.beta) * u[a] + (0.5 + c.ph.beta) * gl[a] - (JUMP ? u[a] : 0.0);
 }
 
 // q = J^-T q~ = (1/J) S^T q~, Eq 10 (:206), in place
@@ -156,23 +158,24 @@ __global__ void k_common_flux(DevConsts c, double *__restrict__ uf, const double
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.npairs) return;
-  const size_t oL = (size_t)c.pLs[i] * NV * c.ld + c.pLe[i], oR = (size_t)c.pRs[i] * NV * c.ld + c.pRe[i];
+  const size_t oL = fp_row(c.blk, c.ld, c.Nf * NV, c.pLs[i] * NV, c.pLe[i]), oR = fp_row(c.blk, c.ld, c.Nf * NV, c.pRs[i] * NV, c.pRe[i]);
+  const size_t vs = fp_rstride(c.blk, c.ld);  // distance between the variables of one flux point
   const size_t blk = (size_t)c.Nf * NV * c.ld;
   double uL[NV], uR[NV], qL[ND][NV], qR[ND][NV], nrm[ND], F[NV];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) { uL[a] = uf[oL + (size_t)a * c.ld]; uR[a] = uf[oR + (size_t)a * c.ld]; }
+  for (int a = 0; a < NV; ++a) { uL[a] = uf[oL + (size_t)a * vs]; uR[a] = uf[oR + (size_t)a * vs]; }
   if (NS) {
 #pragma unroll
     for (int n = 0; n < ND; ++n)
 #pragma unroll
-      for (int a = 0; a < NV; ++a) { qL[n][a] = qf[n * blk + oL + (size_t)a * c.ld]; qR[n][a] = qf[n * blk + oR + (size_t)a * c.ld]; }
+      for (int a = 0; a < NV; ++a) { qL[n][a] = qf[n * blk + oL + (size_t)a * vs]; qR[n][a] = qf[n * blk + oR + (size_t)a * vs]; }
   }
 #pragma unroll
   for (int n = 0; n < ND; ++n) nrm[n] = c.pn[(size_t)n * c.npairs + i];
   common_flux<ND, NS>(uL, uR, uR, qL, qR, nrm, c.ph, F);
   const double jl = c.pJnL[i], jr = c.pJnR[i];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) { uf[oL + (size_t)a * c.ld] = jl * F[a]; uf[oR + (size_t)a * c.ld] = -jr * F[a]; }
+  for (int a = 0; a < NV; ++a) { uf[oL + (size_t)a * vs] = jl * F[a]; uf[oR + (size_t)a * vs] = -jr * F[a]; }
 }
 
 template <int ND, bool NS>
@@ -180,24 +183,25 @@ __global__ void k_common_flux_bnd(DevConsts c, double *__restrict__ uf, const do
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.nbnd) return;
-  const size_t o = (size_t)c.bs[i] * NV * c.ld + c.be[i];
+  const size_t o = fp_row(c.blk, c.ld, c.Nf * NV, c.bs[i] * NV, c.be[i]);
+  const size_t vs = fp_rstride(c.blk, c.ld);
   const size_t blk = (size_t)c.Nf * NV * c.ld;
   double uL[NV], gi[NV], gl[NV], qL[ND][NV], qR[ND][NV], nrm[ND], F[NV];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) uL[a] = uf[o + (size_t)a * c.ld];
+  for (int a = 0; a < NV; ++a) uL[a] = uf[o + (size_t)a * vs];
   const double keep = ghost_states<ND>(c.bcs[c.bbc[i]], uL, c.ph.gamma, gi, gl);
   if (NS) {
 #pragma unroll
     for (int n = 0; n < ND; ++n)
 #pragma unroll
-      for (int a = 0; a < NV; ++a) { qL[n][a] = qf[n * blk + o + (size_t)a * c.ld]; qR[n][a] = keep * qL[n][a]; }
+      for (int a = 0; a < NV; ++a) { qL[n][a] = qf[n * blk + o + (size_t)a * vs]; qR[n][a] = keep * qL[n][a]; }
   }
 #pragma unroll
   for (int n = 0; n < ND; ++n) nrm[n] = c.bn[(size_t)n * c.nbnd + i];
   common_flux<ND, NS>(uL, gl, gi, qL, qR, nrm, c.ph, F);
   const double jn = c.bJn[i];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) uf[o + (size_t)a * c.ld] = jn * F[a];
+  for (int a = 0; a < NV; ++a) uf[o + (size_t)a * vs] = jn * F[a];
 }
 
 // Common normal flux with the viscous part pre-contracted by the element kernels (fr_hex_tma.cu):
@@ -208,13 +212,14 @@ __global__ void k_common_flux_g(DevConsts c, double *__restrict__ uf, const doub
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.npairs) return;
-  const size_t oL = (size_t)c.pLs[i] * NV * c.ld + c.pLe[i], oR = (size_t)c.pRs[i] * NV * c.ld + c.pRe[i];
+  const size_t oL = fp_row(c.blk, c.ld, c.Nf * NV, c.pLs[i] * NV, c.pLe[i]), oR = fp_row(c.blk, c.ld, c.Nf * NV, c.pRs[i] * NV, c.pRe[i]);
+  const size_t vs = fp_rstride(c.blk, c.ld);  // distance between the variables of one flux point
   const double wl = 0.5 + c.ph.beta, wr = 0.5 - c.ph.beta;
   double uL[NV], uR[NV], gL[NV], gR[NV], nrm[ND], F[NV];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) { uL[a] = uf[oL + (size_t)a * c.ld]; uR[a] = uf[oR + (size_t)a * c.ld]; }
+  for (int a = 0; a < NV; ++a) { uL[a] = uf[oL + (size_t)a * vs]; uR[a] = uf[oR + (size_t)a * vs]; }
 #pragma unroll
-  for (int a = 0; a < NV; ++a) { gL[a] = wl != 0.0 ? gf[oL + (size_t)a * c.ld] : 0.0; gR[a] = wr != 0.0 ? gf[oR + (size_t)a * c.ld] : 0.0; }
+  for (int a = 0; a < NV; ++a) { gL[a] = wl != 0.0 ? gf[oL + (size_t)a * vs] : 0.0; gR[a] = wr != 0.0 ? gf[oR + (size_t)a * vs] : 0.0; }
 #pragma unroll
   for (int n = 0; n < ND; ++n) nrm[n] = c.pn[(size_t)n * c.npairs + i];
   rusanov<ND>(uL, uR, nrm, c.ph.gamma, F);
@@ -222,8 +227,8 @@ __global__ void k_common_flux_g(DevConsts c, double *__restrict__ uf, const doub
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
     const double f = F[a] + c.ph.tau * (uL[a] - uR[a]) - (wl * gL[a] - wr * gR[a]);
-    uf[oL + (size_t)a * c.ld] = jl * f;
-    uf[oR + (size_t)a * c.ld] = -jr * f;
+    uf[oL + (size_t)a * vs] = jl * f;
+    uf[oR + (size_t)a * vs] = -jr * f;
   }
 }
 
@@ -233,17 +238,18 @@ __global__ void k_common_flux_bnd_g(DevConsts c, double *__restrict__ uf, const 
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.nbnd) return;
-  const size_t o = (size_t)c.bs[i] * NV * c.ld + c.be[i];
+  const size_t o = fp_row(c.blk, c.ld, c.Nf * NV, c.bs[i] * NV, c.be[i]);
+  const size_t vs = fp_rstride(c.blk, c.ld);
   double uL[NV], gi[NV], gl[NV], nrm[ND], F[NV];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) uL[a] = uf[o + (size_t)a * c.ld];
+  for (int a = 0; a < NV; ++a) uL[a] = uf[o + (size_t)a * vs];
   ghost_states<ND>(c.bcs[c.bbc[i]], uL, c.ph.gamma, gi, gl);
 #pragma unroll
   for (int n = 0; n < ND; ++n) nrm[n] = c.bn[(size_t)n * c.nbnd + i];
   rusanov<ND>(uL, gi, nrm, c.ph.gamma, F);
   const double jn = c.bJn[i];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) uf[o + (size_t)a * c.ld] = jn * (F[a] + c.ph.tau * (uL[a] - gl[a]) - gf[o + (size_t)a * c.ld]);
+  for (int a = 0; a < NV; ++a) uf[o + (size_t)a * vs] = jn * (F[a] + c.ph.tau * (uL[a] - gl[a]) - gf[o + (size_t)a * vs]);
 }
 
 template <typename TIN, typename TOUT, bool SCALE>

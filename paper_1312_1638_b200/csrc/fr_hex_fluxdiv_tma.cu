@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   unsigned char *sSt = sm + L::ST;
   double *sF = (double *)(sm + L::F);  // [NB][2][NV][NFP][E]
   const int tid = threadIdx.x, el = tid % E, ij = tid / E, i = ij % N, j = ij / N;
-  const int e0 = blockIdx.x * E;
+  const int e0 = blockIdx.x * E, l0 = e0 % FR_BLK, eb = e0 / FR_BLK;  // first element: lane and element block (fp_row)
   const int64_t e = (int64_t)e0 + el;
   const bool act = e < Nel;
 
@@ -67,14 +67,14 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   __syncthreads();
   auto issue_stage = [&](int s, int k) {
     mbar_expect_tx(&bar[s], L::S_TX + L::U_TX + L::Q_TX);
-    tma_load_3d(sSt + s * L::ST_BYTES, &tmS, e0, NFP * k, 0, &bar[s]);
+    tma_load_4d(sSt + s * L::ST_BYTES, &tmS, l0, NFP * k, 0, eb, &bar[s]);
     tma_load_3d(sSt + s * L::ST_BYTES + L::ST_U, &tmU, e0, 0, k, &bar[s]);
-    if (NS) tma_load_3d(sSt + s * L::ST_BYTES + L::ST_Q, &tmQ, e0, 0, 3 * k, &bar[s]);
+    if (NS) tma_load_4d(sSt + s * L::ST_BYTES + L::ST_Q, &tmQ, l0, 0, 3 * k, eb, &bar[s]);
   };
   if (tid == 0) {
     issue_stage(0, 0);
     if (N > 1) issue_stage(1, 1);
-    if (L::EPI_DED) { mbar_expect_tx(&bar[2], L::DXY_TX); tma_load_3d(sm + L::DED, &tmD4, e0, 0, 0, &bar[2]); }
+    if (L::EPI_DED) { mbar_expect_tx(&bar[2], L::DXY_TX); tma_load_4d(sm + L::DED, &tmD4, l0, 0, 0, eb, &bar[2]); }
   }
   double acc[N][NV];
 #pragma unroll
@@ -153,17 +153,17 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     if (tid == 0 && k + 2 < N) issue_stage(k & 1, k + 2);
     if (L::EPI_ST && tid == 0 && k == N - 2) {  // this stage is not refilled any more: bring D~ (x/y faces) and 1/J
       mbar_expect_tx(&bar[2], L::DXY_TX);
-      tma_load_3d(sSt + (k & 1) * L::ST_BYTES, &tmD4, e0, 0, 0, &bar[2]);
+      tma_load_4d(sSt + (k & 1) * L::ST_BYTES, &tmD4, l0, 0, 0, eb, &bar[2]);
       mbar_expect_tx(&bar[4], L::RJ_TX);
-      tma_load_3d(sSt + (k & 1) * L::ST_BYTES + L::EP_RJ, &tmR, e0, 0, 0, &bar[4]);
+      tma_load_4d(sSt + (k & 1) * L::ST_BYTES + L::EP_RJ, &tmR, l0, 0, 0, eb, &bar[4]);
     }
     if (L::EPI_DED && tid == 0 && k == N - 2) {
       mbar_expect_tx(&bar[4], L::RJ_TX);
-      tma_load_3d(sSt + (k & 1) * L::ST_BYTES, &tmR, e0, 0, 0, &bar[4]);
+      tma_load_4d(sSt + (k & 1) * L::ST_BYTES, &tmR, l0, 0, 0, eb, &bar[4]);
     }
     if (L::EPI_TMA && tid == 0 && k == N - 1) {  // D~ of the z faces
       mbar_expect_tx(&bar[3], L::DZ_TX);
-      tma_load_3d(sSt + (k & 1) * L::ST_BYTES, &tmD2, e0, 0, 4, &bar[3]);
+      tma_load_4d(sSt + (k & 1) * L::ST_BYTES, &tmD2, l0, 0, 4, eb, &bar[3]);
     }
     // x and y contractions within the slice
 #pragma unroll
@@ -209,23 +209,23 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   double dzm[NV], dzp[NV];
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
-    dzm[a] = dt[((size_t)(4 * NFP + ij) * NV + a) * ld + e];
-    dzp[a] = dt[((size_t)(5 * NFP + ij) * NV + a) * ld + e];
+    dzm[a] = dt[fp_row(true, ld, 6 * NFP * NV, (4 * NFP + ij) * NV + a, e)];
+    dzp[a] = dt[fp_row(true, ld, 6 * NFP * NV, (5 * NFP + ij) * NV + a, e)];
   }
 #pragma unroll
   for (int k = 0; k < N; ++k) {
     const int r = ij + NFP * k;
-    const double rj = rcpj[(size_t)r * ld + e];
+    const double rj = rcpj[fp_row(true, ld, N * NFP, r, e)];
     const int fx = j + N * k, fy = i + N * k;
 #pragma unroll
     for (int a = 0; a < NV; ++a) {
       double v = acc[k][a];
       v = fma(op.gm[k], dzm[a], v);
       v = fma(op.gp[k], dzp[a], v);
-      v = fma(gmi, dt[((size_t)(0 * NFP + fx) * NV + a) * ld + e], v);
-      v = fma(gpi, dt[((size_t)(1 * NFP + fx) * NV + a) * ld + e], v);
-      v = fma(gmj, dt[((size_t)(2 * NFP + fy) * NV + a) * ld + e], v);
-      v = fma(gpj, dt[((size_t)(3 * NFP + fy) * NV + a) * ld + e], v);
+      v = fma(gmi, dt[fp_row(true, ld, 6 * NFP * NV, (0 * NFP + fx) * NV + a, e)], v);
+      v = fma(gpi, dt[fp_row(true, ld, 6 * NFP * NV, (1 * NFP + fx) * NV + a, e)], v);
+      v = fma(gmj, dt[fp_row(true, ld, 6 * NFP * NV, (2 * NFP + fy) * NV + a, e)], v);
+      v = fma(gpj, dt[fp_row(true, ld, 6 * NFP * NV, (3 * NFP + fy) * NV + a, e)], v);
       rhs[((size_t)r * NV + a) * ld + e] = (T)(-v * rj);
     }
   }
@@ -244,13 +244,14 @@ cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *
   constexpr int MINB = min_blocks(L::TOTAL, N * N * E) < CAP ? min_blocks(L::TOTAL, N * N * E) : CAP;
   const uint64_t ld = (uint64_t)c.ld;
   CUtensorMap mS, mU, mQ, mD4, mD2, mR;
-  bool ok = encode3(&mS, true, c.smat, ld, NU, 9, ld, (uint64_t)NU * ld, E, NFP, 9);
-  ok = ok && encode3(&mU, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 1);
-  if (NS) ok = ok && encode3(&mQ, true, q, ld, NV * NFP, 3 * N, ld, (uint64_t)NV * NFP * ld, E, NV * NFP, 3);
+  static_assert(FR_BLK % E == 0, "a CTA's elements must lie in one element block");
+  bool ok = encode_blk(&mS, c.smat, ld, NU, 9, E, NFP, 9);
+  ok = ok && encode3(&mU, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 1);  // caller layout
+  if (NS) ok = ok && encode_blk(&mQ, q, ld, NV * NFP, 3 * N, E, NV * NFP, 3);
   else mQ = mS;
-  ok = ok && encode3(&mD4, true, dt, ld, NFP * NV, 6, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 4);
-  ok = ok && encode3(&mD2, true, dt, ld, NFP * NV, 6, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 2);
-  ok = ok && encode3(&mR, true, c.rcpj, ld, NFP, N, ld, (uint64_t)NFP * ld, E, NFP, N);
+  ok = ok && encode_blk(&mD4, dt, ld, NFP * NV, 6, E, NFP * NV, 4);
+  ok = ok && encode_blk(&mD2, dt, ld, NFP * NV, 6, E, NFP * NV, 2);
+  ok = ok && encode_blk(&mR, c.rcpj, ld, NFP, N, E, NFP, N);
   if (!ok) return cudaErrorNotSupported;
   auto kern = k_hex_fluxdiv_tma<N, E, NS, T, NB, MINB>;
   static bool done = false;
@@ -270,10 +271,8 @@ constexpr bool fd_fits() {
 template <int N, typename T>
 cudaError_t fluxdiv_n(const DevConsts &c, const double *h_ops, const void *u, const double *q, const double *dt, void *rhs, cudaStream_t s) {
   if constexpr (fd_fits<N, T>()) {
-    if constexpr (N == 5 && sizeof(T) == 8) {  // tuning variants (FR_TMA_E = 16 | 81 (E = 8, one CTA per SM))
+    if constexpr (N == 5 && sizeof(T) == 8) {  // tuning variant FR_TMA_E=16
       if (env_e() == 16) return c.ns ? launch_fluxdiv<N, 16, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, 16, false, T>(c, h_ops, u, q, dt, rhs, s);
-      if (env_e() == 4) return c.ns ? launch_fluxdiv<N, 4, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, 4, false, T>(c, h_ops, u, q, dt, rhs, s);
-      if (env_e() == 81) return c.ns ? launch_fluxdiv<N, 8, true, T, 1>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, 8, false, T, 1>(c, h_ops, u, q, dt, rhs, s);
     }
     constexpr int E = Cfg<N>::E;
     return c.ns ? launch_fluxdiv<N, E, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, E, false, T>(c, h_ops, u, q, dt, rhs, s);

@@ -4,7 +4,8 @@
 
 namespace fr {
 
-// true when the sm_100a TMA kernels can run this n = p+1 / precision (shared memory fits, driver exposes the encoder)
+// true when the sm_100a TMA kernels (both of them) can run this n = p+1 / precision: shared memory fits, the driver exposes
+// the tensor-map encoder.  The internal arrays are then element-blocked (fr_dev.hpp: fp_row).
 bool hex_tma_supported(int n, bool f64);
 
 // G^f = n . f_vis(U^f, Q^f) at every flux point, Q computed from u and jump = C - U^f  (parts 2b, 3 of the north_star);
@@ -16,10 +17,6 @@ cudaError_t hex_tma_gradface(const DevConsts &c, const double *h_ops, const void
 cudaError_t hex_tma_fluxdiv(const DevConsts &c, const double *h_ops, const void *u, const double *q, const double *dt, void *rhs,
                             cudaStream_t s);
 bool hex_tma_fluxdiv_supported(int n, bool f64);
-
-// rhs = -(1/J) {(M1 - M3 M2) S f(U, Q) + M3 D~}  (parts 4, 6, 7; Q recomputed for Navier-Stokes)
-cudaError_t hex_tma_rhs(const DevConsts &c, const double *h_ops, const void *u, const double *jump, const double *dt, void *rhs,
-                        cudaStream_t s);
 
 // Eq 15-17 over flux-point pairs with the viscous part taken from G^f; in place over U^f -> D~ (fr_generic.cu)
 void launch_common_flux_g(const DevConsts &c, double *uf, const double *gf, cudaStream_t s);

@@ -62,6 +62,7 @@ struct MeshInput {
 };
 
 // fr_mesh.cpp; returns FR_OK or an error code with text in err
-int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, MeshConsts &out, std::string &err);
+// pair_block > 0: order the flux-point pairs element-block major (blocks of pair_block elements) instead of sigma major
+int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, int pair_block, MeshConsts &out, std::string &err);
 
 }  // namespace fr

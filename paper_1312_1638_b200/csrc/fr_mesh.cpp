@@ -44,7 +44,7 @@ inline long double adjugate(int nd, const long double Jm[3][3], long double S[3]
 
 }  // namespace
 
-int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, MeshConsts &out, std::string &err) {
+int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, int pair_block, MeshConsts &out, std::string &err) {
   const int nd = in.nd, Nu = ops.Nu, Nf = ops.Nf, Nn = ops.Nn, nfp = ops.nfp;
   const int64_t Nel = in.Nel;
   out = MeshConsts();
@@ -144,13 +144,15 @@ int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, MeshCo
   if (badcover) { err = "flux points not covered exactly once by interfaces + boundary faces: " + std::to_string(badcover); return FR_EMESH; }
 
   // iteration order: sort by the L flux point (sigma major, element minor) so that consecutive threads
-  // read consecutive elements of one row
+  // read consecutive elements of one row.  With element-blocked flux-point arrays (pair_block > 0
+  // elements per block) the element block comes first, so that consecutive warps stay inside one block's rows.
   std::vector<int64_t> order(pairs.size());
   std::iota(order.begin(), order.end(), 0);
-  std::sort(order.begin(), order.end(), [&](int64_t a, int64_t b) {
-    int64_t ka = (int64_t)pairs[a].Ls * Nel + pairs[a].Le, kb = (int64_t)pairs[b].Ls * Nel + pairs[b].Le;
-    return ka < kb;
-  });
+  auto key = [&](const Pair &pr) {
+    if (pair_block <= 0) return (int64_t)pr.Ls * Nel + pr.Le;
+    return ((int64_t)(pr.Le / pair_block) * Nf + pr.Ls) * pair_block + pr.Le % pair_block;
+  };
+  std::sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return key(pairs[a]) < key(pairs[b]); });
   const int64_t np = (int64_t)pairs.size();
   out.npairs = np;
   out.pLs.resize(np); out.pLe.resize(np); out.pRs.resize(np); out.pRe.resize(np);

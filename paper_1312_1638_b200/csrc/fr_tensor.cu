@@ -37,12 +37,14 @@ __device__ __forceinline__ int line_base(int d, int idx, int &stride) {
 // U^f = M0 U (Eq 6 / Eq 41) and, with nblk = ND, Q^f = M5 Q (Eq 11 / Eq 43).
 template <int N, int ND, typename TIN>
 __global__ void __launch_bounds__(1024) k_tp_interp(Ops1D<N> op, const TIN *__restrict__ in, double *__restrict__ out, int64_t ncols,
-                                                    int64_t ld, int64_t Nel, int64_t in_blk, int64_t out_blk) {
-  constexpr int NFP = ipow(N, ND - 1);
+                                                    int64_t ld, int64_t Nel, int64_t in_blk, int64_t out_blk, bool blk) {
+  constexpr int NFP = ipow(N, ND - 1), NV = ND + 2;
   const int64_t col = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (col >= ncols || (col % ld) >= Nel) return;
   in += (size_t)blockIdx.z * in_blk + col;
-  out += (size_t)blockIdx.z * out_blk + col;
+  // element-blocked output (fr_dev.hpp: fp_row): row fp*NV + a of 2 ND NFP NV rows; plain: out[fp][a][ld]
+  const size_t rs = blk ? (size_t)NV * FR_BLK : (size_t)ncols;  // distance between consecutive flux points
+  out += blk ? fp_row(true, ld, 2 * ND * NFP * NV, (int)(col / ld), col % ld) : (size_t)blockIdx.z * out_blk + col;
   for (int idx = threadIdx.y; idx < NFP; idx += blockDim.y) {
 #pragma unroll
     for (int d = 0; d < ND; ++d) {
@@ -55,8 +57,8 @@ __global__ void __launch_bounds__(1024) k_tp_interp(Ops1D<N> op, const TIN *__re
         sm = fma(op.lm[m], v, sm);
         sp = fma(op.lp[m], v, sp);
       }
-      out[(size_t)((2 * d) * NFP + idx) * ncols] = sm;
-      out[(size_t)((2 * d + 1) * NFP + idx) * ncols] = sp;
+      out[(size_t)((2 * d) * NFP + idx) * rs] = sm;
+      out[(size_t)((2 * d + 1) * NFP + idx) * rs] = sp;
     }
   }
 }
@@ -201,7 +203,7 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
   const unsigned gx = (unsigned)((ncols + LW - 1) / LW), ge = (unsigned)((c.Nel + LW - 1) / LW);
   const dim3 bf(LW, NFP < rows ? NFP : rows), bu(LW, NU < rows ? NU : rows);
   FR_MARK(prof, "tp_interp");
-  k_tp_interp<N, ND, T><<<dim3(gx, 1, 1), bf, 0, s>>>(op, u, uf, ncols, c.ld, c.Nel, 0, 0);
+  k_tp_interp<N, ND, T><<<dim3(gx, 1, 1), bf, 0, s>>>(op, u, uf, ncols, c.ld, c.Nel, 0, 0, c.blk);
   if (ND == 3 && tp.use_tma) {
     // sm_100a path: 5 launches for Navier-Stokes (3 for Euler); neither Q^f nor F~ is stored
     cudaError_t e = cudaSuccess;
@@ -217,13 +219,8 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
       FR_MARK(prof, "common_flux");
       launch_common_flux(c, uf, qf, s);
     }
-    if (tp.tma_q) {
-      FR_MARK(prof, "hex_fluxdiv_tma");
-      e = hex_tma_fluxdiv(c, tp.h_ops, u, qf, uf, rhs, s);
-    } else {  // Q recomputed from the jumps instead of being read back
-      FR_MARK(prof, "hex_rhs_tma");
-      e = hex_tma_rhs(c, tp.h_ops, u, cf, uf, rhs, s);
-    }
+    FR_MARK(prof, "hex_fluxdiv_tma");
+    e = hex_tma_fluxdiv(c, tp.h_ops, u, qf, uf, rhs, s);
     return e != cudaSuccess ? e : cudaGetLastError();
   }
   if (c.ns) {
@@ -238,7 +235,7 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
       k_tp_grad<N, ND, T><<<dim3(ge, 1, 1), dim3(LW, 256 / LW), 0, s>>>(op, u, cf, c.smat, c.rcpj, qu, ncols, c.ld, c.Nel);
     }
     FR_MARK(prof, "tp_interp_q");
-    k_tp_interp<N, ND, double><<<dim3(gx, 1, ND), bf, 0, s>>>(op, qu, qf, ncols, c.ld, c.Nel, (int64_t)NU * ncols, (int64_t)NF * ncols);
+    k_tp_interp<N, ND, double><<<dim3(gx, 1, ND), bf, 0, s>>>(op, qu, qf, ncols, c.ld, c.Nel, (int64_t)NU * ncols, (int64_t)NF * ncols, false);
   }
   static const bool fuse = !getenv("FR_NOFUSE");
   if (ND == 3 && fuse) {
@@ -296,8 +293,8 @@ cudaError_t tensor_plan(const DevConsts &c, const RefOps &o, const MeshConsts &,
   int64_t off = 0;
   tp.off_uf = off; off = al(off + (int64_t)o.Nf * ncols * 8);
   tp.off_cf = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
-  tp.use_tma = c.etype == FR_HEX && hex_tma_supported(c.n, c.f64);
-  tp.tma_q = tp.use_tma && hex_tma_fluxdiv_supported(c.n, c.f64) && !getenv("FR_TMA_RECOMPUTE");
+  tp.use_tma = c.blk;  // decided with the layout of the internal arrays (fr_api.cu)
+  tp.tma_q = tp.use_tma;
   if (tp.use_tma) {  // G^f (and Q, slice-major) besides U^f and the jumps
     tp.off_qu = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
     tp.off_qf = off; if (c.ns && tp.tma_q) off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
@@ -314,7 +311,7 @@ cudaError_t tensor_rhs(const DevConsts &c, const TensorPlan &tp, const void *u, 
 }
 
 int tensor_rhs_launches(const DevConsts &c) {
-  if (c.etype == FR_HEX && hex_tma_supported(c.n, c.f64)) {
+  if (c.blk) {
     int n = c.ns ? 5 : 3;  // interp, (common sol, gradface,) common flux, rhs
     if (c.nbnd) n += c.ns ? 2 : 1;
     if (!c.npairs) n -= c.ns ? 2 : 1;

@@ -58,6 +58,18 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, in
       : "memory");
 }
 
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, int c3, uint64_t *bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(
+          smem_addr(dst)),
+      "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_addr(bar))
+      : "memory");
+}
+__device__ __forceinline__ void tma_store_4d(const CUtensorMap *tm, int c0, int c1, int c2, int c3, const void *src) {
+  asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4}], [%5];" ::"l"(tm), "r"(c0), "r"(c1),
+               "r"(c2), "r"(c3), "r"(smem_addr(src))
+               : "memory");
+}
 // bulk tensor store shared -> global (bulk async-group completion)
 __device__ __forceinline__ void tma_store_3d(const CUtensorMap *tm, int c0, int c1, int c2, const void *src) {
   asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(tm), "r"(c0), "r"(c1), "r"(c2),
@@ -174,6 +186,19 @@ bool encode3(CUtensorMap *m, bool f64, const void *base, uint64_t d0, uint64_t d
                   box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS;
+}
+
+// Element-blocked internal array (fr_dev.hpp: fp_row) [ld / FR_BLK][r2][r1][FR_BLK] as a 4-D map (lane, r1, r2, block);
+// box (E, b1, b2, 1).  Coordinates of a CTA that starts at element e0: (e0 % FR_BLK, row, block of rows, e0 / FR_BLK).
+inline bool encode_blk(CUtensorMap *m, const void *base, uint64_t ld, uint64_t r1, uint64_t r2, uint32_t E, uint32_t b1, uint32_t b2) {
+  EncodeTiledFn fn = encoder();
+  if (!fn) return false;
+  cuuint64_t dims[4] = {(cuuint64_t)FR_BLK, r1, r2, ld / FR_BLK};
+  cuuint64_t strides[3] = {(cuuint64_t)FR_BLK * 8, r1 * FR_BLK * 8, r1 * r2 * FR_BLK * 8};
+  cuuint32_t box[4] = {E, b1, b2, 1};
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 template <typename K>

@@ -267,22 +267,6 @@ def _ptrs(run):
     return run.u.data_ptr(), run.r.data_ptr(), run.work.data_ptr(), run.stream
 
 
-@pytest.mark.parametrize("p", [1, 2, 3, 4, 5])
-def test_tma_recompute_variant(p, monkeypatch):
-    """The alternative last kernel (k_hex_rhs_tma: Q recomputed from U and the jumps instead of read back)."""
-    monkeypatch.setenv("FR_TMA_RECOMPUTE", "1")
-    mesh, disc = W.config("C3", n=3, p=p)
-    o = FROracle(mesh, disc)
-    U = W.config_state("C3", np.asarray(o.xu_phys, float), n=3, p=p)
-    R = o.rhs(U)
-    bar, _ = _bar(o, U, R)
-    ctx = _ctx(mesh, disc)
-    run = GpuRunner(ctx)
-    got = run.rhs(U)
-    assert "hex_rhs_tma" in [n for n, _ in ctx.rhs_profiled(*_ptrs(run))]
-    _check("recompute-p%d" % p, got, R, bar)
-
-
 def test_tma_curved_all_orders_and_ragged_blocks():
     """Curved hexes at every order the TMA kernels are built for, element counts that are not multiples of the CTA tile
     (E = 32, 16, 8 elements), Euler and Navier-Stokes, fp64 and fp32."""
