@@ -105,6 +105,9 @@ def kernel_words(name, nd, NV, Nu, Nf, ns):
         "common_flux_g": 3 * Nf * NV + (nd + 2 + 2) * Nf // 2,              # U^f, G^f -> D~ (in place), normals, J n
         "hex_rhs_tma": (2 * Nu + 2 * Nf) * NV + met,                        # U, jump, S, 1/J, D~ -> R
         "hex_fluxdiv_tma": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
+        # fused triangle kernels (fr_element.cu)
+        "el_gradface": (Nu + 3 * Nf) * NV + met + nd * Nf + nd * Nu * NV,   # U, C, U^f, S, 1/J, normals -> Q, G^f
+        "el_fluxdiv": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
         "tp_grad": (Nu + Nf) * NV + met + (nd + 1) * Nf + (NV - 1) * Nf + Nf,
         "tp_div": (2 * Nu + Nf) * NV + met + (nd + 1) * Nf + ((NV - 1) * Nf if ns else 0) + Nf,
     }

@@ -9,6 +9,7 @@
 
 #include "fr_dev.hpp"
 #include "fr_host.hpp"
+#include "fr_element.hpp"
 #include "fr_hex_tma.hpp"
 #include "fr_tensor.hpp"
 
@@ -125,6 +126,7 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     dc.nd = o.nd; dc.NV = o.nd + 2; dc.Nu = o.Nu; dc.Nf = o.Nf; dc.n = o.n; dc.nfp = o.nfp; dc.etype = o.etype;
     dc.Nel = mc.Nel; dc.ld = ld; dc.npairs = mc.npairs; dc.nbnd = mc.nbnd;
     dc.ns = d->system == FR_NAVIER_STOKES; dc.f64 = d->precision == FR_F64;
+    dc.staged = (d->flags & FR_FLAG_FORCE_GENERIC) != 0;
     dc.ph = Phys{d->gamma, d->mu, d->Pr, d->ldg_beta, d->ldg_tau};
     c->host_only = (d->flags & FR_FLAG_HOST_ONLY) != 0;
     if (c->host_only) { c->use_tensor = false; c->wl = WorkLayout(); c->ready = true; return FR_OK; }
@@ -147,6 +149,7 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     // element-centric flux-point tables of the fused hexahedral gradient kernel (own normals, boundary ids)
     const bool want_tma = !(d->flags & FR_FLAG_FORCE_GENERIC) && o.etype == FR_HEX && dc.ns && hex_tma_supported(o.n, dc.f64);
     if (want_tma) { UP(reblock(mc.fp_n, o.nd * o.Nf), fp_n); if (mc.nbnd) { UP(reblock(mc.fp_pe, o.Nf), fp_pe); } }
+    if (dc.ns && element_fused_supported(dc)) { UP(mc.fp_n, fp_n); if (mc.nbnd) { UP(mc.fp_pe, fp_pe); } }  // fused triangle kernels
 #undef UP
     std::vector<BcDev> bcs(c->mesh.bcs.size());
     for (size_t i = 0; i < bcs.size(); ++i) {

@@ -13,6 +13,7 @@ struct DevConsts {
   int64_t Nel, ld, npairs, nbnd;
   bool ns;       // Navier-Stokes (gradients, LDG) or Euler
   bool f64;      // storage precision of u / rhs
+  bool staged;   // FR_FLAG_FORCE_GENERIC: the paper's staged kernel sequence, no fused kernels
   bool blk;      // library-internal arrays are element-blocked (FR_BLK elements per block), see fp_row()
   Phys ph;
   // dense operators (device, row-major doubles)

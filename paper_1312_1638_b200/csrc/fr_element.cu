@@ -1,0 +1,255 @@
+// Element-per-thread fused kernels for elements with small dense operators (triangles; App A matrices are
+// 10 x 12 ... 30 x 10 at p = 3).  They replace five of the eight launches of the staged generic sequence
+// (fr_generic.cu) by two:
+//
+//   k_el_gradface : Q = J^-T {(M4 - M6 M0) U + M6 C} (Eq 42 :756, Eq 10), Q^f = M0 Q (Eq 43), and at once
+//                   G^f = n . f_vis(U^f, Q^f) (Eq 22-24) with the element's own outward normal; writes Q and G^f.
+//                   Replaces apply_M46_M6, grad_phys, apply_M5 and makes the N_D N_V N_f array Q^f unnecessary.
+//   k_el_fluxdiv  : F~ = S f(U, Q) (Eq 12) and R = -(1/J) {(M1 - M3 M2) F~ + M3 D~} (Eq 44, Eq 19).
+//                   Replaces tflux and apply_M132_M3; F~ never reaches HBM.
+//
+// A CTA owns EB = 32 consecutive elements and runs one thread per (element, conserved variable): every global access is
+// a 256-byte row segment of consecutive elements, the operators sit in shared memory and are read as broadcasts, the
+// per-variable intermediates live in registers and in a [value][thread] shared-memory scratch (conflict free); the
+// steps that couple the variables (viscous flux at a flux point, flux at a solution point) are redistributed over the
+// CTA's threads after one barrier.
+#include "fr_element.hpp"
+
+#include <cstdlib>
+
+namespace fr {
+namespace {
+
+constexpr int EB = 32;        // elements per CTA
+constexpr int NVT = 4;        // variables (2-D): threads per element
+constexpr int TPB = EB * NVT;
+
+// G at one flux point, ND-dimensional: interior n . f_vis(u, q); boundary the complete LDG viscous flux with the App C
+// ghost state (as face_visc in fr_tma.cuh)
+template <int ND, bool BND>
+__device__ __forceinline__ void face_visc_nd(const double *uf, const double (*qf)[ND + 2], const double *nrm, const Phys &ph, int pe,
+                                             const BcDev *__restrict__ bcs, double *G) {
+  constexpr int NV = ND + 2;
+  normal_viscous_flux<ND>(uf, qf, nrm, ph, G);
+  if (BND && pe < 0) {
+    double gi[NV], gl[NV], qg[ND][NV], GR[NV];
+    const double keep = ghost_states<ND>(bcs[-1 - pe], uf, ph.gamma, gi, gl);
+#pragma unroll
+    for (int n = 0; n < ND; ++n)
+#pragma unroll
+      for (int a = 0; a < NV; ++a) qg[n][a] = keep * qf[n][a];
+    normal_viscous_flux<ND>(gl, qg, nrm, ph, GR);
+    const double wl = 0.5 + ph.beta, wr = 0.5 - ph.beta;
+#pragma unroll
+    for (int a = 0; a < NV; ++a) G[a] = (wl != 0.0 ? wl * G[a] : 0.0) + (wr != 0.0 ? wr * GR[a] : 0.0);
+  }
+}
+
+// u [NU][NV][ld] (T), cf = common solution C [NF][NV][ld], uf = U^f [NF][NV][ld]; out: q [ND][NU][NV][ld], gf [NF][NV][ld]
+template <int NU, int NF, bool BND, typename T>
+__global__ void __launch_bounds__(TPB) k_el_gradface(DevConsts c, const T *__restrict__ u, const double *__restrict__ cf,
+                                                      const double *__restrict__ uf, double *__restrict__ q, double *__restrict__ gf) {
+  constexpr int ND = 2, NV = 4;
+  extern __shared__ double smem[];
+  double *sM46 = smem;                    // [ND*NU][NU]
+  double *sM6 = sM46 + ND * NU * NU;      // [ND*NU][NF]
+  double *sM0 = sM6 + ND * NU * NF;       // [NF][NU]
+  double *sQ = sM0 + NF * NU;             // [ND][NU][TPB]       gradient of the thread's variable
+  double *sQf = sQ + ND * NU * TPB;       // [ND][NV][NF][EB]    gradient at the flux points, all variables
+  const int tid = threadIdx.x, el = tid % EB, a = tid / EB;
+  for (int t = tid; t < ND * NU * NU; t += TPB) sM46[t] = c.M46[t];
+  for (int t = tid; t < ND * NU * NF; t += TPB) sM6[t] = c.M6[t];
+  for (int t = tid; t < NF * NU; t += TPB) sM0[t] = c.M0[t];
+  __syncthreads();
+  const int64_t e0 = (int64_t)blockIdx.x * EB, e = e0 + el;
+  const size_t ld = c.ld;
+  if (e < c.Nel) {
+    double uu[NU], cc[NF];
+#pragma unroll
+    for (int r = 0; r < NU; ++r) uu[r] = (double)u[((size_t)r * NV + a) * ld + e];
+#pragma unroll
+    for (int s = 0; s < NF; ++s) cc[s] = cf[((size_t)s * NV + a) * ld + e];
+#pragma unroll 2
+    for (int r = 0; r < NU; ++r) {
+      double qt[ND];
+#pragma unroll
+      for (int d = 0; d < ND; ++d) {
+        const double *m46 = sM46 + (d * NU + r) * NU, *m6 = sM6 + (d * NU + r) * NF;
+        double s = 0;
+#pragma unroll
+        for (int v = 0; v < NU; ++v) s = fma(m46[v], uu[v], s);
+#pragma unroll
+        for (int v = 0; v < NF; ++v) s = fma(m6[v], cc[v], s);
+        qt[d] = s;
+      }
+      const double rj = c.rcpj[(size_t)r * ld + e];
+      double Sm[ND][ND];
+#pragma unroll
+      for (int d = 0; d < ND; ++d)
+#pragma unroll
+        for (int n = 0; n < ND; ++n) Sm[d][n] = c.smat[((size_t)(d * ND + n) * NU + r) * ld + e];
+#pragma unroll
+      for (int n = 0; n < ND; ++n) {
+        double s = 0;
+#pragma unroll
+        for (int d = 0; d < ND; ++d) s = fma(Sm[d][n], qt[d], s);
+        s *= rj;
+        q[(((size_t)n * NU + r) * NV + a) * ld + e] = s;
+        sQ[(n * NU + r) * TPB + tid] = s;
+      }
+    }
+#pragma unroll 1
+    for (int s = 0; s < NF; ++s) {
+      const double *m0 = sM0 + s * NU;
+#pragma unroll
+      for (int n = 0; n < ND; ++n) {
+        double acc = 0;
+#pragma unroll
+        for (int r = 0; r < NU; ++r) acc = fma(m0[r], sQ[(n * NU + r) * TPB + tid], acc);
+        sQf[((n * NV + a) * NF + s) * EB + el] = acc;
+      }
+    }
+  }
+  __syncthreads();
+  // flux points of the CTA's elements, redistributed over all threads
+#pragma unroll
+  for (int t = tid; t < NF * EB; t += TPB) {
+    const int el2 = t % EB, s = t / EB;
+    const int64_t e2 = e0 + el2;
+    if (e2 >= c.Nel) continue;
+    double us[NV], qf[ND][NV], nrm[ND], G[NV];
+#pragma unroll
+    for (int b = 0; b < NV; ++b) us[b] = uf[((size_t)s * NV + b) * ld + e2];
+#pragma unroll
+    for (int n = 0; n < ND; ++n) {
+      nrm[n] = c.fp_n[((size_t)n * NF + s) * ld + e2];
+#pragma unroll
+      for (int b = 0; b < NV; ++b) qf[n][b] = sQf[((n * NV + b) * NF + s) * EB + el2];
+    }
+    const int pe = BND ? c.fp_pe[(size_t)s * ld + e2] : 0;
+    face_visc_nd<ND, BND>(us, qf, nrm, c.ph, pe, c.bcs, G);
+#pragma unroll
+    for (int b = 0; b < NV; ++b) gf[((size_t)s * NV + b) * ld + e2] = G[b];
+  }
+}
+
+// u as above, q [ND][NU][NV][ld], dt = D~ [NF][NV][ld]; rhs like u
+template <int NU, int NF, bool NS, typename T>
+__global__ void __launch_bounds__(TPB) k_el_fluxdiv(DevConsts c, const T *__restrict__ u, const double *__restrict__ q,
+                                                     const double *__restrict__ dt, T *__restrict__ rhs) {
+  constexpr int ND = 2, NV = 4;
+  extern __shared__ double smem[];
+  double *sM132 = smem;                    // [NU][ND*NU]
+  double *sM3 = sM132 + NU * ND * NU;      // [NU][NF]
+  double *sF = sM3 + NU * NF;              // [ND][NV][NU][EB]
+  const int tid = threadIdx.x, el = tid % EB, a = tid / EB;
+  for (int t = tid; t < NU * ND * NU; t += TPB) sM132[t] = c.M132[t];
+  for (int t = tid; t < NU * NF; t += TPB) sM3[t] = c.M3[t];
+  const int64_t e0 = (int64_t)blockIdx.x * EB, e = e0 + el;
+  const size_t ld = c.ld;
+  // F~ = S f(U, Q) at the solution points of the CTA's elements, one (element, point) per thread and pass
+#pragma unroll
+  for (int t = tid; t < NU * EB; t += TPB) {
+    const int el2 = t % EB, r = t / EB;
+    const int64_t e2 = e0 + el2;
+    if (e2 >= c.Nel) continue;
+    double uu[NV], qq[ND][NV], f[ND][NV], v[ND], p;
+#pragma unroll
+    for (int b = 0; b < NV; ++b) uu[b] = (double)u[((size_t)r * NV + b) * ld + e2];
+    inviscid_flux<ND>(uu, c.ph.gamma, f, v, p);
+    if (NS) {
+#pragma unroll
+      for (int n = 0; n < ND; ++n)
+#pragma unroll
+        for (int b = 0; b < NV; ++b) qq[n][b] = q[(((size_t)n * NU + r) * NV + b) * ld + e2];
+      subtract_viscous_flux<ND>(uu, qq, v, c.ph, f);
+    }
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+      const double s0 = c.smat[((size_t)(d * ND + 0) * NU + r) * ld + e2], s1 = c.smat[((size_t)(d * ND + 1) * NU + r) * ld + e2];
+#pragma unroll
+      for (int b = 0; b < NV; ++b) sF[((d * NV + b) * NU + r) * EB + el2] = fma(s0, f[0][b], s1 * f[1][b]);
+    }
+  }
+  __syncthreads();
+  if (e >= c.Nel) return;
+  double dd[NF];
+#pragma unroll
+  for (int s = 0; s < NF; ++s) dd[s] = dt[((size_t)s * NV + a) * ld + e];
+#pragma unroll 1
+  for (int r = 0; r < NU; ++r) {
+    const double *m132 = sM132 + r * ND * NU, *m3 = sM3 + r * NF;
+    double acc = 0;
+#pragma unroll
+    for (int d = 0; d < ND; ++d)
+#pragma unroll
+      for (int v = 0; v < NU; ++v) acc = fma(m132[d * NU + v], sF[((d * NV + a) * NU + v) * EB + el], acc);
+#pragma unroll
+    for (int s = 0; s < NF; ++s) acc = fma(m3[s], dd[s], acc);
+    rhs[((size_t)r * NV + a) * ld + e] = (T)(-acc * c.rcpj[(size_t)r * ld + e]);
+  }
+}
+
+template <int NU, int NF, typename T>
+cudaError_t gradface_t(const DevConsts &c, const void *u, const double *cf, const double *uf, double *q, double *gf, cudaStream_t s) {
+  const size_t smem = (size_t)(2 * NU * NU + 2 * NU * NF + NF * NU + 2 * NU * TPB + 2 * 4 * NF * EB) * sizeof(double);
+  const unsigned grid = (unsigned)((c.Nel + EB - 1) / EB);
+  if (c.nbnd) {
+    auto kern = k_el_gradface<NU, NF, true, T>;
+    static bool done = false;
+    if (!done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); done = true; }
+    kern<<<grid, TPB, smem, s>>>(c, (const T *)u, cf, uf, q, gf);
+  } else {
+    auto kern = k_el_gradface<NU, NF, false, T>;
+    static bool done = false;
+    if (!done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); done = true; }
+    kern<<<grid, TPB, smem, s>>>(c, (const T *)u, cf, uf, q, gf);
+  }
+  return cudaGetLastError();
+}
+
+template <int NU, int NF, typename T>
+cudaError_t fluxdiv_t(const DevConsts &c, const void *u, const double *q, const double *dt, void *rhs, cudaStream_t s) {
+  const size_t smem = (size_t)(2 * NU * NU + NU * NF + 2 * 4 * NU * EB) * sizeof(double);
+  const unsigned grid = (unsigned)((c.Nel + EB - 1) / EB);
+  if (c.ns) {
+    auto kern = k_el_fluxdiv<NU, NF, true, T>;
+    static bool done = false;
+    if (!done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); done = true; }
+    kern<<<grid, TPB, smem, s>>>(c, (const T *)u, q, dt, (T *)rhs);
+  } else {
+    auto kern = k_el_fluxdiv<NU, NF, false, T>;
+    static bool done = false;
+    if (!done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); done = true; }
+    kern<<<grid, TPB, smem, s>>>(c, (const T *)u, q, dt, (T *)rhs);
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+// triangles, p = 1 .. 4  (N_u = (p+1)(p+2)/2, N_f = 3 (p+1))
+bool element_fused_supported(const DevConsts &c) { return c.etype == FR_TRI && !c.staged && c.n >= 2 && c.n <= 5 && !getenv("FR_NO_ELFUSE"); }
+
+#define FR_TRI_CASES(CALL)                 \
+  switch (c.n) {                           \
+    case 2: return CALL(3, 6);             \
+    case 3: return CALL(6, 9);             \
+    case 4: return CALL(10, 12);           \
+    case 5: return CALL(15, 15);           \
+    default: return cudaErrorNotSupported; \
+  }
+
+cudaError_t element_gradface(const DevConsts &c, const void *u, const double *cf, const double *uf, double *q, double *gf, cudaStream_t s) {
+#define FR_CALL(NU, NF) (c.f64 ? gradface_t<NU, NF, double>(c, u, cf, uf, q, gf, s) : gradface_t<NU, NF, float>(c, u, cf, uf, q, gf, s))
+  FR_TRI_CASES(FR_CALL)
+#undef FR_CALL
+}
+
+cudaError_t element_fluxdiv(const DevConsts &c, const void *u, const double *q, const double *dt, void *rhs, cudaStream_t s) {
+#define FR_CALL(NU, NF) (c.f64 ? fluxdiv_t<NU, NF, double>(c, u, q, dt, rhs, s) : fluxdiv_t<NU, NF, float>(c, u, q, dt, rhs, s))
+  FR_TRI_CASES(FR_CALL)
+#undef FR_CALL
+}
+
+}  // namespace fr

@@ -3,6 +3,7 @@
 // fallback for hexahedra (FR_FLAG_FORCE_GENERIC); the tensor-product kernels in fr_tensor.cu replace it
 // for hexahedra.  All arithmetic in double; u / rhs are stored in T (float or double).
 #include "fr_dev.hpp"
+#include "fr_element.hpp"
 #include "fr_hex_tma.hpp"
 
 namespace fr {
@@ -272,6 +273,27 @@ cudaError_t run(const DevConsts &c, const WorkLayout &w, const T *u, T *rhs, cha
   // (1) U^f = M0 U                                                       Eq 41 :745
   FR_MARK(prof, "apply_M0");
   apply<T, double, false>(s, c, Nf, Nu, c.M0, u, 0, nullptr, nullptr, uf);
+  if (ND == 2 && element_fused_supported(c)) {
+    // triangles: fused kernels with one thread per (element, variable) (fr_element.cu), 5 launches (3 for Euler);
+    // Q^f and F~ are never stored
+    cudaError_t e = cudaSuccess;
+    if (NS) {
+      FR_MARK(prof, "common_sol");
+      if (c.npairs) k_common_sol<ND, false><<<blocks(c.npairs), TB, 0, s>>>(c, uf, cf);
+      if (c.nbnd) k_common_sol_bnd<ND, false><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, cf);
+      FR_MARK(prof, "el_gradface");
+      if ((e = element_gradface(c, u, cf, uf, qu, qf, s)) != cudaSuccess) return e;
+      FR_MARK(prof, "common_flux_g");
+      launch_common_flux_g(c, uf, qf, s);
+    } else {
+      FR_MARK(prof, "common_flux");
+      if (c.npairs) k_common_flux<ND, NS><<<blocks(c.npairs), TB, 0, s>>>(c, uf, qf);
+      if (c.nbnd) k_common_flux_bnd<ND, NS><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, qf);
+    }
+    FR_MARK(prof, "el_fluxdiv");
+    e = element_fluxdiv(c, u, qu, uf, rhs, s);
+    return e != cudaSuccess ? e : cudaGetLastError();
+  }
   if (NS) {
     // (2) C^f                                                            Eq 7, 25
     FR_MARK(prof, "common_sol");
@@ -339,11 +361,22 @@ void launch_common_flux(const DevConsts &c, double *uf, const double *qf, cudaSt
 
 void launch_common_flux_g(const DevConsts &c, double *uf, const double *gf, cudaStream_t s) {
   const int TB = 128;
-  if (c.npairs) k_common_flux_g<3><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
-  if (c.nbnd) k_common_flux_bnd_g<3><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
+  if (c.nd == 2) {
+    if (c.npairs) k_common_flux_g<2><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
+    if (c.nbnd) k_common_flux_bnd_g<2><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
+  } else {
+    if (c.npairs) k_common_flux_g<3><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
+    if (c.nbnd) k_common_flux_bnd_g<3><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
+  }
 }
 
 int generic_rhs_launches(const DevConsts &c) {
+  if (c.nd == 2 && element_fused_supported(c)) {
+    int n = c.ns ? 5 : 3;  // interp, (common sol, gradface,) common flux, fluxdiv
+    if (c.nbnd) n += c.ns ? 2 : 1;
+    if (!c.npairs) n -= c.ns ? 2 : 1;
+    return n;
+  }
   int n = 4;  // interp, tflux, common flux, divergence
   if (c.ns) n += 4;  // common solution, gradient, transform, interp of gradient
   if (c.nbnd) n += c.ns ? 2 : 1;

@@ -341,3 +341,16 @@ def test_pre_tma_hex_kernels_still_match(monkeypatch):
     names = [n for n, _ in ctx.rhs_profiled(*_ptrs(run))]
     assert "hex_grad" in names and "hex_fluxdiv" in names, names
     _check("pre-tma-p3", got, R, bar)
+
+
+def test_fused_triangle_path_is_the_default():
+    """Triangles, p <= 4: 5 launches per Navier-Stokes RHS with the fused element kernels (fr_element.cu); the staged
+    paper sequence stays reachable through FR_FLAG_FORCE_GENERIC (both are compared with the oracle in
+    test_rhs_parity_fp64[C4-24-*])."""
+    mesh, disc = W.config("C4", n=8)
+    ctx = _ctx(mesh, disc)
+    assert ctx.rhs_kernel_launches == 5
+    names = [n for n, _ in ctx.rhs_profiled(*_ptrs(GpuRunner(ctx)))]
+    assert "el_gradface" in names and "el_fluxdiv" in names, names
+    ctx2 = _ctx(mesh, disc, flags=1)
+    assert ctx2.rhs_kernel_launches == 8
