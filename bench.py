@@ -99,11 +99,10 @@ def kernel_words(name, nd, NV, Nu, Nf, ns):
         "tp_interp_q": nd * (Nu + Nf) * NV,
         "hex_grad": (Nu + Nf) * NV + met + nd * Nu * NV,
         "hex_fluxdiv": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
-        "hex_rhs": (2 * Nu + 2 * Nf) * NV + met,
         # TMA-pipelined hexahedral path (fr_hex_tma.cu, fr_hex_fluxdiv_tma.cu)
+        "hex_interp_tma": (Nu + Nf) * NV,
         "hex_gradface": (Nu + 2 * Nf) * NV + met + nd * Nf + nd * Nu * NV,  # U, jump, S, 1/J, normals -> G^f, Q
         "common_flux_g": 3 * Nf * NV + (nd + 2 + 2) * Nf // 2,              # U^f, G^f -> D~ (in place), normals, J n
-        "hex_rhs_tma": (2 * Nu + 2 * Nf) * NV + met,                        # U, jump, S, 1/J, D~ -> R
         "hex_fluxdiv_tma": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
         # fused triangle kernels (fr_element.cu)
         "el_gradface": (Nu + 3 * Nf) * NV + met + nd * Nf + nd * Nu * NV,   # U, C, U^f, S, 1/J, normals -> Q, G^f

@@ -178,124 +178,3 @@ __global__ void __launch_bounds__(N *N *E) k_hex_grad(Ops1D<N> op, const T *__re
     }
   }
 }
-
-// Parts (2b)-(7) for Navier-Stokes in one kernel: Q = J^-T {M4 U + M6 (C - U^f)} is recomputed at every
-// point from U and the interface jumps (never stored), then F~ = S f(U, Q), then
-// rhs = -(1/J) {(M1 - M3 M2) F~ + M3 D~}   (Eq 9, 10, 12, 18, 19).
-// The whole U block of the CTA's E elements sits in shared memory (z lines), F~ slices are double buffered
-// when they fit (NB = 2).
-template <int N, int E, int NB, typename T>
-__global__ void __launch_bounds__(N *N *E) k_hex_rhs(Ops1D<N> op, Phys ph, const T *__restrict__ u, const double *__restrict__ jump,
-                                                     const double *__restrict__ smat, const double *__restrict__ rcpj,
-                                                     const double *__restrict__ dt, T *__restrict__ rhs, int64_t ld, int64_t Nel) {
-  constexpr int NV = 5, NFP = N * N, NU = N * N * N;
-  extern __shared__ double smem[];
-  double *sD = smem;                  // [N*N]
-  double *sDh = sD + N * N;           // [N*N]
-  double *sU = sDh + N * N;           // [NV][NU][E]
-  double *sF = sU + NV * NU * E;      // [NB][2][NV][NFP][E]
-  const int el = threadIdx.x, ij = threadIdx.y, i = ij % N, j = ij / N;
-  const int64_t e = (int64_t)blockIdx.x * E + el;
-  const bool act = e < Nel;
-  for (int t = ij * E + el; t < N * N; t += NFP * E) { sD[t] = op.D[t]; sDh[t] = op.Dh[t]; }
-#pragma unroll
-  for (int k = 0; k < N; ++k)
-#pragma unroll
-    for (int a = 0; a < NV; ++a)
-      sU[(a * NU + ij + NFP * k) * E + el] = act ? (double)u[((size_t)(ij + NFP * k) * NV + a) * ld + e] : 1.0;
-  double jzm[NV], jzp[NV];
-#pragma unroll
-  for (int a = 0; a < NV; ++a) {
-    jzm[a] = act ? jump[((size_t)(4 * NFP + ij) * NV + a) * ld + e] : 0.0;
-    jzp[a] = act ? jump[((size_t)(5 * NFP + ij) * NV + a) * ld + e] : 0.0;
-  }
-  const double gmi = op.gm[i], gpi = op.gp[i], gmj = op.gm[j], gpj = op.gp[j];
-  double acc[N][NV];
-#pragma unroll
-  for (int k = 0; k < N; ++k)
-#pragma unroll
-    for (int a = 0; a < NV; ++a) acc[k][a] = 0.0;
-  __syncthreads();
-
-#pragma unroll
-  for (int k = 0; k < N; ++k) {
-    const int r = ij + NFP * k;
-    double F[3][NV];
-    if (act) {
-      double uu[NV], qq[3][NV], S[3][3];
-#pragma unroll
-      for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b) S[a][b] = smat[((size_t)(a * 3 + b) * NU + r) * ld + e];
-      const double rj = rcpj[(size_t)r * ld + e];
-      const int fx = j + N * k, fy = i + N * k;
-#pragma unroll
-      for (int a = 0; a < NV; ++a) {
-        const double *su = sU + (size_t)a * NU * E + el;
-        uu[a] = su[r * E];
-        double qx = fma(gpi, jump[((size_t)(1 * NFP + fx) * NV + a) * ld + e], -gmi * jump[((size_t)(0 * NFP + fx) * NV + a) * ld + e]);
-        double qy = fma(gpj, jump[((size_t)(3 * NFP + fy) * NV + a) * ld + e], -gmj * jump[((size_t)(2 * NFP + fy) * NV + a) * ld + e]);
-        double qz = fma(op.gp[k], jzp[a], -op.gm[k] * jzm[a]);
-#pragma unroll
-        for (int m = 0; m < N; ++m) {
-          qx = fma(sD[i * N + m], su[(NFP * k + j * N + m) * E], qx);
-          qy = fma(sD[j * N + m], su[(NFP * k + m * N + i) * E], qy);
-          qz = fma(op.D[k * N + m], su[(NFP * m + ij) * E], qz);
-        }
-#pragma unroll
-        for (int n = 0; n < 3; ++n) qq[n][a] = rj * fma(S[0][n], qx, fma(S[1][n], qy, S[2][n] * qz));
-      }
-      point_tflux<true>(uu, qq, S, ph, F);
-    } else {
-#pragma unroll
-      for (int d = 0; d < 3; ++d)
-#pragma unroll
-        for (int a = 0; a < NV; ++a) F[d][a] = 0.0;
-    }
-    if (NB == 1) __syncthreads();
-    double *buf = sF + (NB == 2 ? (k & 1) : 0) * (2 * NV * NFP * E);
-#pragma unroll
-    for (int a = 0; a < NV; ++a) {
-      buf[((0 * NV + a) * NFP + ij) * E + el] = F[0][a];
-      buf[((1 * NV + a) * NFP + ij) * E + el] = F[1][a];
-    }
-#pragma unroll
-    for (int kk = 0; kk < N; ++kk)
-#pragma unroll
-      for (int a = 0; a < NV; ++a) acc[kk][a] = fma(op.Dh[kk * N + k], F[2][a], acc[kk][a]);
-    __syncthreads();
-#pragma unroll
-    for (int m = 0; m < N; ++m) {
-      const double dx = sDh[i * N + m], dy = sDh[j * N + m];
-#pragma unroll
-      for (int a = 0; a < NV; ++a) {
-        acc[k][a] = fma(dx, buf[((0 * NV + a) * NFP + j * N + m) * E + el], acc[k][a]);
-        acc[k][a] = fma(dy, buf[((1 * NV + a) * NFP + m * N + i) * E + el], acc[k][a]);
-      }
-    }
-  }
-  if (!act) return;
-  double dzm[NV], dzp[NV];
-#pragma unroll
-  for (int a = 0; a < NV; ++a) {
-    dzm[a] = dt[((size_t)(4 * NFP + ij) * NV + a) * ld + e];
-    dzp[a] = dt[((size_t)(5 * NFP + ij) * NV + a) * ld + e];
-  }
-#pragma unroll
-  for (int k = 0; k < N; ++k) {
-    const int r = ij + NFP * k;
-    const double rj = rcpj[(size_t)r * ld + e];
-    const int fx = j + N * k, fy = i + N * k;
-#pragma unroll
-    for (int a = 0; a < NV; ++a) {
-      double v = acc[k][a];
-      v = fma(op.gm[k], dzm[a], v);
-      v = fma(op.gp[k], dzp[a], v);
-      v = fma(gmi, dt[((size_t)(0 * NFP + fx) * NV + a) * ld + e], v);
-      v = fma(gpi, dt[((size_t)(1 * NFP + fx) * NV + a) * ld + e], v);
-      v = fma(gmj, dt[((size_t)(2 * NFP + fy) * NV + a) * ld + e], v);
-      v = fma(gpj, dt[((size_t)(3 * NFP + fy) * NV + a) * ld + e], v);
-      rhs[((size_t)r * NV + a) * ld + e] = (T)(-v * rj);
-    }
-  }
-}

@@ -8,6 +8,9 @@ namespace fr {
 // the tensor-map encoder.  The internal arrays are then element-blocked (fr_dev.hpp: fp_row).
 bool hex_tma_supported(int n, bool f64);
 
+// U^f = M0 U, element-blocked output (part 1; fr_hex_interp_tma.cu)
+cudaError_t hex_tma_interp(const DevConsts &c, const double *h_ops, const void *u, double *uf, cudaStream_t s);
+
 // G^f = n . f_vis(U^f, Q^f) at every flux point, Q computed from u and jump = C - U^f  (parts 2b, 3 of the north_star);
 // q != NULL: Q is also stored, slice-major [N][3][NV][NFP][ld], for hex_tma_fluxdiv
 cudaError_t hex_tma_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, double *q,

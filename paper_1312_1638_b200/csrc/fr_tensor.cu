@@ -162,19 +162,6 @@ void launch_hex_fluxdiv(const Ops1D<N> &op, const DevConsts &c, const T *u, cons
   launch_hex_fluxdiv_e<N, E, NS, T>(op, c, u, qu, dt, rhs, s);
 }
 
-template <int N, typename T>
-void launch_hex_rhs(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *jump, const double *dt, T *rhs, cudaStream_t s) {
-  constexpr int E = N <= 3 ? 32 : (N <= 5 ? 16 : 8);
-  constexpr size_t base = (size_t)(2 * N * N + 5 * N * N * N * E) * sizeof(double);
-  constexpr size_t slice = (size_t)(2 * 5 * N * N * E) * sizeof(double);
-  constexpr int NB = (base + 2 * slice <= 200 * 1024) ? 2 : 1;
-  const size_t smem = base + NB * slice;
-  auto kern = k_hex_rhs<N, E, NB, T>;
-  static bool attr_done = false;
-  if (!attr_done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
-  kern<<<(unsigned)((c.Nel + E - 1) / E), dim3(E, N * N), smem, s>>>(op, c.ph, u, jump, c.smat, c.rcpj, dt, rhs, c.ld, c.Nel);
-}
-
 template <int N, int E, typename T>
 void launch_hex_grad_e(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *jump, double *qu, cudaStream_t s) {
   const size_t smem = (size_t)(N * N + 2 * 5 * N * N * E) * sizeof(double);
@@ -202,8 +189,15 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
   const int rows = 1024 / LW;
   const unsigned gx = (unsigned)((ncols + LW - 1) / LW), ge = (unsigned)((c.Nel + LW - 1) / LW);
   const dim3 bf(LW, NFP < rows ? NFP : rows), bu(LW, NU < rows ? NU : rows);
-  FR_MARK(prof, "tp_interp");
-  k_tp_interp<N, ND, T><<<dim3(gx, 1, 1), bf, 0, s>>>(op, u, uf, ncols, c.ld, c.Nel, 0, 0, c.blk);
+  static const bool tma_interp = !getenv("FR_NO_TMA_INTERP");
+  if (ND == 3 && tp.use_tma && tma_interp) {
+    FR_MARK(prof, "hex_interp_tma");
+    cudaError_t e = hex_tma_interp(c, tp.h_ops, u, uf, s);
+    if (e != cudaSuccess) return e;
+  } else {
+    FR_MARK(prof, "tp_interp");
+    k_tp_interp<N, ND, T><<<dim3(gx, 1, 1), bf, 0, s>>>(op, u, uf, ncols, c.ld, c.Nel, 0, 0, c.blk);
+  }
   if (ND == 3 && tp.use_tma) {
     // sm_100a path: 5 launches for Navier-Stokes (3 for Euler); neither Q^f nor F~ is stored
     cudaError_t e = cudaSuccess;
@@ -241,12 +235,6 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
   if (ND == 3 && fuse) {
     FR_MARK(prof, "common_flux");
     launch_common_flux(c, uf, qf, s);
-    static const bool recompute = getenv("FR_RECOMPUTE") != nullptr;  // experimental: recompute Q instead of reading it
-    if (c.ns && recompute) {
-      FR_MARK(prof, "hex_rhs");
-      launch_hex_rhs<N, T>(op, c, u, cf, uf, rhs, s);
-      return cudaGetLastError();
-    }
     FR_MARK(prof, "hex_fluxdiv");
     if (c.ns) launch_hex_fluxdiv<N, true, T>(op, c, u, qu, uf, rhs, s);
     else launch_hex_fluxdiv<N, false, T>(op, c, u, qu, uf, rhs, s);
