@@ -10,6 +10,9 @@ namespace fr {
 namespace {
 
 constexpr int RT = 8;  // rows of the operator per thread
+#ifndef FLUXG_MINB
+#define FLUXG_MINB 6  // resident CTAs of the gather-bound interface kernel: occupancy is what hides its latency
+#endif
 
 // out[blk][r][col] = sum_k A[r][k] in1[blk][k][col] (+ sum_k B[r][k] in2[k][col]),  col = a*ld + e.
 // SCALE: multiply by -rcpj[r][e] (Eq 19 :243, the paper's negdivconf kernel).
@@ -155,7 +158,7 @@ __global__ void k_tflux(DevConsts c, const T *__restrict__ u, double *__restrict
 
 // Common normal flux over flux-point pairs, Eq 15-17 (:227-235); in place over U^f -> D~ (:300)
 template <int ND, bool NS>
-__global__ void k_common_flux(DevConsts c, double *__restrict__ uf, const double *__restrict__ qf) {
+__global__ void __launch_bounds__(128, NS ? 2 : FLUXG_MINB) k_common_flux(DevConsts c, double *__restrict__ uf, const double *__restrict__ qf) {
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.npairs) return;
@@ -209,7 +212,7 @@ __global__ void k_common_flux_bnd(DevConsts c, double *__restrict__ uf, const do
 // gf = n_own . f_vis(u^f, q^f) at every flux point with the element's OWN outward normal, so that
 // n_L . f_R^vis = -gf_R.   F = Rusanov + tau (u_L - u_R) - {(1/2+beta) gf_L - (1/2-beta) gf_R}   (Eq 26-27, A7)
 template <int ND>
-__global__ void k_common_flux_g(DevConsts c, double *__restrict__ uf, const double *__restrict__ gf) {
+__global__ void __launch_bounds__(128, FLUXG_MINB) k_common_flux_g(DevConsts c, double *__restrict__ uf, const double *__restrict__ gf) {
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.npairs) return;
