@@ -213,7 +213,7 @@ cudaError_t set_smem(K kern, size_t smem, bool &done) {
 // elements per CTA for each n = p + 1 (row segments of E*8 bytes)
 template <int N>
 struct Cfg {
-  static constexpr int E = N <= 2 ? 32 : (N == 3 ? 16 : 8);
+  static constexpr int E = N <= 2 ? 32 : (N == 3 ? 16 : (N <= 6 ? 8 : 4));  // N = 7: only 4 elements fit the shared memory
 };
 
 int env_e() {
