@@ -229,7 +229,7 @@ cudaError_t fluxdiv_t(const DevConsts &c, const void *u, const double *q, const 
 }  // namespace
 
 // triangles, p = 1 .. 4  (N_u = (p+1)(p+2)/2, N_f = 3 (p+1))
-bool element_fused_supported(const DevConsts &c) { return c.etype == FR_TRI && !c.staged && c.n >= 2 && c.n <= 5 && !getenv("FR_NO_ELFUSE"); }
+bool element_fused_supported(const DevConsts &c) { return c.etype == FR_TRI && !c.staged && c.n >= 2 && c.n <= 5; }
 
 #define FR_TRI_CASES(CALL)                 \
   switch (c.n) {                           \

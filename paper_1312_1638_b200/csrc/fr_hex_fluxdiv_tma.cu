@@ -231,7 +231,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   }
 }
 
-template <int N, int E, bool NS, typename T, int CAP = 8>
+template <int N, int E, bool NS, typename T>
 cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *u, const double *q, const double *dt, void *rhs,
                            cudaStream_t s) {
   constexpr int NFP = N * N, NU = N * NFP;
@@ -241,7 +241,7 @@ cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *
   constexpr int NB = (L2::TOTAL <= SMEM_MAX && min_blocks(L2::TOTAL, N * N * E) == min_blocks(L1::TOTAL, N * N * E)) ? 2 : 1;
   using L = FdLay<N, E, NS, T, NB>;
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
-  constexpr int MINB = min_blocks(L::TOTAL, N * N * E) < CAP ? min_blocks(L::TOTAL, N * N * E) : CAP;
+  constexpr int MINB = min_blocks(L::TOTAL, N * N * E);
   const uint64_t ld = (uint64_t)c.ld;
   CUtensorMap mS, mU, mQ, mD4, mD2, mR;
   static_assert(FR_BLK % E == 0, "a CTA's elements must lie in one element block");
@@ -271,9 +271,6 @@ constexpr bool fd_fits() {
 template <int N, typename T>
 cudaError_t fluxdiv_n(const DevConsts &c, const double *h_ops, const void *u, const double *q, const double *dt, void *rhs, cudaStream_t s) {
   if constexpr (fd_fits<N, T>()) {
-    if constexpr (N == 5 && sizeof(T) == 8) {  // tuning variant FR_TMA_E=16
-      if (env_e() == 16) return c.ns ? launch_fluxdiv<N, 16, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, 16, false, T>(c, h_ops, u, q, dt, rhs, s);
-    }
     constexpr int E = Cfg<N>::E;
     return c.ns ? launch_fluxdiv<N, E, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, E, false, T>(c, h_ops, u, q, dt, rhs, s);
   } else {

@@ -258,12 +258,12 @@ cudaError_t launch_gradface_k(const DevConsts &c, const Maps<N, E> &m, const Ops
   return cudaGetLastError();
 }
 
-template <int N, int E, typename T, int CAP = 8>
+template <int N, int E, typename T>
 cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, double *q,
                             cudaStream_t s) {
   using L = GfLay<N, E, T>;
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
-  constexpr int MINB = min_blocks(L::TOTAL, N * N * E) < CAP ? min_blocks(L::TOTAL, N * N * E) : CAP;
+  constexpr int MINB = min_blocks(L::TOTAL, N * N * E);
   Maps<N, E> m;
   if (!make_maps<N, E, T>(c, u, jump, m, q)) return cudaErrorNotSupported;
   const Ops1D<N> op = make_ops<N>(h_ops);
@@ -279,9 +279,6 @@ constexpr bool fits() {
 template <int N, typename T>
 cudaError_t gradface_n(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, double *q, cudaStream_t s) {
   if constexpr (fits<N, T>()) {
-    if constexpr (N == 5 && sizeof(T) == 8) {  // tuning variant FR_TMA_E=16: one CTA of 16 elements per SM
-      if (env_e() == 16) return launch_gradface<N, 16, T>(c, h_ops, u, jump, gf, q, s);
-    }
     return launch_gradface<N, Cfg<N>::E, T>(c, h_ops, u, jump, gf, q, s);
   } else {
     return cudaErrorNotSupported;

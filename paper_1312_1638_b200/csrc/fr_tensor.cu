@@ -157,8 +157,6 @@ void launch_hex_fluxdiv_e(const Ops1D<N> &op, const DevConsts &c, const T *u, co
 template <int N, bool NS, typename T>
 void launch_hex_fluxdiv(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *qu, const double *dt, T *rhs, cudaStream_t s) {
   constexpr int E = N <= 3 ? 32 : (N <= 5 ? 16 : 8);
-  static const int e_env = getenv("FR_E") ? atoi(getenv("FR_E")) : 0;
-  if (e_env == 8 && E > 8) return launch_hex_fluxdiv_e<N, 8, NS, T>(op, c, u, qu, dt, rhs, s);
   launch_hex_fluxdiv_e<N, E, NS, T>(op, c, u, qu, dt, rhs, s);
 }
 
@@ -173,8 +171,6 @@ void launch_hex_grad_e(const Ops1D<N> &op, const DevConsts &c, const T *u, const
 template <int N, typename T>
 void launch_hex_grad(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *jump, double *qu, cudaStream_t s) {
   constexpr int E = N <= 3 ? 32 : (N <= 5 ? 16 : 8);
-  static const int e_env = getenv("FR_E") ? atoi(getenv("FR_E")) : 0;
-  if (e_env == 8 && E > 8) return launch_hex_grad_e<N, 8, T>(op, c, u, jump, qu, s);
   launch_hex_grad_e<N, E, T>(op, c, u, jump, qu, s);
 }
 
@@ -185,12 +181,11 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
   const int64_t ncols = (int64_t)c.NV * c.ld;
   double *uf = (double *)(work + tp.off_uf), *cf = (double *)(work + tp.off_cf), *qu = (double *)(work + tp.off_qu),
          *qf = (double *)(work + tp.off_qf);
-  static const int LW = getenv("FR_LW") ? atoi(getenv("FR_LW")) : 32;   // lanes (columns) per CTA row
+  constexpr int LW = 32;  // lanes (columns) per CTA row
   const int rows = 1024 / LW;
   const unsigned gx = (unsigned)((ncols + LW - 1) / LW), ge = (unsigned)((c.Nel + LW - 1) / LW);
   const dim3 bf(LW, NFP < rows ? NFP : rows), bu(LW, NU < rows ? NU : rows);
-  static const bool tma_interp = !getenv("FR_NO_TMA_INTERP");
-  if (ND == 3 && tp.use_tma && tma_interp) {
+  if (ND == 3 && tp.use_tma) {
     FR_MARK(prof, "hex_interp_tma");
     cudaError_t e = hex_tma_interp(c, tp.h_ops, u, uf, s);
     if (e != cudaSuccess) return e;
@@ -205,7 +200,7 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
       FR_MARK(prof, "common_sol");
       launch_common_jump(c, uf, cf, s);
       FR_MARK(prof, "hex_gradface");
-      e = hex_tma_gradface(c, tp.h_ops, u, cf, qu, tp.tma_q ? qf : nullptr, s);
+      e = hex_tma_gradface(c, tp.h_ops, u, cf, qu, qf, s);
       if (e != cudaSuccess) return e;
       FR_MARK(prof, "common_flux_g");
       launch_common_flux_g(c, uf, qu, s);
@@ -220,8 +215,7 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
   if (c.ns) {
     FR_MARK(prof, "common_sol");
     launch_common_jump(c, uf, cf, s);
-    static const bool fuse_g = !getenv("FR_NOFUSE");
-    if (ND == 3 && fuse_g) {
+    if (ND == 3) {
       FR_MARK(prof, "hex_grad");
       launch_hex_grad<N, T>(op, c, u, cf, qu, s);
     } else {
@@ -231,8 +225,7 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
     FR_MARK(prof, "tp_interp_q");
     k_tp_interp<N, ND, double><<<dim3(gx, 1, ND), bf, 0, s>>>(op, qu, qf, ncols, c.ld, c.Nel, (int64_t)NU * ncols, (int64_t)NF * ncols, false);
   }
-  static const bool fuse = !getenv("FR_NOFUSE");
-  if (ND == 3 && fuse) {
+  if (ND == 3) {
     FR_MARK(prof, "common_flux");
     launch_common_flux(c, uf, qf, s);
     FR_MARK(prof, "hex_fluxdiv");
@@ -282,10 +275,9 @@ cudaError_t tensor_plan(const DevConsts &c, const RefOps &o, const MeshConsts &,
   tp.off_uf = off; off = al(off + (int64_t)o.Nf * ncols * 8);
   tp.off_cf = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
   tp.use_tma = c.blk;  // decided with the layout of the internal arrays (fr_api.cu)
-  tp.tma_q = tp.use_tma;
   if (tp.use_tma) {  // G^f (and Q, slice-major) besides U^f and the jumps
     tp.off_qu = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
-    tp.off_qf = off; if (c.ns && tp.tma_q) off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
+    tp.off_qf = off; if (c.ns) off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
   } else {
     tp.off_qu = off; off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
     tp.off_qf = off; if (c.ns) off = al(off + (int64_t)o.nd * o.Nf * ncols * 8);

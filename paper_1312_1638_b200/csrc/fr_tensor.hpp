@@ -12,8 +12,7 @@ struct TensorPlan {
   // workspace offsets (bytes): U^f (-> D~), jump C - U^f, Q~ -> Q -> F~, Q^f
   int64_t off_uf = 0, off_cf = 0, off_qu = 0, off_qf = 0;
   double h_ops[2 * 64 + 4 * 8];   // host copy of the 1-D operators: D, Dhat, lm, lp, gm, gp (n <= 8)
-  bool use_tma = false;           // hexahedra on the TMA-pipelined kernels (fr_hex_tma.cu); off_qu then holds G^f
-  bool tma_q = false;             // Q is stored by the gradient kernel (off_qf) and read back by k_hex_fluxdiv_tma
+  bool use_tma = false;           // hexahedra on the TMA-pipelined kernels (fr_hex_tma.cu); off_qu then holds G^f, off_qf the slice-major Q
 };
 
 bool tensor_supported(const DevConsts &c);

@@ -216,10 +216,5 @@ struct Cfg {
   static constexpr int E = N <= 2 ? 32 : (N == 3 ? 16 : (N <= 6 ? 8 : 4));  // N = 7: only 4 elements fit the shared memory
 };
 
-int env_e() {
-  static const int v = getenv("FR_TMA_E") ? atoi(getenv("FR_TMA_E")) : 0;
-  return v;
-}
-
 }  // namespace
 }  // namespace fr
