@@ -141,7 +141,14 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     };
 #define UP(vec, field) if (e == cudaSuccess) e = upload(c, vec, &dc.field)
     UP(o.M[0], M0); UP(o.M[3], M3); UP(o.M[6], M6); UP(o.M46, M46); UP(o.M132, M132);
-    if (dc.blk) { UP(reblock(mc.smat, o.nd * o.nd * o.Nu), smat); UP(reblock(mc.rcpj, o.Nu), rcpj); }
+    dc.aff = dc.blk && mc.affine;
+    if (dc.aff) {  // affine hexahedra: one point of S and 1/J per element; the tensor maps broadcast it (fr_tma.cuh: encode_blk)
+      const int nn = o.nd * o.nd;
+      std::vector<double> s_el((size_t)nn * ld), r_el((size_t)ld);
+      for (int cc = 0; cc < nn; ++cc) std::memcpy(&s_el[(size_t)cc * ld], &mc.smat[(size_t)cc * o.Nu * ld], ld * sizeof(double));
+      std::memcpy(r_el.data(), mc.rcpj.data(), ld * sizeof(double));
+      UP(reblock(s_el, nn), smat); UP(reblock(r_el, 1), rcpj);
+    } else if (dc.blk) { UP(reblock(mc.smat, o.nd * o.nd * o.Nu), smat); UP(reblock(mc.rcpj, o.Nu), rcpj); }
     else { UP(mc.smat, smat); UP(mc.rcpj, rcpj); }
     UP(mc.pLs, pLs); UP(mc.pLe, pLe); UP(mc.pRs, pRs); UP(mc.pRe, pRe);
     UP(mc.pn, pn); UP(mc.pJnL, pJnL); UP(mc.pJnR, pJnR);

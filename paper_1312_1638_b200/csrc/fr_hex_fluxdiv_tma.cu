@@ -42,8 +42,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     k_hex_fluxdiv_tma(const __grid_constant__ CUtensorMap tmS, const __grid_constant__ CUtensorMap tmU,
                       const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmD4,
                       const __grid_constant__ CUtensorMap tmD2, const __grid_constant__ CUtensorMap tmR, Ops1D<N> op, Phys ph,
-                      const double *__restrict__ rcpj,
-                      const double *__restrict__ dt, T *__restrict__ rhs, int64_t ld, int64_t Nel) {
+                      const double *__restrict__ rcpj, bool aff, const double *__restrict__ dt, T *__restrict__ rhs, int64_t ld,
+                      int64_t Nel) {
   using L = FdLay<N, E, NS, T, NB>;
   constexpr int NFP = N * N;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -215,7 +215,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
   for (int k = 0; k < N; ++k) {
     const int r = ij + NFP * k;
-    const double rj = rcpj[fp_row(true, ld, N * NFP, r, e)];
+    const double rj = aff ? rcpj[fp_row(true, ld, 1, 0, e)] : rcpj[fp_row(true, ld, N * NFP, r, e)];
     const int fx = j + N * k, fy = i + N * k;
 #pragma unroll
     for (int a = 0; a < NV; ++a) {
@@ -245,20 +245,20 @@ cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *
   const uint64_t ld = (uint64_t)c.ld;
   CUtensorMap mS, mU, mQ, mD4, mD2, mR;
   static_assert(FR_BLK % E == 0, "a CTA's elements must lie in one element block");
-  bool ok = encode_blk(&mS, c.smat, ld, NU, 9, E, NFP, 9);
+  bool ok = encode_blk(&mS, c.smat, ld, NU, 9, E, NFP, 9, c.aff ? 1 : 0);
   ok = ok && encode3(&mU, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 1);  // caller layout
   if (NS) ok = ok && encode_blk(&mQ, q, ld, NV * NFP, 3 * N, E, NV * NFP, 3);
   else mQ = mS;
   ok = ok && encode_blk(&mD4, dt, ld, NFP * NV, 6, E, NFP * NV, 4);
   ok = ok && encode_blk(&mD2, dt, ld, NFP * NV, 6, E, NFP * NV, 2);
-  ok = ok && encode_blk(&mR, c.rcpj, ld, NFP, N, E, NFP, N);
+  ok = ok && encode_blk(&mR, c.rcpj, ld, NFP, N, E, NFP, N, c.aff ? 2 : 0);
   if (!ok) return cudaErrorNotSupported;
   auto kern = k_hex_fluxdiv_tma<N, E, NS, T, NB, MINB>;
   static bool done = false;
   cudaError_t err = set_smem(kern, L::TOTAL, done);
   if (err != cudaSuccess) return err;
   const Ops1D<N> op = make_ops<N>(h_ops);
-  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(mS, mU, mQ, mD4, mD2, mR, op, c.ph, c.rcpj, dt, (T *)rhs, c.ld,
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(mS, mU, mQ, mD4, mD2, mR, op, c.ph, c.rcpj, c.aff, dt, (T *)rhs, c.ld,
                                                                   c.Nel);
   return cudaGetLastError();
 }

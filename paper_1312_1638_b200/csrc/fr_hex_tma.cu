@@ -236,8 +236,8 @@ bool make_maps(const DevConsts &c, const void *u, const double *jump, Maps<N, E>
   static_assert(FR_BLK % E == 0, "a CTA's elements must lie in one element block");
   const uint64_t ld = (uint64_t)c.ld;
   bool ok = encode3(&m.U, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, N);  // caller layout
-  ok = ok && encode_blk(&m.S, c.smat, ld, NU, 9, E, NFP, 9);
-  ok = ok && encode_blk(&m.R1, c.rcpj, ld, NFP, N, E, NFP, 1);
+  ok = ok && encode_blk(&m.S, c.smat, ld, NU, 9, E, NFP, 9, c.aff ? 1 : 0);
+  ok = ok && encode_blk(&m.R1, c.rcpj, ld, NFP, N, E, NFP, 1, c.aff ? 2 : 0);
   ok = ok && encode_blk(&m.J, jump, ld, NFP * NV, 6, E, N * NV, 4);
   ok = ok && encode_blk(&m.Jz, jump, ld, NFP * NV, 6, E, NFP * NV, 2);
   if (q) ok = ok && encode_blk(&m.Q, q, ld, NV * NFP, 3 * N, E, NV * NFP, 3);

@@ -190,11 +190,16 @@ bool encode3(CUtensorMap *m, bool f64, const void *base, uint64_t d0, uint64_t d
 
 // Element-blocked internal array (fr_dev.hpp: fp_row) [ld / FR_BLK][r2][r1][FR_BLK] as a 4-D map (lane, r1, r2, block);
 // box (E, b1, b2, 1).  Coordinates of a CTA that starts at element e0: (e0 % FR_BLK, row, block of rows, e0 / FR_BLK).
-inline bool encode_blk(CUtensorMap *m, const void *base, uint64_t ld, uint64_t r1, uint64_t r2, uint32_t E, uint32_t b1, uint32_t b2) {
+inline bool encode_blk(CUtensorMap *m, const void *base, uint64_t ld, uint64_t r1, uint64_t r2, uint32_t E, uint32_t b1, uint32_t b2,
+                       int bcast = 0) {
   EncodeTiledFn fn = encoder();
   if (!fn) return false;
   cuuint64_t dims[4] = {(cuuint64_t)FR_BLK, r1, r2, ld / FR_BLK};
   cuuint64_t strides[3] = {(cuuint64_t)FR_BLK * 8, r1 * FR_BLK * 8, r1 * r2 * FR_BLK * 8};
+  // affine meshes store one point per element: the point dimension(s) are broadcast through a zero stride, so the
+  // kernels see the same [rows][E] boxes while DRAM holds (and serves) each value once
+  if (bcast == 1) { strides[0] = 0; strides[1] = FR_BLK * 8; strides[2] = r2 * FR_BLK * 8; }       // r1 broadcast: [block][r2][FR_BLK]
+  if (bcast == 2) { strides[0] = 0; strides[1] = 0; strides[2] = FR_BLK * 8; }                      // r1 and r2 broadcast: [block][FR_BLK]
   cuuint32_t box[4] = {E, b1, b2, 1};
   cuuint32_t estr[4] = {1, 1, 1, 1};
   return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
