@@ -81,8 +81,9 @@ def rhs_algorithmic_words(nd, NV, Nu, Nf, ns, affine):
     return w
 
 
-def kernel_words(name, nd, NV, Nu, Nf, ns):
-    """compulsory words per element for one launch group (inputs once + outputs once)."""
+def kernel_words(name, nd, NV, Nu, Nf, ns, gfrac=1.0):
+    """compulsory words per element for one launch group (inputs once + outputs once).
+    gfrac: fraction of the faces whose G^f is produced (1/2 when the LDG weight of one side is zero, |beta| = 1/2)."""
     met = (nd * nd + 1) * Nu
     t = {
         # generic staged path (PAPER.md App A sequence)
@@ -101,8 +102,8 @@ def kernel_words(name, nd, NV, Nu, Nf, ns):
         "hex_fluxdiv": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
         # TMA-pipelined hexahedral path (fr_hex_tma.cu, fr_hex_fluxdiv_tma.cu)
         "hex_interp_tma": (Nu + Nf) * NV,
-        "hex_gradface": (Nu + 2 * Nf) * NV + met + nd * Nf + nd * Nu * NV,  # U, jump, S, 1/J, normals -> G^f, Q
-        "common_flux_g": 3 * Nf * NV + (nd + 2 + 2) * Nf // 2,              # U^f, G^f -> D~ (in place), normals, J n
+        "hex_gradface": (Nu + Nf + gfrac * Nf) * NV + met + gfrac * nd * Nf + nd * Nu * NV,  # U, jump, S, 1/J, normals -> G^f, Q
+        "common_flux_g": (2 + gfrac) * Nf * NV + (nd + 2 + 2) * Nf // 2,      # U^f, G^f -> D~ (in place), normals, J n
         "hex_fluxdiv_tma": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
         # fused triangle kernels (fr_element.cu)
         "el_gradface": (Nu + 3 * Nf) * NV + met + nd * Nf + nd * Nu * NV,   # U, C, U^f, S, 1/J, normals -> Q, G^f
@@ -309,7 +310,7 @@ def main():
     affine = mesh["p_g"] == 1
     kern = []
     for name, ms in acc.items():
-        wds = kernel_words(name, nd, NV, Nu, Nf, ns)
+        wds = kernel_words(name, nd, NV, Nu, Nf, ns, 0.5 if abs(abs(disc.get("beta", 0.5)) - 0.5) < 1e-15 else 1.0)
         gbs = (wds * esz * ctx.n_elems / (ms * 1e-3) / 1e9) if (wds and ms > 0) else None
         kern.append({"name": name, "ms": ms, "share": ms / sum(acc.values()), "algorithmic_GBps": gbs})
     kern.sort(key=lambda k: -k["ms"])

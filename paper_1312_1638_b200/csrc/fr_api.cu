@@ -155,7 +155,19 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     UP(mc.bs, bs); UP(mc.be, be); UP(mc.bbc, bbc); UP(mc.bn, bn); UP(mc.bJn, bJn);
     // element-centric flux-point tables of the fused hexahedral gradient kernel (own normals, boundary ids)
     const bool want_tma = !(d->flags & FR_FLAG_FORCE_GENERIC) && o.etype == FR_HEX && dc.ns && hex_tma_supported(o.n, dc.f64);
-    if (want_tma) { UP(reblock(mc.fp_n, o.nd * o.Nf), fp_n); if (mc.nbnd) { UP(reblock(mc.fp_pe, o.Nf), fp_pe); } }
+    if (want_tma) {
+      UP(reblock(mc.fp_n, o.nd * o.Nf), fp_n);
+      if (mc.nbnd) { UP(reblock(mc.fp_pe, o.Nf), fp_pe); }
+      // faces whose G^f enters the common flux: L sides weigh 1/2 + beta, R sides 1/2 - beta (Eq 27), boundaries always
+      std::vector<uint8_t> need((size_t)o.nfaces * ld, 0);
+      for (int f = 0; f < o.nfaces; ++f)
+        for (int64_t el = 0; el < mc.Nel; ++el) {
+          const size_t i0 = (size_t)(f * o.nfp) * ld + el;
+          const bool bnd = mc.fp_pe[i0] < 0, rside = mc.fp_Jn[i0] < 0;
+          need[(size_t)f * ld + el] = bnd || (rside ? 0.5 - d->ldg_beta : 0.5 + d->ldg_beta) != 0.0;
+        }
+      UP(need, face_need);
+    }
     if (dc.ns && element_fused_supported(dc)) { UP(mc.fp_n, fp_n); if (mc.nbnd) { UP(mc.fp_pe, fp_pe); } }  // fused triangle kernels
 #undef UP
     std::vector<BcDev> bcs(c->mesh.bcs.size());

@@ -32,6 +32,7 @@ struct DevConsts {
   int nbcs;
   // element-centric tables (tensor-product kernels)
   const int32_t *fp_pe, *fp_ps;
+  const uint8_t *face_need;  // [6][ld] (hexahedra): 1 where the element kernels must produce G^f of the face
   const double *fp_n, *fp_Jn;
 };
 

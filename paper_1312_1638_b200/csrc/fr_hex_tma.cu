@@ -55,7 +55,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
                    const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmJ,
                    const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmJz, Ops1D<N> op, Phys ph,
                    const double *__restrict__ jump, const double *__restrict__ fp_n, const int32_t *__restrict__ fp_pe,
-                   const BcDev *__restrict__ bcs, double *__restrict__ gf, int64_t ld, int64_t Nel) {
+                   const uint8_t *__restrict__ face_need, const BcDev *__restrict__ bcs, double *__restrict__ gf, int64_t ld,
+                   int64_t Nel) {
   using L = GfLay<N, E, T>;
   constexpr int NFP = N * N, NF = 6 * NFP;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -98,6 +99,17 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     issue_stage(0, 0);
     if (N > 1) issue_stage(1, 1);
   }
+  // G^f of a face is needed only if its LDG weight (1/2 + beta on L sides, 1/2 - beta on R sides, Eq 27) is non-zero or it
+  // lies on a boundary: with the paper's beta = 1/2 half of the faces are skipped.  x/y tasks visit the +1 faces first
+  // (the L sides of structured meshes) so that skipped tasks fall into the same warps.
+  constexpr int TPT = (4 * N + NFP - 1) / NFP;  // x/y-face tasks of a thread per slice
+  bool need_xy[TPT];
+#pragma unroll
+  for (int q = 0; q < TPT; ++q) {
+    const int t = ij + q * NFP;
+    need_xy[q] = t < 4 * N && act && face_need[(size_t)(t < 2 * N ? 2 * (t / N) + 1 : 2 * (t / N - 2)) * ld + e] != 0;
+  }
+  const bool need_z[2] = {act && face_need[(size_t)4 * ld + e] != 0, act && face_need[(size_t)5 * ld + e] != 0};
   double zm[3][NV], zp[3][NV];  // Q interpolated to the two z faces of this column
 #pragma unroll
   for (int n = 0; n < 3; ++n)
@@ -147,8 +159,11 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     if (tid == 0 && k + 2 < N) issue_stage(k & 1, k + 2);
     if (SQ && tid == 0) { tma_store_4d(&tmQ, l0, 0, 3 * k, eb, sQ); tma_store_commit(); }
     // x / y faces of the slice: 4 N flux points per element, one thread each
-    for (int t = ij; t < 4 * N; t += NFP) {
-      const int f = t / N, m = t % N;
+#pragma unroll
+    for (int q = 0; q < TPT; ++q) {
+      if (!need_xy[q]) continue;
+      const int t = ij + q * NFP;
+      const int f = t < 2 * N ? 2 * (t / N) + 1 : 2 * (t / N - 2), m = t % N;  // faces 1, 3 (+x, +y), then 0, 2
       const int base = f < 2 ? m * N : m, stride = f < 2 ? 1 : N;
       const double *lc = sL + (f & 1) * N;
       const int fp = f * NFP + m + N * k;
@@ -198,6 +213,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   // z faces of the column
 #pragma unroll
   for (int s = 0; s < 2; ++s) {
+    if (!need_z[s]) continue;
     const int fp = (4 + s) * NFP + ij;
     double nrm[3], uf[NV], G[NV];
 #pragma unroll
@@ -252,7 +268,7 @@ cudaError_t launch_gradface_k(const DevConsts &c, const Maps<N, E> &m, const Ops
   static bool done = false;
   cudaError_t err = set_smem(kern, L::TOTAL, done);
   if (err != cudaSuccess) return err;
-  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.J, m.Q, m.Jz, op, c.ph, jump, c.fp_n, c.fp_pe, c.bcs, gf,
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.J, m.Q, m.Jz, op, c.ph, jump, c.fp_n, c.fp_pe, c.face_need, c.bcs, gf,
                                                                   c.ld,
                                                                   c.Nel);
   return cudaGetLastError();
