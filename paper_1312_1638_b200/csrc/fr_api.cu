@@ -158,6 +158,10 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     if (want_tma) {
       UP(reblock(mc.fp_n, o.nd * o.Nf), fp_n);
       if (mc.nbnd) { UP(reblock(mc.fp_pe, o.Nf), fp_pe); }
+    }
+    const bool want_el = dc.ns && element_fused_supported(dc);  // fused triangle kernels
+    if (want_el) { UP(mc.fp_n, fp_n); if (mc.nbnd) { UP(mc.fp_pe, fp_pe); } }
+    if (want_tma) {
       // faces whose G^f enters the common flux: L sides weigh 1/2 + beta, R sides 1/2 - beta (Eq 27), boundaries always
       std::vector<uint8_t> need((size_t)o.nfaces * ld, 0);
       for (int f = 0; f < o.nfaces; ++f)
@@ -168,7 +172,6 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
         }
       UP(need, face_need);
     }
-    if (dc.ns && element_fused_supported(dc)) { UP(mc.fp_n, fp_n); if (mc.nbnd) { UP(mc.fp_pe, fp_pe); } }  // fused triangle kernels
 #undef UP
     std::vector<BcDev> bcs(c->mesh.bcs.size());
     for (size_t i = 0; i < bcs.size(); ++i) {
