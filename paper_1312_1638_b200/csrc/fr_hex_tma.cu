@@ -76,6 +76,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 
   if (tid == 0) {
     mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); mbar_init(&bar[2], 1); mbar_init(&bar[3], 1);
+    mbar_init(&bar[4], 1); mbar_init(&bar[5], 1);  // second pass over the Q slices (z faces)
     fence_barrier_init();
     fence_proxy_async();
   }
@@ -110,11 +111,6 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     need_xy[q] = t < 4 * N && act && face_need[(size_t)(t < 2 * N ? 2 * (t / N) + 1 : 2 * (t / N - 2)) * ld + e] != 0;
   }
   const bool need_z[2] = {act && face_need[(size_t)4 * ld + e] != 0, act && face_need[(size_t)5 * ld + e] != 0};
-  double zm[3][NV], zp[3][NV];  // Q interpolated to the two z faces of this column
-#pragma unroll
-  for (int n = 0; n < 3; ++n)
-#pragma unroll
-    for (int a = 0; a < NV; ++a) zm[n][a] = zp[n][a] = 0.0;
   mbar_wait(&bar[0], 0);
 
 #pragma unroll
@@ -148,8 +144,6 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
         for (int n = 0; n < 3; ++n) {
           sQ[((n * NFP + ij) * NV + a) * E + el] = q3[n];
-          zm[n][a] = fma(op.lm[k], q3[n], zm[n][a]);
-          zp[n][a] = fma(op.lp[k], q3[n], zp[n][a]);
         }
       }
     }
@@ -210,31 +204,73 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     if (SQ && tid == 0) tma_store_wait_read();  // the bulk store has read sQ
     if (k + 1 < N) __syncthreads();  // before the next slice overwrites sQ
   }
-  // z faces of the column
+  // ---- z faces.  Q^f on them is sum_k l(+-1)_k Q(i, j, k): instead of carrying 2 x 15 accumulators through the slice
+  // loop, the Q slices just stored are streamed once more (TMA loads, L2 hits) through two buffers that the slice loop
+  // no longer needs: [SS .. Q) (S, 1/J, x/y jumps) and [U .. SS) (U block, z jumps).  The last slice is still in sQ.
+  static_assert(L::Q - L::SS >= L::Q_BYTES && L::SS - L::U >= L::Q_BYTES, "Q slice does not fit the reused buffers");
+  double ufz[2][NV];
+#pragma unroll
+  for (int s = 0; s < 2; ++s)
+#pragma unroll
+    for (int a = 0; a < NV; ++a) ufz[s][a] = 0.0;
+#pragma unroll
+  for (int m = 0; m < N; ++m)
+#pragma unroll
+    for (int a = 0; a < NV; ++a) {
+      const double v = (double)sU[((size_t)(NFP * m + ij) * NV + a) * E + el];
+      ufz[0][a] = fma(op.lm[m], v, ufz[0][a]);
+      ufz[1][a] = fma(op.lp[m], v, ufz[1][a]);
+    }
+  __syncthreads();  // U block, z jumps and the stages are dead from here on
+  unsigned char *zb[2] = {sm + L::SS, sm + L::U};
+  if (tid == 0) {
+    tma_store_wait_all();  // every Q slice of this CTA has reached global memory
+#pragma unroll
+    for (int k = 0; k < 2; ++k)
+      if (k < N - 1) { mbar_expect_tx(&bar[4 + k], (uint32_t)L::Q_BYTES); tma_load_4d(zb[k], &tmQ, l0, 0, 3 * k, eb, &bar[4 + k]); }
+  }
+  double zq[2][3][NV];
+#pragma unroll
+  for (int s = 0; s < 2; ++s)
+#pragma unroll
+    for (int n = 0; n < 3; ++n)
+#pragma unroll
+      for (int a = 0; a < NV; ++a) zq[s][n][a] = 0.0;
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    const double *src = sQ;
+    if (k < N - 1) {
+      mbar_wait(&bar[4 + (k & 1)], (k >> 1) & 1);
+      src = (const double *)zb[k & 1];
+    }
+#pragma unroll
+    for (int n = 0; n < 3; ++n)
+#pragma unroll
+      for (int a = 0; a < NV; ++a) {
+        const double q = src[((n * NFP + ij) * NV + a) * E + el];
+        zq[0][n][a] = fma(op.lm[k], q, zq[0][n][a]);
+        zq[1][n][a] = fma(op.lp[k], q, zq[1][n][a]);
+      }
+    if (k + 2 < N - 1) {  // refill this buffer with slice k + 2
+      __syncthreads();
+      if (tid == 0) { mbar_expect_tx(&bar[4 + (k & 1)], (uint32_t)L::Q_BYTES); tma_load_4d(zb[k & 1], &tmQ, l0, 0, 3 * (k + 2), eb, &bar[4 + (k & 1)]); }
+    }
+  }
 #pragma unroll
   for (int s = 0; s < 2; ++s) {
     if (!need_z[s]) continue;
     const int fp = (4 + s) * NFP + ij;
-    double nrm[3], uf[NV], G[NV];
+    double nrm[3], G[NV];
 #pragma unroll
     for (int n = 0; n < 3; ++n) nrm[n] = fp_n[fp_row(true, ld, 3 * NF, n * NF + fp, e)];
     const int pe = BND ? fp_pe[fp_row(true, ld, NF, fp, e)] : 0;
+    if constexpr (BND) face_visc<BND>(ufz[s], zq[s], nrm, ph, pe, bcs, G);
+    else visc_normal_stream(ufz[s], nrm, ph, [&](int a, double *g) {
 #pragma unroll
-    for (int a = 0; a < NV; ++a) uf[a] = 0.0;
-#pragma unroll
-    for (int m = 0; m < N; ++m)
-#pragma unroll
-      for (int a = 0; a < NV; ++a)
-        uf[a] = fma(s ? op.lp[m] : op.lm[m], (double)sU[((size_t)(NFP * m + ij) * NV + a) * E + el], uf[a]);
-    if constexpr (BND) face_visc<BND>(uf, s ? zp : zm, nrm, ph, pe, bcs, G);
-    else visc_normal_stream(uf, nrm, ph, [&](int a, double *g) {
-#pragma unroll
-      for (int n = 0; n < 3; ++n) g[n] = s ? zp[n][a] : zm[n][a];
+      for (int n = 0; n < 3; ++n) g[n] = zq[s][n][a];
     }, G);
-    if (act) {
 #pragma unroll
-      for (int a = 0; a < NV; ++a) gf[fp_row(true, ld, NF * NV, fp * NV + a, e)] = G[a];
-    }
+    for (int a = 0; a < NV; ++a) gf[fp_row(true, ld, NF * NV, fp * NV + a, e)] = G[a];
   }
 }
 
@@ -283,8 +319,8 @@ cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void 
   Maps<N, E> m;
   if (!make_maps<N, E, T>(c, u, jump, m, q)) return cudaErrorNotSupported;
   const Ops1D<N> op = make_ops<N>(h_ops);
-  if (c.nbnd) return q ? launch_gradface_k<N, E, true, true, T, MINB>(c, m, op, jump, gf, s) : launch_gradface_k<N, E, true, false, T, MINB>(c, m, op, jump, gf, s);
-  return q ? launch_gradface_k<N, E, false, true, T, MINB>(c, m, op, jump, gf, s) : launch_gradface_k<N, E, false, false, T, MINB>(c, m, op, jump, gf, s);
+  if (!q) return cudaErrorInvalidValue;  // the z-face pass re-reads the stored Q slices
+  return c.nbnd ? launch_gradface_k<N, E, true, true, T, MINB>(c, m, op, jump, gf, s) : launch_gradface_k<N, E, false, true, T, MINB>(c, m, op, jump, gf, s);
 }
 
 template <int N, typename T>

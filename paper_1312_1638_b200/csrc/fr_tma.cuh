@@ -77,6 +77,7 @@ __device__ __forceinline__ void tma_store_3d(const CUtensorMap *tm, int c0, int 
                : "memory");
 }
 __device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 
 // resident CTAs per SM the kernel is compiled for: limited by shared memory, by >= 128 registers per thread
