@@ -354,3 +354,26 @@ def test_fused_triangle_path_is_the_default():
     assert "el_gradface" in names and "el_fluxdiv" in names, names
     ctx2 = _ctx(mesh, disc, flags=1)
     assert ctx2.rhs_kernel_launches == 8
+
+
+def test_arbitrary_left_right_order_of_interfaces():
+    """The L/R order of each interface is the caller's (A12).  Flipping a seeded random half of the interfaces makes the
+    faces that carry an LDG weight (beta = 1/2: the L sides) vary from element to element inside a CTA, which the
+    face-skipping logic of k_hex_gradface must follow."""
+    mesh, disc = W.config("C3", n=3, p=3)
+    rng = np.random.default_rng(11)
+    flip = rng.random(mesh["ifaces"].shape[0]) < 0.5
+    m2 = dict(mesh)
+    ifc = mesh["ifaces"].copy()
+    ifc[flip] = mesh["ifaces"][flip][:, [2, 3, 0, 1]]
+    sh = mesh["shifts"].copy()
+    sh[flip] = -sh[flip]
+    m2["ifaces"], m2["shifts"] = ifc, sh
+    o = FROracle(m2, disc)
+    U = W.config_state("C3", np.asarray(o.xu_phys, float), n=3, p=3)
+    R = o.rhs(U)
+    bar, _ = _bar(o, U, R)
+    _check("flipped-LR", GpuRunner(_ctx(m2, disc)).rhs(U), R, bar)
+    # and it is a different discretisation from the unflipped one (beta = 1/2 is one-sided)
+    R0 = FROracle(mesh, disc).rhs(U)
+    assert np.max(np.abs(R0 - R)) > 1e-8 * np.max(np.abs(R))
