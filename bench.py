@@ -106,6 +106,7 @@ def kernel_words(name, nd, NV, Nu, Nf, ns, gfrac=1.0):
         "common_flux_g": (2 + gfrac) * Nf * NV + (nd + 2 + 2) * Nf // 2,      # U^f, G^f -> D~ (in place), normals, J n
         "hex_fluxdiv_tma": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
         # fused triangle kernels (fr_element.cu)
+        "el_interp": (Nu + Nf) * NV,
         "el_gradface": (Nu + 3 * Nf) * NV + met + nd * Nf + nd * Nu * NV,   # U, C, U^f, S, 1/J, normals -> Q, G^f
         "el_fluxdiv": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
         "tp_grad": (Nu + Nf) * NV + met + (nd + 1) * Nf + (NV - 1) * Nf + Nf,

@@ -45,6 +45,29 @@ __device__ __forceinline__ void face_visc_nd(const double *uf, const double (*qf
   }
 }
 
+// U^f = M0 U (Eq 41): u [NU][NV][ld] (T) -> uf [NF][NV][ld]
+template <int NU, int NF, typename T>
+__global__ void __launch_bounds__(TPB) k_el_interp(DevConsts c, const T *__restrict__ u, double *__restrict__ uf) {
+  constexpr int NV = 4;
+  __shared__ double sM0[NF * NU];
+  const int tid = threadIdx.x, el = tid % EB, a = tid / EB;
+  for (int t = tid; t < NF * NU; t += TPB) sM0[t] = c.M0[t];
+  __syncthreads();
+  const int64_t e = (int64_t)blockIdx.x * EB + el;
+  if (e >= c.Nel) return;
+  const size_t ld = c.ld;
+  double uu[NU];
+#pragma unroll
+  for (int r = 0; r < NU; ++r) uu[r] = (double)u[((size_t)r * NV + a) * ld + e];
+#pragma unroll 4
+  for (int s = 0; s < NF; ++s) {
+    double acc = 0;
+#pragma unroll
+    for (int r = 0; r < NU; ++r) acc = fma(sM0[s * NU + r], uu[r], acc);
+    uf[((size_t)s * NV + a) * ld + e] = acc;
+  }
+}
+
 // u [NU][NV][ld] (T), cf = common solution C [NF][NV][ld], uf = U^f [NF][NV][ld]; out: q [ND][NU][NV][ld], gf [NF][NV][ld]
 template <int NU, int NF, bool BND, typename T>
 __global__ void __launch_bounds__(TPB) k_el_gradface(DevConsts c, const T *__restrict__ u, const double *__restrict__ cf,
@@ -69,6 +92,15 @@ __global__ void __launch_bounds__(TPB) k_el_gradface(DevConsts c, const T *__res
     for (int r = 0; r < NU; ++r) uu[r] = (double)u[((size_t)r * NV + a) * ld + e];
 #pragma unroll
     for (int s = 0; s < NF; ++s) cc[s] = cf[((size_t)s * NV + a) * ld + e];
+    // affine elements: the metric terms of point 0 serve every point (one load instead of N_u)
+    double Sa[ND][ND], rja = 0;
+    if (c.affine) {
+      rja = c.rcpj[e];
+#pragma unroll
+      for (int d = 0; d < ND; ++d)
+#pragma unroll
+        for (int n = 0; n < ND; ++n) Sa[d][n] = c.smat[(size_t)(d * ND + n) * NU * ld + e];
+    }
 #pragma unroll 2
     for (int r = 0; r < NU; ++r) {
       double qt[ND];
@@ -82,12 +114,12 @@ __global__ void __launch_bounds__(TPB) k_el_gradface(DevConsts c, const T *__res
         for (int v = 0; v < NF; ++v) s = fma(m6[v], cc[v], s);
         qt[d] = s;
       }
-      const double rj = c.rcpj[(size_t)r * ld + e];
+      const double rj = c.affine ? rja : c.rcpj[(size_t)r * ld + e];
       double Sm[ND][ND];
 #pragma unroll
       for (int d = 0; d < ND; ++d)
 #pragma unroll
-        for (int n = 0; n < ND; ++n) Sm[d][n] = c.smat[((size_t)(d * ND + n) * NU + r) * ld + e];
+        for (int n = 0; n < ND; ++n) Sm[d][n] = c.affine ? Sa[d][n] : c.smat[((size_t)(d * ND + n) * NU + r) * ld + e];
 #pragma unroll
       for (int n = 0; n < ND; ++n) {
         double s = 0;
@@ -166,7 +198,8 @@ __global__ void __launch_bounds__(TPB) k_el_fluxdiv(DevConsts c, const T *__rest
     }
 #pragma unroll
     for (int d = 0; d < ND; ++d) {
-      const double s0 = c.smat[((size_t)(d * ND + 0) * NU + r) * ld + e2], s1 = c.smat[((size_t)(d * ND + 1) * NU + r) * ld + e2];
+      const int rm = c.affine ? 0 : r;  // affine elements: point 0 serves every point
+      const double s0 = c.smat[((size_t)(d * ND + 0) * NU + rm) * ld + e2], s1 = c.smat[((size_t)(d * ND + 1) * NU + rm) * ld + e2];
 #pragma unroll
       for (int b = 0; b < NV; ++b) sF[((d * NV + b) * NU + r) * EB + el2] = fma(s0, f[0][b], s1 * f[1][b]);
     }
@@ -186,7 +219,7 @@ __global__ void __launch_bounds__(TPB) k_el_fluxdiv(DevConsts c, const T *__rest
       for (int v = 0; v < NU; ++v) acc = fma(m132[d * NU + v], sF[((d * NV + a) * NU + v) * EB + el], acc);
 #pragma unroll
     for (int s = 0; s < NF; ++s) acc = fma(m3[s], dd[s], acc);
-    rhs[((size_t)r * NV + a) * ld + e] = (T)(-acc * c.rcpj[(size_t)r * ld + e]);
+    rhs[((size_t)r * NV + a) * ld + e] = (T)(-acc * c.rcpj[(size_t)(c.affine ? 0 : r) * ld + e]);
   }
 }
 
@@ -239,6 +272,16 @@ bool element_fused_supported(const DevConsts &c) { return c.etype == FR_TRI && !
     case 5: return CALL(15, 15);           \
     default: return cudaErrorNotSupported; \
   }
+
+cudaError_t element_interp(const DevConsts &c, const void *u, double *uf, cudaStream_t s) {
+  const unsigned grid = (unsigned)((c.Nel + EB - 1) / EB);
+#define FR_CALL(NU, NF)                                                                                            \
+  ((c.f64 ? k_el_interp<NU, NF, double><<<grid, TPB, 0, s>>>(c, (const double *)u, uf)                               \
+          : k_el_interp<NU, NF, float><<<grid, TPB, 0, s>>>(c, (const float *)u, uf)),                               \
+   cudaGetLastError())
+  FR_TRI_CASES(FR_CALL)
+#undef FR_CALL
+}
 
 cudaError_t element_gradface(const DevConsts &c, const void *u, const double *cf, const double *uf, double *q, double *gf, cudaStream_t s) {
 #define FR_CALL(NU, NF) (c.f64 ? gradface_t<NU, NF, double>(c, u, cf, uf, q, gf, s) : gradface_t<NU, NF, float>(c, u, cf, uf, q, gf, s))

@@ -6,6 +6,9 @@ namespace fr {
 
 bool element_fused_supported(const DevConsts &c);
 
+// U^f = M0 U -> uf [Nf][NV][ld]
+cudaError_t element_interp(const DevConsts &c, const void *u, double *uf, cudaStream_t s);
+
 // Q = J^-T {(M4 - M6 M0) U + M6 C} -> q [nd][Nu][NV][ld];  G^f = n . f_vis(U^f, M0 Q) -> gf [Nf][NV][ld]
 cudaError_t element_gradface(const DevConsts &c, const void *u, const double *cf, const double *uf, double *q, double *gf, cudaStream_t s);
 

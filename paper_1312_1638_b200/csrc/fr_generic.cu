@@ -273,13 +273,12 @@ cudaError_t run(const DevConsts &c, const WorkLayout &w, const T *u, T *rhs, cha
   const int TB = 128;
   auto blocks = [&](int64_t n) { return (unsigned)((n + TB - 1) / TB); };
   const int64_t npts = (int64_t)Nu * c.ld;
-  // (1) U^f = M0 U                                                       Eq 41 :745
-  FR_MARK(prof, "apply_M0");
-  apply<T, double, false>(s, c, Nf, Nu, c.M0, u, 0, nullptr, nullptr, uf);
   if (ND == 2 && element_fused_supported(c)) {
     // triangles: fused kernels with one thread per (element, variable) (fr_element.cu), 5 launches (3 for Euler);
     // Q^f and F~ are never stored
-    cudaError_t e = cudaSuccess;
+    FR_MARK(prof, "el_interp");
+    cudaError_t e = element_interp(c, u, uf, s);
+    if (e != cudaSuccess) return e;
     if (NS) {
       FR_MARK(prof, "common_sol");
       if (c.npairs) k_common_sol<ND, false><<<blocks(c.npairs), TB, 0, s>>>(c, uf, cf);
@@ -297,6 +296,9 @@ cudaError_t run(const DevConsts &c, const WorkLayout &w, const T *u, T *rhs, cha
     e = element_fluxdiv(c, u, qu, uf, rhs, s);
     return e != cudaSuccess ? e : cudaGetLastError();
   }
+  // (1) U^f = M0 U                                                       Eq 41 :745
+  FR_MARK(prof, "apply_M0");
+  apply<T, double, false>(s, c, Nf, Nu, c.M0, u, 0, nullptr, nullptr, uf);
   if (NS) {
     // (2) C^f                                                            Eq 7, 25
     FR_MARK(prof, "common_sol");
