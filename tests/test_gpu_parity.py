@@ -377,3 +377,40 @@ def test_arbitrary_left_right_order_of_interfaces():
     # and it is a different discretisation from the unflipped one (beta = 1/2 is one-sided)
     R0 = FROracle(mesh, disc).rhs(U)
     assert np.max(np.abs(R0 - R)) > 1e-8 * np.max(np.abs(R))
+
+
+def test_no_write_outside_caller_buffers():
+    """u, rhs and the workspace sit between guard bands filled with a byte pattern; after fr_rhs and fr_rk4_step on ragged
+    element counts (hexahedra NS / Euler, triangles, quads) the guards are untouched and u is unchanged by fr_rhs."""
+    import torch
+
+    G = 1 << 16
+    cases = [("C3", dict(n=3, p=4), "navier-stokes"), ("C3", dict(n=3, p=2), "euler"), ("C4", dict(n=5), "navier-stokes"), ("C1", {}, "euler")]
+    for name, over, system in cases:
+        mesh, disc = W.config(name, **over)
+        if name == "C3":
+            mesh = W.box_mesh((3, 2, 3) if over["p"] == 4 else (5, 3, 1), (2 * np.pi,) * 3, p_g=over["p"], warp=W.sine_warp(0.05))
+        disc = dict(disc, system=system)
+        ctx = _ctx(mesh, disc)
+        nb, wb = ctx.state_bytes, ctx.workspace_bytes
+        big = torch.full((4 * G + 2 * nb + wb + 1024,), 0xAB, dtype=torch.uint8, device="cuda")
+        o_u, o_r = G, 2 * G + nb
+        o_w = (3 * G + 2 * nb + 255) // 256 * 256
+        X = ctx.solution_point_coords()
+        kw = {k: v for k, v in over.items() if k in ("p", "n")}
+        U = ctx.pad(W.config_state(name, X, **kw))
+        big[o_u:o_u + nb] = torch.from_numpy(U.view(np.uint8).reshape(-1)).cuda()
+        base = big.data_ptr()
+        assert base % 256 == 0
+        stream = torch.cuda.current_stream().cuda_stream
+        ctx.rhs(base + o_u, base + o_r, base + o_w, stream)
+        torch.cuda.synchronize()
+        host = big.cpu().numpy()
+        assert np.array_equal(host[o_u:o_u + nb], U.view(np.uint8).reshape(-1)), name  # u untouched
+        ctx.rk4_step(base + o_u, 1e-5, base + o_w, stream)
+        torch.cuda.synchronize()
+        host = big.cpu().numpy()
+        for lo, hi in ((0, o_u), (o_u + nb, o_r), (o_r + nb, o_w), (o_w + wb, host.size)):
+            assert np.all(host[lo:hi] == 0xAB), (name, lo, hi)
+        got = host[o_u:o_u + nb].view(ctx.dtype).reshape(U.shape)
+        assert np.all(np.isfinite(ctx.unpad(got)))
