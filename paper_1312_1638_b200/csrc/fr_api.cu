@@ -190,7 +190,7 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     int64_t off = 0;
     auto take = [&](int64_t bytes) { int64_t o2 = off; off = align_up(off + bytes, 256); return o2; };
     c->use_tensor = false;
-    if (!(d->flags & FR_FLAG_FORCE_GENERIC) && tensor_supported(dc)) {
+    if (!(d->flags & FR_FLAG_FORCE_GENERIC) && tensor_supported(dc) && !element_fused_supported(dc)) {
       e = tensor_plan(dc, o, mc, c->tp, c->dev_allocs);
       if (e != cudaSuccess) { free_dev(c); return fail(c, FR_ECUDA, std::string("tensor plan: ") + cudaGetErrorString(e)); }
       c->use_tensor = true;

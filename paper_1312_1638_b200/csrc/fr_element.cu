@@ -1,5 +1,5 @@
-// Element-per-thread fused kernels for elements with small dense operators (triangles; App A matrices are
-// 10 x 12 ... 30 x 10 at p = 3).  They replace five of the eight launches of the staged generic sequence
+// Fused kernels for 2-D elements with small dense operators (triangles, low-order quadrilaterals; App A matrices
+// are 10 x 12 ... 30 x 10 for a p = 3 triangle).  They replace five of the eight launches of the staged generic sequence
 // (fr_generic.cu) by two:
 //
 //   k_el_gradface : Q = J^-T {(M4 - M6 M0) U + M6 C} (Eq 42 :756, Eq 10), Q^f = M0 Q (Eq 43), and at once
@@ -261,16 +261,30 @@ cudaError_t fluxdiv_t(const DevConsts &c, const void *u, const double *q, const 
 
 }  // namespace
 
-// triangles, p = 1 .. 4  (N_u = (p+1)(p+2)/2, N_f = 3 (p+1))
-bool element_fused_supported(const DevConsts &c) { return c.etype == FR_TRI && !c.staged && c.n >= 2 && c.n <= 5; }
+// triangles p = 1 .. 4 (N_u = (p+1)(p+2)/2, N_f = 3 (p+1)) and quadrilaterals p = 1 .. 3 (N_u = (p+1)^2, N_f = 4 (p+1)): at these
+// sizes the dense operators cost less than the extra launches and HBM round trips of the staged / sum-factorised sequences
+bool element_fused_supported(const DevConsts &c) {
+  if (c.staged) return false;
+  if (c.etype == FR_TRI) return c.n >= 2 && c.n <= 5;
+  if (c.etype == FR_QUAD) return c.n >= 2 && c.n <= 4;
+  return false;
+}
 
-#define FR_TRI_CASES(CALL)                 \
-  switch (c.n) {                           \
-    case 2: return CALL(3, 6);             \
-    case 3: return CALL(6, 9);             \
-    case 4: return CALL(10, 12);           \
-    case 5: return CALL(15, 15);           \
-    default: return cudaErrorNotSupported; \
+#define FR_TRI_CASES(CALL)                     \
+  if (c.etype == FR_TRI) {                     \
+    switch (c.n) {                             \
+      case 2: return CALL(3, 6);               \
+      case 3: return CALL(6, 9);               \
+      case 4: return CALL(10, 12);             \
+      case 5: return CALL(15, 15);             \
+      default: return cudaErrorNotSupported;   \
+    }                                          \
+  }                                            \
+  switch (c.n) {                               \
+    case 2: return CALL(4, 8);                 \
+    case 3: return CALL(9, 12);                \
+    case 4: return CALL(16, 16);               \
+    default: return cudaErrorNotSupported;     \
   }
 
 cudaError_t element_interp(const DevConsts &c, const void *u, double *uf, cudaStream_t s) {
