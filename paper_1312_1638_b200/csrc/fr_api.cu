@@ -141,6 +141,7 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     };
 #define UP(vec, field) if (e == cudaSuccess) e = upload(c, vec, &dc.field)
     UP(o.M[0], M0); UP(o.M[3], M3); UP(o.M[6], M6); UP(o.M46, M46); UP(o.M132, M132);
+    dc.hM0 = o.M[0].data(); dc.hM3 = o.M[3].data(); dc.hM6 = o.M[6].data(); dc.hM46 = o.M46.data(); dc.hM132 = o.M132.data();
     dc.affine = mc.affine;
     dc.aff = dc.blk && mc.affine;
     if (dc.aff) {  // affine hexahedra: one point of S and 1/J per element; the tensor maps broadcast it (fr_tma.cuh: encode_blk)

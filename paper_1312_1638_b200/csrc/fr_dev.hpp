@@ -20,6 +20,7 @@ struct DevConsts {
   Phys ph;
   // dense operators (device, row-major doubles)
   const double *M0, *M3, *M6, *M46, *M132;
+  const double *hM0, *hM3, *hM6, *hM46, *hM132;  // host copies (owned by the context): operators passed as kernel parameters
   // metrics at solution points
   const double *smat;   // [nd*nd][Nu][ld]
   const double *rcpj;   // [Nu][ld]

@@ -16,9 +16,28 @@
 #include "fr_element.hpp"
 
 #include <cstdlib>
+#include <cstring>
 
 namespace fr {
 namespace {
+
+// Operators as kernel parameters: they live in the constant bank, every loop over them is fully unrolled, and each FMA takes
+// its operator entry as a constant operand (no load instruction, no register) -- the operators are the same for all threads.
+template <int NU, int NF>
+struct OpsGrad {
+  double M46[2 * NU * NU];  // [ND*NU][NU]   M4 - M6 M0
+  double M6[2 * NU * NF];   // [ND*NU][NF]
+  double M0[NF * NU];       // [NF][NU]
+};
+template <int NU, int NF>
+struct OpsDiv {
+  double M132[NU * 2 * NU];  // [NU][ND*NU]  M1 - M3 M2
+  double M3[NU * NF];        // [NU][NF]
+};
+template <int NU, int NF>
+struct OpsInterp {
+  double M0[NF * NU];
+};
 
 constexpr int EB = 32;        // elements per CTA
 constexpr int NVT = 4;        // variables (2-D): threads per element
@@ -47,47 +66,38 @@ __device__ __forceinline__ void face_visc_nd(const double *uf, const double (*qf
 
 // U^f = M0 U (Eq 41): u [NU][NV][ld] (T) -> uf [NF][NV][ld]
 template <int NU, int NF, typename T>
-__global__ void __launch_bounds__(TPB) k_el_interp(DevConsts c, const T *__restrict__ u, double *__restrict__ uf) {
+__global__ void __launch_bounds__(TPB) k_el_interp(const __grid_constant__ OpsInterp<NU, NF> op, DevConsts c, const T *__restrict__ u,
+                                                    double *__restrict__ uf) {
   constexpr int NV = 4;
-  __shared__ double sM0[NF * NU];
   const int tid = threadIdx.x, el = tid % EB, a = tid / EB;
-  for (int t = tid; t < NF * NU; t += TPB) sM0[t] = c.M0[t];
-  __syncthreads();
   const int64_t e = (int64_t)blockIdx.x * EB + el;
   if (e >= c.Nel) return;
   const size_t ld = c.ld;
   double uu[NU];
 #pragma unroll
   for (int r = 0; r < NU; ++r) uu[r] = (double)u[((size_t)r * NV + a) * ld + e];
-#pragma unroll 4
+#pragma unroll
   for (int s = 0; s < NF; ++s) {
     double acc = 0;
 #pragma unroll
-    for (int r = 0; r < NU; ++r) acc = fma(sM0[s * NU + r], uu[r], acc);
+    for (int r = 0; r < NU; ++r) acc = fma(op.M0[s * NU + r], uu[r], acc);
     uf[((size_t)s * NV + a) * ld + e] = acc;
   }
 }
 
 // u [NU][NV][ld] (T), cf = common solution C [NF][NV][ld], uf = U^f [NF][NV][ld]; out: q [ND][NU][NV][ld], gf [NF][NV][ld]
 template <int NU, int NF, bool BND, typename T>
-__global__ void __launch_bounds__(TPB) k_el_gradface(DevConsts c, const T *__restrict__ u, const double *__restrict__ cf,
-                                                      const double *__restrict__ uf, double *__restrict__ q, double *__restrict__ gf) {
+__global__ void __launch_bounds__(TPB) k_el_gradface(const __grid_constant__ OpsGrad<NU, NF> op, DevConsts c, const T *__restrict__ u,
+                                                      const double *__restrict__ cf, const double *__restrict__ uf,
+                                                      double *__restrict__ q, double *__restrict__ gf) {
   constexpr int ND = 2, NV = 4;
   extern __shared__ double smem[];
-  double *sM46 = smem;                    // [ND*NU][NU]
-  double *sM6 = sM46 + ND * NU * NU;      // [ND*NU][NF]
-  double *sM0 = sM6 + ND * NU * NF;       // [NF][NU]
-  double *sQ = sM0 + NF * NU;             // [ND][NU][TPB]       gradient of the thread's variable
-  double *sQf = sQ + ND * NU * TPB;       // [ND][NV][NF][EB]    gradient at the flux points, all variables
+  double *sQf = smem;  // [ND][NV][NF][EB]  gradient at the flux points, all variables
   const int tid = threadIdx.x, el = tid % EB, a = tid / EB;
-  for (int t = tid; t < ND * NU * NU; t += TPB) sM46[t] = c.M46[t];
-  for (int t = tid; t < ND * NU * NF; t += TPB) sM6[t] = c.M6[t];
-  for (int t = tid; t < NF * NU; t += TPB) sM0[t] = c.M0[t];
-  __syncthreads();
   const int64_t e0 = (int64_t)blockIdx.x * EB, e = e0 + el;
   const size_t ld = c.ld;
   if (e < c.Nel) {
-    double uu[NU], cc[NF];
+    double uu[NU], cc[NF], qq[ND][NU];
 #pragma unroll
     for (int r = 0; r < NU; ++r) uu[r] = (double)u[((size_t)r * NV + a) * ld + e];
 #pragma unroll
@@ -101,46 +111,38 @@ __global__ void __launch_bounds__(TPB) k_el_gradface(DevConsts c, const T *__res
 #pragma unroll
         for (int n = 0; n < ND; ++n) Sa[d][n] = c.smat[(size_t)(d * ND + n) * NU * ld + e];
     }
-#pragma unroll 2
+#pragma unroll
     for (int r = 0; r < NU; ++r) {
       double qt[ND];
 #pragma unroll
       for (int d = 0; d < ND; ++d) {
-        const double *m46 = sM46 + (d * NU + r) * NU, *m6 = sM6 + (d * NU + r) * NF;
         double s = 0;
 #pragma unroll
-        for (int v = 0; v < NU; ++v) s = fma(m46[v], uu[v], s);
+        for (int v = 0; v < NU; ++v) s = fma(op.M46[(d * NU + r) * NU + v], uu[v], s);
 #pragma unroll
-        for (int v = 0; v < NF; ++v) s = fma(m6[v], cc[v], s);
+        for (int v = 0; v < NF; ++v) s = fma(op.M6[(d * NU + r) * NF + v], cc[v], s);
         qt[d] = s;
       }
       const double rj = c.affine ? rja : c.rcpj[(size_t)r * ld + e];
-      double Sm[ND][ND];
-#pragma unroll
-      for (int d = 0; d < ND; ++d)
-#pragma unroll
-        for (int n = 0; n < ND; ++n) Sm[d][n] = c.affine ? Sa[d][n] : c.smat[((size_t)(d * ND + n) * NU + r) * ld + e];
 #pragma unroll
       for (int n = 0; n < ND; ++n) {
         double s = 0;
 #pragma unroll
-        for (int d = 0; d < ND; ++d) s = fma(Sm[d][n], qt[d], s);
+        for (int d = 0; d < ND; ++d) s = fma(c.affine ? Sa[d][n] : c.smat[((size_t)(d * ND + n) * NU + r) * ld + e], qt[d], s);
         s *= rj;
         q[(((size_t)n * NU + r) * NV + a) * ld + e] = s;
-        sQ[(n * NU + r) * TPB + tid] = s;
+        qq[n][r] = s;
       }
     }
-#pragma unroll 1
-    for (int s = 0; s < NF; ++s) {
-      const double *m0 = sM0 + s * NU;
+#pragma unroll
+    for (int s = 0; s < NF; ++s)
 #pragma unroll
       for (int n = 0; n < ND; ++n) {
         double acc = 0;
 #pragma unroll
-        for (int r = 0; r < NU; ++r) acc = fma(m0[r], sQ[(n * NU + r) * TPB + tid], acc);
+        for (int r = 0; r < NU; ++r) acc = fma(op.M0[s * NU + r], qq[n][r], acc);
         sQf[((n * NV + a) * NF + s) * EB + el] = acc;
       }
-    }
   }
   __syncthreads();
   // flux points of the CTA's elements, redistributed over all threads
@@ -167,16 +169,12 @@ __global__ void __launch_bounds__(TPB) k_el_gradface(DevConsts c, const T *__res
 
 // u as above, q [ND][NU][NV][ld], dt = D~ [NF][NV][ld]; rhs like u
 template <int NU, int NF, bool NS, typename T>
-__global__ void __launch_bounds__(TPB) k_el_fluxdiv(DevConsts c, const T *__restrict__ u, const double *__restrict__ q,
-                                                     const double *__restrict__ dt, T *__restrict__ rhs) {
+__global__ void __launch_bounds__(TPB) k_el_fluxdiv(const __grid_constant__ OpsDiv<NU, NF> op, DevConsts c, const T *__restrict__ u,
+                                                     const double *__restrict__ q, const double *__restrict__ dt, T *__restrict__ rhs) {
   constexpr int ND = 2, NV = 4;
   extern __shared__ double smem[];
-  double *sM132 = smem;                    // [NU][ND*NU]
-  double *sM3 = sM132 + NU * ND * NU;      // [NU][NF]
-  double *sF = sM3 + NU * NF;              // [ND][NV][NU][EB]
+  double *sF = smem;  // [ND][NV][NU][EB]
   const int tid = threadIdx.x, el = tid % EB, a = tid / EB;
-  for (int t = tid; t < NU * ND * NU; t += TPB) sM132[t] = c.M132[t];
-  for (int t = tid; t < NU * NF; t += TPB) sM3[t] = c.M3[t];
   const int64_t e0 = (int64_t)blockIdx.x * EB, e = e0 + el;
   const size_t ld = c.ld;
   // F~ = S f(U, Q) at the solution points of the CTA's elements, one (element, point) per thread and pass
@@ -209,53 +207,54 @@ __global__ void __launch_bounds__(TPB) k_el_fluxdiv(DevConsts c, const T *__rest
   double dd[NF];
 #pragma unroll
   for (int s = 0; s < NF; ++s) dd[s] = dt[((size_t)s * NV + a) * ld + e];
-#pragma unroll 1
+  double fa[ND][NU];  // F~ of this variable at all points of the element
+#pragma unroll
+  for (int d = 0; d < ND; ++d)
+#pragma unroll
+    for (int v = 0; v < NU; ++v) fa[d][v] = sF[((d * NV + a) * NU + v) * EB + el];
+#pragma unroll
   for (int r = 0; r < NU; ++r) {
-    const double *m132 = sM132 + r * ND * NU, *m3 = sM3 + r * NF;
     double acc = 0;
 #pragma unroll
     for (int d = 0; d < ND; ++d)
 #pragma unroll
-      for (int v = 0; v < NU; ++v) acc = fma(m132[d * NU + v], sF[((d * NV + a) * NU + v) * EB + el], acc);
+      for (int v = 0; v < NU; ++v) acc = fma(op.M132[r * ND * NU + d * NU + v], fa[d][v], acc);
 #pragma unroll
-    for (int s = 0; s < NF; ++s) acc = fma(m3[s], dd[s], acc);
+    for (int s = 0; s < NF; ++s) acc = fma(op.M3[r * NF + s], dd[s], acc);
     rhs[((size_t)r * NV + a) * ld + e] = (T)(-acc * c.rcpj[(size_t)(c.affine ? 0 : r) * ld + e]);
   }
 }
 
 template <int NU, int NF, typename T>
 cudaError_t gradface_t(const DevConsts &c, const void *u, const double *cf, const double *uf, double *q, double *gf, cudaStream_t s) {
-  const size_t smem = (size_t)(2 * NU * NU + 2 * NU * NF + NF * NU + 2 * NU * TPB + 2 * 4 * NF * EB) * sizeof(double);
+  OpsGrad<NU, NF> op;
+  std::memcpy(op.M46, c.hM46, sizeof(op.M46));
+  std::memcpy(op.M6, c.hM6, sizeof(op.M6));
+  std::memcpy(op.M0, c.hM0, sizeof(op.M0));
+  const size_t smem = (size_t)(2 * 4 * NF * EB) * sizeof(double);
   const unsigned grid = (unsigned)((c.Nel + EB - 1) / EB);
-  if (c.nbnd) {
-    auto kern = k_el_gradface<NU, NF, true, T>;
-    static bool done = false;
-    if (!done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); done = true; }
-    kern<<<grid, TPB, smem, s>>>(c, (const T *)u, cf, uf, q, gf);
-  } else {
-    auto kern = k_el_gradface<NU, NF, false, T>;
-    static bool done = false;
-    if (!done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); done = true; }
-    kern<<<grid, TPB, smem, s>>>(c, (const T *)u, cf, uf, q, gf);
-  }
+  if (c.nbnd) k_el_gradface<NU, NF, true, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
+  else k_el_gradface<NU, NF, false, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
   return cudaGetLastError();
 }
 
 template <int NU, int NF, typename T>
 cudaError_t fluxdiv_t(const DevConsts &c, const void *u, const double *q, const double *dt, void *rhs, cudaStream_t s) {
-  const size_t smem = (size_t)(2 * NU * NU + NU * NF + 2 * 4 * NU * EB) * sizeof(double);
+  OpsDiv<NU, NF> op;
+  std::memcpy(op.M132, c.hM132, sizeof(op.M132));
+  std::memcpy(op.M3, c.hM3, sizeof(op.M3));
+  const size_t smem = (size_t)(2 * 4 * NU * EB) * sizeof(double);
   const unsigned grid = (unsigned)((c.Nel + EB - 1) / EB);
-  if (c.ns) {
-    auto kern = k_el_fluxdiv<NU, NF, true, T>;
-    static bool done = false;
-    if (!done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); done = true; }
-    kern<<<grid, TPB, smem, s>>>(c, (const T *)u, q, dt, (T *)rhs);
-  } else {
-    auto kern = k_el_fluxdiv<NU, NF, false, T>;
-    static bool done = false;
-    if (!done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); done = true; }
-    kern<<<grid, TPB, smem, s>>>(c, (const T *)u, q, dt, (T *)rhs);
-  }
+  if (c.ns) k_el_fluxdiv<NU, NF, true, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, q, dt, (T *)rhs);
+  else k_el_fluxdiv<NU, NF, false, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, q, dt, (T *)rhs);
+  return cudaGetLastError();
+}
+
+template <int NU, int NF, typename T>
+cudaError_t interp_t(const DevConsts &c, const void *u, double *uf, cudaStream_t s) {
+  OpsInterp<NU, NF> op;
+  std::memcpy(op.M0, c.hM0, sizeof(op.M0));
+  k_el_interp<NU, NF, T><<<(unsigned)((c.Nel + EB - 1) / EB), TPB, 0, s>>>(op, c, (const T *)u, uf);
   return cudaGetLastError();
 }
 
@@ -288,11 +287,7 @@ bool element_fused_supported(const DevConsts &c) {
   }
 
 cudaError_t element_interp(const DevConsts &c, const void *u, double *uf, cudaStream_t s) {
-  const unsigned grid = (unsigned)((c.Nel + EB - 1) / EB);
-#define FR_CALL(NU, NF)                                                                                            \
-  ((c.f64 ? k_el_interp<NU, NF, double><<<grid, TPB, 0, s>>>(c, (const double *)u, uf)                               \
-          : k_el_interp<NU, NF, float><<<grid, TPB, 0, s>>>(c, (const float *)u, uf)),                               \
-   cudaGetLastError())
+#define FR_CALL(NU, NF) (c.f64 ? interp_t<NU, NF, double>(c, u, uf, s) : interp_t<NU, NF, float>(c, u, uf, s))
   FR_TRI_CASES(FR_CALL)
 #undef FR_CALL
 }
