@@ -1,7 +1,8 @@
-// Fused kernels for 2-D elements with small dense operators (triangles, low-order quadrilaterals; App A matrices
-// are 10 x 12 ... 30 x 10 for a p = 3 triangle).  They replace five of the eight launches of the staged generic sequence
-// (fr_generic.cu) by two:
+// Fused kernels for 2-D elements with small dense operators (triangles p <= 4, quadrilaterals p <= 4; App A
+// matrices are 10 x 12 ... 30 x 10 for a p = 3 triangle).  They replace six of the eight launches of the staged generic
+// sequence (fr_generic.cu) by three:
 //
+//   k_el_interp   : U^f = M0 U (Eq 41).
 //   k_el_gradface : Q = J^-T {(M4 - M6 M0) U + M6 C} (Eq 42 :756, Eq 10), Q^f = M0 Q (Eq 43), and at once
 //                   G^f = n . f_vis(U^f, Q^f) (Eq 22-24) with the element's own outward normal; writes Q and G^f.
 //                   Replaces apply_M46_M6, grad_phys, apply_M5 and makes the N_D N_V N_f array Q^f unnecessary.
@@ -9,10 +10,10 @@
 //                   Replaces tflux and apply_M132_M3; F~ never reaches HBM.
 //
 // A CTA owns EB = 32 consecutive elements and runs one thread per (element, conserved variable): every global access is
-// a 256-byte row segment of consecutive elements, the operators sit in shared memory and are read as broadcasts, the
-// per-variable intermediates live in registers and in a [value][thread] shared-memory scratch (conflict free); the
-// steps that couple the variables (viscous flux at a flux point, flux at a solution point) are redistributed over the
-// CTA's threads after one barrier.
+// a 256-byte row segment of consecutive elements; the operators are kernel parameters (constant bank) read as FMA operands
+// by fully unrolled loops; the per-variable intermediates live in registers; the steps that couple the variables
+// (viscous flux at a flux point, flux at a solution point) are redistributed over the CTA's threads through a
+// [value][element] shared-memory scratch after one barrier.
 #include "fr_element.hpp"
 
 #include <cstdlib>
@@ -233,6 +234,12 @@ cudaError_t gradface_t(const DevConsts &c, const void *u, const double *cf, cons
   std::memcpy(op.M0, c.hM0, sizeof(op.M0));
   const size_t smem = (size_t)(2 * 4 * NF * EB) * sizeof(double);
   const unsigned grid = (unsigned)((c.Nel + EB - 1) / EB);
+  static bool done = false;
+  if (!done && smem > 48 * 1024) {
+    cudaFuncSetAttribute(k_el_gradface<NU, NF, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_el_gradface<NU, NF, false, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  }
+  done = true;
   if (c.nbnd) k_el_gradface<NU, NF, true, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
   else k_el_gradface<NU, NF, false, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
   return cudaGetLastError();
@@ -245,6 +252,12 @@ cudaError_t fluxdiv_t(const DevConsts &c, const void *u, const double *q, const 
   std::memcpy(op.M3, c.hM3, sizeof(op.M3));
   const size_t smem = (size_t)(2 * 4 * NU * EB) * sizeof(double);
   const unsigned grid = (unsigned)((c.Nel + EB - 1) / EB);
+  static bool done = false;
+  if (!done && smem > 48 * 1024) {
+    cudaFuncSetAttribute(k_el_fluxdiv<NU, NF, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_el_fluxdiv<NU, NF, false, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  }
+  done = true;
   if (c.ns) k_el_fluxdiv<NU, NF, true, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, q, dt, (T *)rhs);
   else k_el_fluxdiv<NU, NF, false, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, q, dt, (T *)rhs);
   return cudaGetLastError();
@@ -260,12 +273,12 @@ cudaError_t interp_t(const DevConsts &c, const void *u, double *uf, cudaStream_t
 
 }  // namespace
 
-// triangles p = 1 .. 4 (N_u = (p+1)(p+2)/2, N_f = 3 (p+1)) and quadrilaterals p = 1 .. 3 (N_u = (p+1)^2, N_f = 4 (p+1)): at these
+// triangles p = 1 .. 4 (N_u = (p+1)(p+2)/2, N_f = 3 (p+1)) and quadrilaterals p = 1 .. 4 (N_u = (p+1)^2, N_f = 4 (p+1)): at these
 // sizes the dense operators cost less than the extra launches and HBM round trips of the staged / sum-factorised sequences
 bool element_fused_supported(const DevConsts &c) {
   if (c.staged) return false;
   if (c.etype == FR_TRI) return c.n >= 2 && c.n <= 5;
-  if (c.etype == FR_QUAD) return c.n >= 2 && c.n <= 4;
+  if (c.etype == FR_QUAD) return c.n >= 2 && c.n <= 5;
   return false;
 }
 
@@ -283,6 +296,7 @@ bool element_fused_supported(const DevConsts &c) {
     case 2: return CALL(4, 8);                 \
     case 3: return CALL(9, 12);                \
     case 4: return CALL(16, 16);               \
+    case 5: return CALL(25, 20);               \
     default: return cudaErrorNotSupported;     \
   }
 
