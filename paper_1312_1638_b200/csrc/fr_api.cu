@@ -128,9 +128,10 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     dc.ns = d->system == FR_NAVIER_STOKES; dc.f64 = d->precision == FR_F64;
     dc.staged = (d->flags & FR_FLAG_FORCE_GENERIC) != 0;
     dc.ph = Phys{d->gamma, d->mu, d->Pr, d->ldg_beta, d->ldg_tau};
-    c->host_only = (d->flags & FR_FLAG_HOST_ONLY) != 0;
+    dc.dev = -1;
     if (c->host_only) { c->use_tensor = false; c->wl = WorkLayout(); c->ready = true; return FR_OK; }
-    cudaError_t e = cudaSuccess;
+    cudaError_t e = cudaGetDevice(&dc.dev);
+    if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
     dc.blk = blk;
     auto reblock = [&](const auto &src, int rows) {  // [rows][ld] -> [ld / FR_BLK][rows][FR_BLK]
       typename std::decay<decltype(src)>::type dst(src.size());
@@ -275,6 +276,9 @@ static int rhs_impl(fr_ctx *c, const void *u, void *rhs, void *work, void *strea
   if (!u || !rhs || !work) return fail(c, FR_EINVAL, "fr_rhs: NULL device pointer");
   if (u == rhs) return fail(c, FR_EINVAL, "fr_rhs: rhs must not alias u");
   if (c->host_only) return fail(c, FR_EINVAL, "fr_rhs: context was set up with FR_FLAG_HOST_ONLY");
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != c->dc.dev)
+    return fail(c, FR_EINVAL, "fr_rhs: the current CUDA device is not the one fr_setup_operators uploaded the constants to");
   cudaStream_t s = (cudaStream_t)stream;
   cudaError_t e = c->use_tensor ? tensor_rhs(c->dc, c->tp, u, rhs, (char *)work + c->wl.uf, s, prof)
                                 : generic_rhs(c->dc, c->wl, u, rhs, (char *)work, s, prof);
@@ -313,22 +317,22 @@ int fr_rk4_step(fr_ctx *c, void *u, double dt, void *work, void *stream) {
   cudaStream_t s = (cudaStream_t)stream;
   char *wk = (char *)work;
   void *k = wk + c->wl.rk_k, *tmp = wk + c->wl.rk_tmp, *acc = wk + c->wl.rk_acc;
-  const int64_t n = (int64_t)c->ops.Nu * c->dc.NV * c->dc.ld;
+  const int64_t n = (int64_t)c->ops.Nu * c->dc.NV;  // rows of ld values; pad columns (e >= n_elems) are left untouched
   const bool f64 = c->dc.f64;
   int rc;
   cudaError_t e;
   // k1; tmp = u + dt/2 k1; acc = u + dt/6 k1
   if ((rc = fr_rhs(c, u, k, work, stream)) != FR_OK) return rc;
-  e = rk_axpy2(f64, n, u, k, dt / 2, tmp, dt / 6, acc, 0, s);
+  e = rk_axpy2(f64, n, c->dc.ld, c->dc.Nel, u, k, dt / 2, tmp, dt / 6, acc, 0, s);
   // k2; tmp = u + dt/2 k2; acc += dt/3 k2
   if (e == cudaSuccess && (rc = fr_rhs(c, tmp, k, work, stream)) != FR_OK) return rc;
-  if (e == cudaSuccess) e = rk_axpy2(f64, n, u, k, dt / 2, tmp, dt / 3, acc, 1, s);
+  if (e == cudaSuccess) e = rk_axpy2(f64, n, c->dc.ld, c->dc.Nel, u, k, dt / 2, tmp, dt / 3, acc, 1, s);
   // k3; tmp = u + dt k3; acc += dt/3 k3
   if (e == cudaSuccess && (rc = fr_rhs(c, tmp, k, work, stream)) != FR_OK) return rc;
-  if (e == cudaSuccess) e = rk_axpy2(f64, n, u, k, dt, tmp, dt / 3, acc, 1, s);
+  if (e == cudaSuccess) e = rk_axpy2(f64, n, c->dc.ld, c->dc.Nel, u, k, dt, tmp, dt / 3, acc, 1, s);
   // k4; u = acc + dt/6 k4
   if (e == cudaSuccess && (rc = fr_rhs(c, tmp, k, work, stream)) != FR_OK) return rc;
-  if (e == cudaSuccess) e = rk_axpy2(f64, n, u, k, 0.0, u, dt / 6, acc, 2, s);
+  if (e == cudaSuccess) e = rk_axpy2(f64, n, c->dc.ld, c->dc.Nel, u, k, 0.0, u, dt / 6, acc, 2, s);
   if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("fr_rk4_step launch: ") + cudaGetErrorString(e));
   return FR_OK;
 }

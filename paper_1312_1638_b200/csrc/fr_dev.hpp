@@ -8,8 +8,16 @@
 
 namespace fr {
 
+// one bit per device ordinal (cudaFuncSetAttribute is per device)
+struct DevFlags {
+  uint64_t bits[4] = {0, 0, 0, 0};
+  bool test(int d) const { return d >= 0 && d < 256 && ((bits[d >> 6] >> (d & 63)) & 1u); }
+  void set(int d) { if (d >= 0 && d < 256) bits[d >> 6] |= 1ull << (d & 63); }
+};
+
 struct DevConsts {
   int nd, NV, Nu, Nf, n, nfp, etype;
+  int dev;       // device ordinal the constants were uploaded to (fr_setup_operators); fr_rhs refuses any other current device
   int64_t Nel, ld, npairs, nbnd;
   bool ns;       // Navier-Stokes (gradients, LDG) or Euler
   bool f64;      // storage precision of u / rhs
@@ -78,8 +86,16 @@ void launch_common_jump(const DevConsts &c, const double *uf, double *cf, cudaSt
 void launch_tflux(const DevConsts &c, const void *u, double *qu, cudaStream_t s);           // Eq 12, in place over Q^u
 void launch_common_flux(const DevConsts &c, double *uf, const double *qf, cudaStream_t s);  // Eq 15-17, in place over U^f
 
-// RK4 register updates (fr_rk.cu)
-cudaError_t rk_axpy2(bool f64, int64_t n, const void *u, const void *k, double a, void *out1, double b, void *out2,
-                     int mode, cudaStream_t s);
+// register updates of the time steppers (fr_rk.cu): rows x ld matrices of which the first nel columns are updated
+constexpr int RK_MAX_IN = 8;
+constexpr int RK_MAX_PARTIALS = 4096;
+// out1 = sum_i a[i] in[i], out2 = sum_i b[i] in[i]  (either output may be NULL or alias an input)
+cudaError_t rk_lincomb(bool f64, int64_t rows, int64_t ld, int64_t nel, int nin, const void *const *in, const double *a, const double *b,
+                       void *out1, void *out2, cudaStream_t s);
+cudaError_t rk_axpy2(bool f64, int64_t rows, int64_t ld, int64_t nel, const void *u, const void *k, double a, void *out1, double b,
+                     void *out2, int mode, cudaStream_t s);
+// *out = sqrt(mean (x - y)^2) over the rows x nel values, deterministic; part: RK_MAX_PARTIALS doubles of scratch
+cudaError_t rk_rms_diff(bool f64, int64_t rows, int64_t ld, int64_t nel, const void *x, const void *y, double *part, double *out,
+                        cudaStream_t s);
 
 }  // namespace fr

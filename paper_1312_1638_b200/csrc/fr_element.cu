@@ -234,12 +234,12 @@ cudaError_t gradface_t(const DevConsts &c, const void *u, const double *cf, cons
   std::memcpy(op.M0, c.hM0, sizeof(op.M0));
   const size_t smem = (size_t)(2 * 4 * NF * EB) * sizeof(double);
   const unsigned grid = (unsigned)((c.Nel + EB - 1) / EB);
-  static bool done = false;
-  if (!done && smem > 48 * 1024) {
+  static DevFlags done;  // function attributes are per device
+  if (!done.test(c.dev) && smem > 48 * 1024) {
     cudaFuncSetAttribute(k_el_gradface<NU, NF, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(k_el_gradface<NU, NF, false, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
-  done = true;
+  done.set(c.dev);
   if (c.nbnd) k_el_gradface<NU, NF, true, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
   else k_el_gradface<NU, NF, false, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
   return cudaGetLastError();
@@ -252,12 +252,12 @@ cudaError_t fluxdiv_t(const DevConsts &c, const void *u, const double *q, const 
   std::memcpy(op.M3, c.hM3, sizeof(op.M3));
   const size_t smem = (size_t)(2 * 4 * NU * EB) * sizeof(double);
   const unsigned grid = (unsigned)((c.Nel + EB - 1) / EB);
-  static bool done = false;
-  if (!done && smem > 48 * 1024) {
+  static DevFlags done;
+  if (!done.test(c.dev) && smem > 48 * 1024) {
     cudaFuncSetAttribute(k_el_fluxdiv<NU, NF, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(k_el_fluxdiv<NU, NF, false, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
-  done = true;
+  done.set(c.dev);
   if (c.ns) k_el_fluxdiv<NU, NF, true, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, q, dt, (T *)rhs);
   else k_el_fluxdiv<NU, NF, false, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, q, dt, (T *)rhs);
   return cudaGetLastError();

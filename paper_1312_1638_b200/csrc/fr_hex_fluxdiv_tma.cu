@@ -254,8 +254,8 @@ cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *
   ok = ok && encode_blk(&mR, c.rcpj, ld, NFP, N, E, NFP, N, c.aff ? 2 : 0);
   if (!ok) return cudaErrorNotSupported;
   auto kern = k_hex_fluxdiv_tma<N, E, NS, T, NB, MINB>;
-  static bool done = false;
-  cudaError_t err = set_smem(kern, L::TOTAL, done);
+  static DevFlags done;
+  cudaError_t err = set_smem(kern, L::TOTAL, done, c.dev);
   if (err != cudaSuccess) return err;
   const Ops1D<N> op = make_ops<N>(h_ops);
   kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(mS, mU, mQ, mD4, mD2, mR, op, c.ph, c.rcpj, c.aff, dt, (T *)rhs, c.ld,
@@ -281,7 +281,7 @@ cudaError_t fluxdiv_n(const DevConsts &c, const double *h_ops, const void *u, co
 }  // namespace
 
 bool hex_tma_fluxdiv_supported(int n, bool f64) {
-  if (getenv("FR_NO_TMA") || !encoder()) return false;
+  if (!encoder()) return false;
   switch (n) {
 #define FR_CASE(NN) case NN: return f64 ? fd_fits<NN, double>() : fd_fits<NN, float>();
     FR_CASE(2) FR_CASE(3) FR_CASE(4) FR_CASE(5) FR_CASE(6) FR_CASE(7)

@@ -82,8 +82,8 @@ cudaError_t launch_interp(const DevConsts &c, const double *h_ops, const void *u
   CUtensorMap mU;
   if (!encode3(&mU, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, N)) return cudaErrorNotSupported;
   auto kern = k_hex_interp_tma<N, E, T>;
-  static bool done = false;
-  cudaError_t err = set_smem(kern, SMEM, done);
+  static DevFlags done;
+  cudaError_t err = set_smem(kern, SMEM, done, c.dev);
   if (err != cudaSuccess) return err;
   kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, SMEM, s>>>(mU, make_ops<N>(h_ops), uf, c.ld, c.Nel);
   return cudaGetLastError();

@@ -301,8 +301,8 @@ template <int N, int E, bool BND, bool SQ, typename T, int MINB>
 cudaError_t launch_gradface_k(const DevConsts &c, const Maps<N, E> &m, const Ops1D<N> &op, const double *jump, double *gf, cudaStream_t s) {
   using L = GfLay<N, E, T>;
   auto kern = k_hex_gradface<N, E, BND, SQ, T, MINB>;
-  static bool done = false;
-  cudaError_t err = set_smem(kern, L::TOTAL, done);
+  static DevFlags done;
+  cudaError_t err = set_smem(kern, L::TOTAL, done, c.dev);
   if (err != cudaSuccess) return err;
   kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.J, m.Q, m.Jz, op, c.ph, jump, c.fp_n, c.fp_pe, c.face_need, c.bcs, gf,
                                                                   c.ld,
@@ -340,7 +340,6 @@ cudaError_t gradface_n(const DevConsts &c, const double *h_ops, const void *u, c
 }  // namespace
 
 bool hex_tma_supported(int n, bool f64) {
-  if (getenv("FR_NO_TMA")) return false;
   if (!encoder() || !hex_tma_fluxdiv_supported(n, f64)) return false;
   switch (n) {
 #define FR_CASE(NN) case NN: return f64 ? fits<NN, double>() : fits<NN, float>();

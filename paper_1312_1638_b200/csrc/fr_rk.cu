@@ -1,39 +1,115 @@
-// RK4 register updates ("classical fourth order Runge-Kutta"), vectorised streaming.
+// Register updates of the explicit time steppers (PAPER.md:247 RK4; Table 1 :263 Euler, RK4, DOPRI5): one streaming
+// kernel forms up to two linear combinations of state-sized registers per pass.  Registers are [rows][ld] matrices in the
+// storage precision; only the first nel columns of a row are touched (the pad columns of the caller's u stay as they are).
 #include "fr_dev.hpp"
 
 namespace fr {
 namespace {
 
-// mode 0: out1 = u + a k ; out2 = u + b k          (stage 1: next stage state, accumulator)
-// mode 1: out1 = u + a k ; out2 = out2 + b k       (stages 2, 3)
-// mode 2: out1 = out2 + b k                        (stage 4: u <- acc + dt/6 k4; out1 == u)
+struct LinComb {
+  int nin;
+  const void *in[RK_MAX_IN];
+  double a[RK_MAX_IN], b[RK_MAX_IN];  // out1 = sum a_i in_i,  out2 = sum b_i in_i  (zero coefficients: operand not read)
+  void *out1, *out2;                  // either may be NULL; may alias an input (element-wise update)
+};
+
 template <typename T>
-__global__ void k_rk(int64_t n, const T *__restrict__ u, const T *__restrict__ k, double a, T *out1, double b, T *out2, int mode) {
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const double kk = (double)k[i];
-    if (mode == 0) {
-      const double uu = (double)u[i];
-      out1[i] = (T)fma(a, kk, uu);
-      out2[i] = (T)fma(b, kk, uu);
-    } else if (mode == 1) {
-      out1[i] = (T)fma(a, kk, (double)u[i]);
-      out2[i] = (T)fma(b, kk, (double)out2[i]);
-    } else {
-      out1[i] = (T)fma(b, kk, (double)out2[i]);
+__global__ void __launch_bounds__(256) k_lincomb(const __grid_constant__ LinComb lc, int64_t rows, int64_t ld, int64_t nel) {
+  const int64_t col = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (col >= nel) return;
+  for (int64_t r = blockIdx.y; r < rows; r += gridDim.y) {
+    const size_t o = (size_t)r * ld + col;
+    double s1 = 0.0, s2 = 0.0;
+#pragma unroll
+    for (int i = 0; i < RK_MAX_IN; ++i) {
+      if (i < lc.nin && (lc.a[i] != 0.0 || lc.b[i] != 0.0)) {
+        const double v = (double)((const T *)lc.in[i])[o];
+        s1 = fma(lc.a[i], v, s1);
+        s2 = fma(lc.b[i], v, s2);
+      }
     }
+    if (lc.out1) ((T *)lc.out1)[o] = (T)s1;
+    if (lc.out2) ((T *)lc.out2)[o] = (T)s2;
   }
+}
+
+// sum over the first nel columns of (x - y)^2, deterministic: one partial per CTA row chunk, then a single-CTA pass
+template <typename T>
+__global__ void __launch_bounds__(256) k_sqdiff_partial(const T *__restrict__ x, const T *__restrict__ y, int64_t rows, int64_t ld, int64_t nel,
+                                                        double *__restrict__ part) {
+  __shared__ double sh[256];
+  double s = 0.0;
+  const int64_t col0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  for (int64_t r = blockIdx.y; r < rows; r += gridDim.y)
+    for (int64_t col = col0; col < nel; col += (int64_t)gridDim.x * blockDim.x) {
+      const double d = (double)x[(size_t)r * ld + col] - (double)y[(size_t)r * ld + col];
+      s = fma(d, d, s);
+    }
+  sh[threadIdx.x] = s;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if ((int)threadIdx.x < w) sh[threadIdx.x] += sh[threadIdx.x + w];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) part[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = sh[0];
+}
+
+__global__ void __launch_bounds__(256) k_rms_final(const double *__restrict__ part, int n, double count, double *__restrict__ out) {
+  __shared__ double sh[256];
+  double s = 0.0;
+  for (int i = threadIdx.x; i < n; i += 256) s += part[i];
+  sh[threadIdx.x] = s;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if ((int)threadIdx.x < w) sh[threadIdx.x] += sh[threadIdx.x + w];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *out = sqrt(sh[0] / count);
 }
 
 }  // namespace
 
-cudaError_t rk_axpy2(bool f64, int64_t n, const void *u, const void *k, double a, void *out1, double b, void *out2, int mode,
-                     cudaStream_t s) {
+cudaError_t rk_lincomb(bool f64, int64_t rows, int64_t ld, int64_t nel, int nin, const void *const *in, const double *a, const double *b,
+                       void *out1, void *out2, cudaStream_t s) {
+  if (nin < 1 || nin > RK_MAX_IN) return cudaErrorInvalidValue;
+  LinComb lc{};
+  lc.nin = nin;
+  for (int i = 0; i < nin; ++i) { lc.in[i] = in[i]; lc.a[i] = a ? a[i] : 0.0; lc.b[i] = b ? b[i] : 0.0; }
+  lc.out1 = out1; lc.out2 = out2;
   const int TB = 256;
-  int64_t nb = (n + TB - 1) / TB;
-  if (nb > 148 * 16) nb = 148 * 16;
-  if (f64) k_rk<double><<<(unsigned)nb, TB, 0, s>>>(n, (const double *)u, (const double *)k, a, (double *)out1, b, (double *)out2, mode);
-  else k_rk<float><<<(unsigned)nb, TB, 0, s>>>(n, (const float *)u, (const float *)k, a, (float *)out1, b, (float *)out2, mode);
+  const unsigned gx = (unsigned)((nel + TB - 1) / TB);
+  int64_t gy = (148 * 16 + gx - 1) / gx;  // about 16 CTAs per SM in total
+  if (gy > rows) gy = rows;
+  if (gy < 1) gy = 1;
+  if (gy > 65535) gy = 65535;
+  if (f64) k_lincomb<double><<<dim3(gx, (unsigned)gy), TB, 0, s>>>(lc, rows, ld, nel);
+  else k_lincomb<float><<<dim3(gx, (unsigned)gy), TB, 0, s>>>(lc, rows, ld, nel);
+  return cudaGetLastError();
+}
+
+cudaError_t rk_axpy2(bool f64, int64_t rows, int64_t ld, int64_t nel, const void *u, const void *k, double a, void *out1, double b,
+                     void *out2, int mode, cudaStream_t s) {
+  // mode 0: out1 = u + a k ; out2 = u + b k          (RK4 stage 1: next stage state, accumulator)
+  // mode 1: out1 = u + a k ; out2 = out2 + b k       (stages 2, 3)
+  // mode 2: out1 = out2 + b k                        (stage 4: u <- acc + dt/6 k4; out1 == u)
+  const void *in[3] = {u, k, out2};
+  if (mode == 0) { const double ca[3] = {1, a, 0}, cb[3] = {1, b, 0}; return rk_lincomb(f64, rows, ld, nel, 2, in, ca, cb, out1, out2, s); }
+  if (mode == 1) { const double ca[3] = {1, a, 0}, cb[3] = {0, b, 1}; return rk_lincomb(f64, rows, ld, nel, 3, in, ca, cb, out1, out2, s); }
+  const double ca[3] = {0, b, 1};
+  return rk_lincomb(f64, rows, ld, nel, 3, in, ca, nullptr, out1, nullptr, s);
+}
+
+cudaError_t rk_rms_diff(bool f64, int64_t rows, int64_t ld, int64_t nel, const void *x, const void *y, double *part, double *out,
+                        cudaStream_t s) {
+  const int TB = 256;
+  unsigned gx = (unsigned)((nel + TB - 1) / TB);
+  if (gx > 64) gx = 64;
+  unsigned gy = (unsigned)(RK_MAX_PARTIALS / gx);
+  if (gy > rows) gy = (unsigned)rows;
+  if (gy < 1) gy = 1;
+  if (f64) k_sqdiff_partial<double><<<dim3(gx, gy), TB, 0, s>>>((const double *)x, (const double *)y, rows, ld, nel, part);
+  else k_sqdiff_partial<float><<<dim3(gx, gy), TB, 0, s>>>((const float *)x, (const float *)y, rows, ld, nel, part);
+  k_rms_final<<<1, 256, 0, s>>>(part, (int)(gx * gy), (double)rows * (double)nel, out);
   return cudaGetLastError();
 }
 

@@ -37,14 +37,13 @@ __device__ __forceinline__ int line_base(int d, int idx, int &stride) {
 // U^f = M0 U (Eq 6 / Eq 41) and, with nblk = ND, Q^f = M5 Q (Eq 11 / Eq 43).
 template <int N, int ND, typename TIN>
 __global__ void __launch_bounds__(1024) k_tp_interp(Ops1D<N> op, const TIN *__restrict__ in, double *__restrict__ out, int64_t ncols,
-                                                    int64_t ld, int64_t Nel, int64_t in_blk, int64_t out_blk, bool blk) {
-  constexpr int NFP = ipow(N, ND - 1), NV = ND + 2;
+                                                    int64_t ld, int64_t Nel, int64_t in_blk, int64_t out_blk) {
+  constexpr int NFP = ipow(N, ND - 1);
   const int64_t col = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (col >= ncols || (col % ld) >= Nel) return;
   in += (size_t)blockIdx.z * in_blk + col;
-  // element-blocked output (fr_dev.hpp: fp_row): row fp*NV + a of 2 ND NFP NV rows; plain: out[fp][a][ld]
-  const size_t rs = blk ? (size_t)NV * FR_BLK : (size_t)ncols;  // distance between consecutive flux points
-  out += blk ? fp_row(true, ld, 2 * ND * NFP * NV, (int)(col / ld), col % ld) : (size_t)blockIdx.z * out_blk + col;
+  const size_t rs = (size_t)ncols;  // distance between consecutive flux points: out[fp][a][ld]
+  out += (size_t)blockIdx.z * out_blk + col;
   for (int idx = threadIdx.y; idx < NFP; idx += blockDim.y) {
 #pragma unroll
     for (int d = 0; d < ND; ++d) {
@@ -144,58 +143,16 @@ __global__ void __launch_bounds__(1024) k_tp_div(Ops1D<N> op, const double *__re
   }
 }
 
-#include "fr_hex.cuh"
-
-template <int N, int E, bool NS, typename T>
-void launch_hex_fluxdiv_e(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *qu, const double *dt, T *rhs, cudaStream_t s) {
-  const size_t smem = (size_t)(N * N + 2 * 2 * 5 * N * N * E) * sizeof(double);
-  auto kern = k_hex_fluxdiv<N, E, NS, T>;
-  static bool attr_done = false;
-  if (!attr_done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
-  kern<<<(unsigned)((c.Nel + E - 1) / E), dim3(E, N * N), smem, s>>>(op, c.ph, u, qu, c.smat, c.rcpj, dt, rhs, c.ld, c.Nel);
-}
-template <int N, bool NS, typename T>
-void launch_hex_fluxdiv(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *qu, const double *dt, T *rhs, cudaStream_t s) {
-  constexpr int E = N <= 3 ? 32 : (N <= 5 ? 16 : 8);
-  launch_hex_fluxdiv_e<N, E, NS, T>(op, c, u, qu, dt, rhs, s);
-}
-
-template <int N, int E, typename T>
-void launch_hex_grad_e(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *jump, double *qu, cudaStream_t s) {
-  const size_t smem = (size_t)(N * N + 2 * 5 * N * N * E) * sizeof(double);
-  auto kern = k_hex_grad<N, E, T>;
-  static bool attr_done = false;
-  if (!attr_done) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_done = true; }
-  kern<<<(unsigned)((c.Nel + E - 1) / E), dim3(E, N * N), smem, s>>>(op, u, jump, c.smat, c.rcpj, qu, c.ld, c.Nel);
-}
-template <int N, typename T>
-void launch_hex_grad(const Ops1D<N> &op, const DevConsts &c, const T *u, const double *jump, double *qu, cudaStream_t s) {
-  constexpr int E = N <= 3 ? 32 : (N <= 5 ? 16 : 8);
-  launch_hex_grad_e<N, E, T>(op, c, u, jump, qu, s);
-}
-
 template <int N, int ND, typename T>
 cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, char *work, cudaStream_t s, Prof *prof) {
   constexpr int NU = ipow(N, ND), NFP = ipow(N, ND - 1), NF = 2 * ND * NFP;
-  const Ops1D<N> op = make_ops<N>(tp.h_ops);
-  const int64_t ncols = (int64_t)c.NV * c.ld;
   double *uf = (double *)(work + tp.off_uf), *cf = (double *)(work + tp.off_cf), *qu = (double *)(work + tp.off_qu),
          *qf = (double *)(work + tp.off_qf);
-  constexpr int LW = 32;  // lanes (columns) per CTA row
-  const int rows = 1024 / LW;
-  const unsigned gx = (unsigned)((ncols + LW - 1) / LW), ge = (unsigned)((c.Nel + LW - 1) / LW);
-  const dim3 bf(LW, NFP < rows ? NFP : rows), bu(LW, NU < rows ? NU : rows);
-  if (ND == 3 && tp.use_tma) {
+  if constexpr (ND == 3) {
+    // hexahedra: sm_100a TMA path, 5 launches for Navier-Stokes (3 for Euler); neither Q^f nor F~ is stored
     FR_MARK(prof, "hex_interp_tma");
     cudaError_t e = hex_tma_interp(c, tp.h_ops, u, uf, s);
     if (e != cudaSuccess) return e;
-  } else {
-    FR_MARK(prof, "tp_interp");
-    k_tp_interp<N, ND, T><<<dim3(gx, 1, 1), bf, 0, s>>>(op, u, uf, ncols, c.ld, c.Nel, 0, 0, c.blk);
-  }
-  if (ND == 3 && tp.use_tma) {
-    // sm_100a path: 5 launches for Navier-Stokes (3 for Euler); neither Q^f nor F~ is stored
-    cudaError_t e = cudaSuccess;
     if (c.ns) {
       FR_MARK(prof, "common_sol");
       launch_common_jump(c, uf, cf, s);
@@ -211,35 +168,32 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
     FR_MARK(prof, "hex_fluxdiv_tma");
     e = hex_tma_fluxdiv(c, tp.h_ops, u, qf, uf, rhs, s);
     return e != cudaSuccess ? e : cudaGetLastError();
-  }
-  if (c.ns) {
-    FR_MARK(prof, "common_sol");
-    launch_common_jump(c, uf, cf, s);
-    if (ND == 3) {
-      FR_MARK(prof, "hex_grad");
-      launch_hex_grad<N, T>(op, c, u, cf, qu, s);
-    } else {
+  } else {
+    // quadrilaterals (p = 0 and p >= 5; lower orders run the fused element kernels): L1-gather line kernels
+    const Ops1D<N> op = make_ops<N>(tp.h_ops);
+    const int64_t ncols = (int64_t)c.NV * c.ld;
+    constexpr int LW = 32;  // lanes (columns) per CTA row
+    const int rows = 1024 / LW;
+    const unsigned gx = (unsigned)((ncols + LW - 1) / LW), ge = (unsigned)((c.Nel + LW - 1) / LW);
+    const dim3 bf(LW, NFP < rows ? NFP : rows), bu(LW, NU < rows ? NU : rows);
+    FR_MARK(prof, "tp_interp");
+    k_tp_interp<N, ND, T><<<dim3(gx, 1, 1), bf, 0, s>>>(op, u, uf, ncols, c.ld, c.Nel, 0, 0);
+    if (c.ns) {
+      FR_MARK(prof, "common_sol");
+      launch_common_jump(c, uf, cf, s);
       FR_MARK(prof, "tp_grad");
       k_tp_grad<N, ND, T><<<dim3(ge, 1, 1), dim3(LW, 256 / LW), 0, s>>>(op, u, cf, c.smat, c.rcpj, qu, ncols, c.ld, c.Nel);
+      FR_MARK(prof, "tp_interp_q");
+      k_tp_interp<N, ND, double><<<dim3(gx, 1, ND), bf, 0, s>>>(op, qu, qf, ncols, c.ld, c.Nel, (int64_t)NU * ncols, (int64_t)NF * ncols);
     }
-    FR_MARK(prof, "tp_interp_q");
-    k_tp_interp<N, ND, double><<<dim3(gx, 1, ND), bf, 0, s>>>(op, qu, qf, ncols, c.ld, c.Nel, (int64_t)NU * ncols, (int64_t)NF * ncols, false);
-  }
-  if (ND == 3) {
+    FR_MARK(prof, "tflux");
+    launch_tflux(c, u, qu, s);
     FR_MARK(prof, "common_flux");
     launch_common_flux(c, uf, qf, s);
-    FR_MARK(prof, "hex_fluxdiv");
-    if (c.ns) launch_hex_fluxdiv<N, true, T>(op, c, u, qu, uf, rhs, s);
-    else launch_hex_fluxdiv<N, false, T>(op, c, u, qu, uf, rhs, s);
+    FR_MARK(prof, "tp_div");
+    k_tp_div<N, ND, T><<<dim3(gx, 1, 1), bu, 0, s>>>(op, qu, uf, c.rcpj, rhs, ncols, c.ld, c.Nel);
     return cudaGetLastError();
   }
-  FR_MARK(prof, "tflux");
-  launch_tflux(c, u, qu, s);
-  FR_MARK(prof, "common_flux");
-  launch_common_flux(c, uf, qf, s);
-  FR_MARK(prof, "tp_div");
-  k_tp_div<N, ND, T><<<dim3(gx, 1, 1), bu, 0, s>>>(op, qu, uf, c.rcpj, rhs, ncols, c.ld, c.Nel);
-  return cudaGetLastError();
 }
 
 template <int ND>
@@ -257,7 +211,11 @@ cudaError_t dispatch_n(const DevConsts &c, const TensorPlan &tp, const void *u, 
 
 }  // namespace
 
-bool tensor_supported(const DevConsts &c) { return (c.etype == FR_QUAD || c.etype == FR_HEX) && c.n >= 1 && c.n <= 8; }
+// quadrilaterals at any order 0 <= p <= 7; hexahedra when the TMA kernels can run (c.blk: decided in fr_api.cu with the layout)
+bool tensor_supported(const DevConsts &c) {
+  if (c.n < 1 || c.n > 8) return false;
+  return c.etype == FR_QUAD || (c.etype == FR_HEX && c.blk);
+}
 
 cudaError_t tensor_plan(const DevConsts &c, const RefOps &o, const MeshConsts &, TensorPlan &tp, std::vector<void *> &) {
   tp = TensorPlan();
@@ -274,7 +232,7 @@ cudaError_t tensor_plan(const DevConsts &c, const RefOps &o, const MeshConsts &,
   int64_t off = 0;
   tp.off_uf = off; off = al(off + (int64_t)o.Nf * ncols * 8);
   tp.off_cf = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
-  tp.use_tma = c.blk;  // decided with the layout of the internal arrays (fr_api.cu)
+  tp.use_tma = c.blk;
   if (tp.use_tma) {  // G^f (and Q, slice-major) besides U^f and the jumps
     tp.off_qu = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
     tp.off_qf = off; if (c.ns) off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
@@ -291,13 +249,9 @@ cudaError_t tensor_rhs(const DevConsts &c, const TensorPlan &tp, const void *u, 
 }
 
 int tensor_rhs_launches(const DevConsts &c) {
-  if (c.blk) {
-    int n = c.ns ? 5 : 3;  // interp, (common sol, gradface,) common flux, rhs
-    if (c.nbnd) n += c.ns ? 2 : 1;
-    if (!c.npairs) n -= c.ns ? 2 : 1;
-    return n;
-  }
-  int n = 4 + (c.ns ? 3 : 0);  // interp, tflux, common flux, div (+ common sol, grad, interp q)
+  int n;
+  if (c.nd == 3) n = c.ns ? 5 : 3;  // interp, (common sol, gradface,) common flux, fluxdiv
+  else n = c.ns ? 7 : 4;            // interp, (common sol, grad, interp q,) tflux, common flux, div
   if (c.nbnd) n += c.ns ? 2 : 1;
   if (!c.npairs) n -= c.ns ? 2 : 1;
   return n;

@@ -207,12 +207,13 @@ inline bool encode_blk(CUtensorMap *m, const void *base, uint64_t ld, uint64_t r
             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// function attributes are per device: one flag per (kernel instantiation, device ordinal)
 template <typename K>
-cudaError_t set_smem(K kern, size_t smem, bool &done) {
-  if (done) return cudaSuccess;
+cudaError_t set_smem(K kern, size_t smem, DevFlags &done, int dev) {
+  if (done.test(dev)) return cudaSuccess;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-  done = e == cudaSuccess;
+  if (e == cudaSuccess) done.set(dev);
   return e;
 }
 

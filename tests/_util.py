@@ -11,6 +11,17 @@ def rel_l2_per_field(a, b):
     return np.asarray(num / den, dtype=np.float64)
 
 
+def rel_max_per_field(a, b):
+    """max|a-b| / max|b| per variable (the max-abs companion of the L2 norm)."""
+    a = np.asarray(a, dtype=np.longdouble)
+    b = np.asarray(b, dtype=np.longdouble)
+    return np.asarray(np.max(np.abs(a - b), axis=(0, 2)) / np.max(np.abs(b), axis=(0, 2)), dtype=np.float64)
+
+
+# parity triples of the current pytest session (written to gpurun_out/parity_records.jsonl by conftest.py)
+RECORDS = []
+
+
 class GpuRunner:
     """Allocates device buffers with torch and calls the C-ABI through the binding."""
 

@@ -197,6 +197,24 @@ def tri_mesh(n, length=1.0, jitter=0.1, seed=4321, periodic=True):
     }
 
 
+def curve_tri_mesh(mesh, p_g=2, amplitude=0.01):
+    """Raises a straight-sided triangle mesh to geometry degree p_g: lattice nodes (rows j = 0..p_g, i = 0..p_g-j) of each
+    straight triangle, displaced by amplitude*sin(2 pi x/L)*sin(2 pi y/L) in both coordinates (smooth, zero on the box
+    boundary, so periodic images and shared edges still match).  Topology unchanged."""
+    V = mesh["nodes"]  # [n_el, 3, 2]
+    L = np.array(mesh["lengths"])
+    pts = []
+    for j in range(p_g + 1):
+        for i in range(p_g + 1 - j):
+            pts.append(V[:, 0] + (i / p_g) * (V[:, 1] - V[:, 0]) + (j / p_g) * (V[:, 2] - V[:, 0]))
+    X = np.stack(pts, axis=1)  # [n_el, n_nodes, 2]
+    d = amplitude * np.prod(np.sin(2 * np.pi * X / L[None, None, :]), axis=-1, keepdims=True)
+    out = dict(mesh)
+    out["nodes"] = np.ascontiguousarray(X + np.repeat(d, 2, axis=-1))
+    out["p_g"] = p_g
+    return out
+
+
 # ----------------------------------------------------------------------------
 # analytic states, evaluated at physical coordinates X[..., nd] -> U[..., nd+2]
 # (conserved variables rho, rho*v, E with E = p/(gamma-1) + rho|v|^2/2, PAPER.md:481 Eq 21)
