@@ -35,6 +35,8 @@ enum { FR_QUAD = 0, FR_TRI = 1, FR_HEX = 2 };                  /* element types,
 enum { FR_EULER = 0, FR_NAVIER_STOKES = 1 };                   /* governing systems */
 enum { FR_F32 = 0, FR_F64 = 1 };                               /* storage precision of u / rhs */
 enum { FR_BC_SUP_INFLOW = 0, FR_BC_SUB_OUTFLOW = 1, FR_BC_NOSLIP_WALL = 2 }; /* App C :799-825 */
+enum { FR_CORR_DG = 0, FR_CORR_SD = 1, FR_CORR_HU = 2 };      /* FR schemes, "DG, SD, and HU as defined in [10]" */
+enum { FR_STEPPER_EULER = 0, FR_STEPPER_RK4 = 1, FR_STEPPER_DOPRI5 = 2 }; /* time steppers, Table 1 :263 */
 
 enum {
   FR_OK = 0,
@@ -71,13 +73,24 @@ typedef struct {
 
 /* Discretisation: order p, system (§4), storage precision, gas constants gamma (Eq 21),
  * mu, Pr (Eq 22-23; mu constant, A9), LDG beta / tau (Eq 25-27 :506-516; tau enters with the dissipative
- * sign, A7).  Point sets and the DG correction function are fixed (A5, A6). */
+ * sign, A7).  Point sets are fixed (A6).  correction: FR_CORR_DG (A5; every element type), FR_CORR_SD / FR_CORR_HU
+ * (:568; the one-parameter family of the paper's ref [10] with c_SD / c_HU, reading A23; quadrilaterals and hexahedra,
+ * FR_CORR_HU needs p >= 1; FR_EINVAL otherwise).
+ * rho_ref, v_ref, p_ref: an optional constant reference state (all zero = none).  It is a CONDITIONING hint, not a
+ * parameter of the method: the fused kernels then evaluate the inviscid flux and the interface flux in perturbation
+ * form about it (constant fluxes have zero discrete divergence, Eq 18 with M1 const = 0), which removes
+ * the cancellation of O(p_ref) terms from the rounding error.  The result is the same function of u up to rounding on
+ * meshes whose metric terms satisfy the discrete metric identities (affine elements; 2-D elements with p_g <= p; the
+ * 3-D cases of reading A10); elsewhere it differs by the freestream residual of the reference state. */
 typedef struct {
   int32_t p;
   int32_t system;
   int32_t precision;
   int32_t flags;           /* FR_FLAG_* bits */
+  int32_t correction;      /* FR_CORR_* */
+  int32_t reserved;        /* 0 */
   double gamma, mu, Pr, ldg_beta, ldg_tau;
+  double rho_ref, v_ref[3], p_ref;
 } fr_disc_desc;
 
 #define FR_FLAG_FORCE_GENERIC 1
@@ -102,6 +115,7 @@ int64_t fr_num_pairs(const fr_ctx *ctx);           /* interior+periodic flux-poi
 int64_t fr_leading_dim(const fr_ctx *ctx);         /* ld of every state matrix */
 int64_t fr_state_bytes(const fr_ctx *ctx);         /* N_u*N_V*ld*sizeof(precision) */
 int64_t fr_workspace_bytes(const fr_ctx *ctx);     /* scratch for fr_rhs + RK registers for fr_rk4_step */
+int64_t fr_stepper_workspace_bytes(const fr_ctx *ctx, int stepper); /* the same for FR_STEPPER_*: Euler 1, RK4 3, DOPRI5 7 registers */
 int64_t fr_rhs_kernel_launches(const fr_ctx *ctx); /* kernels one fr_rhs call launches */
 
 /* Physical coordinates of the solution points, host buffer [N_u][n_elems][ndims] doubles. */
@@ -131,8 +145,18 @@ int fr_rhs(fr_ctx *ctx, const void *u_dev, void *rhs_dev, void *work_dev, void *
 int fr_rhs_profiled(fr_ctx *ctx, const void *u_dev, void *rhs_dev, void *work_dev, void *stream, int max_kernels,
                     int *n_kernels, float *ms_host, char *names_host);
 
-/* One classical RK4 step, u advanced in place; four fr_rhs evaluations. */
+/* One classical RK4 step, u advanced in place; four fr_rhs evaluations.  Pad columns (element index
+ * >= n_elems) of u are left untouched by every stepper. */
 int fr_rk4_step(fr_ctx *ctx, void *u_dev, double dt, void *work_dev, void *stream);
+
+/* One forward Euler step u <- u + dt R(u) (Table 1 :263).  work_dev: >= fr_stepper_workspace_bytes(FR_STEPPER_EULER). */
+int fr_euler_step(fr_ctx *ctx, void *u_dev, double dt, void *work_dev, void *stream);
+
+/* One step of the Dormand-Prince 5(4) pair (Table 1 :263 "DOPRI5"; the published tableau, reading A24): seven fr_rhs
+ * evaluations; u advanced in place with the fifth-order weights.  err_dev (device, may be NULL): receives the RMS over
+ * all n_elems*N_u*N_V values of the embedded error estimate dt * sum_i (b5_i - b4_i) k_i, reduced in a fixed order
+ * (bit-reproducible).  Step-size control is the caller's.  work_dev: >= fr_stepper_workspace_bytes(FR_STEPPER_DOPRI5). */
+int fr_dopri5_step(fr_ctx *ctx, void *u_dev, double dt, void *work_dev, void *stream, double *err_dev);
 
 /* End-to-end variant with HOST buffers: copies u_host -> u_dev (H2D), evaluates fr_rhs, copies
  * rhs_dev -> rhs_host (D2H), all asynchronously on `stream` (pinned host memory recommended).

@@ -28,8 +28,11 @@ M0/M4/M1, zero divergence of a constant flux, w^T M3 = w^f, Radau closed form of
 correction on tensor elements, fused == unfused Eq 42/44, gradient exactness for continuous
 polynomials, flux consistency/antisymmetry, closed-form stresses, p=0 == first-order finite
 volume (hand-written loops), freestream, conservation, vortex order p+1, RK4 stability
-polynomial.  PARITY UNPINNED by the paper (fixed by documentation only): A6 (triangle
-solution-point set), A7 (sign of the LDG penalty tau), A12/A13 (which side is L; beta, tau).
+polynomial; SD / HU correction functions: end values, zeros at the Gauss / Gauss-Lobatto points;
+DOPRI5: row sums, order conditions to order 5 / 4, stability polynomial.
+PARITY UNPINNED by the paper (fixed by documentation only): A6 (triangle solution-point set), A7 (sign of
+the LDG penalty tau), A12/A13 (which side is L; beta, tau), A23 (which published correction functions the
+names SD and HU denote), A24 (the DOPRI5 tableau: named, not printed).
 """
 import numpy as np
 
@@ -270,13 +273,41 @@ class RefElement:
 
 
 # =============================================================================
+# correction functions of the FR schemes the paper runs ("DG, SD, and HU as defined in [10]")
+# =============================================================================
+def correction_derivative_1d(scheme, p, x):
+    """g_R'(x) of the 1-D right-boundary correction function g_R (degree p+1, g_R(-1) = 0, g_R(1) = 1) on [-1,1];
+    the left one is g_L(x) = g_R(-x).  Closed forms (reading A23; the paper only names the schemes):
+      dg  g_R = R_{p+1},  R_k = (P_{k-1} + P_k)/2 the right Radau polynomial of degree k  (reading A5)
+      sd  g_R = (1 + x)/2 * P_p(x): zero at the p Gauss points, which recovers the spectral difference scheme
+      hu  g_R = ((p+1) R_p + p R_{p+1}) / (2p+1): Huynh's g_2, whose derivative vanishes at the interior
+          Gauss-Lobatto points and at -1."""
+    x = np.asarray(x, dtype=LD)
+
+    def radau_d(k):  # R_k' = (P_{k-1}' + P_k')/2
+        return (legendre(k - 1, x)[1] + legendre(k, x)[1]) / 2
+
+    if scheme == "dg":
+        return radau_d(p + 1)
+    if scheme == "sd":
+        P, dP = legendre(p, x)
+        return P / 2 + (1 + x) / 2 * dP
+    if scheme == "hu":
+        if p < 1:
+            raise ValueError("the HU scheme needs p >= 1")
+        return ((p + 1) * radau_d(p) + p * radau_d(p + 1)) / (2 * p + 1)
+    raise KeyError(scheme)
+
+
+# =============================================================================
 # O3: constant operator matrices (PAPER.md:737-768 App A)
 # =============================================================================
 class Operators:
     """M0..M6 of Appendix A for one element type, long double.
-    Vector rows are packed with stride N_u (or N_f): row = d*N_u + rho."""
+    Vector rows are packed with stride N_u (or N_f): row = d*N_u + rho.
+    scheme: 'dg' (any element type) or 'sd' / 'hu' (quadrilaterals and hexahedra, tensor product of the 1-D functions)."""
 
-    def __init__(self, ref):
+    def __init__(self, ref, scheme="dg"):
         nd, Nu, Nf = ref.nd, ref.Nu, ref.Nf
         Lf, _ = ref.basis(ref.xf)  # [Nf, Nu]
         _, dLu = ref.basis(ref.xu)  # [nd, Nu(points), Nu(basis)]
@@ -291,6 +322,20 @@ class Operators:
         # M3[rho, sigma] = (div g_sigma)(x^u_rho), DG correction (reading A5):
         # div g_sigma = sum_rho l_rho * (Mass^-1 M0^T diag(w^f))[rho, sigma]
         self.M3 = _solve_ld(ref.mass, Lf.T * ref.wf[None, :])
+        if scheme != "dg":
+            # SD / HU on tensor elements: the correction field of flux point sigma on face (d, s) is the 1-D function along d
+            # times the face's Lagrange polynomials in the other directions, so (div g_sigma)(x_rho) = g'(xi_d) on the line
+            # of solution points through sigma and zero off it; outward normals: +g_R'(xi) at s = 1, g_R'(-xi) at s = 0
+            if ref.etype not in ("quad", "hex"):
+                raise ValueError("SD / HU correction functions are defined on quadrilaterals and hexahedra only")
+            n, M3 = ref.p + 1, np.zeros((Nu, Nf), dtype=LD)
+            for sig in range(Nf):
+                d, side = (sig // ref.nfp) // 2, (sig // ref.nfp) % 2
+                others = [dd for dd in range(nd) if dd != d]
+                on_line = np.all(np.abs(ref.xu[:, others] - ref.xf[sig, others][None, :]) < 1e-14, axis=1)
+                xi = ref.xu[on_line, d]
+                M3[on_line, sig] = correction_derivative_1d(scheme, ref.p, xi if side else -xi)
+            self.M3 = M3
         # M6[(d,rho), sigma] = n_sigma,d * M3[rho, sigma]  (reading A1)           :749
         self.M6 = np.concatenate([self.M3 * ref.nf[None, :, d] for d in range(nd)], axis=0)
         # M5 = diag(M0,...,M0)                                                    :760
@@ -397,13 +442,27 @@ def ghost_states(kind, par, uL, gamma):
     raise KeyError(kind)
 
 
+# Dormand-Prince 5(4): nodes c_i = sum_j a_ij, 5th-order weights b5 (= row 7 of A: first-same-as-last), 4th-order weights b4
+DOPRI5_A = [
+    [],
+    [1 / 5],
+    [3 / 40, 9 / 40],
+    [44 / 45, -56 / 15, 32 / 9],
+    [19372 / 6561, -25360 / 2187, 64448 / 6561, -212 / 729],
+    [9017 / 3168, -355 / 33, 46732 / 5247, 49 / 176, -5103 / 18656],
+    [35 / 384, 0, 500 / 1113, 125 / 192, -2187 / 6784, 11 / 84],
+]
+DOPRI5_B5 = [35 / 384, 0, 500 / 1113, 125 / 192, -2187 / 6784, 11 / 84, 0]
+DOPRI5_B4 = [5179 / 57600, 0, 7571 / 16695, 393 / 640, -92097 / 339200, 187 / 2100, 1 / 40]
+
+
 # =============================================================================
 # the discretisation on a mesh of one element type
 # =============================================================================
 class FROracle:
     """FR semi-discretisation on a single-element-type mesh (workloads.py mesh dict).
 
-    prm: p, system ('euler'|'navier-stokes'), gamma, mu, Pr, beta, tau.
+    prm: p, system ('euler'|'navier-stokes'), gamma, mu, Pr, beta, tau, correction ('dg' default | 'sd' | 'hu').
     bcs: {bc_id: (kind, params)} for boundary faces.
     dtype: np.float64 or np.longdouble for the STATE arithmetic (operators and metrics are
     always built in long double and rounded once to dtype)."""
@@ -411,7 +470,7 @@ class FROracle:
     def __init__(self, mesh, prm, bcs=None, dtype=np.float64):
         self.mesh, self.prm, self.bcs, self.dtype = mesh, dict(prm), bcs or {}, dtype
         self.ref = ref = RefElement(mesh["etype"], prm["p"])
-        self.ops = Operators(ref)
+        self.ops = Operators(ref, self.prm.get("correction", "dg"))
         self.nd, self.Nu, self.Nf = ref.nd, ref.Nu, ref.Nf
         self.NV = ref.nd + 2
         self.Nel = mesh["nodes"].shape[0]
@@ -581,6 +640,28 @@ class FROracle:
         k3 = self.rhs(u + (dt / 2) * k2)
         k4 = self.rhs(u + dt * k3)
         return u + (dt / 6) * (k1 + 2 * k2 + 2 * k3 + k4)
+
+    def euler_step(self, u, dt):
+        """Forward Euler (Table 1 :263)."""
+        return u + dt * self.rhs(u)
+
+    def dopri5_step(self, u, dt):
+        """One step of the Dormand-Prince 5(4) pair (Table 1 :263 names DOPRI5; the tableau is the published one, reading
+        A24).  Returns (u advanced with the 5th-order weights, dt * sum (b5 - b4)_i k_i = the embedded error estimate)."""
+        k = []
+        for i in range(7):
+            ui = u
+            for j in range(i):
+                if DOPRI5_A[i][j] != 0:
+                    ui = ui + (dt * DOPRI5_A[i][j]) * k[j]
+            k.append(self.rhs(ui))
+        new = u
+        err = 0
+        for i in range(7):
+            if DOPRI5_B5[i] != 0:
+                new = new + (dt * DOPRI5_B5[i]) * k[i]
+            err = err + (dt * (DOPRI5_B5[i] - DOPRI5_B4[i])) * k[i]
+        return new, err
 
     # ---- O12: quadrature functionals ----
     def integrate(self, g):

@@ -18,6 +18,8 @@ EULER, NAVIER_STOKES = 0, 1
 F32, F64 = 0, 1
 BC_SUP_INFLOW, BC_SUB_OUTFLOW, BC_NOSLIP_WALL = 0, 1, 2
 FLAG_FORCE_GENERIC, FLAG_HOST_ONLY = 1, 2
+CORRECTIONS = {"dg": 0, "sd": 1, "hu": 2}
+STEPPERS = {"euler": 0, "rk4": 1, "dopri5": 2}
 ETYPES = {"quad": QUAD, "tri": TRI, "hex": HEX}
 SYSTEMS = {"euler": EULER, "navier-stokes": NAVIER_STOKES}
 BC_KINDS = {"sup-inflow": BC_SUP_INFLOW, "sub-outflow": BC_SUB_OUTFLOW, "noslip-wall": BC_NOSLIP_WALL}
@@ -44,7 +46,9 @@ class fr_mesh_desc(C.Structure):
 class fr_disc_desc(C.Structure):
     _fields_ = [
         ("p", C.c_int32), ("system", C.c_int32), ("precision", C.c_int32), ("flags", C.c_int32),
+        ("correction", C.c_int32), ("reserved", C.c_int32),
         ("gamma", C.c_double), ("mu", C.c_double), ("Pr", C.c_double), ("ldg_beta", C.c_double), ("ldg_tau", C.c_double),
+        ("rho_ref", C.c_double), ("v_ref", C.c_double * 3), ("p_ref", C.c_double),
     ]
 
 
@@ -61,6 +65,9 @@ def _load():
         "fr_num_solution_points": (I64, [P]), "fr_num_flux_points": (I64, [P]), "fr_num_vars": (I64, [P]),
         "fr_num_pairs": (I64, [P]), "fr_leading_dim": (I64, [P]), "fr_state_bytes": (I64, [P]),
         "fr_workspace_bytes": (I64, [P]), "fr_rhs_kernel_launches": (I64, [P]),
+        "fr_stepper_workspace_bytes": (I64, [P, C.c_int]),
+        "fr_euler_step": (C.c_int, [P, P, C.c_double, P, P]),
+        "fr_dopri5_step": (C.c_int, [P, P, C.c_double, P, P, P]),
         "fr_solution_point_coords": (C.c_int, [P, P]),
         "fr_operator_dims": (C.c_int, [P, C.c_int, C.POINTER(I64), C.POINTER(I64)]),
         "fr_get_operator": (C.c_int, [P, C.c_int, P]),
@@ -81,7 +88,8 @@ def _load():
 
 lib = _load()
 EXPORTS = ["fr_setup_mesh", "fr_setup_operators", "fr_num_solution_points", "fr_num_flux_points", "fr_num_vars", "fr_num_pairs",
-           "fr_leading_dim", "fr_state_bytes", "fr_workspace_bytes", "fr_rhs_kernel_launches", "fr_solution_point_coords",
+           "fr_leading_dim", "fr_state_bytes", "fr_workspace_bytes", "fr_stepper_workspace_bytes", "fr_rhs_kernel_launches",
+           "fr_euler_step", "fr_dopri5_step", "fr_solution_point_coords",
            "fr_operator_dims", "fr_get_operator", "fr_get_pairs", "fr_get_metrics", "fr_rhs", "fr_rhs_profiled", "fr_rk4_step", "fr_rhs_host",
            "fr_teardown", "fr_last_error"]
 
@@ -130,9 +138,15 @@ class Context:
         if rc != 0:
             raise FrError(rc, (lib.fr_last_error(self._h) or b"").decode())
 
-    def setup_operators(self, p, system, precision="f64", gamma=1.4, mu=0.0, Pr=0.71, beta=0.5, tau=0.1, flags=0, **_):
+    def setup_operators(self, p, system, precision="f64", gamma=1.4, mu=0.0, Pr=0.71, beta=0.5, tau=0.1, flags=0, correction="dg",
+                        ref=None, **_):
+        """ref: optional constant reference state dict(rho=, v=(..), p=) (fr.h: conditioning hint)."""
         d = fr_disc_desc(p=p, system=SYSTEMS[system], precision=F64 if precision in ("f64", F64) else F32, flags=flags,
-                         gamma=gamma, mu=mu, Pr=Pr, ldg_beta=beta, ldg_tau=tau)
+                         correction=CORRECTIONS[correction], gamma=gamma, mu=mu, Pr=Pr, ldg_beta=beta, ldg_tau=tau)
+        if ref:
+            d.rho_ref, d.p_ref = float(ref["rho"]), float(ref["p"])
+            for i, v in enumerate(ref.get("v", ())):
+                d.v_ref[i] = float(v)
         self._check(lib.fr_setup_operators(self._h, C.byref(d)))
         self.Nu = lib.fr_num_solution_points(self._h)
         self.Nf = lib.fr_num_flux_points(self._h)
@@ -186,6 +200,15 @@ class Context:
 
     def rk4_step(self, u_ptr, dt, work_ptr, stream=0):
         self._check(lib.fr_rk4_step(self._h, u_ptr, float(dt), work_ptr, stream))
+
+    def stepper_workspace_bytes(self, stepper):
+        return lib.fr_stepper_workspace_bytes(self._h, STEPPERS[stepper])
+
+    def euler_step(self, u_ptr, dt, work_ptr, stream=0):
+        self._check(lib.fr_euler_step(self._h, u_ptr, float(dt), work_ptr, stream))
+
+    def dopri5_step(self, u_ptr, dt, work_ptr, stream=0, err_ptr=None):
+        self._check(lib.fr_dopri5_step(self._h, u_ptr, float(dt), work_ptr, stream, err_ptr))
 
     def rhs_host(self, u_host_ptr, rhs_host_ptr, u_ptr, rhs_ptr, work_ptr, stream=0):
         self._check(lib.fr_rhs_host(self._h, u_host_ptr, rhs_host_ptr, u_ptr, rhs_ptr, work_ptr, stream))

@@ -108,7 +108,7 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
   try {
     c->ready = false;
     free_dev(c);
-    build_ref_ops(c->mesh.etype, d->p, c->mesh.p_g, c->ops);
+    build_ref_ops(c->mesh.etype, d->p, c->mesh.p_g, d->correction, c->ops);
     const int64_t lane = FR_BLK;  // rows start on 128-byte boundaries (north_star) and hold whole element blocks (fp_row)
     const int64_t ld = align_up(c->mesh.Nel, lane);
     std::string err;
@@ -204,8 +204,9 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
       w.qu = take((int64_t)o.nd * o.Nu * dc.NV * ld * 8);
       w.qf = dc.ns ? take((int64_t)o.nd * o.Nf * dc.NV * ld * 8) : 0;
     }
-    w.rk_k = take(state); w.rk_tmp = take(state); w.rk_acc = take(state);
-    w.total = off;
+    w.partials = take((int64_t)RK_MAX_PARTIALS * 8);
+    w.reg0 = off; w.reg_stride = align_up(state, 256);
+    w.total = w.reg0 + 3 * w.reg_stride;
     c->ready = true;
     return FR_OK;
   } catch (const std::bad_alloc &) {
@@ -226,6 +227,12 @@ int64_t fr_num_pairs(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return c->mc
 int64_t fr_leading_dim(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return c->dc.ld; }
 int64_t fr_state_bytes(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return (int64_t)c->ops.Nu * c->dc.NV * c->dc.ld * (c->dc.f64 ? 8 : 4); }
 int64_t fr_workspace_bytes(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return c->wl.total; }
+int64_t fr_stepper_workspace_bytes(const fr_ctx *c, int stepper) {
+  FR_NEED_READY(c, FR_EINVAL)
+  const int regs = stepper == FR_STEPPER_EULER ? 1 : stepper == FR_STEPPER_RK4 ? 3 : stepper == FR_STEPPER_DOPRI5 ? 7 : -1;
+  if (regs < 0) return fail(c, FR_EINVAL, "unknown stepper");
+  return c->wl.reg0 + regs * c->wl.reg_stride;
+}
 int64_t fr_rhs_kernel_launches(const fr_ctx *c) {
   FR_NEED_READY(c, FR_EINVAL)
   return c->use_tensor ? tensor_rhs_launches(c->dc) : generic_rhs_launches(c->dc);
@@ -310,30 +317,86 @@ int fr_rhs_profiled(fr_ctx *c, const void *u, void *rhs, void *work, void *strea
   return FR_OK;
 }
 
+// ---- time steppers (Table 1 :263).  Registers: work + reg0 + i * reg_stride ----
+#define FR_STEPPER_PROLOGUE(name)                                                                       \
+  FR_NEED_READY(c, FR_EINVAL)                                                                           \
+  if (c->host_only) return fail(c, FR_EINVAL, name ": context was set up with FR_FLAG_HOST_ONLY");       \
+  if (!u || !work) return fail(c, FR_EINVAL, name ": NULL device pointer");                              \
+  cudaStream_t s = (cudaStream_t)stream;                                                                \
+  char *wk = (char *)work;                                                                              \
+  auto reg = [&](int i) { return (void *)(wk + c->wl.reg0 + i * c->wl.reg_stride); };                   \
+  const int64_t rows = (int64_t)c->ops.Nu * c->dc.NV, ld = c->dc.ld, nel = c->dc.Nel;                   \
+  const bool f64 = c->dc.f64;                                                                           \
+  int rc;                                                                                               \
+  cudaError_t e = cudaSuccess;
+
 int fr_rk4_step(fr_ctx *c, void *u, double dt, void *work, void *stream) {
-  FR_NEED_READY(c, FR_EINVAL)
-  if (c->host_only) return fail(c, FR_EINVAL, "fr_rk4_step: context was set up with FR_FLAG_HOST_ONLY");
-  if (!u || !work) return fail(c, FR_EINVAL, "fr_rk4_step: NULL device pointer");
-  cudaStream_t s = (cudaStream_t)stream;
-  char *wk = (char *)work;
-  void *k = wk + c->wl.rk_k, *tmp = wk + c->wl.rk_tmp, *acc = wk + c->wl.rk_acc;
-  const int64_t n = (int64_t)c->ops.Nu * c->dc.NV;  // rows of ld values; pad columns (e >= n_elems) are left untouched
-  const bool f64 = c->dc.f64;
-  int rc;
-  cudaError_t e;
+  FR_STEPPER_PROLOGUE("fr_rk4_step")
+  void *k = reg(0), *tmp = reg(1), *acc = reg(2);
   // k1; tmp = u + dt/2 k1; acc = u + dt/6 k1
   if ((rc = fr_rhs(c, u, k, work, stream)) != FR_OK) return rc;
-  e = rk_axpy2(f64, n, c->dc.ld, c->dc.Nel, u, k, dt / 2, tmp, dt / 6, acc, 0, s);
+  e = rk_axpy2(f64, rows, ld, nel, u, k, dt / 2, tmp, dt / 6, acc, 0, s);
   // k2; tmp = u + dt/2 k2; acc += dt/3 k2
   if (e == cudaSuccess && (rc = fr_rhs(c, tmp, k, work, stream)) != FR_OK) return rc;
-  if (e == cudaSuccess) e = rk_axpy2(f64, n, c->dc.ld, c->dc.Nel, u, k, dt / 2, tmp, dt / 3, acc, 1, s);
+  if (e == cudaSuccess) e = rk_axpy2(f64, rows, ld, nel, u, k, dt / 2, tmp, dt / 3, acc, 1, s);
   // k3; tmp = u + dt k3; acc += dt/3 k3
   if (e == cudaSuccess && (rc = fr_rhs(c, tmp, k, work, stream)) != FR_OK) return rc;
-  if (e == cudaSuccess) e = rk_axpy2(f64, n, c->dc.ld, c->dc.Nel, u, k, dt, tmp, dt / 3, acc, 1, s);
+  if (e == cudaSuccess) e = rk_axpy2(f64, rows, ld, nel, u, k, dt, tmp, dt / 3, acc, 1, s);
   // k4; u = acc + dt/6 k4
   if (e == cudaSuccess && (rc = fr_rhs(c, tmp, k, work, stream)) != FR_OK) return rc;
-  if (e == cudaSuccess) e = rk_axpy2(f64, n, c->dc.ld, c->dc.Nel, u, k, 0.0, u, dt / 6, acc, 2, s);
+  if (e == cudaSuccess) e = rk_axpy2(f64, rows, ld, nel, u, k, 0.0, u, dt / 6, acc, 2, s);
   if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("fr_rk4_step launch: ") + cudaGetErrorString(e));
+  return FR_OK;
+}
+
+int fr_euler_step(fr_ctx *c, void *u, double dt, void *work, void *stream) {
+  FR_STEPPER_PROLOGUE("fr_euler_step")
+  void *k = reg(0);
+  if ((rc = fr_rhs(c, u, k, work, stream)) != FR_OK) return rc;
+  const void *in[2] = {u, k};
+  const double a[2] = {1.0, dt};
+  e = rk_lincomb(f64, rows, ld, nel, 2, in, a, nullptr, u, nullptr, s);
+  if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("fr_euler_step launch: ") + cudaGetErrorString(e));
+  return FR_OK;
+}
+
+int fr_dopri5_step(fr_ctx *c, void *u, double dt, void *work, void *stream, double *err_dev) {
+  FR_STEPPER_PROLOGUE("fr_dopri5_step")
+  // Dormand-Prince 5(4), reading A24.  Row i+1 of A gives the state of stage i+1; row 7 = the fifth-order weights (FSAL).
+  static const double A[7][6] = {
+      {0, 0, 0, 0, 0, 0},
+      {1.0 / 5, 0, 0, 0, 0, 0},
+      {3.0 / 40, 9.0 / 40, 0, 0, 0, 0},
+      {44.0 / 45, -56.0 / 15, 32.0 / 9, 0, 0, 0},
+      {19372.0 / 6561, -25360.0 / 2187, 64448.0 / 6561, -212.0 / 729, 0, 0},
+      {9017.0 / 3168, -355.0 / 33, 46732.0 / 5247, 49.0 / 176, -5103.0 / 18656, 0},
+      {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84}};
+  static const double B4[7] = {5179.0 / 57600, 0, 7571.0 / 16695, 393.0 / 640, -92097.0 / 339200, 187.0 / 2100, 1.0 / 40};
+  void *tmp = reg(6);  // registers 0..5 hold k1..k6; k7 = R(u_new) overwrites k2, whose weights are zero in both rules
+  if ((rc = fr_rhs(c, u, reg(0), work, stream)) != FR_OK) return rc;
+  for (int i = 1; i < 6 && e == cudaSuccess; ++i) {
+    const void *in[7] = {u, reg(0), reg(1), reg(2), reg(3), reg(4), reg(5)};
+    double a[7] = {1.0, 0, 0, 0, 0, 0, 0};
+    for (int j = 0; j < i; ++j) a[1 + j] = dt * A[i][j];
+    e = rk_lincomb(f64, rows, ld, nel, 1 + i, in, a, nullptr, tmp, nullptr, s);
+    if (e == cudaSuccess && (rc = fr_rhs(c, tmp, reg(i), work, stream)) != FR_OK) return rc;
+  }
+  if (e == cudaSuccess) {  // u <- u + dt sum b5_i k_i ; tmp <- the fourth-order solution minus the same (without k7)
+    const void *in[7] = {u, reg(0), reg(1), reg(2), reg(3), reg(4), reg(5)};
+    double a[7] = {1.0, 0, 0, 0, 0, 0, 0}, b[7] = {0, 0, 0, 0, 0, 0, 0};
+    for (int j = 0; j < 6; ++j) { a[1 + j] = dt * A[6][j]; b[1 + j] = dt * (A[6][j] - B4[j]); }
+    e = rk_lincomb(f64, rows, ld, nel, 7, in, a, err_dev ? b : nullptr, u, err_dev ? tmp : nullptr, s);
+  }
+  if (err_dev && e == cudaSuccess) {
+    if ((rc = fr_rhs(c, u, reg(1), work, stream)) != FR_OK) return rc;  // k7
+    const void *in[2] = {tmp, reg(1)};
+    const double a[2] = {1.0, -dt * B4[6]};  // + dt (b5_7 - b4_7) k7, b5_7 = 0
+    e = rk_lincomb(f64, rows, ld, nel, 2, in, a, nullptr, tmp, nullptr, s);
+    // RMS of the error estimate: distance of tmp from zero = rms_diff(tmp, 0 * tmp); reuse k7's register as the zero operand
+    if (e == cudaSuccess) { const void *z[1] = {tmp}; const double za[1] = {0.0}; e = rk_lincomb(f64, rows, ld, nel, 1, z, za, nullptr, reg(1), nullptr, s); }
+    if (e == cudaSuccess) e = rk_rms_diff(f64, rows, ld, nel, tmp, reg(1), (double *)(wk + c->wl.partials), err_dev, s);
+  }
+  if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("fr_dopri5_step launch: ") + cudaGetErrorString(e));
   return FR_OK;
 }
 

@@ -148,8 +148,11 @@ int ipowi(int b, int e) { int r = 1; for (int i = 0; i < e; ++i) r *= b; return 
 
 }  // namespace
 
-void build_ref_ops(int etype, int p, int p_g, RefOps &o) {
+void build_ref_ops(int etype, int p, int p_g, int correction, RefOps &o) {
   if (p < 0 || p > 12) throw std::runtime_error("polynomial order p out of range [0,12]");
+  if (correction != FR_CORR_DG && correction != FR_CORR_SD && correction != FR_CORR_HU) throw std::runtime_error("unknown correction function");
+  if (correction != FR_CORR_DG && etype == FR_TRI) throw std::runtime_error("SD / HU correction functions are available on quadrilaterals and hexahedra only");
+  if (correction == FR_CORR_HU && p < 1) throw std::runtime_error("the HU correction function needs p >= 1");
   if (p_g < 1 || p_g > 8) throw std::runtime_error("geometry degree p_g out of range [1,8]");
   o = RefOps();
   o.etype = etype; o.p = p; o.n = p + 1; o.p_g = p_g;
@@ -169,11 +172,24 @@ void build_ref_ops(int etype, int p, int p_g, RefOps &o) {
     for (int i = 0; i < n; ++i) { lagrange1d(g, g[i], L, dL); for (int j = 0; j < n; ++j) D[i * n + j] = dL[j]; }
     lagrange1d(g, -1, lm, dL);
     lagrange1d(g, 1, lp, dL);
-    for (int i = 0; i < n; ++i) {  // g_R' = (P_p' + P_{p+1}')/2; the -1 face uses g_R'(-xi) (outward-normal convention)
-      real a, da, b, db;
-      legendre(p, g[i], a, da); legendre(p + 1, g[i], b, db); gp[i] = (da + db) / 2;
-      legendre(p, -g[i], a, da); legendre(p + 1, -g[i], b, db); gm[i] = (da + db) / 2;
+    // One-parameter family of energy-stable correction functions of the paper's ref [10] ("DG, SD, and HU as
+    // defined in [10]"; reading A23):  g_R = {P_p + (eta P_{p-1} + P_{p+1}) / (1 + eta)} / 2,  eta = c (2p+1) (a_p p!)^2 / 2,
+    // a_p = (2p)! / (2^p (p!)^2);  c = 0 (DG: g_R = Radau, A5),  c_SD = 2p / ((2p+1)(p+1)(a_p p!)^2),
+    // c_HU = 2(p+1) / ((2p+1) p (a_p p!)^2).  The -1 face uses g_R'(-xi) (outward-normal convention).
+    real eta = 0;
+    if (correction != FR_CORR_DG) {
+      const real ap = fact(2 * p) / (ipow(2, p) * fact(p) * fact(p));
+      const real apf2 = (ap * fact(p)) * (ap * fact(p));
+      const real c = correction == FR_CORR_SD ? (real)(2 * p) / ((2 * p + 1) * (p + 1) * apf2) : (real)(2 * (p + 1)) / ((2 * p + 1) * p * apf2);
+      eta = c * (2 * p + 1) * apf2 / 2;
     }
+    auto dgr = [&](real x) {
+      real a, da, b, db, m = 0, dm = 0;
+      legendre(p, x, a, da); legendre(p + 1, x, b, db);
+      if (p >= 1) legendre(p - 1, x, m, dm);
+      return (da + (eta * dm + db) / (1 + eta)) / 2;
+    };
+    for (int i = 0; i < n; ++i) { gp[i] = dgr(g[i]); gm[i] = dgr(-g[i]); }
     std::vector<real> Dh(n * n);
     for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) Dh[i * n + j] = D[i * n + j] + gm[i] * lm[j] - gp[i] * lp[j];  // M2 carries the reference normal: -1 on the -1 face
     o.D1 = round_to_double(D); o.lm = round_to_double(lm); o.lp = round_to_double(lp);

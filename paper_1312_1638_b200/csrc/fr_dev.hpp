@@ -62,8 +62,9 @@ __host__ __device__ inline size_t fp_rstride(bool blk, int64_t ld) { return blk 
 // Workspace layout (doubles unless noted); offsets in bytes from work_dev
 struct WorkLayout {
   int64_t uf, cf, qu, qf;          // generic path: U^f (-> D~), C^f, Q~ -> Q -> F~, Q^f
-  int64_t rk_k, rk_tmp, rk_acc;    // RK4 registers in the storage precision
-  int64_t total;
+  int64_t partials;                // RK_MAX_PARTIALS doubles (error norm of fr_dopri5_step)
+  int64_t reg0, reg_stride;        // stepper registers in the storage precision: reg0 + i * reg_stride, i < 7
+  int64_t total;                   // through register 2 (fr_rk4_step)
 };
 
 // Optional per-kernel timing: an event is recorded before every kernel and after the last one.

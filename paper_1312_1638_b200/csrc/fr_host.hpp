@@ -29,7 +29,7 @@ struct RefOps {
   std::vector<long double> Gu, dGu, Gf, dGf;  // [Nu][Nn], [nd][Nu][Nn], [Nf][Nn], [nd][Nf][Nn]
 };
 
-void build_ref_ops(int etype, int p, int p_g, RefOps &out);  // fr_basis.cpp
+void build_ref_ops(int etype, int p, int p_g, int correction, RefOps &out);  // fr_basis.cpp
 
 // Per-mesh geometric constants and the interface lookup tables, host copies.
 struct MeshConsts {

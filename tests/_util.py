@@ -34,7 +34,7 @@ class GpuRunner:
         shape = (ctx.Nu, ctx.NV, ctx.ld)
         self.u = torch.zeros(shape, dtype=self.tdtype, device="cuda")
         self.r = torch.zeros(shape, dtype=self.tdtype, device="cuda")
-        self.work = torch.zeros(max(ctx.workspace_bytes, 256), dtype=torch.uint8, device="cuda")
+        self.work = torch.zeros(max(ctx.stepper_workspace_bytes("dopri5"), 256), dtype=torch.uint8, device="cuda")
         self.stream = torch.cuda.current_stream().cuda_stream
 
     def set_state(self, U):
@@ -48,9 +48,18 @@ class GpuRunner:
         self.torch.cuda.synchronize()
         return self.ctx.unpad(self.r.cpu().numpy())
 
-    def rk4(self, U, dt, steps):
+    def rk4(self, U, dt, steps, stepper="rk4"):
         self.set_state(U)
+        step = {"rk4": self.ctx.rk4_step, "euler": self.ctx.euler_step, "dopri5": self.ctx.dopri5_step}[stepper]
         for _ in range(steps):
-            self.ctx.rk4_step(self.u.data_ptr(), dt, self.work.data_ptr(), self.stream)
+            step(self.u.data_ptr(), dt, self.work.data_ptr(), self.stream)
         self.torch.cuda.synchronize()
         return self.ctx.unpad(self.u.cpu().numpy())
+
+    def dopri5(self, U, dt):
+        """one DOPRI5 step -> (new state, RMS of the embedded error estimate)"""
+        self.set_state(U)
+        err = self.torch.zeros(1, dtype=self.torch.float64, device="cuda")
+        self.ctx.dopri5_step(self.u.data_ptr(), dt, self.work.data_ptr(), self.stream, err.data_ptr())
+        self.torch.cuda.synchronize()
+        return self.ctx.unpad(self.u.cpu().numpy()), float(err.item())

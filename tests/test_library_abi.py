@@ -36,12 +36,18 @@ def test_build_targets_sm_100a():
     assert "arch=compute_100a,code=sm_100a" in src
 
 
-CASES = [("C1", {}), ("C2", dict(n=3)), ("C3", dict(n=3, p=4)), ("C3", dict(n=2, p=2)), ("C4", dict(n=6)), ("C5", dict(n=2, p=6))]
+CASES = [("C1", {}), ("C2", dict(n=3)), ("C3", dict(n=3, p=4)), ("C3", dict(n=2, p=2)), ("C4", dict(n=6)), ("C5", dict(n=2, p=6)),
+         ("C1", dict(correction="sd")), ("C1", dict(correction="hu")), ("C2", dict(n=2, correction="hu")), ("C5", dict(n=2, p=5, correction="sd"))]
 
 
 @pytest.mark.parametrize("name,over", CASES)
 def test_host_tables_match_oracle(fr, name, over):
+    """M0..M6 (DG, SD and HU correction functions: the library builds the family of the paper's ref [10] from its parameter c,
+    the oracle from the closed forms), metrics, coordinates and the pair set."""
+    over = dict(over)
+    corr = over.pop("correction", "dg")
     mesh, disc = W.config(name, **over)
+    disc = dict(disc, correction=corr)
     ctx = fr.Context(mesh).setup_operators(flags=fr.FLAG_HOST_ONLY, **disc)
     o = FROracle(mesh, disc)
     ops = o.ops
