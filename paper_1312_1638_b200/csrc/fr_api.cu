@@ -127,7 +127,11 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     dc.Nel = mc.Nel; dc.ld = ld; dc.npairs = mc.npairs; dc.nbnd = mc.nbnd;
     dc.ns = d->system == FR_NAVIER_STOKES; dc.f64 = d->precision == FR_F64;
     dc.staged = (d->flags & FR_FLAG_FORCE_GENERIC) != 0;
-    dc.ph = Phys{d->gamma, d->mu, d->Pr, d->ldg_beta, d->ldg_tau};
+    // the reference state (perturbation form, fr_physics.cuh) serves the fused kernel families; the staged sequence and the
+    // line kernels of high-order quadrilaterals evaluate the plain formulas
+    const bool fused = !dc.staged && (o.etype == FR_HEX ? blk : (o.n >= 2 && o.n <= (o.etype == FR_TRI ? 6 : 5)));
+    const double zero3[3] = {0, 0, 0};
+    dc.ph = make_phys(d->gamma, d->mu, d->Pr, d->ldg_beta, d->ldg_tau, fused ? d->rho_ref : 0.0, fused ? d->v_ref : zero3, fused ? d->p_ref : 0.0);
     dc.dev = -1;
     if (c->host_only) { c->use_tensor = false; c->wl = WorkLayout(); c->ready = true; return FR_OK; }
     cudaError_t e = cudaGetDevice(&dc.dev);

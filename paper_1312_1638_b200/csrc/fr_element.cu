@@ -77,6 +77,17 @@ __global__ void __launch_bounds__(TPB) k_el_interp(const __grid_constant__ OpsIn
   double uu[NU];
 #pragma unroll
   for (int r = 0; r < NU; ++r) uu[r] = (double)u[((size_t)r * NV + a) * ld + e];
+  // perturbation variables (fr_physics.cuh) BEFORE the interpolation, so that its rounding error scales with the deviation
+  // from the reference state: w_rho = rho - rho0, w_mj = m_j - v0_j rho, w_E = (E - E0) - h0 (rho - rho0)
+  if (c.ph.rho0 != 0.0) {
+    const double ka = a == 0 ? 0.0 : (a == NV - 1 ? c.ph.h0 : c.ph.v0[a - 1]);
+    const double da = a == 0 ? c.ph.rho0 : (a == NV - 1 ? c.ph.E0 : 0.0);
+#pragma unroll
+    for (int r = 0; r < NU; ++r) {
+      const double rho = a == 0 ? uu[r] : (double)u[((size_t)r * NV) * ld + e];
+      uu[r] = a == NV - 1 ? fma(-ka, rho - c.ph.rho0, uu[r] - da) : fma(-ka, rho, uu[r] - da);
+    }
+  }
 #pragma unroll
   for (int s = 0; s < NF; ++s) {
     double acc = 0;
@@ -155,6 +166,7 @@ __global__ void __launch_bounds__(TPB) k_el_gradface(const __grid_constant__ Ops
     double us[NV], qf[ND][NV], nrm[ND], G[NV];
 #pragma unroll
     for (int b = 0; b < NV; ++b) us[b] = uf[((size_t)s * NV + b) * ld + e2];
+    from_pert<ND>(c.ph, us, us);
 #pragma unroll
     for (int n = 0; n < ND; ++n) {
       nrm[n] = c.fp_n[((size_t)n * NF + s) * ld + e2];
@@ -184,10 +196,11 @@ __global__ void __launch_bounds__(TPB) k_el_fluxdiv(const __grid_constant__ OpsD
     const int el2 = t % EB, r = t / EB;
     const int64_t e2 = e0 + el2;
     if (e2 >= c.Nel) continue;
-    double uu[NV], qq[ND][NV], f[ND][NV], v[ND], p;
+    double uu[NV], ww[NV], qq[ND][NV], f[ND][NV], v[ND], p;
 #pragma unroll
     for (int b = 0; b < NV; ++b) uu[b] = (double)u[((size_t)r * NV + b) * ld + e2];
-    inviscid_flux<ND>(uu, c.ph.gamma, f, v, p);
+    to_pert<ND>(c.ph, uu, ww);
+    inviscid_flux<ND>(ww, c.ph, f, v, p);
     if (NS) {
 #pragma unroll
       for (int n = 0; n < ND; ++n)
@@ -204,26 +217,43 @@ __global__ void __launch_bounds__(TPB) k_el_fluxdiv(const __grid_constant__ OpsD
     }
   }
   __syncthreads();
-  if (e >= c.Nel) return;
+  const bool act = e < c.Nel;
+  const int64_t ec = act ? e : c.Nel - 1;  // inactive lanes of the last CTA repeat a valid element (they take part in the barriers)
   double dd[NF];
 #pragma unroll
-  for (int s = 0; s < NF; ++s) dd[s] = dt[((size_t)s * NV + a) * ld + e];
+  for (int s = 0; s < NF; ++s) dd[s] = dt[((size_t)s * NV + a) * ld + ec];
   double fa[ND][NU];  // F~ of this variable at all points of the element
 #pragma unroll
   for (int d = 0; d < ND; ++d)
 #pragma unroll
     for (int v = 0; v < NU; ++v) fa[d][v] = sF[((d * NV + a) * NU + v) * EB + el];
+  double acc[NU];
 #pragma unroll
   for (int r = 0; r < NU; ++r) {
-    double acc = 0;
+    double t = 0;
 #pragma unroll
     for (int d = 0; d < ND; ++d)
 #pragma unroll
-      for (int v = 0; v < NU; ++v) acc = fma(op.M132[r * ND * NU + d * NU + v], fa[d][v], acc);
+      for (int v = 0; v < NU; ++v) t = fma(op.M132[r * ND * NU + d * NU + v], fa[d][v], t);
 #pragma unroll
-    for (int s = 0; s < NF; ++s) acc = fma(op.M3[r * NF + s], dd[s], acc);
-    rhs[((size_t)r * NV + a) * ld + e] = (T)(-acc * c.rcpj[(size_t)(c.affine ? 0 : r) * ld + e]);
+    for (int s = 0; s < NF; ++s) t = fma(op.M3[r * NF + s], dd[s], t);
+    acc[r] = t;
   }
+  if (c.ph.rho0 != 0.0) {
+    // back to conserved variables: R_mj = R_wmj + v0_j R_wrho, R_E = R_wE + h0 R_wrho (the mass row through shared memory)
+    __syncthreads();  // every thread has taken its F~ out of sF
+    if (a == 0) {
+#pragma unroll
+      for (int r = 0; r < NU; ++r) sF[r * EB + el] = acc[r];
+    }
+    __syncthreads();
+    const double ka = a == 0 ? 0.0 : (a == NV - 1 ? c.ph.h0 : c.ph.v0[a - 1]);
+#pragma unroll
+    for (int r = 0; r < NU; ++r) acc[r] = fma(ka, sF[r * EB + el], acc[r]);
+  }
+  if (!act) return;
+#pragma unroll
+  for (int r = 0; r < NU; ++r) rhs[((size_t)r * NV + a) * ld + e] = (T)(-acc[r] * c.rcpj[(size_t)(c.affine ? 0 : r) * ld + e]);
 }
 
 template <int NU, int NF, typename T>
@@ -273,11 +303,11 @@ cudaError_t interp_t(const DevConsts &c, const void *u, double *uf, cudaStream_t
 
 }  // namespace
 
-// triangles p = 1 .. 4 (N_u = (p+1)(p+2)/2, N_f = 3 (p+1)) and quadrilaterals p = 1 .. 4 (N_u = (p+1)^2, N_f = 4 (p+1)): at these
+// triangles p = 1 .. 5 (N_u = (p+1)(p+2)/2, N_f = 3 (p+1)) and quadrilaterals p = 1 .. 4 (N_u = (p+1)^2, N_f = 4 (p+1)): at these
 // sizes the dense operators cost less than the extra launches and HBM round trips of the staged / sum-factorised sequences
 bool element_fused_supported(const DevConsts &c) {
   if (c.staged) return false;
-  if (c.etype == FR_TRI) return c.n >= 2 && c.n <= 5;
+  if (c.etype == FR_TRI) return c.n >= 2 && c.n <= 6;
   if (c.etype == FR_QUAD) return c.n >= 2 && c.n <= 5;
   return false;
 }
@@ -289,6 +319,7 @@ bool element_fused_supported(const DevConsts &c) {
       case 3: return CALL(6, 9);               \
       case 4: return CALL(10, 12);             \
       case 5: return CALL(15, 15);             \
+      case 6: return CALL(21, 18);             \
       default: return cudaErrorNotSupported;   \
     }                                          \
   }                                            \

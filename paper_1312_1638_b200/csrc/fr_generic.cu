@@ -1,7 +1,8 @@
 // Generic FR right-hand side: the paper's staged kernel sequence (App A) with dense
-// operator matrices, for any element type.  This is the path triangles and quadrilaterals run and the
-// fallback for hexahedra (FR_FLAG_FORCE_GENERIC); the tensor-product kernels in fr_tensor.cu replace it
-// for hexahedra.  All arithmetic in double; u / rhs are stored in T (float or double).
+// operator matrices, for any element type (FR_FLAG_FORCE_GENERIC; triangles with p = 0 or p > 4; hexahedra with p = 0 or
+// p > 6), and the interface (flux-point pair) kernels every path shares.  Triangles and quadrilaterals with 1 <= p <= 4 run
+// the fused kernels of fr_element.cu, quadrilaterals of other orders the line kernels of fr_tensor.cu, hexahedra with
+// 1 <= p <= 6 the TMA kernels.  All arithmetic in double; u / rhs are stored in T (float or double).
 #include "fr_dev.hpp"
 #include "fr_element.hpp"
 #include "fr_hex_tma.hpp"
@@ -10,9 +11,7 @@ namespace fr {
 namespace {
 
 constexpr int RT = 8;  // rows of the operator per thread
-#ifndef FLUXG_MINB
-#define FLUXG_MINB 6  // resident CTAs of the gather-bound interface kernel: occupancy is what hides its latency
-#endif
+constexpr int FLUXG_MINB = 6;  // resident CTAs of the gather-bound interface kernels: occupancy is what hides their latency
 
 // out[blk][r][col] = sum_k A[r][k] in1[blk][k][col] (+ sum_k B[r][k] in2[k][col]),  col = a*ld + e.
 // SCALE: multiply by -rcpj[r][e] (Eq 19 :243, the paper's negdivconf kernel).
@@ -57,7 +56,8 @@ __global__ void __launch_bounds__(128) k_apply(int M, int K1, const double *__re
     }
 }
 
-// Common solution, Eq 7 + Eq 25 (:192, :506): each pair visited once, same value to both sides.
+// Common solution, Eq 7 + Eq 25 (:192, :506): each pair visited once, same value to both sides.  The flux-point states
+// arrive in perturbation variables w (fr_physics.cuh); the output is in CONSERVED variables (it feeds the gradient of u).
 template <int ND, bool JUMP>
 __global__ void k_common_sol(DevConsts c, const double *__restrict__ uf, double *__restrict__ cf) {
   constexpr int NV = ND + 2;
@@ -66,13 +66,18 @@ __global__ void k_common_sol(DevConsts c, const double *__restrict__ uf, double 
   const size_t oL = fp_row(c.blk, c.ld, c.Nf * NV, c.pLs[i] * NV, c.pLe[i]), oR = fp_row(c.blk, c.ld, c.Nf * NV, c.pRs[i] * NV, c.pRe[i]);
   const size_t vs = fp_rstride(c.blk, c.ld);  // distance between the variables of one flux point
   const double wl = 0.5 - c.ph.beta, wr = 0.5 + c.ph.beta;
+  double oa[NV], ob[NV];
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
     const double ul = uf[oL + (size_t)a * vs], ur = uf[oR + (size_t)a * vs];
     const double v = wl * ul + wr * ur;
-    cf[oL + (size_t)a * vs] = JUMP ? v - ul : v;   // JUMP: the {C - u^f} of Eq 9 directly
-    cf[oR + (size_t)a * vs] = JUMP ? v - ur : v;
+    oa[a] = JUMP ? v - ul : v;   // JUMP: the {C - u^f} of Eq 9 directly
+    ob[a] = JUMP ? v - ur : v;
   }
+  if (JUMP) { from_pert_delta<ND>(c.ph, oa); from_pert_delta<ND>(c.ph, ob); }
+  else { from_pert<ND>(c.ph, oa, oa); from_pert<ND>(c.ph, ob, ob); }
+#pragma unroll
+  for (int a = 0; a < NV; ++a) { cf[oL + (size_t)a * vs] = oa[a]; cf[oR + (size_t)a * vs] = ob[a]; }
 }
 
 // Boundary common solution C(u_L, B_ldg u_L)  (:797)
@@ -86,6 +91,7 @@ __global__ void k_common_sol_bnd(DevConsts c, const double *__restrict__ uf, dou
   double u[NV], gi[NV], gl[NV];
 #pragma unroll
   for (int a = 0; a < NV; ++a) u[a] = uf[o + (size_t)a * vs];
+  from_pert<ND>(c.ph, u, u);
   ghost_states<ND>(c.bcs[c.bbc[i]], u, c.ph.gamma, gi, gl);
 #pragma unroll
   for (int a = 0; a < NV; ++a) cf[o + (size_t)a * vs] = (0.5 - c.ph.beta) * u[a] + (0.5 + c.ph.beta) * gl[a] - (JUMP ? u[a] : 0.0);
@@ -131,7 +137,7 @@ __global__ void k_tflux(DevConsts c, const T *__restrict__ u, double *__restrict
   double uu[NV], f[ND][NV], v[ND], p;
 #pragma unroll
   for (int a = 0; a < NV; ++a) uu[a] = (double)u[((size_t)r * NV + a) * c.ld + e];
-  inviscid_flux<ND>(uu, c.ph.gamma, f, v, p);
+  inviscid_flux<ND>(uu, c.ph, f, v, p);  // staged path: no reference state (w = u)
   if (NS) {
     double q[ND][NV];
 #pragma unroll
@@ -193,7 +199,11 @@ __global__ void k_common_flux_bnd(DevConsts c, double *__restrict__ uf, const do
   double uL[NV], gi[NV], gl[NV], qL[ND][NV], qR[ND][NV], nrm[ND], F[NV];
 #pragma unroll
   for (int a = 0; a < NV; ++a) uL[a] = uf[o + (size_t)a * vs];
-  const double keep = ghost_states<ND>(c.bcs[c.bbc[i]], uL, c.ph.gamma, gi, gl);
+  double uc[NV];
+  from_pert<ND>(c.ph, uL, uc);
+  const double keep = ghost_states<ND>(c.bcs[c.bbc[i]], uc, c.ph.gamma, gi, gl);
+  to_pert<ND>(c.ph, gi, gi);
+  to_pert<ND>(c.ph, gl, gl);
   if (NS) {
 #pragma unroll
     for (int n = 0; n < ND; ++n)
@@ -226,7 +236,7 @@ __global__ void __launch_bounds__(128, FLUXG_MINB) k_common_flux_g(DevConsts c, 
   for (int a = 0; a < NV; ++a) { gL[a] = wl != 0.0 ? gf[oL + (size_t)a * vs] : 0.0; gR[a] = wr != 0.0 ? gf[oR + (size_t)a * vs] : 0.0; }
 #pragma unroll
   for (int n = 0; n < ND; ++n) nrm[n] = c.pn[(size_t)n * c.npairs + i];
-  rusanov<ND>(uL, uR, nrm, c.ph.gamma, F);
+  rusanov<ND>(uL, uR, nrm, c.ph, F);
   const double jl = c.pJnL[i], jr = c.pJnR[i];
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
@@ -247,10 +257,14 @@ __global__ void k_common_flux_bnd_g(DevConsts c, double *__restrict__ uf, const 
   double uL[NV], gi[NV], gl[NV], nrm[ND], F[NV];
 #pragma unroll
   for (int a = 0; a < NV; ++a) uL[a] = uf[o + (size_t)a * vs];
-  ghost_states<ND>(c.bcs[c.bbc[i]], uL, c.ph.gamma, gi, gl);
+  double uc[NV];
+  from_pert<ND>(c.ph, uL, uc);
+  ghost_states<ND>(c.bcs[c.bbc[i]], uc, c.ph.gamma, gi, gl);
+  to_pert<ND>(c.ph, gi, gi);
+  to_pert<ND>(c.ph, gl, gl);
 #pragma unroll
   for (int n = 0; n < ND; ++n) nrm[n] = c.bn[(size_t)n * c.nbnd + i];
-  rusanov<ND>(uL, gi, nrm, c.ph.gamma, F);
+  rusanov<ND>(uL, gi, nrm, c.ph, F);
   const double jn = c.bJn[i];
 #pragma unroll
   for (int a = 0; a < NV; ++a) uf[o + (size_t)a * vs] = jn * (F[a] + c.ph.tau * (uL[a] - gl[a]) - gf[o + (size_t)a * vs]);

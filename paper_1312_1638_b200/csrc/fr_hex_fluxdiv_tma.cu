@@ -97,12 +97,19 @@ __global__ void __launch_bounds__(N *N *E, MINB)
         for (int b = 0; b < 3; ++b) S[a][b] = stS[((a * 3 + b) * NFP + ij) * E + el];
 #pragma unroll
       for (int a = 0; a < NV; ++a) uu[a] = (double)stU[(ij * NV + a) * E + el];
-      // primitive variables (Eq 20-21)
+      // primitive variables (Eq 20-21) through the perturbation variables w about the reference state (fr_physics.cuh):
+      // v = v0 + w_m / rho,  pp = p - p0;  with no reference state w = u and pp = p
       const double rrho = 1.0 / uu[0], En = uu[4];
-      double v[3], ke = 0;
+      double ww[NV], v[3], ke = 0, vw = 0;
+      to_pert<3>(ph, uu, ww);
 #pragma unroll
-      for (int d = 0; d < 3; ++d) { v[d] = uu[1 + d] * rrho; ke += uu[1 + d] * v[d]; }
-      const double p = (ph.gamma - 1.0) * (En - 0.5 * ke);
+      for (int d = 0; d < 3; ++d) {
+        const double dv = ww[1 + d] * rrho;
+        v[d] = ph.v0[d] + dv;
+        ke += ww[1 + d] * dv;
+        vw += ph.v0[d] * ww[1 + d];
+      }
+      const double pp = (ph.gamma - 1.0) * (fma(ph.hs0, ww[0], ww[4]) - vw - 0.5 * ke);
       // viscous stress Tm and energy flux w = v.Tm + (mu gamma / Pr) grad e  (Eq 22-24, A8), built variable by variable
       double Tm[3][3], w[3];
       if (NS) {
@@ -131,15 +138,15 @@ __global__ void __launch_bounds__(N *N *E, MINB)
         }
       }
       if (NB == 1 && k > 0) __syncthreads();  // the previous slice's contraction has finished reading sF
-      // F~_i = sum_n S[i][n] (f_inv - f_vis)_n  (Eq 12), one variable at a time
+      // F~_i = sum_n S[i][n] (g_inv - f_vis)_n  (Eq 12; g = the inviscid flux in perturbation form), one variable at a time
 #pragma unroll
       for (int a = 0; a < NV; ++a) {
         double f[3];
 #pragma unroll
         for (int n = 0; n < 3; ++n) {
-          if (a == 0) f[n] = uu[1 + n];
-          else if (a < 4) { f[n] = uu[1 + n] * v[a - 1] + (a - 1 == n ? p : 0.0); if (NS) f[n] -= Tm[n][a - 1]; }
-          else { f[n] = v[n] * (En + p); if (NS) f[n] -= w[n]; }
+          if (a == 0) f[n] = fma(ph.v0[n], ww[0], ww[1 + n]);
+          else if (a < 4) { f[n] = v[n] * ww[a] + (a - 1 == n ? pp : 0.0); if (NS) f[n] -= Tm[n][a - 1]; }
+          else { f[n] = v[n] * (ww[4] + pp); if (NS) f[n] -= w[n]; }
         }
         buf[((0 * NV + a) * NFP + ij) * E + el] = fma(S[0][0], f[0], fma(S[0][1], f[1], S[0][2] * f[2]));
         buf[((1 * NV + a) * NFP + ij) * E + el] = fma(S[1][0], f[0], fma(S[1][1], f[1], S[1][2] * f[2]));
@@ -191,6 +198,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       const int r = ij + NFP * k;
       const double rj = sRJ[r * E + el];
       const int fx = j + N * k, fy = i + N * k;
+      double r0 = 0;  // R~ of the mass equation: R_mj = R_wmj + v0_j R_wrho, R_E = R_wE + h0 R_wrho (fr_physics.cuh)
 #pragma unroll
       for (int a = 0; a < NV; ++a) {
         double v = acc[k][a];
@@ -200,6 +208,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
         v = fma(gpi, sDxy[((1 * NFP + fx) * NV + a) * E + el], v);
         v = fma(gmj, sDxy[((2 * NFP + fy) * NV + a) * E + el], v);
         v = fma(gpj, sDxy[((3 * NFP + fy) * NV + a) * E + el], v);
+        if (a == 0) r0 = v;
+        else v = fma(a < 4 ? ph.v0[a - 1] : ph.h0, r0, v);
         rhs[((size_t)r * NV + a) * ld + e] = (T)(-v * rj);
       }
     }
@@ -217,6 +227,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     const int r = ij + NFP * k;
     const double rj = aff ? rcpj[fp_row(true, ld, 1, 0, e)] : rcpj[fp_row(true, ld, N * NFP, r, e)];
     const int fx = j + N * k, fy = i + N * k;
+    double r0 = 0;
 #pragma unroll
     for (int a = 0; a < NV; ++a) {
       double v = acc[k][a];
@@ -226,6 +237,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       v = fma(gpi, dt[fp_row(true, ld, 6 * NFP * NV, (1 * NFP + fx) * NV + a, e)], v);
       v = fma(gmj, dt[fp_row(true, ld, 6 * NFP * NV, (2 * NFP + fy) * NV + a, e)], v);
       v = fma(gpj, dt[fp_row(true, ld, 6 * NFP * NV, (3 * NFP + fy) * NV + a, e)], v);
+      if (a == 0) r0 = v;
+      else v = fma(a < 4 ? ph.v0[a - 1] : ph.h0, r0, v);
       rhs[((size_t)r * NV + a) * ld + e] = (T)(-v * rj);
     }
   }

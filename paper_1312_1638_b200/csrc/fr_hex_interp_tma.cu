@@ -1,4 +1,5 @@
 // k_hex_interp_tma: U^f = M0 U on hexahedra (Eq 6 :186 / Eq 41 :745), part (1) of the right-hand side, as a TMA-fed
+// (stored in the perturbation variables w = T (u - u_ref) of fr_physics.cuh; with no reference state w = u)
 // z-slab kernel.  A CTA owns E consecutive elements; their whole U block ([N_u*N_V] rows of E values, caller layout)
 // arrives by ONE 3-D TMA box load; thread (e, i, j) interpolates its column to the two z faces from shared memory,
 // and the 4 N x/y-face flux points of every slice are interpolated along their lines by one thread each.  U^f is
@@ -10,8 +11,8 @@ namespace fr {
 namespace {
 
 template <int N, int E, typename T>
-__global__ void __launch_bounds__(N *N *E) k_hex_interp_tma(const __grid_constant__ CUtensorMap tmU, Ops1D<N> op, double *__restrict__ uf,
-                                                            int64_t ld, int64_t Nel) {
+__global__ void __launch_bounds__(N *N *E) k_hex_interp_tma(const __grid_constant__ CUtensorMap tmU, Ops1D<N> op, Phys ph,
+                                                            double *__restrict__ uf, int64_t ld, int64_t Nel) {
   constexpr int NFP = N * N, NU = N * NFP, NF = 6 * NFP;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char *sm = smem_raw + ((128u - (smem_addr(smem_raw) & 127u)) & 127u);
@@ -40,13 +41,17 @@ __global__ void __launch_bounds__(N *N *E) k_hex_interp_tma(const __grid_constan
 #pragma unroll
     for (int a = 0; a < NV; ++a) zm[a] = zp[a] = 0.0;
 #pragma unroll
-    for (int m = 0; m < N; ++m)
+    for (int m = 0; m < N; ++m) {
+      double w[NV];
+#pragma unroll
+      for (int a = 0; a < NV; ++a) w[a] = (double)sU[((size_t)(NFP * m + ij) * NV + a) * E + el];
+      to_pert<3>(ph, w, w);  // perturbation variables before the interpolation (fr_physics.cuh)
 #pragma unroll
       for (int a = 0; a < NV; ++a) {
-        const double v = (double)sU[((size_t)(NFP * m + ij) * NV + a) * E + el];
-        zm[a] = fma(op.lm[m], v, zm[a]);
-        zp[a] = fma(op.lp[m], v, zp[a]);
+        zm[a] = fma(op.lm[m], w[a], zm[a]);
+        zp[a] = fma(op.lp[m], w[a], zp[a]);
       }
+    }
 #pragma unroll
     for (int a = 0; a < NV; ++a) {
       uf[fp_row(true, ld, NF * NV, (4 * NFP + ij) * NV + a, e)] = zm[a];
@@ -64,8 +69,12 @@ __global__ void __launch_bounds__(N *N *E) k_hex_interp_tma(const __grid_constan
 #pragma unroll
     for (int mm = 0; mm < N; ++mm) {
       const double l = lc[mm];
+      double w[NV];
 #pragma unroll
-      for (int a = 0; a < NV; ++a) v[a] = fma(l, (double)sU[((size_t)(base + mm * stride) * NV + a) * E + el], v[a]);
+      for (int a = 0; a < NV; ++a) w[a] = (double)sU[((size_t)(base + mm * stride) * NV + a) * E + el];
+      to_pert<3>(ph, w, w);
+#pragma unroll
+      for (int a = 0; a < NV; ++a) v[a] = fma(l, w[a], v[a]);
     }
     const int fp = f * NFP + m + N * k;
 #pragma unroll
@@ -85,7 +94,7 @@ cudaError_t launch_interp(const DevConsts &c, const double *h_ops, const void *u
   static DevFlags done;
   cudaError_t err = set_smem(kern, SMEM, done, c.dev);
   if (err != cudaSuccess) return err;
-  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, SMEM, s>>>(mU, make_ops<N>(h_ops), uf, c.ld, c.Nel);
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, SMEM, s>>>(mU, make_ops<N>(h_ops), c.ph, uf, c.ld, c.Nel);
   return cudaGetLastError();
 }
 

@@ -8,30 +8,90 @@
 
 namespace fr {
 
+// Gas constants, LDG parameters and the optional constant reference state (fr.h: fr_disc_desc rho_ref, v_ref, p_ref).
+//
+// Perturbation form.  With a reference state (rho0, v0, p0), E0 = p0/(gamma-1) + rho0 |v0|^2 / 2,
+// h0 = (E0 + p0)/rho0, the fused kernels carry the flux-point states and evaluate the inviscid fluxes in the variables
+//     w_rho = rho - rho0,   w_mj = m_j - v0_j rho,   w_E = (E - E0) - h0 (rho - rho0)          (w = T (u - u_ref), T constant)
+// whose equations are  d_t w + div g = 0  with  g = T f - const:
+//     g_rho,n = w_mn + v0_n w_rho,   g_mj,n = v_n w_mj + p' delta_nj,   g_E,n = v_n (w_E + p'),
+//     p' = p - p0 = (gamma-1) {w_E + hs0 w_rho - v0 . w_m - |w_m|^2 / (2 rho)},   hs0 = h0 - |v0|^2/2,   v = v0 + w_m / rho.
+// T is linear and constant, so interpolation, jumps, Rusanov dissipation s/2 (w_L - w_R), lifting and divergence commute
+// with it; the subtracted constant flux has zero discrete divergence (Eq 18: M1 const = 0, common flux of equal states =
+// the flux itself).  The right-hand side returns to conserved variables by R_mj = R_wmj + v0_j R_wrho, R_E = R_wE + h0 R_wrho.
+// Every O(p0), O(E0) term is gone from the arithmetic: rounding errors scale with the deviation from the reference state.
+// The viscous flux is unchanged (f_vis,rho = 0, so T f_vis = f_vis) and is evaluated from conserved variables.
+// All-zero reference: w = u, g = f, p' = p -- the plain formulas of Eq 20-21.
 struct Phys {
   double gamma, mu, Pr, beta, tau;
+  double rho0, v0[3], p0, E0, h0, hs0;
 };
+
+inline Phys make_phys(double gamma, double mu, double Pr, double beta, double tau, double rho0, const double *v0, double p0) {
+  Phys ph{};
+  ph.gamma = gamma; ph.mu = mu; ph.Pr = Pr; ph.beta = beta; ph.tau = tau;
+  if (rho0 > 0.0 && p0 > 0.0) {
+    double ke = 0;
+    for (int d = 0; d < 3; ++d) { ph.v0[d] = v0[d]; ke += v0[d] * v0[d]; }
+    ph.rho0 = rho0; ph.p0 = p0;
+    ph.E0 = p0 / (gamma - 1.0) + 0.5 * rho0 * ke;
+    ph.h0 = (ph.E0 + p0) / rho0;
+    ph.hs0 = ph.h0 - 0.5 * ke;
+  }
+  return ph;
+}
 
 struct BcDev {
   int kind;
   double rho, v[3], p, cpTw;
 };
 
-// f_inv[n][a] of Eq 20 for state u[NV]; also returns pressure and velocities
+// conserved u -> perturbation variables w (may alias)
 template <int ND>
-__device__ __forceinline__ void inviscid_flux(const double *u, double gamma, double (*f)[ND + 2], double *v, double &p) {
-  const double rrho = 1.0 / u[0];
-  double ke = 0;
+__device__ __forceinline__ void to_pert(const Phys &ph, const double *u, double *w) {
+  const double rho = u[0], dr = rho - ph.rho0;
+  w[ND + 1] = fma(-ph.h0, dr, u[ND + 1] - ph.E0);
 #pragma unroll
-  for (int d = 0; d < ND; ++d) { v[d] = u[1 + d] * rrho; ke += u[1 + d] * v[d]; }
-  const double E = u[ND + 1];
-  p = (gamma - 1.0) * (E - 0.5 * ke);
+  for (int d = 0; d < ND; ++d) w[1 + d] = fma(-ph.v0[d], rho, u[1 + d]);
+  w[0] = dr;
+}
+// w -> conserved u (may alias)
+template <int ND>
+__device__ __forceinline__ void from_pert(const Phys &ph, const double *w, double *u) {
+  const double dr = w[0], rho = dr + ph.rho0;
+  u[ND + 1] = fma(ph.h0, dr, w[ND + 1]) + ph.E0;
+#pragma unroll
+  for (int d = 0; d < ND; ++d) u[1 + d] = fma(ph.v0[d], rho, w[1 + d]);
+  u[0] = rho;
+}
+// a difference (jump, increment) of w -> the same difference of u, in place
+template <int ND>
+__device__ __forceinline__ void from_pert_delta(const Phys &ph, double *d) {
+#pragma unroll
+  for (int j = 0; j < ND; ++j) d[1 + j] = fma(ph.v0[j], d[0], d[1 + j]);
+  d[ND + 1] = fma(ph.h0, d[0], d[ND + 1]);
+}
+
+// g[n][a] (Eq 20 in perturbation form) for the perturbation state w[NV]; also returns the full velocities and p' = p - p0
+template <int ND>
+__device__ __forceinline__ void inviscid_flux(const double *w, const Phys &ph, double (*g)[ND + 2], double *v, double &pp) {
+  const double rrho = 1.0 / (w[0] + ph.rho0);
+  double ke = 0, vw = 0;
+#pragma unroll
+  for (int d = 0; d < ND; ++d) {
+    const double dv = w[1 + d] * rrho;
+    v[d] = ph.v0[d] + dv;
+    ke += w[1 + d] * dv;
+    vw += ph.v0[d] * w[1 + d];
+  }
+  const double wE = w[ND + 1];
+  pp = (ph.gamma - 1.0) * (fma(ph.hs0, w[0], wE) - vw - 0.5 * ke);
 #pragma unroll
   for (int n = 0; n < ND; ++n) {
-    f[n][0] = u[1 + n];
+    g[n][0] = fma(ph.v0[n], w[0], w[1 + n]);
 #pragma unroll
-    for (int j = 0; j < ND; ++j) f[n][1 + j] = u[1 + n] * v[j] + (j == n ? p : 0.0);
-    f[n][ND + 1] = v[n] * (E + p);
+    for (int j = 0; j < ND; ++j) g[n][1 + j] = v[n] * w[1 + j] + (j == n ? pp : 0.0);
+    g[n][ND + 1] = v[n] * (wE + pp);
   }
 }
 
@@ -91,32 +151,39 @@ __device__ __forceinline__ void normal_viscous_flux(const double *u, const doubl
   }
 }
 
-// n . f_inv(u) of Eq 20 contracted with the unit normal directly (5 values instead of the 15 of the flux tensor):
-// [rho vn, rho v_j vn + p n_j, (E + p) vn] with vn = n . v; also returns vn and the pressure
+// n . g(w) contracted with the unit normal directly (5 values instead of the 15 of the flux tensor):
+// [w_m.n + (v0.n) w_rho,  vn w_mj + p' n_j,  vn (w_E + p')]  with vn = n . v (full velocity); also returns vn, p' and rho
 template <int ND>
-__device__ __forceinline__ void normal_inviscid_flux(const double *u, const double *nrm, double gamma, double *fn, double &vn, double &p) {
-  const double rrho = 1.0 / u[0];
-  double ke = 0, mn = 0;
+__device__ __forceinline__ void normal_inviscid_flux(const double *w, const double *nrm, const Phys &ph, double *gn, double &vn, double &pp,
+                                                     double &rho) {
+  rho = w[0] + ph.rho0;
+  const double rrho = 1.0 / rho;
+  double ke = 0, vw = 0, wn = 0, v0n = 0;
 #pragma unroll
-  for (int d = 0; d < ND; ++d) { ke += u[1 + d] * (u[1 + d] * rrho); mn += nrm[d] * u[1 + d]; }
-  const double E = u[ND + 1];
-  p = (gamma - 1.0) * (E - 0.5 * ke);
-  vn = mn * rrho;
-  fn[0] = mn;
+  for (int d = 0; d < ND; ++d) {
+    ke += w[1 + d] * (w[1 + d] * rrho);
+    vw += ph.v0[d] * w[1 + d];
+    wn += nrm[d] * w[1 + d];
+    v0n += nrm[d] * ph.v0[d];
+  }
+  const double wE = w[ND + 1];
+  pp = (ph.gamma - 1.0) * (fma(ph.hs0, w[0], wE) - vw - 0.5 * ke);
+  vn = fma(wn, rrho, v0n);
+  gn[0] = fma(v0n, w[0], wn);
 #pragma unroll
-  for (int j = 0; j < ND; ++j) fn[1 + j] = fma(u[1 + j], vn, p * nrm[j]);
-  fn[ND + 1] = vn * (E + p);
+  for (int j = 0; j < ND; ++j) gn[1 + j] = fma(w[1 + j], vn, pp * nrm[j]);
+  gn[ND + 1] = vn * (wE + pp);
 }
 
-// Rusanov, Eq 45-46 with the printed wave-speed estimate (A14)
+// Rusanov, Eq 45-46 with the printed wave-speed estimate (A14), on perturbation states: the dissipation acts on w_L - w_R
 template <int ND>
-__device__ __forceinline__ void rusanov(const double *uL, const double *uR, const double *nrm, double gamma, double *F) {
-  double fL[ND + 2], fR[ND + 2], vnL, vnR, pL, pR;
-  normal_inviscid_flux<ND>(uL, nrm, gamma, fL, vnL, pL);
-  normal_inviscid_flux<ND>(uR, nrm, gamma, fR, vnR, pR);
-  const double s = sqrt(gamma * (pL + pR) / (uL[0] + uR[0])) + 0.5 * fabs(vnL + vnR);
+__device__ __forceinline__ void rusanov(const double *wL, const double *wR, const double *nrm, const Phys &ph, double *F) {
+  double fL[ND + 2], fR[ND + 2], vnL, vnR, pL, pR, rL, rR;
+  normal_inviscid_flux<ND>(wL, nrm, ph, fL, vnL, pL, rL);
+  normal_inviscid_flux<ND>(wR, nrm, ph, fR, vnR, pR, rR);
+  const double s = sqrt(ph.gamma * (2.0 * ph.p0 + pL + pR) / (rL + rR)) + 0.5 * fabs(vnL + vnR);
 #pragma unroll
-  for (int a = 0; a < ND + 2; ++a) F[a] = 0.5 * (fL[a] + fR[a]) + 0.5 * s * (uL[a] - uR[a]);
+  for (int a = 0; a < ND + 2; ++a) F[a] = 0.5 * (fL[a] + fR[a]) + 0.5 * s * (wL[a] - wR[a]);
 }
 
 // Ghost states of Appendix C.  gi: B_inv u_L, gl: B_ldg u_L; returns the factor of q_L in B_ldg q_L.
@@ -158,15 +225,18 @@ __device__ __forceinline__ double ghost_states(const BcDev &bc, const double *uL
   return 1.0;
 }
 
-// Common normal flux Eq 26 with the penalty in its dissipative sign (A7):
-// F = F_inv(uL, uRinv) - n.{(1/2+beta) f_L^vis + (1/2-beta) f_R^vis} + tau (uL - uR)
+// Common normal flux Eq 26 with the penalty in its dissipative sign (A7), on perturbation states w (the viscous part is
+// evaluated from the conserved variables; its mass row is zero, so it is the same in both sets of variables):
+// F = F_inv(wL, wRinv) - n.{(1/2+beta) f_L^vis + (1/2-beta) f_R^vis} + tau (wL - wR)
 template <int ND, bool NS>
-__device__ __forceinline__ void common_flux(const double *uL, const double *uR, const double *uRinv, const double (*qL)[ND + 2],
+__device__ __forceinline__ void common_flux(const double *wL, const double *wR, const double *wRinv, const double (*qL)[ND + 2],
                                             const double (*qR)[ND + 2], const double *nrm, const Phys &ph, double *F) {
-  rusanov<ND>(uL, uRinv, nrm, ph.gamma, F);
+  rusanov<ND>(wL, wRinv, nrm, ph, F);
   if (NS) {
-    double fvL[ND + 2], fvR[ND + 2];
+    double fvL[ND + 2], fvR[ND + 2], uL[ND + 2], uR[ND + 2];
     const double wl = 0.5 + ph.beta, wr = 0.5 - ph.beta;
+    from_pert<ND>(ph, wL, uL);
+    from_pert<ND>(ph, wR, uR);
     if (wl != 0.0) normal_viscous_flux<ND>(uL, qL, nrm, ph, fvL);
     if (wr != 0.0) normal_viscous_flux<ND>(uR, qR, nrm, ph, fvR);
 #pragma unroll
@@ -174,7 +244,7 @@ __device__ __forceinline__ void common_flux(const double *uL, const double *uR, 
       double fv = 0;
       if (wl != 0.0) fv += wl * fvL[a];
       if (wr != 0.0) fv += wr * fvR[a];
-      F[a] += ph.tau * (uL[a] - uR[a]) - fv;
+      F[a] += ph.tau * (wL[a] - wR[a]) - fv;
     }
   }
 }

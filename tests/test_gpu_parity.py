@@ -46,12 +46,12 @@ def _check(name, got, ref, bar, floor=None):
     return err
 
 
-def _check_ld(name, got, o, U, R=None, sel=None, tol=TOL64):
+def _check_ld(name, got, o, U, R=None, sel=None, tol=TOL64, floor_mult=2):
     """fp64 comparison against the long-double oracle; bar = max(tol, 2 x floor of plain double arithmetic)."""
     R = o.rhs(U) if R is None else R
     R_ld = _ld(o, U, sel)
     floor = rel_l2_per_field(R if sel is None else R[:, :, sel], R_ld)
-    return _check(name, got, R_ld, np.maximum(tol, 2 * floor), floor)
+    return _check(name, got, R_ld, np.maximum(tol, floor_mult * floor), floor)
 
 
 def _check32(name, got, o, U32, sel=None):
@@ -177,6 +177,8 @@ def test_error_paths_on_device():
 # every kernel instantiation the dispatcher can reach
 # ------------------------------------------------------------------------------------------
 NS = dict(system="navier-stokes", gamma=1.4, mu=0.02, Pr=0.71, beta=0.5, tau=0.1)
+REF2 = dict(rho=1.0, v=(1.0, 0.5), p=1.0 / (1.4 * 0.3 ** 2))  # the freestream of workloads.fourier_state
+REF3 = dict(rho=1.0, v=(1.0, 0.5, 0.25), p=1.0 / (1.4 * 0.3 ** 2))
 BC2 = {0: ("sup-inflow", dict(rho=1.0, v=(1.0, 0.5), p=7.9)), 1: ("sub-outflow", dict(p=7.5)),
        2: ("noslip-wall", dict(cpTw=28.0, v=(0.2, 0.0))), 3: ("noslip-wall", dict(cpTw=27.0, v=(0.0, 0.0)))}
 BC3 = {4: ("noslip-wall", dict(cpTw=28.0, v=(0.2, 0.0, 0.0))), 5: ("sub-outflow", dict(p=7.5))}
@@ -187,9 +189,11 @@ def _state(mesh, o, seed):
     return np.ascontiguousarray(np.moveaxis(W.fourier_state(X, seed), -1, 1))
 
 
-def _sweep(label, mesh, p, bcs=None, systems=("navier-stokes", "euler"), precisions=("f64", "f32"), expect=None):
+def _sweep(label, mesh, p, bcs=None, systems=("navier-stokes", "euler"), precisions=("f64", "f32"), expect=None, ref=True, floor_mult=2):
     for system in systems:
         disc = dict(NS, p=p, system=system)
+        if ref:  # the library evaluates the fluxes in perturbation form about this state (include/fr.h); the oracle ignores it
+            disc["ref"] = REF2 if mesh["ndims"] == 2 else REF3
         o = FROracle(mesh, disc, bcs)
         U = _state(mesh, o, 100 + p)
         R = o.rhs(U)
@@ -203,7 +207,7 @@ def _sweep(label, mesh, p, bcs=None, systems=("navier-stokes", "euler"), precisi
                 if not bcs:  # boundary kernels are extra launches inside the same profiled groups
                     assert len(names) == ctx.rhs_kernel_launches, (name, names, ctx.rhs_kernel_launches)
             if precision == "f64":
-                _check_ld(name, run.rhs(U), o, U, R)
+                _check_ld(name, run.rhs(U), o, U, R, floor_mult=floor_mult)
             else:
                 U32 = U.astype(np.float32)
                 _check32(name, run.rhs(U32), o, U32)
@@ -244,14 +248,45 @@ def test_quads_every_order_curved_affine_boundary(p):
            precisions=("f64",), expect=expect)
 
 
-@pytest.mark.parametrize("p", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("p", [0, 1, 2, 3, 4, 5, 6])
 def test_triangles_every_order_straight_curved_boundary(p):
-    """Triangles: fused element kernels (1 <= p <= 4), staged dense path (p = 0, p >= 5); straight-sided jittered, curved
-    (p_g = 2), periodic and with boundary faces on all four sides."""
-    expect = "el_" if 1 <= p <= 4 else "apply_M0"
-    _sweep("tri-straight", W.tri_mesh(5, 1.0, 0.1, 77), p, expect=expect)
-    _sweep("tri-curved", W.curve_tri_mesh(W.tri_mesh(4, 1.0, 0.1, 78), 2, 0.02), p, expect=expect)
-    _sweep("tri-bnd", W.curve_tri_mesh(W.tri_mesh(3, 1.0, 0.1, 79, periodic=False), 2, 0.01), p, bcs=BC2, precisions=("f64",), expect=expect)
+    """Triangles: fused element kernels (1 <= p <= 5), staged dense path (p = 0, p >= 6); straight-sided jittered, curved
+    (p_g = 2), periodic and with boundary faces on all four sides.  The dense operators of the lattice point set (A6) are
+    ill-conditioned at p = 6 (the double oracle itself is 1e-12 from the long-double one): the staged path, which sums in
+    another order and has no reference state, is held to 4 x that floor there."""
+    expect = "el_" if 1 <= p <= 5 else "apply_M0"
+    fm = 4 if p >= 6 else 2
+    _sweep("tri-straight", W.tri_mesh(5, 1.0, 0.1, 77), p, expect=expect, floor_mult=fm)
+    _sweep("tri-curved", W.curve_tri_mesh(W.tri_mesh(4, 1.0, 0.1, 78), 2, 0.02), p, expect=expect, floor_mult=fm)
+    _sweep("tri-bnd", W.curve_tri_mesh(W.tri_mesh(3, 1.0, 0.1, 79, periodic=False), 2, 0.01), p, bcs=BC2, precisions=("f64",), expect=expect,
+           floor_mult=fm)
+
+
+def test_plain_formulas_without_a_reference_state():
+    """No reference state (fr_disc_desc rho_ref = p_ref = 0): the kernels evaluate the plain Eq 20-21 formulas; every fused
+    family once, with boundary faces."""
+    L3, L2 = (2 * np.pi,) * 3, (2 * np.pi,) * 2
+    _sweep("hex-noref", W.box_mesh((3, 2, 2), L3, p_g=2, warp=W.sine_warp(0.05)), 3, ref=False, precisions=("f64",))
+    _sweep("hex-noref-bnd", W.box_mesh((2, 1, 3), L3, periodic=(True, True, False)), 2, bcs=BC3, ref=False, precisions=("f64",))
+    _sweep("quad-noref", W.box_mesh((3, 4), L2, p_g=2, warp=W.sine_warp(0.05), periodic=(False, False)), 3, bcs=BC2, ref=False, precisions=("f64",))
+    _sweep("tri-noref", W.tri_mesh(4, 1.0, 0.1, 80, periodic=False), 2, bcs=BC2, ref=False, precisions=("f64",))
+
+
+def test_reference_state_removes_the_cancellation_error():
+    """on the clean Taylor-Green state of C2 (p0 = 71.4, E = 179, |R| << |f|) the perturbation form about
+    the freestream brings the GPU's distance from the long-double oracle well below the floor of plain double arithmetic,
+    which is where the same kernels sit without the reference state."""
+    mesh, disc = W.config("C2", n=8)
+    o = FROracle(mesh, disc)
+    U = W.config_state("C2", np.asarray(o.xu_phys, float))
+    R, R_ld = o.rhs(U), _ld(o, U)
+    floor = rel_l2_per_field(R, R_ld)
+    e_ref = rel_l2_per_field(GpuRunner(_ctx(mesh, disc)).rhs(U), R_ld)
+    e_plain = rel_l2_per_field(GpuRunner(_ctx(mesh, dict(disc, ref=None))).rhs(U), R_ld)
+    print("floor", floor, "with reference", e_ref, "without", e_plain)
+    assert np.all(e_ref <= TOL64) and np.all(e_ref <= 0.5 * floor), (e_ref, floor)
+    assert np.all(e_plain <= 2 * floor)
+    assert np.max(e_plain) > 3 * np.max(e_ref)
 
 
 # ------------------------------------------------------------------------------------------
@@ -501,7 +536,8 @@ def test_euler_and_dopri5_steppers_parity(case):
     name, over = CASES[case]
     mesh, disc = W.config(name, **over)
     o = FROracle(mesh, disc)
-    U = W.config_state(name, np.asarray(o.xu_phys, float), **over)
+    # C2's clean Taylor-Green state has rho w = 0 identically (no scale for a relative norm): use the noisy one of C3
+    U = W.config_state("C3" if name == "C2" else name, np.asarray(o.xu_phys, float), **over)
     run = GpuRunner(_ctx(mesh, disc))
     dt = disc["dt"]
     ref = U

@@ -307,7 +307,18 @@ def fourier_state(X, seed, gamma=1.4, mach=0.3, n_modes=8, amp=0.02):
 # the BASELINE.json configs
 # ----------------------------------------------------------------------------
 def config(name, **over):
-    """Returns (mesh, disc) for C1..C5 (C5 takes p=, n=, system=)."""
+    """Returns (mesh, disc) for C1..C5 (C5 takes p=, n=, system=).  disc["ref"] is the freestream the state generator of the
+    config perturbs (density, velocity, pressure): the library takes it as its constant reference state (a conditioning
+    hint, include/fr.h); the oracle ignores it."""
+    mesh, disc = _config(name, **over)
+    nd = mesh["ndims"]
+    p0 = {"C1": 1.0, "C2": 1.0 / (1.4 * 0.1 ** 2), "C3": 1.0 / (1.4 * 0.1 ** 2), "C4": 1.0 / (1.4 * 0.2 ** 2), "C5": 1.0 / (1.4 * 0.3 ** 2)}[name]
+    v0 = {"C1": (1.0, 1.0), "C2": (0.0,) * 3, "C3": (0.0,) * 3, "C4": (1.0, 1.0), "C5": (1.0, 0.5, 0.25)}[name]
+    disc["ref"] = dict(rho=1.0, v=v0[:nd], p=p0)
+    return mesh, disc
+
+
+def _config(name, **over):
     g = 1.4
     if name == "C1":
         mesh = box_mesh((8, 8), (10.0, 10.0))
