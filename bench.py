@@ -81,36 +81,39 @@ def rhs_algorithmic_words(nd, NV, Nu, Nf, ns, affine):
     return w
 
 
-def kernel_words(name, nd, NV, Nu, Nf, ns, gfrac=1.0):
-    """compulsory words per element for one launch group (inputs once + outputs once).
-    gfrac: fraction of the faces whose G^f is produced (1/2 when the LDG weight of one side is zero, |beta| = 1/2)."""
-    met = (nd * nd + 1) * Nu
+def kernel_bytes(name, nd, NV, Nu, Nf, ns, gfrac=1.0, sz=8, szi=8):
+    """compulsory bytes per element for one launch group (inputs once + outputs once).
+    sz: bytes of a state / metric word (8 | 4: the algorithmic size in the context's precision); szi: bytes of a flux-point /
+    gradient intermediate as the path stores it (= sz on the hexahedral TMA path, 8 elsewhere); index words are 4 bytes,
+    gather offsets 8.  gfrac: fraction of the faces that carry an LDG weight (1/2 when |beta| = 1/2)."""
+    met = (nd * nd + 1) * Nu * sz
+    pair_tab = (4 * 4 + (nd + 2) * sz) * Nf // 2  # per flux-point pair: 4 indices, unit normal, two J n
+    U, R = Nu * NV * sz, Nu * NV * sz
     t = {
         # generic staged path (PAPER.md App A sequence)
-        "apply_M0": (Nu + Nf) * NV,
-        "common_sol": 2 * Nf * NV + Nf,
-        "apply_M46_M6": (Nu + Nf + nd * Nu) * NV,
-        "grad_phys": 2 * nd * Nu * NV + met,
-        "apply_M5": nd * (Nu + Nf) * NV,
-        "tflux": Nu * NV + (2 if ns else 1) * nd * Nu * NV + nd * nd * Nu,
-        "common_flux": (2 + (nd if ns else 0)) * Nf * NV + (nd + 2 + 2) * Nf // 2,
-        "apply_M132_M3_negdivconf": (nd * Nu + Nf + Nu) * NV + Nu,
-        # tensor-product path (fr_tensor.cu)
-        "tp_interp": (Nu + Nf) * NV,
-        "tp_interp_q": nd * (Nu + Nf) * NV,
-        "hex_grad": (Nu + Nf) * NV + met + nd * Nu * NV,
-        "hex_fluxdiv": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
-        # TMA-pipelined hexahedral path (fr_hex_tma.cu, fr_hex_fluxdiv_tma.cu)
-        "hex_interp_tma": (Nu + Nf) * NV,
-        "hex_gradface": (Nu + Nf + gfrac * Nf) * NV + met + gfrac * nd * Nf + nd * Nu * NV,  # U, jump, S, 1/J, normals -> G^f, Q
-        "common_flux_g": (2 + gfrac) * Nf * NV + (nd + 2 + 2) * Nf // 2,      # U^f, G^f -> D~ (in place), normals, J n
-        "hex_fluxdiv_tma": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
-        # fused triangle kernels (fr_element.cu)
-        "el_interp": (Nu + Nf) * NV,
-        "el_gradface": (Nu + 3 * Nf) * NV + met + nd * Nf + nd * Nu * NV,   # U, C, U^f, S, 1/J, normals -> Q, G^f
-        "el_fluxdiv": (2 * Nu + Nf) * NV + (nd * Nu * NV if ns else 0) + met,
-        "tp_grad": (Nu + Nf) * NV + met + (nd + 1) * Nf + (NV - 1) * Nf + Nf,
-        "tp_div": (2 * Nu + Nf) * NV + met + (nd + 1) * Nf + ((NV - 1) * Nf if ns else 0) + Nf,
+        "apply_M0": U + Nf * NV * szi,
+        "common_sol": 2 * Nf * NV * szi + 4 * 4 * Nf // 2,
+        "apply_M46_M6": U + (Nf + nd * Nu) * NV * szi,
+        "grad_phys": 2 * nd * Nu * NV * szi + met,
+        "apply_M5": nd * (Nu + Nf) * NV * szi,
+        "tflux": U + (2 if ns else 1) * nd * Nu * NV * szi + nd * nd * Nu * sz,
+        "common_flux": (2 + (nd if ns else 0)) * Nf * NV * szi + pair_tab,
+        "apply_M132_M3_negdivconf": (nd * Nu + Nf) * NV * szi + R + Nu * sz,
+        # quadrilateral line kernels (fr_tensor.cu)
+        "tp_interp": U + Nf * NV * szi,
+        "tp_interp_q": nd * (Nu + Nf) * NV * szi,
+        "tp_grad": U + Nf * NV * szi + met + nd * Nu * NV * szi,
+        "tp_div": (nd * Nu + Nf) * NV * szi + R + Nu * sz,
+        # TMA-pipelined hexahedral path (fr_hex_interp_tma.cu, fr_hex_tma.cu, fr_hex_fluxdiv_tma.cu)
+        "hex_interp_tma": U + Nf * NV * szi,
+        # U, partner U^f and its offset (faces with an LDG weight), S, 1/J, own normals -> G^f, Q
+        "hex_gradface": U + 2 * gfrac * Nf * NV * szi + gfrac * Nf * 8 + met + gfrac * nd * Nf * sz + nd * Nu * NV * szi,
+        "common_flux_g": (2 + gfrac) * Nf * NV * szi + pair_tab,      # U^f, G^f -> D~ (in place), normals, J n
+        "hex_fluxdiv_tma": U + R + Nf * NV * szi + (nd * Nu * NV * szi if ns else 0) + met,
+        # fused triangle / quadrilateral kernels (fr_element.cu)
+        "el_interp": U + Nf * NV * szi,
+        "el_gradface": U + 3 * Nf * NV * szi + met + nd * Nf * sz + nd * Nu * NV * szi,   # U, C, U^f, S, 1/J, normals -> Q, G^f
+        "el_fluxdiv": U + R + Nf * NV * szi + (nd * Nu * NV * szi if ns else 0) + met,
     }
     return t.get(name)
 
@@ -306,13 +309,14 @@ def main():
         peaks = json.load(open(pk_path))
     peak_gbs = float(peaks.get("hbm_gbs", 6650.0))
     peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s"
-    esz = 8  # intermediates are fp64 in both precisions; state words counted at the storage size below
     nd, NV, Nu, Nf, ns = ctx.ndims, ctx.NV, ctx.Nu, ctx.Nf, disc["system"] == "navier-stokes"
     affine = mesh["p_g"] == 1
+    sz = 8 if args.precision == "f64" else 4
+    szi = sz if any(n.startswith("hex_") for n in acc) else 8  # the hexahedral TMA path stores its intermediates in the storage precision
     kern = []
     for name, ms in acc.items():
-        wds = kernel_words(name, nd, NV, Nu, Nf, ns, 0.5 if abs(abs(disc.get("beta", 0.5)) - 0.5) < 1e-15 else 1.0)
-        gbs = (wds * esz * ctx.n_elems / (ms * 1e-3) / 1e9) if (wds and ms > 0) else None
+        byt = kernel_bytes(name, nd, NV, Nu, Nf, ns, 0.5 if abs(abs(disc.get("beta", 0.5)) - 0.5) < 1e-15 else 1.0, sz, szi)
+        gbs = (byt * ctx.n_elems / (ms * 1e-3) / 1e9) if (byt and ms > 0) else None
         kern.append({"name": name, "ms": ms, "share": ms / sum(acc.values()), "algorithmic_GBps": gbs})
     kern.sort(key=lambda k: -k["ms"])
     top = kern[0]

@@ -149,37 +149,59 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     dc.hM0 = o.M[0].data(); dc.hM3 = o.M[3].data(); dc.hM6 = o.M[6].data(); dc.hM46 = o.M46.data(); dc.hM132 = o.M132.data();
     dc.affine = mc.affine;
     dc.aff = dc.blk && mc.affine;
+    // The hexahedral TMA path keeps its metric terms, normals and J n in the STORAGE precision (single precision halves
+    // their traffic too; with a reference state their rounding multiplies deviation-sized fluxes only, fr_physics.cuh).
+    const bool f32tab = dc.blk && !dc.f64;
+    auto up_t = [&](const std::vector<double> &v, const double **dst) {  // upload as double, or as float behind the same pointer
+      if (!f32tab) return upload(c, v, dst);
+      std::vector<float> f(v.begin(), v.end());
+      const float *p = nullptr;
+      cudaError_t er = upload(c, f, &p);
+      *dst = (const double *)(const void *)p;
+      return er;
+    };
+#define UPT(vec, field) if (e == cudaSuccess) e = up_t(vec, &dc.field)
     if (dc.aff) {  // affine hexahedra: one point of S and 1/J per element; the tensor maps broadcast it (fr_tma.cuh: encode_blk)
       const int nn = o.nd * o.nd;
       std::vector<double> s_el((size_t)nn * ld), r_el((size_t)ld);
       for (int cc = 0; cc < nn; ++cc) std::memcpy(&s_el[(size_t)cc * ld], &mc.smat[(size_t)cc * o.Nu * ld], ld * sizeof(double));
       std::memcpy(r_el.data(), mc.rcpj.data(), ld * sizeof(double));
-      UP(reblock(s_el, nn), smat); UP(reblock(r_el, 1), rcpj);
-    } else if (dc.blk) { UP(reblock(mc.smat, o.nd * o.nd * o.Nu), smat); UP(reblock(mc.rcpj, o.Nu), rcpj); }
+      UPT(reblock(s_el, nn), smat); UPT(reblock(r_el, 1), rcpj);
+    } else if (dc.blk) { UPT(reblock(mc.smat, o.nd * o.nd * o.Nu), smat); UPT(reblock(mc.rcpj, o.Nu), rcpj); }
     else { UP(mc.smat, smat); UP(mc.rcpj, rcpj); }
     UP(mc.pLs, pLs); UP(mc.pLe, pLe); UP(mc.pRs, pRs); UP(mc.pRe, pRe);
-    UP(mc.pn, pn); UP(mc.pJnL, pJnL); UP(mc.pJnR, pJnR);
+    UPT(mc.pn, pn); UPT(mc.pJnL, pJnL); UPT(mc.pJnR, pJnR);
     UP(mc.bs, bs); UP(mc.be, be); UP(mc.bbc, bbc); UP(mc.bn, bn); UP(mc.bJn, bJn);
     // element-centric flux-point tables of the fused hexahedral gradient kernel (own normals, boundary ids)
     const bool want_tma = !(d->flags & FR_FLAG_FORCE_GENERIC) && o.etype == FR_HEX && dc.ns && hex_tma_supported(o.n, dc.f64);
     if (want_tma) {
-      UP(reblock(mc.fp_n, o.nd * o.Nf), fp_n);
-      if (mc.nbnd) { UP(reblock(mc.fp_pe, o.Nf), fp_pe); }
+      UPT(reblock(mc.fp_n, o.nd * o.Nf), fp_n);
+      // partner of every flux point as an offset into the element-blocked U^f array (row sigma * N_V of N_f * N_V rows)
+      std::vector<int64_t> poff((size_t)o.Nf * ld, 0);
+      for (int sg = 0; sg < o.Nf; ++sg)
+        for (int64_t el = 0; el < mc.Nel; ++el) {
+          const size_t i0 = (size_t)sg * ld + el;
+          const int32_t pe = mc.fp_pe[i0];
+          poff[i0] = pe < 0 ? (int64_t)pe : (int64_t)fp_row(true, ld, o.Nf * dc.NV, mc.fp_ps[i0] * dc.NV, pe);
+        }
+      UP(reblock(poff, o.Nf), fp_poff);
     }
     const bool want_el = dc.ns && element_fused_supported(dc);  // fused triangle kernels
     if (want_el) { UP(mc.fp_n, fp_n); if (mc.nbnd) { UP(mc.fp_pe, fp_pe); } }
     if (want_tma) {
-      // faces whose G^f enters the common flux: L sides weigh 1/2 + beta, R sides 1/2 - beta (Eq 27), boundaries always
-      std::vector<uint8_t> need((size_t)o.nfaces * ld, 0);
+      // faces that carry an LDG weight (jump of Eq 9 and G^f of Eq 27): L sides weigh 1/2 + beta, R sides 1/2 - beta
+      std::vector<uint8_t> code((size_t)o.nfaces * ld, 0);
       for (int f = 0; f < o.nfaces; ++f)
         for (int64_t el = 0; el < mc.Nel; ++el) {
           const size_t i0 = (size_t)(f * o.nfp) * ld + el;
           const bool bnd = mc.fp_pe[i0] < 0, rside = mc.fp_Jn[i0] < 0;
-          need[(size_t)f * ld + el] = bnd || (rside ? 0.5 - d->ldg_beta : 0.5 + d->ldg_beta) != 0.0;
+          const double wgt = rside ? 0.5 - d->ldg_beta : 0.5 + d->ldg_beta;
+          code[(size_t)f * ld + el] = bnd ? 3 : (wgt == 0.0 ? 0 : (rside ? 2 : 1));
         }
-      UP(need, face_need);
+      UP(code, face_code);
     }
 #undef UP
+#undef UPT
     std::vector<BcDev> bcs(c->mesh.bcs.size());
     for (size_t i = 0; i < bcs.size(); ++i) {
       const fr_bc_desc &b = c->mesh.bcs[i];

@@ -42,7 +42,8 @@ struct DevConsts {
   int nbcs;
   // element-centric tables (tensor-product kernels)
   const int32_t *fp_pe, *fp_ps;
-  const uint8_t *face_need;  // [6][ld] (hexahedra): 1 where the element kernels must produce G^f of the face
+  const int64_t *fp_poff;    // hexahedral TMA path, [block][Nf][FR_BLK]: offset of the partner's first variable in U^f, or -1 - bc_id
+  const uint8_t *face_code;  // [6][ld] (hexahedra): 0 = face without LDG weight, 1 = L side, 2 = R side, 3 = boundary (fr_hex_tma.cu)
   const double *fp_n, *fp_Jn;
 };
 
@@ -85,7 +86,7 @@ int generic_rhs_launches(const DevConsts &c);
 // point-wise / pair kernels of the generic path reused by the tensor-product path
 void launch_common_jump(const DevConsts &c, const double *uf, double *cf, cudaStream_t s);  // {C - u^f} of Eq 9
 void launch_tflux(const DevConsts &c, const void *u, double *qu, cudaStream_t s);           // Eq 12, in place over Q^u
-void launch_common_flux(const DevConsts &c, double *uf, const double *qf, cudaStream_t s);  // Eq 15-17, in place over U^f
+void launch_common_flux(const DevConsts &c, void *uf, const void *qf, bool f32, cudaStream_t s);  // Eq 15-17, in place over U^f (f32: float arrays)
 
 // register updates of the time steppers (fr_rk.cu): rows x ld matrices of which the first nel columns are updated
 constexpr int RK_MAX_IN = 8;

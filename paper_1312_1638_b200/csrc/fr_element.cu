@@ -50,10 +50,12 @@ template <int ND, bool BND>
 __device__ __forceinline__ void face_visc_nd(const double *uf, const double (*qf)[ND + 2], const double *nrm, const Phys &ph, int pe,
                                              const BcDev *__restrict__ bcs, double *G) {
   constexpr int NV = ND + 2;
-  normal_viscous_flux<ND>(uf, qf, nrm, ph, G);
+  normal_viscous_flux<ND>(uf, qf, nrm, ph, G);  // uf: perturbation state w^f, qf: its gradient
   if (BND && pe < 0) {
-    double gi[NV], gl[NV], qg[ND][NV], GR[NV];
-    const double keep = ghost_states<ND>(bcs[-1 - pe], uf, ph.gamma, gi, gl);
+    double uc[NV], gi[NV], gl[NV], qg[ND][NV], GR[NV];
+    from_pert<ND>(ph, uf, uc);
+    const double keep = ghost_states<ND>(bcs[-1 - pe], uc, ph.gamma, gi, gl);
+    to_pert<ND>(ph, gl, gl);
 #pragma unroll
     for (int n = 0; n < ND; ++n)
 #pragma unroll
@@ -62,6 +64,22 @@ __device__ __forceinline__ void face_visc_nd(const double *uf, const double (*qf
     const double wl = 0.5 + ph.beta, wr = 0.5 - ph.beta;
 #pragma unroll
     for (int a = 0; a < NV; ++a) G[a] = (wl != 0.0 ? wl * G[a] : 0.0) + (wr != 0.0 ? wr * GR[a] : 0.0);
+  }
+}
+
+// Variable a of the conserved state at the NU points of element e (uu, read from u) -> the same component of the perturbation
+// variables: w_rho = rho - rho0, w_mj = m_j - v0_j rho, w_E = (E - E0) - h0 (rho - rho0); the other threads' density rows are
+// re-read (L1 hits: the thread of variable 0 has just loaded them)
+template <int NU, typename T>
+__device__ __forceinline__ void pert_rows(const Phys &ph, int a, const T *__restrict__ u, size_t ld, int64_t e, double *uu) {
+  constexpr int NV = 4;
+  if (ph.rho0 == 0.0) return;
+  const double ka = a == 0 ? 0.0 : (a == NV - 1 ? ph.h0 : ph.v0[a - 1]);
+  const double da = a == 0 ? ph.rho0 : (a == NV - 1 ? ph.E0 : 0.0);
+#pragma unroll
+  for (int r = 0; r < NU; ++r) {
+    const double rho = a == 0 ? uu[r] : (double)u[((size_t)r * NV) * ld + e];
+    uu[r] = a == NV - 1 ? fma(-ka, rho - ph.rho0, uu[r] - da) : fma(-ka, rho, uu[r] - da);
   }
 }
 
@@ -78,16 +96,8 @@ __global__ void __launch_bounds__(TPB) k_el_interp(const __grid_constant__ OpsIn
 #pragma unroll
   for (int r = 0; r < NU; ++r) uu[r] = (double)u[((size_t)r * NV + a) * ld + e];
   // perturbation variables (fr_physics.cuh) BEFORE the interpolation, so that its rounding error scales with the deviation
-  // from the reference state: w_rho = rho - rho0, w_mj = m_j - v0_j rho, w_E = (E - E0) - h0 (rho - rho0)
-  if (c.ph.rho0 != 0.0) {
-    const double ka = a == 0 ? 0.0 : (a == NV - 1 ? c.ph.h0 : c.ph.v0[a - 1]);
-    const double da = a == 0 ? c.ph.rho0 : (a == NV - 1 ? c.ph.E0 : 0.0);
-#pragma unroll
-    for (int r = 0; r < NU; ++r) {
-      const double rho = a == 0 ? uu[r] : (double)u[((size_t)r * NV) * ld + e];
-      uu[r] = a == NV - 1 ? fma(-ka, rho - c.ph.rho0, uu[r] - da) : fma(-ka, rho, uu[r] - da);
-    }
-  }
+  // from the reference state
+  pert_rows<NU, T>(c.ph, a, u, ld, e, uu);
 #pragma unroll
   for (int s = 0; s < NF; ++s) {
     double acc = 0;
@@ -112,6 +122,7 @@ __global__ void __launch_bounds__(TPB) k_el_gradface(const __grid_constant__ Ops
     double uu[NU], cc[NF], qq[ND][NU];
 #pragma unroll
     for (int r = 0; r < NU; ++r) uu[r] = (double)u[((size_t)r * NV + a) * ld + e];
+    pert_rows<NU, T>(c.ph, a, u, ld, e, uu);  // the gradient is taken of the perturbation variables (fr_physics.cuh)
 #pragma unroll
     for (int s = 0; s < NF; ++s) cc[s] = cf[((size_t)s * NV + a) * ld + e];
     // affine elements: the metric terms of point 0 serve every point (one load instead of N_u)
@@ -166,7 +177,6 @@ __global__ void __launch_bounds__(TPB) k_el_gradface(const __grid_constant__ Ops
     double us[NV], qf[ND][NV], nrm[ND], G[NV];
 #pragma unroll
     for (int b = 0; b < NV; ++b) us[b] = uf[((size_t)s * NV + b) * ld + e2];
-    from_pert<ND>(c.ph, us, us);
 #pragma unroll
     for (int n = 0; n < ND; ++n) {
       nrm[n] = c.fp_n[((size_t)n * NF + s) * ld + e2];
@@ -206,7 +216,7 @@ __global__ void __launch_bounds__(TPB) k_el_fluxdiv(const __grid_constant__ OpsD
       for (int n = 0; n < ND; ++n)
 #pragma unroll
         for (int b = 0; b < NV; ++b) qq[n][b] = q[(((size_t)n * NU + r) * NV + b) * ld + e2];
-      subtract_viscous_flux<ND>(uu, qq, v, c.ph, f);
+      subtract_viscous_flux<ND>(ww, qq, v, c.ph, f);
     }
 #pragma unroll
     for (int d = 0; d < ND; ++d) {

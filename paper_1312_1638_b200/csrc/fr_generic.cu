@@ -56,8 +56,8 @@ __global__ void __launch_bounds__(128) k_apply(int M, int K1, const double *__re
     }
 }
 
-// Common solution, Eq 7 + Eq 25 (:192, :506): each pair visited once, same value to both sides.  The flux-point states
-// arrive in perturbation variables w (fr_physics.cuh); the output is in CONSERVED variables (it feeds the gradient of u).
+// Common solution, Eq 7 + Eq 25 (:192, :506): each pair visited once, same value to both sides.  Flux-point states and the
+// output are in the perturbation variables w (fr_physics.cuh): the gradient kernels differentiate w.
 template <int ND, bool JUMP>
 __global__ void k_common_sol(DevConsts c, const double *__restrict__ uf, double *__restrict__ cf) {
   constexpr int NV = ND + 2;
@@ -66,18 +66,13 @@ __global__ void k_common_sol(DevConsts c, const double *__restrict__ uf, double 
   const size_t oL = fp_row(c.blk, c.ld, c.Nf * NV, c.pLs[i] * NV, c.pLe[i]), oR = fp_row(c.blk, c.ld, c.Nf * NV, c.pRs[i] * NV, c.pRe[i]);
   const size_t vs = fp_rstride(c.blk, c.ld);  // distance between the variables of one flux point
   const double wl = 0.5 - c.ph.beta, wr = 0.5 + c.ph.beta;
-  double oa[NV], ob[NV];
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
     const double ul = uf[oL + (size_t)a * vs], ur = uf[oR + (size_t)a * vs];
     const double v = wl * ul + wr * ur;
-    oa[a] = JUMP ? v - ul : v;   // JUMP: the {C - u^f} of Eq 9 directly
-    ob[a] = JUMP ? v - ur : v;
+    cf[oL + (size_t)a * vs] = JUMP ? v - ul : v;   // JUMP: the {C - u^f} of Eq 9 directly
+    cf[oR + (size_t)a * vs] = JUMP ? v - ur : v;
   }
-  if (JUMP) { from_pert_delta<ND>(c.ph, oa); from_pert_delta<ND>(c.ph, ob); }
-  else { from_pert<ND>(c.ph, oa, oa); from_pert<ND>(c.ph, ob, ob); }
-#pragma unroll
-  for (int a = 0; a < NV; ++a) { cf[oL + (size_t)a * vs] = oa[a]; cf[oR + (size_t)a * vs] = ob[a]; }
 }
 
 // Boundary common solution C(u_L, B_ldg u_L)  (:797)
@@ -88,13 +83,14 @@ __global__ void k_common_sol_bnd(DevConsts c, const double *__restrict__ uf, dou
   if (i >= c.nbnd) return;
   const size_t o = fp_row(c.blk, c.ld, c.Nf * NV, c.bs[i] * NV, c.be[i]);
   const size_t vs = fp_rstride(c.blk, c.ld);
-  double u[NV], gi[NV], gl[NV];
+  double w[NV], u[NV], gi[NV], gl[NV];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) u[a] = uf[o + (size_t)a * vs];
-  from_pert<ND>(c.ph, u, u);
+  for (int a = 0; a < NV; ++a) w[a] = uf[o + (size_t)a * vs];
+  from_pert<ND>(c.ph, w, u);
   ghost_states<ND>(c.bcs[c.bbc[i]], u, c.ph.gamma, gi, gl);
+  to_pert<ND>(c.ph, gl, gl);
 #pragma unroll
-  for (int a = 0; a < NV; ++a) cf[o + (size_t)a * vs] = (0.5 - c.ph.beta) * u[a] + (0.5 + c.ph.beta) * gl[a] - (JUMP ? u[a] : 0.0);
+  for (int a = 0; a < NV; ++a) cf[o + (size_t)a * vs] = (0.5 - c.ph.beta) * w[a] + (0.5 + c.ph.beta) * gl[a] - (JUMP ? w[a] : 0.0);
 }
 
 // q = J^-T q~ = (1/J) S^T q~, Eq 10 (:206), in place
@@ -163,8 +159,9 @@ __global__ void k_tflux(DevConsts c, const T *__restrict__ u, double *__restrict
 }
 
 // Common normal flux over flux-point pairs, Eq 15-17 (:227-235); in place over U^f -> D~ (:300)
-template <int ND, bool NS>
-__global__ void __launch_bounds__(128, NS ? 2 : FLUXG_MINB) k_common_flux(DevConsts c, double *__restrict__ uf, const double *__restrict__ qf) {
+// TI: storage type of the flux-point arrays (double; float on the hexahedral TMA path in single precision)
+template <int ND, bool NS, typename TI>
+__global__ void __launch_bounds__(128, NS ? 2 : FLUXG_MINB) k_common_flux(DevConsts c, TI *__restrict__ uf, const TI *__restrict__ qf) {
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.npairs) return;
@@ -173,23 +170,23 @@ __global__ void __launch_bounds__(128, NS ? 2 : FLUXG_MINB) k_common_flux(DevCon
   const size_t blk = (size_t)c.Nf * NV * c.ld;
   double uL[NV], uR[NV], qL[ND][NV], qR[ND][NV], nrm[ND], F[NV];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) { uL[a] = uf[oL + (size_t)a * vs]; uR[a] = uf[oR + (size_t)a * vs]; }
+  for (int a = 0; a < NV; ++a) { uL[a] = (double)uf[oL + (size_t)a * vs]; uR[a] = (double)uf[oR + (size_t)a * vs]; }
   if (NS) {
 #pragma unroll
     for (int n = 0; n < ND; ++n)
 #pragma unroll
-      for (int a = 0; a < NV; ++a) { qL[n][a] = qf[n * blk + oL + (size_t)a * vs]; qR[n][a] = qf[n * blk + oR + (size_t)a * vs]; }
+      for (int a = 0; a < NV; ++a) { qL[n][a] = (double)qf[n * blk + oL + (size_t)a * vs]; qR[n][a] = (double)qf[n * blk + oR + (size_t)a * vs]; }
   }
 #pragma unroll
-  for (int n = 0; n < ND; ++n) nrm[n] = c.pn[(size_t)n * c.npairs + i];
+  for (int n = 0; n < ND; ++n) nrm[n] = (double)((const TI *)c.pn)[(size_t)n * c.npairs + i];  // tables in TI (fr_api.cu)
   common_flux<ND, NS>(uL, uR, uR, qL, qR, nrm, c.ph, F);
-  const double jl = c.pJnL[i], jr = c.pJnR[i];
+  const double jl = (double)((const TI *)c.pJnL)[i], jr = (double)((const TI *)c.pJnR)[i];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) { uf[oL + (size_t)a * vs] = jl * F[a]; uf[oR + (size_t)a * vs] = -jr * F[a]; }
+  for (int a = 0; a < NV; ++a) { uf[oL + (size_t)a * vs] = (TI)(jl * F[a]); uf[oR + (size_t)a * vs] = (TI)(-jr * F[a]); }
 }
 
-template <int ND, bool NS>
-__global__ void k_common_flux_bnd(DevConsts c, double *__restrict__ uf, const double *__restrict__ qf) {
+template <int ND, bool NS, typename TI>
+__global__ void k_common_flux_bnd(DevConsts c, TI *__restrict__ uf, const TI *__restrict__ qf) {
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.nbnd) return;
@@ -198,7 +195,7 @@ __global__ void k_common_flux_bnd(DevConsts c, double *__restrict__ uf, const do
   const size_t blk = (size_t)c.Nf * NV * c.ld;
   double uL[NV], gi[NV], gl[NV], qL[ND][NV], qR[ND][NV], nrm[ND], F[NV];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) uL[a] = uf[o + (size_t)a * vs];
+  for (int a = 0; a < NV; ++a) uL[a] = (double)uf[o + (size_t)a * vs];
   double uc[NV];
   from_pert<ND>(c.ph, uL, uc);
   const double keep = ghost_states<ND>(c.bcs[c.bbc[i]], uc, c.ph.gamma, gi, gl);
@@ -208,21 +205,21 @@ __global__ void k_common_flux_bnd(DevConsts c, double *__restrict__ uf, const do
 #pragma unroll
     for (int n = 0; n < ND; ++n)
 #pragma unroll
-      for (int a = 0; a < NV; ++a) { qL[n][a] = qf[n * blk + o + (size_t)a * vs]; qR[n][a] = keep * qL[n][a]; }
+      for (int a = 0; a < NV; ++a) { qL[n][a] = (double)qf[n * blk + o + (size_t)a * vs]; qR[n][a] = keep * qL[n][a]; }
   }
 #pragma unroll
-  for (int n = 0; n < ND; ++n) nrm[n] = c.bn[(size_t)n * c.nbnd + i];
+  for (int n = 0; n < ND; ++n) nrm[n] = c.bn[(size_t)n * c.nbnd + i];  // boundary tables stay double
   common_flux<ND, NS>(uL, gl, gi, qL, qR, nrm, c.ph, F);
   const double jn = c.bJn[i];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) uf[o + (size_t)a * vs] = jn * F[a];
+  for (int a = 0; a < NV; ++a) uf[o + (size_t)a * vs] = (TI)(jn * F[a]);
 }
 
 // Common normal flux with the viscous part pre-contracted by the element kernels (fr_hex_tma.cu):
 // gf = n_own . f_vis(u^f, q^f) at every flux point with the element's OWN outward normal, so that
 // n_L . f_R^vis = -gf_R.   F = Rusanov + tau (u_L - u_R) - {(1/2+beta) gf_L - (1/2-beta) gf_R}   (Eq 26-27, A7)
-template <int ND>
-__global__ void __launch_bounds__(128, FLUXG_MINB) k_common_flux_g(DevConsts c, double *__restrict__ uf, const double *__restrict__ gf) {
+template <int ND, typename TI>
+__global__ void __launch_bounds__(128, FLUXG_MINB) k_common_flux_g(DevConsts c, TI *__restrict__ uf, const TI *__restrict__ gf) {
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.npairs) return;
@@ -231,24 +228,24 @@ __global__ void __launch_bounds__(128, FLUXG_MINB) k_common_flux_g(DevConsts c, 
   const double wl = 0.5 + c.ph.beta, wr = 0.5 - c.ph.beta;
   double uL[NV], uR[NV], gL[NV], gR[NV], nrm[ND], F[NV];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) { uL[a] = uf[oL + (size_t)a * vs]; uR[a] = uf[oR + (size_t)a * vs]; }
+  for (int a = 0; a < NV; ++a) { uL[a] = (double)uf[oL + (size_t)a * vs]; uR[a] = (double)uf[oR + (size_t)a * vs]; }
 #pragma unroll
-  for (int a = 0; a < NV; ++a) { gL[a] = wl != 0.0 ? gf[oL + (size_t)a * vs] : 0.0; gR[a] = wr != 0.0 ? gf[oR + (size_t)a * vs] : 0.0; }
+  for (int a = 0; a < NV; ++a) { gL[a] = wl != 0.0 ? (double)gf[oL + (size_t)a * vs] : 0.0; gR[a] = wr != 0.0 ? (double)gf[oR + (size_t)a * vs] : 0.0; }
 #pragma unroll
-  for (int n = 0; n < ND; ++n) nrm[n] = c.pn[(size_t)n * c.npairs + i];
+  for (int n = 0; n < ND; ++n) nrm[n] = (double)((const TI *)c.pn)[(size_t)n * c.npairs + i];
   rusanov<ND>(uL, uR, nrm, c.ph, F);
-  const double jl = c.pJnL[i], jr = c.pJnR[i];
+  const double jl = (double)((const TI *)c.pJnL)[i], jr = (double)((const TI *)c.pJnR)[i];
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
     const double f = F[a] + c.ph.tau * (uL[a] - uR[a]) - (wl * gL[a] - wr * gR[a]);
-    uf[oL + (size_t)a * vs] = jl * f;
-    uf[oR + (size_t)a * vs] = -jr * f;
+    uf[oL + (size_t)a * vs] = (TI)(jl * f);
+    uf[oR + (size_t)a * vs] = (TI)(-jr * f);
   }
 }
 
 // boundary flux points: gf already holds the complete LDG viscous flux with the ghost state (App C)
-template <int ND>
-__global__ void k_common_flux_bnd_g(DevConsts c, double *__restrict__ uf, const double *__restrict__ gf) {
+template <int ND, typename TI>
+__global__ void k_common_flux_bnd_g(DevConsts c, TI *__restrict__ uf, const TI *__restrict__ gf) {
   constexpr int NV = ND + 2;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= c.nbnd) return;
@@ -256,7 +253,7 @@ __global__ void k_common_flux_bnd_g(DevConsts c, double *__restrict__ uf, const 
   const size_t vs = fp_rstride(c.blk, c.ld);
   double uL[NV], gi[NV], gl[NV], nrm[ND], F[NV];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) uL[a] = uf[o + (size_t)a * vs];
+  for (int a = 0; a < NV; ++a) uL[a] = (double)uf[o + (size_t)a * vs];
   double uc[NV];
   from_pert<ND>(c.ph, uL, uc);
   ghost_states<ND>(c.bcs[c.bbc[i]], uc, c.ph.gamma, gi, gl);
@@ -267,7 +264,7 @@ __global__ void k_common_flux_bnd_g(DevConsts c, double *__restrict__ uf, const 
   rusanov<ND>(uL, gi, nrm, c.ph, F);
   const double jn = c.bJn[i];
 #pragma unroll
-  for (int a = 0; a < NV; ++a) uf[o + (size_t)a * vs] = jn * (F[a] + c.ph.tau * (uL[a] - gl[a]) - gf[o + (size_t)a * vs]);
+  for (int a = 0; a < NV; ++a) uf[o + (size_t)a * vs] = (TI)(jn * (F[a] + c.ph.tau * (uL[a] - gl[a]) - (double)gf[o + (size_t)a * vs]));
 }
 
 template <typename TIN, typename TOUT, bool SCALE>
@@ -300,11 +297,11 @@ cudaError_t run(const DevConsts &c, const WorkLayout &w, const T *u, T *rhs, cha
       FR_MARK(prof, "el_gradface");
       if ((e = element_gradface(c, u, cf, uf, qu, qf, s)) != cudaSuccess) return e;
       FR_MARK(prof, "common_flux_g");
-      launch_common_flux_g(c, uf, qf, s);
+      launch_common_flux_g(c, uf, qf, false, s);
     } else {
       FR_MARK(prof, "common_flux");
-      if (c.npairs) k_common_flux<ND, NS><<<blocks(c.npairs), TB, 0, s>>>(c, uf, qf);
-      if (c.nbnd) k_common_flux_bnd<ND, NS><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, qf);
+      if (c.npairs) k_common_flux<ND, NS, double><<<blocks(c.npairs), TB, 0, s>>>(c, uf, qf);
+      if (c.nbnd) k_common_flux_bnd<ND, NS, double><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, qf);
     }
     FR_MARK(prof, "el_fluxdiv");
     e = element_fluxdiv(c, u, qu, uf, rhs, s);
@@ -332,8 +329,8 @@ cudaError_t run(const DevConsts &c, const WorkLayout &w, const T *u, T *rhs, cha
   k_tflux<ND, NS, T><<<blocks(npts), TB, 0, s>>>(c, u, qu);
   // (5) D~ = J n F(...)  in place over U^f                               Eq 15-17
   FR_MARK(prof, "common_flux");
-  if (c.npairs) k_common_flux<ND, NS><<<blocks(c.npairs), TB, 0, s>>>(c, uf, qf);
-  if (c.nbnd) k_common_flux_bnd<ND, NS><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, qf);
+  if (c.npairs) k_common_flux<ND, NS, double><<<blocks(c.npairs), TB, 0, s>>>(c, uf, qf);
+  if (c.nbnd) k_common_flux_bnd<ND, NS, double><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, qf);
   // (6,7) R = -(1/J) {(M1 - M3 M2) F~ + M3 D~}                           Eq 44, Eq 19
   FR_MARK(prof, "apply_M132_M3_negdivconf");
   apply<double, T, true>(s, c, Nu, ND * Nu, c.M132, qu, Nf, c.M3, uf, rhs);
@@ -355,38 +352,45 @@ void launch_common_jump(const DevConsts &c, const double *uf, double *cf, cudaSt
 }
 
 template <int ND, bool NS>
-static void launch_flux_t(const DevConsts &c, const void *u, double *qu, double *uf, const double *qf, bool do_tflux, bool do_common, cudaStream_t s) {
+static void launch_tflux_t(const DevConsts &c, const void *u, double *qu, cudaStream_t s) {
   const int TB = 128;
   const int64_t npts = (int64_t)c.Nu * c.ld;
-  if (do_tflux) {
-    if (c.f64) k_tflux<ND, NS, double><<<(unsigned)((npts + TB - 1) / TB), TB, 0, s>>>(c, (const double *)u, qu);
-    else k_tflux<ND, NS, float><<<(unsigned)((npts + TB - 1) / TB), TB, 0, s>>>(c, (const float *)u, qu);
-  }
-  if (do_common) {
-    if (c.npairs) k_common_flux<ND, NS><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, uf, qf);
-    if (c.nbnd) k_common_flux_bnd<ND, NS><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, uf, qf);
-  }
+  if (c.f64) k_tflux<ND, NS, double><<<(unsigned)((npts + TB - 1) / TB), TB, 0, s>>>(c, (const double *)u, qu);
+  else k_tflux<ND, NS, float><<<(unsigned)((npts + TB - 1) / TB), TB, 0, s>>>(c, (const float *)u, qu);
 }
 
 void launch_tflux(const DevConsts &c, const void *u, double *qu, cudaStream_t s) {
-  if (c.nd == 2) { if (c.ns) launch_flux_t<2, true>(c, u, qu, nullptr, nullptr, true, false, s); else launch_flux_t<2, false>(c, u, qu, nullptr, nullptr, true, false, s); }
-  else { if (c.ns) launch_flux_t<3, true>(c, u, qu, nullptr, nullptr, true, false, s); else launch_flux_t<3, false>(c, u, qu, nullptr, nullptr, true, false, s); }
+  if (c.nd == 2) { if (c.ns) launch_tflux_t<2, true>(c, u, qu, s); else launch_tflux_t<2, false>(c, u, qu, s); }
+  else { if (c.ns) launch_tflux_t<3, true>(c, u, qu, s); else launch_tflux_t<3, false>(c, u, qu, s); }
 }
 
-void launch_common_flux(const DevConsts &c, double *uf, const double *qf, cudaStream_t s) {
-  if (c.nd == 2) { if (c.ns) launch_flux_t<2, true>(c, nullptr, nullptr, uf, qf, false, true, s); else launch_flux_t<2, false>(c, nullptr, nullptr, uf, qf, false, true, s); }
-  else { if (c.ns) launch_flux_t<3, true>(c, nullptr, nullptr, uf, qf, false, true, s); else launch_flux_t<3, false>(c, nullptr, nullptr, uf, qf, false, true, s); }
-}
-
-void launch_common_flux_g(const DevConsts &c, double *uf, const double *gf, cudaStream_t s) {
+template <int ND, bool NS, typename TI>
+static void launch_common_flux_t(const DevConsts &c, void *uf, const void *qf, cudaStream_t s) {
   const int TB = 128;
-  if (c.nd == 2) {
-    if (c.npairs) k_common_flux_g<2><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
-    if (c.nbnd) k_common_flux_bnd_g<2><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
-  } else {
-    if (c.npairs) k_common_flux_g<3><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
-    if (c.nbnd) k_common_flux_bnd_g<3><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, uf, gf);
+  if (c.npairs) k_common_flux<ND, NS, TI><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, (TI *)uf, (const TI *)qf);
+  if (c.nbnd) k_common_flux_bnd<ND, NS, TI><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, (TI *)uf, (const TI *)qf);
+}
+
+void launch_common_flux(const DevConsts &c, void *uf, const void *qf, bool f32, cudaStream_t s) {
+  if (f32) {  // Euler on the hexahedral TMA path in single precision
+    if (c.nd == 3 && !c.ns) launch_common_flux_t<3, false, float>(c, uf, qf, s);
+    return;
   }
+  if (c.nd == 2) { if (c.ns) launch_common_flux_t<2, true, double>(c, uf, qf, s); else launch_common_flux_t<2, false, double>(c, uf, qf, s); }
+  else { if (c.ns) launch_common_flux_t<3, true, double>(c, uf, qf, s); else launch_common_flux_t<3, false, double>(c, uf, qf, s); }
+}
+
+template <int ND, typename TI>
+static void launch_common_flux_g_t(const DevConsts &c, void *uf, const void *gf, cudaStream_t s) {
+  const int TB = 128;
+  if (c.npairs) k_common_flux_g<ND, TI><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, (TI *)uf, (const TI *)gf);
+  if (c.nbnd) k_common_flux_bnd_g<ND, TI><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, (TI *)uf, (const TI *)gf);
+}
+
+void launch_common_flux_g(const DevConsts &c, void *uf, const void *gf, bool f32, cudaStream_t s) {
+  if (c.nd == 2) launch_common_flux_g_t<2, double>(c, uf, gf, s);
+  else if (f32) launch_common_flux_g_t<3, float>(c, uf, gf, s);
+  else launch_common_flux_g_t<3, double>(c, uf, gf, s);
 }
 
 int generic_rhs_launches(const DevConsts &c) {

@@ -15,7 +15,7 @@ struct FdLay {
   static constexpr size_t BAR = 0;
   static constexpr size_t OPS = 128;  // sDh [N*N], sGm [N], sGp [N]
   static constexpr size_t ST = OPS + al128((N * N + 2 * N) * 8);
-  static constexpr uint32_t S_TX = 9 * NFP * E * 8, U_TX = NFP * NV * E * sizeof(T), Q_TX = NS ? 3 * NV * NFP * E * 8 : 0;
+  static constexpr uint32_t S_TX = 9 * NFP * E * sizeof(T), U_TX = NFP * NV * E * sizeof(T), Q_TX = NS ? 3 * NV * NFP * E * sizeof(T) : 0;
   static constexpr size_t ST_U = al128(S_TX);
   static constexpr size_t ST_Q = ST_U + al128(U_TX);
   static constexpr size_t ST_BYTES = ST_Q + al128(Q_TX);
@@ -24,7 +24,7 @@ struct FdLay {
   // epilogue operands by TMA: D~ of the x/y faces, 1/J, D~ of the z faces.  EPI_ST: all into the stage buffers once they
   // are free (Navier-Stokes: the stages are large).  EPI_DED: the stages are too small for D~ of the x/y faces (Euler), which
   // gets a buffer of its own, loaded at kernel start; 1/J and the z faces still reuse the freed stages.
-  static constexpr uint32_t DXY_TX = 4 * NFP * NV * E * 8, RJ_TX = NU * E * 8, DZ_TX = 2 * NFP * NV * E * 8;
+  static constexpr uint32_t DXY_TX = 4 * NFP * NV * E * sizeof(T), RJ_TX = NU * E * sizeof(T), DZ_TX = 2 * NFP * NV * E * sizeof(T);
   static constexpr size_t EP_RJ = al128(DXY_TX);
   static constexpr bool EPI_ST = N >= 2 && EP_RJ + RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
   static constexpr bool EPI_DED = N >= 2 && !EPI_ST && RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     k_hex_fluxdiv_tma(const __grid_constant__ CUtensorMap tmS, const __grid_constant__ CUtensorMap tmU,
                       const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmD4,
                       const __grid_constant__ CUtensorMap tmD2, const __grid_constant__ CUtensorMap tmR, Ops1D<N> op, Phys ph,
-                      const double *__restrict__ rcpj, bool aff, const double *__restrict__ dt, T *__restrict__ rhs, int64_t ld,
+                      const T *__restrict__ rcpj, bool aff, const T *__restrict__ dt, T *__restrict__ rhs, int64_t ld,
                       int64_t Nel) {
   using L = FdLay<N, E, NS, T, NB>;
   constexpr int NFP = N * N;
@@ -85,32 +85,34 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
   for (int k = 0; k < N; ++k) {
     mbar_wait(&bar[k & 1], (k >> 1) & 1);
-    const double *stS = (const double *)(sSt + (k & 1) * L::ST_BYTES);
+    const T *stS = (const T *)(sSt + (k & 1) * L::ST_BYTES);
     const T *stU = (const T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_U);
-    const double *stQ = (const double *)(sSt + (k & 1) * L::ST_BYTES + L::ST_Q);
+    const T *stQ = (const T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_Q);
     double *buf = sF + (NB == 2 ? (k & 1) : 0) * (2 * NV * NFP * E);
     {
       double S[3][3], uu[NV];
 #pragma unroll
       for (int a = 0; a < 3; ++a)
 #pragma unroll
-        for (int b = 0; b < 3; ++b) S[a][b] = stS[((a * 3 + b) * NFP + ij) * E + el];
+        for (int b = 0; b < 3; ++b) S[a][b] = (double)stS[((a * 3 + b) * NFP + ij) * E + el];
 #pragma unroll
       for (int a = 0; a < NV; ++a) uu[a] = (double)stU[(ij * NV + a) * E + el];
       // primitive variables (Eq 20-21) through the perturbation variables w about the reference state (fr_physics.cuh):
       // v = v0 + w_m / rho,  pp = p - p0;  with no reference state w = u and pp = p
-      const double rrho = 1.0 / uu[0], En = uu[4];
-      double ww[NV], v[3], ke = 0, vw = 0;
+      const double rrho = 1.0 / uu[0];
+      double ww[NV], v[3], dvl[3], ke = 0, vw = 0;
       to_pert<3>(ph, uu, ww);
+      const double Es = (ww[4] - ph.p0) * rrho;
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
-        const double dv = ww[1 + d] * rrho;
-        v[d] = ph.v0[d] + dv;
-        ke += ww[1 + d] * dv;
+        dvl[d] = ww[1 + d] * rrho;
+        v[d] = ph.v0[d] + dvl[d];
+        ke += ww[1 + d] * dvl[d];
         vw += ph.v0[d] * ww[1 + d];
       }
       const double pp = (ph.gamma - 1.0) * (fma(ph.hs0, ww[0], ww[4]) - vw - 0.5 * ke);
-      // viscous stress Tm and energy flux w = v.Tm + (mu gamma / Pr) grad e  (Eq 22-24, A8), built variable by variable
+      // viscous stress Tm and energy flux w = v.Tm + (mu gamma / Pr) grad e  (Eq 22-24, A8), built variable by variable from
+      // the gradient of the perturbation variables (formulas of subtract_viscous_flux, fr_physics.cuh)
       double Tm[3][3], w[3];
       if (NS) {
         double g0[3], dv[3][3], de[3];
@@ -118,10 +120,10 @@ __global__ void __launch_bounds__(N *N *E, MINB)
         for (int a = 0; a < NV; ++a)
 #pragma unroll
           for (int n = 0; n < 3; ++n) {
-            const double g = stQ[((n * NFP + ij) * NV + a) * E + el];
+            const double g = (double)stQ[((n * NFP + ij) * NV + a) * E + el];
             if (a == 0) g0[n] = g;
-            else if (a < 4) dv[n][a - 1] = (g - v[a - 1] * g0[n]) * rrho;  // d_n v_j by the quotient rule
-            else de[n] = (g - (En * rrho) * g0[n]) * rrho;
+            else if (a < 4) dv[n][a - 1] = (g - dvl[a - 1] * g0[n]) * rrho;  // d_n v_j by the quotient rule (Q = grad w)
+            else de[n] = (g - Es * g0[n]) * rrho;
           }
         const double lam = -2.0 / 3.0 * ph.mu * (dv[0][0] + dv[1][1] + dv[2][2]);
 #pragma unroll
@@ -186,9 +188,9 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   // lifting M3 D~ and the -1/J scale (Eq 19); faces: 0,1 = x-,x+ (idx j + N k); 2,3 = y (i + N k); 4,5 = z (i + N j)
   const double gmi = sGm[i], gpi = sGp[i], gmj = sGm[j], gpj = sGp[j];
   if (L::EPI_TMA) {
-    const double *sDxy = (const double *)(L::EPI_DED ? sm + L::DED : sSt + ((N - 2) & 1) * L::ST_BYTES);  // [4][NFP*NV][E]
-    const double *sRJ = (const double *)(sSt + ((N - 2) & 1) * L::ST_BYTES + (L::EPI_DED ? 0 : L::EP_RJ));  // [NU][E]
-    const double *sDz = (const double *)(sSt + ((N - 1) & 1) * L::ST_BYTES);                               // [2][NFP*NV][E]
+    const T *sDxy = (const T *)(L::EPI_DED ? sm + L::DED : sSt + ((N - 2) & 1) * L::ST_BYTES);  // [4][NFP*NV][E]
+    const T *sRJ = (const T *)(sSt + ((N - 2) & 1) * L::ST_BYTES + (L::EPI_DED ? 0 : L::EP_RJ));  // [NU][E]
+    const T *sDz = (const T *)(sSt + ((N - 1) & 1) * L::ST_BYTES);                                         // [2][NFP*NV][E]
     mbar_wait(&bar[2], 0);
     mbar_wait(&bar[3], 0);
     mbar_wait(&bar[4], 0);
@@ -196,18 +198,18 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
     for (int k = 0; k < N; ++k) {
       const int r = ij + NFP * k;
-      const double rj = sRJ[r * E + el];
+      const double rj = (double)sRJ[r * E + el];
       const int fx = j + N * k, fy = i + N * k;
       double r0 = 0;  // R~ of the mass equation: R_mj = R_wmj + v0_j R_wrho, R_E = R_wE + h0 R_wrho (fr_physics.cuh)
 #pragma unroll
       for (int a = 0; a < NV; ++a) {
         double v = acc[k][a];
-        v = fma(op.gm[k], sDz[((0 * NFP + ij) * NV + a) * E + el], v);
-        v = fma(op.gp[k], sDz[((1 * NFP + ij) * NV + a) * E + el], v);
-        v = fma(gmi, sDxy[((0 * NFP + fx) * NV + a) * E + el], v);
-        v = fma(gpi, sDxy[((1 * NFP + fx) * NV + a) * E + el], v);
-        v = fma(gmj, sDxy[((2 * NFP + fy) * NV + a) * E + el], v);
-        v = fma(gpj, sDxy[((3 * NFP + fy) * NV + a) * E + el], v);
+        v = fma(op.gm[k], (double)sDz[((0 * NFP + ij) * NV + a) * E + el], v);
+        v = fma(op.gp[k], (double)sDz[((1 * NFP + ij) * NV + a) * E + el], v);
+        v = fma(gmi, (double)sDxy[((0 * NFP + fx) * NV + a) * E + el], v);
+        v = fma(gpi, (double)sDxy[((1 * NFP + fx) * NV + a) * E + el], v);
+        v = fma(gmj, (double)sDxy[((2 * NFP + fy) * NV + a) * E + el], v);
+        v = fma(gpj, (double)sDxy[((3 * NFP + fy) * NV + a) * E + el], v);
         if (a == 0) r0 = v;
         else v = fma(a < 4 ? ph.v0[a - 1] : ph.h0, r0, v);
         rhs[((size_t)r * NV + a) * ld + e] = (T)(-v * rj);
@@ -219,13 +221,13 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   double dzm[NV], dzp[NV];
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
-    dzm[a] = dt[fp_row(true, ld, 6 * NFP * NV, (4 * NFP + ij) * NV + a, e)];
-    dzp[a] = dt[fp_row(true, ld, 6 * NFP * NV, (5 * NFP + ij) * NV + a, e)];
+    dzm[a] = (double)dt[fp_row(true, ld, 6 * NFP * NV, (4 * NFP + ij) * NV + a, e)];
+    dzp[a] = (double)dt[fp_row(true, ld, 6 * NFP * NV, (5 * NFP + ij) * NV + a, e)];
   }
 #pragma unroll
   for (int k = 0; k < N; ++k) {
     const int r = ij + NFP * k;
-    const double rj = aff ? rcpj[fp_row(true, ld, 1, 0, e)] : rcpj[fp_row(true, ld, N * NFP, r, e)];
+    const double rj = (double)(aff ? rcpj[fp_row(true, ld, 1, 0, e)] : rcpj[fp_row(true, ld, N * NFP, r, e)]);
     const int fx = j + N * k, fy = i + N * k;
     double r0 = 0;
 #pragma unroll
@@ -233,10 +235,10 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       double v = acc[k][a];
       v = fma(op.gm[k], dzm[a], v);
       v = fma(op.gp[k], dzp[a], v);
-      v = fma(gmi, dt[fp_row(true, ld, 6 * NFP * NV, (0 * NFP + fx) * NV + a, e)], v);
-      v = fma(gpi, dt[fp_row(true, ld, 6 * NFP * NV, (1 * NFP + fx) * NV + a, e)], v);
-      v = fma(gmj, dt[fp_row(true, ld, 6 * NFP * NV, (2 * NFP + fy) * NV + a, e)], v);
-      v = fma(gpj, dt[fp_row(true, ld, 6 * NFP * NV, (3 * NFP + fy) * NV + a, e)], v);
+      v = fma(gmi, (double)dt[fp_row(true, ld, 6 * NFP * NV, (0 * NFP + fx) * NV + a, e)], v);
+      v = fma(gpi, (double)dt[fp_row(true, ld, 6 * NFP * NV, (1 * NFP + fx) * NV + a, e)], v);
+      v = fma(gmj, (double)dt[fp_row(true, ld, 6 * NFP * NV, (2 * NFP + fy) * NV + a, e)], v);
+      v = fma(gpj, (double)dt[fp_row(true, ld, 6 * NFP * NV, (3 * NFP + fy) * NV + a, e)], v);
       if (a == 0) r0 = v;
       else v = fma(a < 4 ? ph.v0[a - 1] : ph.h0, r0, v);
       rhs[((size_t)r * NV + a) * ld + e] = (T)(-v * rj);
@@ -245,7 +247,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 }
 
 template <int N, int E, bool NS, typename T>
-cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *u, const double *q, const double *dt, void *rhs,
+cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *u, const void *q, const void *dt, void *rhs,
                            cudaStream_t s) {
   constexpr int NFP = N * N, NU = N * NFP;
   using L2 = FdLay<N, E, NS, T, 2>;
@@ -258,33 +260,34 @@ cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *
   const uint64_t ld = (uint64_t)c.ld;
   CUtensorMap mS, mU, mQ, mD4, mD2, mR;
   static_assert(FR_BLK % E == 0, "a CTA's elements must lie in one element block");
-  bool ok = encode_blk(&mS, c.smat, ld, NU, 9, E, NFP, 9, c.aff ? 1 : 0);
+  constexpr bool F64 = sizeof(T) == 8;
+  bool ok = encode_blk(&mS, F64, c.smat, ld, NU, 9, E, NFP, 9, c.aff ? 1 : 0);  // metric terms in T on this path (fr_api.cu)
   ok = ok && encode3(&mU, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 1);  // caller layout
-  if (NS) ok = ok && encode_blk(&mQ, q, ld, NV * NFP, 3 * N, E, NV * NFP, 3);
+  if (NS) ok = ok && encode_blk(&mQ, F64, q, ld, NV * NFP, 3 * N, E, NV * NFP, 3);
   else mQ = mS;
-  ok = ok && encode_blk(&mD4, dt, ld, NFP * NV, 6, E, NFP * NV, 4);
-  ok = ok && encode_blk(&mD2, dt, ld, NFP * NV, 6, E, NFP * NV, 2);
-  ok = ok && encode_blk(&mR, c.rcpj, ld, NFP, N, E, NFP, N, c.aff ? 2 : 0);
+  ok = ok && encode_blk(&mD4, F64, dt, ld, NFP * NV, 6, E, NFP * NV, 4);
+  ok = ok && encode_blk(&mD2, F64, dt, ld, NFP * NV, 6, E, NFP * NV, 2);
+  ok = ok && encode_blk(&mR, F64, c.rcpj, ld, NFP, N, E, NFP, N, c.aff ? 2 : 0);
   if (!ok) return cudaErrorNotSupported;
   auto kern = k_hex_fluxdiv_tma<N, E, NS, T, NB, MINB>;
   static DevFlags done;
   cudaError_t err = set_smem(kern, L::TOTAL, done, c.dev);
   if (err != cudaSuccess) return err;
   const Ops1D<N> op = make_ops<N>(h_ops);
-  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(mS, mU, mQ, mD4, mD2, mR, op, c.ph, c.rcpj, c.aff, dt, (T *)rhs, c.ld,
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(mS, mU, mQ, mD4, mD2, mR, op, c.ph, (const T *)c.rcpj, c.aff, (const T *)dt, (T *)rhs, c.ld,
                                                                   c.Nel);
   return cudaGetLastError();
 }
 
 template <int N, typename T>
 constexpr bool fd_fits() {
-  return FdLay<N, Cfg<N>::E, true, T, 1>::TOTAL <= SMEM_MAX && N * N * Cfg<N>::E <= 1024 && N * N * NV <= 256;
+  return FdLay<N, Cfg<N, T>::E, true, T, 1>::TOTAL <= SMEM_MAX && N * N * Cfg<N, T>::E <= 1024 && N * N * NV <= 256;
 }
 
 template <int N, typename T>
-cudaError_t fluxdiv_n(const DevConsts &c, const double *h_ops, const void *u, const double *q, const double *dt, void *rhs, cudaStream_t s) {
+cudaError_t fluxdiv_n(const DevConsts &c, const double *h_ops, const void *u, const void *q, const void *dt, void *rhs, cudaStream_t s) {
   if constexpr (fd_fits<N, T>()) {
-    constexpr int E = Cfg<N>::E;
+    constexpr int E = Cfg<N, T>::E;
     return c.ns ? launch_fluxdiv<N, E, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, E, false, T>(c, h_ops, u, q, dt, rhs, s);
   } else {
     return cudaErrorNotSupported;
@@ -303,7 +306,7 @@ bool hex_tma_fluxdiv_supported(int n, bool f64) {
   }
 }
 
-cudaError_t hex_tma_fluxdiv(const DevConsts &c, const double *h_ops, const void *u, const double *q, const double *dt, void *rhs,
+cudaError_t hex_tma_fluxdiv(const DevConsts &c, const double *h_ops, const void *u, const void *q, const void *dt, void *rhs,
                             cudaStream_t s) {
   switch (c.n) {
 #define FR_CASE(NN) case NN: return c.f64 ? fluxdiv_n<NN, double>(c, h_ops, u, q, dt, rhs, s) : fluxdiv_n<NN, float>(c, h_ops, u, q, dt, rhs, s);

@@ -3,7 +3,7 @@
 // z-slab kernel.  A CTA owns E consecutive elements; their whole U block ([N_u*N_V] rows of E values, caller layout)
 // arrives by ONE 3-D TMA box load; thread (e, i, j) interpolates its column to the two z faces from shared memory,
 // and the 4 N x/y-face flux points of every slice are interpolated along their lines by one thread each.  U^f is
-// written element-blocked (fr_dev.hpp: fp_row).  Several CTAs are resident per SM (40 KB at p = 4), so the load of
+// written element-blocked (fr_dev.hpp: fp_row) in the storage precision T of the context (all arithmetic in double).  Several CTAs are resident per SM (40 KB at p = 4), so the load of
 // one CTA overlaps the arithmetic and the stores of the others.
 #include "fr_tma.cuh"
 
@@ -12,7 +12,7 @@ namespace {
 
 template <int N, int E, typename T>
 __global__ void __launch_bounds__(N *N *E) k_hex_interp_tma(const __grid_constant__ CUtensorMap tmU, Ops1D<N> op, Phys ph,
-                                                            double *__restrict__ uf, int64_t ld, int64_t Nel) {
+                                                            T *__restrict__ uf, int64_t ld, int64_t Nel) {
   constexpr int NFP = N * N, NU = N * NFP, NF = 6 * NFP;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char *sm = smem_raw + ((128u - (smem_addr(smem_raw) & 127u)) & 127u);
@@ -54,8 +54,8 @@ __global__ void __launch_bounds__(N *N *E) k_hex_interp_tma(const __grid_constan
     }
 #pragma unroll
     for (int a = 0; a < NV; ++a) {
-      uf[fp_row(true, ld, NF * NV, (4 * NFP + ij) * NV + a, e)] = zm[a];
-      uf[fp_row(true, ld, NF * NV, (5 * NFP + ij) * NV + a, e)] = zp[a];
+      uf[fp_row(true, ld, NF * NV, (4 * NFP + ij) * NV + a, e)] = (T)zm[a];
+      uf[fp_row(true, ld, NF * NV, (5 * NFP + ij) * NV + a, e)] = (T)zp[a];
     }
   }
   // x / y faces: 4 N flux points per slice, N slices; task t = (slice k, face f, line m)
@@ -78,12 +78,12 @@ __global__ void __launch_bounds__(N *N *E) k_hex_interp_tma(const __grid_constan
     }
     const int fp = f * NFP + m + N * k;
 #pragma unroll
-    for (int a = 0; a < NV; ++a) uf[fp_row(true, ld, NF * NV, fp * NV + a, e)] = v[a];
+    for (int a = 0; a < NV; ++a) uf[fp_row(true, ld, NF * NV, fp * NV + a, e)] = (T)v[a];
   }
 }
 
 template <int N, int E, typename T>
-cudaError_t launch_interp(const DevConsts &c, const double *h_ops, const void *u, double *uf, cudaStream_t s) {
+cudaError_t launch_interp(const DevConsts &c, const double *h_ops, const void *u, void *uf, cudaStream_t s) {
   constexpr int NFP = N * N, NU = N * NFP;
   constexpr size_t SMEM = 128 + al128(2 * N * 8) + al128(NU * NV * E * sizeof(T)) + 128;
   static_assert(SMEM <= SMEM_MAX && FR_BLK % E == 0, "configuration");
@@ -94,16 +94,16 @@ cudaError_t launch_interp(const DevConsts &c, const double *h_ops, const void *u
   static DevFlags done;
   cudaError_t err = set_smem(kern, SMEM, done, c.dev);
   if (err != cudaSuccess) return err;
-  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, SMEM, s>>>(mU, make_ops<N>(h_ops), c.ph, uf, c.ld, c.Nel);
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, SMEM, s>>>(mU, make_ops<N>(h_ops), c.ph, (T *)uf, c.ld, c.Nel);
   return cudaGetLastError();
 }
 
 }  // namespace
 
-cudaError_t hex_tma_interp(const DevConsts &c, const double *h_ops, const void *u, double *uf, cudaStream_t s) {
+cudaError_t hex_tma_interp(const DevConsts &c, const double *h_ops, const void *u, void *uf, cudaStream_t s) {
   switch (c.n) {
 #define FR_CASE(NN) \
-  case NN: return c.f64 ? launch_interp<NN, Cfg<NN>::E, double>(c, h_ops, u, uf, s) : launch_interp<NN, Cfg<NN>::E, float>(c, h_ops, u, uf, s);
+  case NN: return c.f64 ? launch_interp<NN, Cfg<NN, double>::E, double>(c, h_ops, u, uf, s) : launch_interp<NN, Cfg<NN, float>::E, float>(c, h_ops, u, uf, s);
     FR_CASE(2) FR_CASE(3) FR_CASE(4) FR_CASE(5) FR_CASE(6) FR_CASE(7)
 #undef FR_CASE
     default: return cudaErrorNotSupported;

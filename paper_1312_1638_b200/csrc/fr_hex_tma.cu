@@ -1,20 +1,29 @@
-// TMA-fed, mbarrier-pipelined "z-slab" kernels for hexahedral elements (sm_100a).
+// TMA-fed, mbarrier-pipelined "z-slab" kernel for hexahedral elements (sm_100a): parts (2)-(3) of the Navier-Stokes
+// right-hand side and the viscous half of part (5) (BASELINE.json north_star) in ONE launch.
 //
-// Two kernels carry parts (2b)-(7) of the Navier-Stokes right-hand side (BASELINE.json north_star):
-//
-//   k_hex_gradface : Q = J^-T {M4 U + M6 (C - U^f)} at the solution points (Eq 9-10 / Eq 42 :753), interpolated
-//                    to the element's own flux points (Eq 11 / Eq 43 :764) and contracted at once with the
-//                    outward unit normal: G^f = n . f_vis(U^f, Q^f)  (Eq 22-24, the viscous part of Eq 26-27).
-//                    Only G^f (N_V values per flux point) goes to HBM: neither Q (3 N_V N_u) nor Q^f
-//                    (3 N_V N_f) is ever stored.  Boundary flux points get the complete LDG viscous flux
-//                    with the ghost state of App C.
+//   k_hex_gradface : common solution and its jump at the element's own flux points (Eq 7, 25), gathered from the partner's
+//                    U^f;  Q = J^-T {M4 U + M6 (C - U^f)} at the solution points (Eq 9-10 / Eq 42 :753), stored slice-major for
+//                    k_hex_fluxdiv_tma;  Q interpolated to the element's own flux points (Eq 11 / Eq 43 :764) and contracted at
+//                    once with the outward unit normal: G^f = n . f_vis(U^f, Q^f)  (Eq 22-24, the viscous part of Eq 26-27).
+//                    Q^f (3 N_V N_f) and the common solution C^f (N_V N_f) are never stored.  Boundary flux points get the
+//                    complete LDG viscous flux with the ghost state of App C.
 //   (k_hex_fluxdiv_tma, fr_hex_fluxdiv_tma.cu: F~ = S f(U, Q), R = -(1/J) {(M1 - M3 M2) F~ + M3 D~}.)
 //
-// Data movement: a CTA owns E consecutive elements.  The U block of those elements ([N_u*N_V] rows of E
-// values) is brought into shared memory by ONE 3-D TMA box load; the metric terms S (9 rows per point), 1/J
-// and the x/y-face jumps stream slice by slice (z = k) through a two-stage ring of TMA box loads completing on
-// mbarriers, issued two slices ahead by one thread, so HBM latency is covered without registers or occupancy.
-// Thread (e, i, j) owns the column of points (i, j, .); contractions along x and y read shared memory,
+// The jump C - U^f of Eq 9 at a flux point is  w_f (u_partner - u_own)  with  w_f = 1/2 + beta on the L side of its interface
+// and 1/2 - beta on the R side (Eq 25): it needs the partner's U^f only where w_f != 0 (the paper's beta = 1/2: on L sides), and
+// the same faces are the ones whose G^f carries a non-zero LDG weight (Eq 27).  The partner values are gathered by per-thread
+// cp.async copies issued one slice ahead (offsets from the element-centric table fp_poff); there is no separate
+// common-solution kernel and no jump array in HBM.
+//
+// Arithmetic: in the context's storage precision T.  Everything this kernel produces (Q, G^f) enters the right-hand side
+// through the viscous flux only, whose share of the RHS is O(1/Re_h): single-precision arithmetic on the perturbation
+// variables (O(1) values) keeps the single-precision bar of 1e-5 with a wide margin, and avoids a float <-> double conversion
+// per shared-memory operand.  The inviscid path (k_hex_interp_tma, the pair kernels, k_hex_fluxdiv_tma) computes in double.
+//
+// Data movement: a CTA owns E consecutive elements.  The U block of those elements ([N_u*N_V] rows of E values) is brought
+// into shared memory by ONE 3-D TMA box load; the metric terms S (9 rows per point) and 1/J stream slice by slice (z = k)
+// through TMA box loads completing on mbarriers, issued ahead by one thread, so HBM latency is covered without registers or
+// occupancy.  Thread (e, i, j) owns the column of points (i, j, .); contractions along x and y read shared memory,
 // contractions along z use operator entries from the constant bank.
 #include "fr_tma.cuh"
 
@@ -22,7 +31,7 @@ namespace fr {
 namespace {
 
 // ---------------------------------------------------------------------------------------------
-// shared-memory layouts (byte offsets from a 128-byte aligned base)
+// shared-memory layout (byte offsets from a 128-byte aligned base)
 // ---------------------------------------------------------------------------------------------
 template <int N, int E, typename T>
 struct GfLay {
@@ -31,48 +40,51 @@ struct GfLay {
   static constexpr size_t OPS = 128;  // sD [N*N], sL [2][N], sGm [N], sGp [N]
   static constexpr size_t U = OPS + al128((N * N + 4 * N) * 8);
   static constexpr uint32_t U_TX = NU * NV * E * sizeof(T);
-  static constexpr size_t JZ = U + al128(U_TX);                   // jumps of the two z faces [2][NFP*NV][E], loaded once
-  static constexpr uint32_t JZ_TX = 2 * NFP * NV * E * 8;
-  static constexpr size_t SS = JZ + al128(JZ_TX);                 // S of the current slice: ONE buffer, refilled during the face phase
-  static constexpr uint32_t S_TX = 9 * NFP * E * 8, R_TX = NFP * E * 8, J_TX = 4 * N * NV * E * 8;
-  static constexpr size_t ST = SS + al128(S_TX);                  // two stages of {1/J, x/y-face jumps}
-  static constexpr size_t ST_J = al128(R_TX);
-  static constexpr size_t ST_BYTES = ST_J + al128(J_TX);
+  static constexpr size_t PZ = U + al128(U_TX);                   // partner U^f of the two z faces [2][NFP][NV][E], then their jumps
+  static constexpr size_t PZ_BYTES = 2 * NFP * NV * E * sizeof(T);
+  static constexpr size_t SS = PZ + al128(PZ_BYTES);              // S of the current slice: ONE buffer, refilled during the face phase
+  static constexpr uint32_t S_TX = 9 * NFP * E * sizeof(T), R_TX = NFP * E * sizeof(T);  // metric terms in the storage precision
+  static constexpr size_t ST = SS + al128(S_TX);                  // two stages of {1/J (TMA), partner U^f of the x/y faces -> jumps (cp.async)}
+  static constexpr size_t ST_P = al128(R_TX);
+  static constexpr size_t P_BYTES = 4 * N * NV * E * sizeof(T);   // [slot 0..3 = faces 1, 3, 0, 2][N][NV][E]
+  static constexpr size_t ST_BYTES = ST_P + al128(P_BYTES);
   static constexpr size_t Q = ST + 2 * ST_BYTES;
-  static constexpr size_t Q_BYTES = 3 * NV * NFP * E * 8;
-  static constexpr size_t TOTAL = Q + Q_BYTES + 128;
+  static constexpr size_t Q_BYTES = 3 * NV * NFP * E * sizeof(T);
+  static constexpr size_t TOTAL = Q + al128(Q_BYTES) + 128;
 };
 
 // ---------------------------------------------------------------------------------------------
 // k_hex_gradface
 // ---------------------------------------------------------------------------------------------
-// tmU, tmS, tmJ as above; tmR: rcpj as (ld, NFP, N), box (E, NFP, 1).
-// SQ: also store Q slice by slice (bulk tensor store of the shared-memory slice) for k_hex_fluxdiv_tma;
-// tmQ: Q workspace as (ld, NV*NFP, 3N), box (E, NV*NFP, 3): slice k, component n, variable a, point ij.
-template <int N, int E, bool BND, bool SQ, typename T, int MINB>
+// tmU: u as (ld, NFP*NV, N) box (E, NFP*NV, N); tmS: smat blocked, box (E, NFP, 9); tmR: rcpj blocked, box (E, NFP, 1);
+// tmQ: Q workspace as (lane, NV*NFP, 3N, block), box (E, NV*NFP, 3): slice k, component n, point ij, variable a.
+// uf: U^f of all elements in perturbation variables (k_hex_interp_tma), element-blocked; fp_poff: for every flux point the
+// offset of its partner's first variable in uf, or -1 - bc_id on a boundary; face_code [6][ld]: 0 = no LDG weight (skip),
+// 1 = L side (1/2 + beta), 2 = R side (1/2 - beta), 3 = boundary.
+template <int N, int E, bool BND, typename T, int MINB>
 __global__ void __launch_bounds__(N *N *E, MINB)
     k_hex_gradface(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS,
-                   const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmJ,
-                   const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmJz, Ops1D<N> op, Phys ph,
-                   const double *__restrict__ jump, const double *__restrict__ fp_n, const int32_t *__restrict__ fp_pe,
-                   const uint8_t *__restrict__ face_need, const BcDev *__restrict__ bcs, double *__restrict__ gf, int64_t ld,
-                   int64_t Nel) {
+                   const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmQ, Ops1D<N, T> op, Phys ph,
+                   const T *__restrict__ uf, const int64_t *__restrict__ fp_poff, const T *__restrict__ fp_n,
+                   const uint8_t *__restrict__ face_code, const BcDev *__restrict__ bcs, T *__restrict__ gf, int64_t ld, int64_t Nel) {
   using L = GfLay<N, E, T>;
+  using R = T;  // arithmetic type of this kernel: the gradient feeds the viscous flux only (see the header comment)
   constexpr int NFP = N * N, NF = 6 * NFP;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char *sm = smem_raw + ((128u - (smem_addr(smem_raw) & 127u)) & 127u);  // stays in the shared address space
   uint64_t *bar = (uint64_t *)(sm + L::BAR);
-  double *sD = (double *)(sm + L::OPS), *sL = sD + N * N;  // sL[0][m] = l_m(-1), sL[1][m] = l_m(+1)
-  double *sGm = sL + 2 * N, *sGp = sGm + N;
-  const T *sU = (const T *)(sm + L::U);
-  const double *sJz = (const double *)(sm + L::JZ);
-  const double *stS = (const double *)(sm + L::SS);
+  R *sD = (R *)(sm + L::OPS), *sL = sD + N * N;  // sL[0][m] = l_m(-1), sL[1][m] = l_m(+1)
+  R *sGm = sL + 2 * N, *sGp = sGm + N;
+  T *sU = (T *)(sm + L::U);
+  T *sPz = (T *)(sm + L::PZ);
+  const T *stS = (const T *)(sm + L::SS);
   unsigned char *sSt = sm + L::ST;
-  double *sQ = (double *)(sm + L::Q);  // [3][NFP][NV][E]
+  T *sQ = (T *)(sm + L::Q);  // [3][NFP][NV][E]
   const int tid = threadIdx.x, el = tid % E, ij = tid / E, i = ij % N, j = ij / N;
   const int e0 = blockIdx.x * E, l0 = e0 % FR_BLK, eb = e0 / FR_BLK;  // first element: lane and element block (fp_row)
   const int64_t e = (int64_t)e0 + el;
   const bool act = e < Nel;
+  const R wL = (R)(0.5 + ph.beta), wR = (R)(0.5 - ph.beta);
 
   if (tid == 0) {
     mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); mbar_init(&bar[2], 1); mbar_init(&bar[3], 1);
@@ -83,141 +95,284 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   for (int t = tid; t < N * N; t += NFP * E) sD[t] = op.D[t];
   for (int t = tid; t < N; t += NFP * E) { sL[t] = op.lm[t]; sL[N + t] = op.lp[t]; sGm[t] = op.gm[t]; sGp[t] = op.gp[t]; }
   __syncthreads();
-  auto issue_stage = [&](int s, int k) {
-    mbar_expect_tx(&bar[1 + s], L::R_TX + L::J_TX);
+  auto issue_R = [&](int s, int k) {
+    mbar_expect_tx(&bar[1 + s], L::R_TX);
     tma_load_4d(sSt + s * L::ST_BYTES, &tmR, l0, 0, k, eb, &bar[1 + s]);
-    tma_load_4d(sSt + s * L::ST_BYTES + L::ST_J, &tmJ, l0, N * k * NV, 0, eb, &bar[1 + s]);
   };
   auto issue_S = [&](int k) {
     mbar_expect_tx(&bar[3], L::S_TX);
     tma_load_4d(sm + L::SS, &tmS, l0, NFP * k, 0, eb, &bar[3]);
   };
   if (tid == 0) {
-    mbar_expect_tx(&bar[0], L::U_TX + L::JZ_TX);
+    mbar_expect_tx(&bar[0], L::U_TX);
     tma_load_3d(sm + L::U, &tmU, e0, 0, 0, &bar[0]);
-    tma_load_4d(sm + L::JZ, &tmJz, l0, 0, 4, eb, &bar[0]);
     issue_S(0);
-    issue_stage(0, 0);
-    if (N > 1) issue_stage(1, 1);
+    issue_R(0, 0);
+    if (N > 1) issue_R(1, 1);
   }
-  // G^f of a face is needed only if its LDG weight (1/2 + beta on L sides, 1/2 - beta on R sides, Eq 27) is non-zero or it
-  // lies on a boundary: with the paper's beta = 1/2 half of the faces are skipped.  x/y tasks visit the +1 faces first
-  // (the L sides of structured meshes) so that skipped tasks fall into the same warps.
-  constexpr int TPT = (4 * N + NFP - 1) / NFP;  // x/y-face tasks of a thread per slice
-  bool need_xy[TPT];
+  // x/y-face tasks of a thread per slice: task t = ij + q NFP < 4 N handles flux point (slot t / N, line m = t % N) of the
+  // thread's element; slots 0..3 = faces 1, 3 (+x, +y: the L sides of structured meshes, so that skipped tasks fall into the
+  // same warps), then 0, 2.  code: 0 skip, 1 / 2 interior with weight 1/2 +- beta, 3 boundary.
+  constexpr int TPT = (4 * N + NFP - 1) / NFP;
+  auto face_of = [](int t) { return t < 2 * N ? 2 * (t / N) + 1 : 2 * (t / N - 2); };
+  int code_xy[TPT];
+  int64_t off_nx[TPT];  // partner offset of the task's flux point in the next slice to gather
 #pragma unroll
   for (int q = 0; q < TPT; ++q) {
     const int t = ij + q * NFP;
-    need_xy[q] = t < 4 * N && act && face_need[(size_t)(t < 2 * N ? 2 * (t / N) + 1 : 2 * (t / N - 2)) * ld + e] != 0;
+    code_xy[q] = (t < 4 * N && act) ? face_code[(size_t)face_of(t) * ld + e] : 0;
+    off_nx[q] = 0;
   }
-  const bool need_z[2] = {act && face_need[(size_t)4 * ld + e] != 0, act && face_need[(size_t)5 * ld + e] != 0};
+  int code_z[2];
+#pragma unroll
+  for (int s = 0; s < 2; ++s) code_z[s] = act ? face_code[(size_t)(4 + s) * ld + e] : 0;
+
+  auto poff = [&](int fp) { return fp_poff[fp_row(true, ld, NF, fp, e)]; };
+  // gather of the partner's U^f (N_V values) of one flux point: per-thread asynchronous copies, consumed by the same thread
+  auto gather = [&](T *dst, int64_t off) {
+#pragma unroll
+    for (int a = 0; a < NV; ++a) cp_async<sizeof(T)>(dst + a * E, uf + off + (int64_t)a * FR_BLK);
+  };
+  auto gather_xy = [&](int k, int64_t *off) {  // slice k into stage k & 1
+    T *sP = (T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_P);
+#pragma unroll
+    for (int q = 0; q < TPT; ++q) {
+      const int t = ij + q * NFP;
+      if (code_xy[q] == 1 || code_xy[q] == 2) gather(sP + (size_t)t * NV * E + el, off[q]);
+    }
+  };
+  {
+    // z faces and slice 0 (group 0), slice 1 (group 1); the offsets of slice 2 wait in registers
+    int64_t off[TPT];
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+      if (code_z[s] == 1 || code_z[s] == 2) gather(sPz + (size_t)(s * NFP + ij) * NV * E + el, poff((4 + s) * NFP + ij));
+#pragma unroll
+    for (int q = 0; q < TPT; ++q) {
+      const int t = ij + q * NFP;
+      off[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N) : 0;
+    }
+    gather_xy(0, off);
+    cp_async_commit();
+    if (N > 1) {
+#pragma unroll
+      for (int q = 0; q < TPT; ++q) {
+        const int t = ij + q * NFP;
+        off[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N + N) : 0;
+      }
+      gather_xy(1, off);
+    }
+    cp_async_commit();
+    if (N > 2) {
+#pragma unroll
+      for (int q = 0; q < TPT; ++q) {
+        const int t = ij + q * NFP;
+        off_nx[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N + 2 * N) : 0;
+      }
+    }
+  }
+  // jump C - U^f (Eq 9) from the partner's U^f and the own interpolated state, both in the perturbation variables w (whose
+  // gradient this kernel takes); boundary: C = (1/2 - beta) u + (1/2 + beta) B_ldg u  (:797)
+  auto jump_of = [&](int code, int64_t off_or_bc, const R *uown, T *slot) {
+    R d[NV];
+    if (code == 1 || code == 2) {
+      const R w = code == 1 ? wL : wR;
+#pragma unroll
+      for (int a = 0; a < NV; ++a) d[a] = w * ((R)slot[a * E] - uown[a]);
+    } else if (BND && code == 3) {
+      double uw[NV], uc[NV], gi[NV], gl[NV];
+#pragma unroll
+      for (int a = 0; a < NV; ++a) uw[a] = (double)uown[a];
+      from_pert<3>(ph, uw, uc);
+      ghost_states<3>(bcs[-1 - off_or_bc], uc, ph.gamma, gi, gl);
+      to_pert<3>(ph, gl, gl);
+#pragma unroll
+      for (int a = 0; a < NV; ++a) d[a] = wL * ((R)gl[a] - uown[a]);
+    } else {
+#pragma unroll
+      for (int a = 0; a < NV; ++a) d[a] = 0;
+    }
+#pragma unroll
+    for (int a = 0; a < NV; ++a) slot[a * E] = (T)d[a];
+  };
+  // own state at the x/y flux point of task t in slice k (interpolation along its line, Eq 6)
+  auto own_xy = [&](int t, int k, R *uo) {
+    const int slot = t / N, m = t % N;
+    const int base = NFP * k + (slot % 2 == 0 ? m * N : m), stride = slot % 2 == 0 ? 1 : N;  // slots 0, 2: x faces (line j = m)
+    const R *lc = sL + (slot < 2 ? N : 0);
+#pragma unroll
+    for (int a = 0; a < NV; ++a) uo[a] = 0;
+#pragma unroll
+    for (int mm = 0; mm < N; ++mm) {
+      const R l = lc[mm];
+#pragma unroll
+      for (int a = 0; a < NV; ++a) uo[a] = fma(l, (R)sU[((size_t)(base + mm * stride) * NV + a) * E + el], uo[a]);
+    }
+  };
+  auto phase_A = [&](int k) {  // jumps of the x/y faces of slice k, in place over the gathered partner values
+    T *sP = (T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_P);
+#pragma unroll
+    for (int q = 0; q < TPT; ++q) {
+      const int t = ij + q * NFP;
+      if (t >= 4 * N) continue;
+      R uo[NV];
+      if (code_xy[q] != 0) own_xy(t, k, uo);
+      int64_t bc = 0;
+      if (BND && code_xy[q] == 3) bc = poff(face_of(t) * NFP + t % N + N * k);
+      jump_of(code_xy[q], bc, uo, sP + (size_t)t * NV * E + el);
+    }
+  };
   mbar_wait(&bar[0], 0);
+  if (ph.rho0 != 0.0) {
+    // the U block becomes w = T (u - u_ref) in place (fr_physics.cuh): every thread converts its own column
+#pragma unroll
+    for (int m = 0; m < N; ++m) {
+      double w[NV];
+      T *col = sU + ((size_t)(NFP * m + ij) * NV) * E + el;
+#pragma unroll
+      for (int a = 0; a < NV; ++a) w[a] = (double)col[a * E];
+      if (act) to_pert<3>(ph, w, w);
+#pragma unroll
+      for (int a = 0; a < NV; ++a) col[a * E] = (T)w[a];
+    }
+    __syncthreads();
+  }
+  cp_async_wait<1>();  // z faces and slice 0 have arrived (this thread's own copies)
+  {
+    R uz[2][NV];
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+#pragma unroll
+      for (int a = 0; a < NV; ++a) uz[s][a] = 0;
+#pragma unroll
+    for (int m = 0; m < N; ++m)
+#pragma unroll
+      for (int a = 0; a < NV; ++a) {
+        const R v = (R)sU[((size_t)(NFP * m + ij) * NV + a) * E + el];
+        uz[0][a] = fma(op.lm[m], v, uz[0][a]);
+        uz[1][a] = fma(op.lp[m], v, uz[1][a]);
+      }
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+      int64_t bc = 0;
+      if (BND && code_z[s] == 3) bc = poff((4 + s) * NFP + ij);
+      jump_of(code_z[s], bc, uz[s], sPz + (size_t)(s * NFP + ij) * NV * E + el);
+    }
+  }
+  phase_A(0);
+  __syncthreads();  // jumps of the z faces and of slice 0 are visible
 
 #pragma unroll
   for (int k = 0; k < N; ++k) {
     mbar_wait(&bar[1 + (k & 1)], (k >> 1) & 1);
     mbar_wait(&bar[3], k & 1);
-    const double *stR = (const double *)(sSt + (k & 1) * L::ST_BYTES);
-    const double *stJ = (const double *)(sSt + (k & 1) * L::ST_BYTES + L::ST_J);
+    const T *stR = (const T *)(sSt + (k & 1) * L::ST_BYTES);
+    const T *stJ = (const T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_P);  // [slot][line][NV][E]: slots 0, 1 = +x, +y; 2, 3 = -x, -y
     const T *su = sU + (size_t)(NFP * k) * NV * E + el;  // slice k
     {
-      double S[3][3];
+      R S[3][3];
 #pragma unroll
       for (int a = 0; a < 3; ++a)
 #pragma unroll
-        for (int b = 0; b < 3; ++b) S[a][b] = stS[((a * 3 + b) * NFP + ij) * E + el];
-      const double rj = stR[ij * E + el];
-      const double gmi = sGm[i], gpi = sGp[i], gmj = sGm[j], gpj = sGp[j];
+        for (int b = 0; b < 3; ++b) S[a][b] = (R)stS[((a * 3 + b) * NFP + ij) * E + el];
+      const R rj = (R)stR[ij * E + el];
+      const R gmi = sGm[i], gpi = sGp[i], gmj = sGm[j], gpj = sGp[j];
 #pragma unroll
       for (int a = 0; a < NV; ++a) {
-        double qx = fma(gpi, stJ[((1 * N + j) * NV + a) * E + el], -gmi * stJ[((0 * N + j) * NV + a) * E + el]);
-        double qy = fma(gpj, stJ[((3 * N + i) * NV + a) * E + el], -gmj * stJ[((2 * N + i) * NV + a) * E + el]);
-        double qz = fma(op.gp[k], sJz[((1 * NFP + ij) * NV + a) * E + el], -op.gm[k] * sJz[((0 * NFP + ij) * NV + a) * E + el]);
+        // M6 = n~ (x) M3 (A1): the reference normal is -1 on the -1 faces (jumps of faces without an LDG weight are zero;
+        // skipping their reads under a predicate was 4 % slower)
+        R qx = fma(gpi, (R)stJ[((0 * N + j) * NV + a) * E + el], -gmi * (R)stJ[((2 * N + j) * NV + a) * E + el]);
+        R qy = fma(gpj, (R)stJ[((1 * N + i) * NV + a) * E + el], -gmj * (R)stJ[((3 * N + i) * NV + a) * E + el]);
+        R qz = fma(op.gp[k], (R)sPz[((1 * NFP + ij) * NV + a) * E + el], -op.gm[k] * (R)sPz[((0 * NFP + ij) * NV + a) * E + el]);
 #pragma unroll
         for (int m = 0; m < N; ++m) {
-          qx = fma(sD[i * N + m], (double)su[((j * N + m) * NV + a) * E], qx);
-          qy = fma(sD[j * N + m], (double)su[((m * N + i) * NV + a) * E], qy);
-          qz = fma(op.D[k * N + m], (double)sU[((size_t)(NFP * m + ij) * NV + a) * E + el], qz);
+          qx = fma(sD[i * N + m], (R)su[((j * N + m) * NV + a) * E], qx);
+          qy = fma(sD[j * N + m], (R)su[((m * N + i) * NV + a) * E], qy);
+          qz = fma(op.D[k * N + m], (R)sU[((size_t)(NFP * m + ij) * NV + a) * E + el], qz);
         }
-        double q3[3];
+        R q3[3];
         to_physical(S, rj, qx, qy, qz, q3);
 #pragma unroll
-        for (int n = 0; n < 3; ++n) {
-          sQ[((n * NFP + ij) * NV + a) * E + el] = q3[n];
+        for (int n = 0; n < 3; ++n) sQ[((n * NFP + ij) * NV + a) * E + el] = (T)q3[n];
+      }
+    }
+    fence_proxy_async();  // make the sQ writes visible to the bulk store
+    __syncthreads();      // Q of the slice is complete; S, 1/J and the jumps of stage k&1 have been consumed
+    if (tid == 0 && k + 1 < N) issue_S(k + 1);
+    if (tid == 0 && k + 2 < N) issue_R(k & 1, k + 2);
+    if (tid == 0) { tma_store_4d(&tmQ, l0, 0, 3 * k, eb, sQ); tma_store_commit(); }
+    if (k + 2 < N) {  // partner values of slice k + 2 into the freed stage; the offsets of slice k + 3 start their way
+      gather_xy(k + 2, off_nx);
+      if (k + 3 < N) {
+#pragma unroll
+        for (int q = 0; q < TPT; ++q) {
+          const int t = ij + q * NFP;
+          off_nx[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N + N * (k + 3)) : 0;
         }
       }
     }
-    if (SQ) fence_proxy_async();  // make the sQ writes visible to the bulk store
-    __syncthreads();  // Q of the slice is complete; stage k&1 has been consumed
-    if (tid == 0 && k + 1 < N) issue_S(k + 1);
-    if (tid == 0 && k + 2 < N) issue_stage(k & 1, k + 2);
-    if (SQ && tid == 0) { tma_store_4d(&tmQ, l0, 0, 3 * k, eb, sQ); tma_store_commit(); }
-    // x / y faces of the slice: 4 N flux points per element, one thread each
+    cp_async_commit();
+    // x / y faces of the slice: G^f at the flux points that carry an LDG weight, one thread each
 #pragma unroll
     for (int q = 0; q < TPT; ++q) {
-      if (!need_xy[q]) continue;
+      if (code_xy[q] == 0) continue;
       const int t = ij + q * NFP;
-      const int f = t < 2 * N ? 2 * (t / N) + 1 : 2 * (t / N - 2), m = t % N;  // faces 1, 3 (+x, +y), then 0, 2
-      const int base = f < 2 ? m * N : m, stride = f < 2 ? 1 : N;
-      const double *lc = sL + (f & 1) * N;
+      const int slot = t / N, f = face_of(t), m = t % N;
+      const int base = slot % 2 == 0 ? m * N : m, stride = slot % 2 == 0 ? 1 : N;
+      const R *lc = sL + (slot < 2 ? N : 0);
       const int fp = f * NFP + m + N * k;
-      double nrm[3], uf[NV], G[NV];
+      R nrm[3], uo[NV], G[NV];
 #pragma unroll
-      for (int n = 0; n < 3; ++n) nrm[n] = fp_n[fp_row(true, ld, 3 * NF, n * NF + fp, e)];
-#pragma unroll
-      for (int a = 0; a < NV; ++a) uf[a] = 0.0;
-#pragma unroll
-      for (int mm = 0; mm < N; ++mm) {
-        const double l = lc[mm];
-#pragma unroll
-        for (int a = 0; a < NV; ++a) uf[a] = fma(l, (double)su[((base + mm * stride) * NV + a) * E], uf[a]);
-      }
+      for (int n = 0; n < 3; ++n) nrm[n] = (R)fp_n[fp_row(true, ld, 3 * NF, n * NF + fp, e)];
+      own_xy(t, k, uo);
       if constexpr (BND) {
-        const int pe = fp_pe[fp_row(true, ld, NF, fp, e)];
-        double qf[3][NV];
+        const int pe = code_xy[q] == 3 ? (int)poff(fp) : 0;
+        R qf[3][NV];
 #pragma unroll
         for (int n = 0; n < 3; ++n)
 #pragma unroll
           for (int a = 0; a < NV; ++a) {
-            double q = 0;
+            R qq = 0;
 #pragma unroll
-            for (int mm = 0; mm < N; ++mm) q = fma(lc[mm], sQ[((n * NFP + base + mm * stride) * NV + a) * E + el], q);
-            qf[n][a] = q;
+            for (int mm = 0; mm < N; ++mm) qq = fma(lc[mm], (R)sQ[((n * NFP + base + mm * stride) * NV + a) * E + el], qq);
+            qf[n][a] = qq;
           }
-        face_visc<BND>(uf, qf, nrm, ph, pe, bcs, G);
+        face_visc_r<BND, R>(uo, qf, nrm, ph, pe, bcs, G);
       } else {
-        visc_normal_stream(uf, nrm, ph, [&](int a, double *g) {
+        visc_normal_stream<R>(uo, nrm, ph, [&](int a, R *g) {
 #pragma unroll
           for (int n = 0; n < 3; ++n) {
-            double q = 0;
+            R qq = 0;
 #pragma unroll
-            for (int mm = 0; mm < N; ++mm) q = fma(lc[mm], sQ[((n * NFP + base + mm * stride) * NV + a) * E + el], q);
-            g[n] = q;
+            for (int mm = 0; mm < N; ++mm) qq = fma(lc[mm], (R)sQ[((n * NFP + base + mm * stride) * NV + a) * E + el], qq);
+            g[n] = qq;
           }
         }, G);
       }
-      if (act) {
 #pragma unroll
-        for (int a = 0; a < NV; ++a) gf[fp_row(true, ld, NF * NV, fp * NV + a, e)] = G[a];
-      }
+      for (int a = 0; a < NV; ++a) gf[fp_row(true, ld, NF * NV, fp * NV + a, e)] = (T)G[a];
     }
-    if (SQ && tid == 0) tma_store_wait_read();  // the bulk store has read sQ
-    if (k + 1 < N) __syncthreads();  // before the next slice overwrites sQ
+    if (k + 1 < N) {
+      cp_async_wait<1>();  // slice k + 1 has arrived (slice k + 2 may still be in flight)
+      phase_A(k + 1);
+    }
+    if (tid == 0) tma_store_wait_read();  // the bulk store has read sQ
+    if (k + 1 < N) __syncthreads();  // jumps of slice k + 1 visible; sQ free
   }
   // ---- z faces.  Q^f on them is sum_k l(+-1)_k Q(i, j, k): instead of carrying 2 x 15 accumulators through the slice
   // loop, the Q slices just stored are streamed once more (TMA loads, L2 hits) through two buffers that the slice loop
   // no longer needs: [SS .. Q) (S, 1/J, x/y jumps) and [U .. SS) (U block, z jumps).  The last slice is still in sQ.
   static_assert(L::Q - L::SS >= L::Q_BYTES && L::SS - L::U >= L::Q_BYTES, "Q slice does not fit the reused buffers");
-  double ufz[2][NV];
+  R ufz[2][NV];
 #pragma unroll
   for (int s = 0; s < 2; ++s)
 #pragma unroll
-    for (int a = 0; a < NV; ++a) ufz[s][a] = 0.0;
+    for (int a = 0; a < NV; ++a) ufz[s][a] = 0;
 #pragma unroll
   for (int m = 0; m < N; ++m)
 #pragma unroll
     for (int a = 0; a < NV; ++a) {
-      const double v = (double)sU[((size_t)(NFP * m + ij) * NV + a) * E + el];
+      const R v = (R)sU[((size_t)(NFP * m + ij) * NV + a) * E + el];
       ufz[0][a] = fma(op.lm[m], v, ufz[0][a]);
       ufz[1][a] = fma(op.lp[m], v, ufz[1][a]);
     }
@@ -229,25 +384,25 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     for (int k = 0; k < 2; ++k)
       if (k < N - 1) { mbar_expect_tx(&bar[4 + k], (uint32_t)L::Q_BYTES); tma_load_4d(zb[k], &tmQ, l0, 0, 3 * k, eb, &bar[4 + k]); }
   }
-  double zq[2][3][NV];
+  R zq[2][3][NV];
 #pragma unroll
   for (int s = 0; s < 2; ++s)
 #pragma unroll
     for (int n = 0; n < 3; ++n)
 #pragma unroll
-      for (int a = 0; a < NV; ++a) zq[s][n][a] = 0.0;
+      for (int a = 0; a < NV; ++a) zq[s][n][a] = 0;
 #pragma unroll
   for (int k = 0; k < N; ++k) {
-    const double *src = sQ;
+    const T *src = sQ;
     if (k < N - 1) {
       mbar_wait(&bar[4 + (k & 1)], (k >> 1) & 1);
-      src = (const double *)zb[k & 1];
+      src = (const T *)zb[k & 1];
     }
 #pragma unroll
     for (int n = 0; n < 3; ++n)
 #pragma unroll
       for (int a = 0; a < NV; ++a) {
-        const double q = src[((n * NFP + ij) * NV + a) * E + el];
+        const R q = (R)src[((n * NFP + ij) * NV + a) * E + el];
         zq[0][n][a] = fma(op.lm[k], q, zq[0][n][a]);
         zq[1][n][a] = fma(op.lp[k], q, zq[1][n][a]);
       }
@@ -258,80 +413,75 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   }
 #pragma unroll
   for (int s = 0; s < 2; ++s) {
-    if (!need_z[s]) continue;
+    if (code_z[s] == 0) continue;
     const int fp = (4 + s) * NFP + ij;
-    double nrm[3], G[NV];
+    R nrm[3], G[NV];
 #pragma unroll
-    for (int n = 0; n < 3; ++n) nrm[n] = fp_n[fp_row(true, ld, 3 * NF, n * NF + fp, e)];
-    const int pe = BND ? fp_pe[fp_row(true, ld, NF, fp, e)] : 0;
-    if constexpr (BND) face_visc<BND>(ufz[s], zq[s], nrm, ph, pe, bcs, G);
-    else visc_normal_stream(ufz[s], nrm, ph, [&](int a, double *g) {
+    for (int n = 0; n < 3; ++n) nrm[n] = (R)fp_n[fp_row(true, ld, 3 * NF, n * NF + fp, e)];
+    const int pe = (BND && code_z[s] == 3) ? (int)poff(fp) : 0;
+    if constexpr (BND) face_visc_r<BND, R>(ufz[s], zq[s], nrm, ph, pe, bcs, G);
+    else visc_normal_stream<R>(ufz[s], nrm, ph, [&](int a, R *g) {
 #pragma unroll
       for (int n = 0; n < 3; ++n) g[n] = zq[s][n][a];
     }, G);
 #pragma unroll
-    for (int a = 0; a < NV; ++a) gf[fp_row(true, ld, NF * NV, fp * NV + a, e)] = G[a];
+    for (int a = 0; a < NV; ++a) gf[fp_row(true, ld, NF * NV, fp * NV + a, e)] = (T)G[a];
   }
 }
 
 // ---------------------------------------------------------------------------------------------
 // host side: tensor maps and launches
 // ---------------------------------------------------------------------------------------------
-template <int N, int E>
 struct Maps {
-  CUtensorMap U, S, R1, J, Jz, Q;
+  CUtensorMap U, S, R1, Q;
 };
 
 template <int N, int E, typename T>
-bool make_maps(const DevConsts &c, const void *u, const double *jump, Maps<N, E> &m, const double *q) {
+bool make_maps(const DevConsts &c, const void *u, Maps &m, const void *q) {
   constexpr int NFP = N * N, NU = N * NFP;
   static_assert(FR_BLK % E == 0, "a CTA's elements must lie in one element block");
   const uint64_t ld = (uint64_t)c.ld;
   bool ok = encode3(&m.U, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, N);  // caller layout
-  ok = ok && encode_blk(&m.S, c.smat, ld, NU, 9, E, NFP, 9, c.aff ? 1 : 0);
-  ok = ok && encode_blk(&m.R1, c.rcpj, ld, NFP, N, E, NFP, 1, c.aff ? 2 : 0);
-  ok = ok && encode_blk(&m.J, jump, ld, NFP * NV, 6, E, N * NV, 4);
-  ok = ok && encode_blk(&m.Jz, jump, ld, NFP * NV, 6, E, NFP * NV, 2);
-  if (q) ok = ok && encode_blk(&m.Q, q, ld, NV * NFP, 3 * N, E, NV * NFP, 3);
-  else m.Q = m.R1;
+  ok = ok && encode_blk(&m.S, sizeof(T) == 8, c.smat, ld, NU, 9, E, NFP, 9, c.aff ? 1 : 0);  // metric terms in T on this path (fr_api.cu)
+  ok = ok && encode_blk(&m.R1, sizeof(T) == 8, c.rcpj, ld, NFP, N, E, NFP, 1, c.aff ? 2 : 0);
+  ok = ok && encode_blk(&m.Q, sizeof(T) == 8, q, ld, NV * NFP, 3 * N, E, NV * NFP, 3);
   return ok;
 }
 
-template <int N, int E, bool BND, bool SQ, typename T, int MINB>
-cudaError_t launch_gradface_k(const DevConsts &c, const Maps<N, E> &m, const Ops1D<N> &op, const double *jump, double *gf, cudaStream_t s) {
+template <int N, int E, bool BND, typename T, int MINB>
+cudaError_t launch_gradface_k(const DevConsts &c, const Maps &m, const Ops1D<N, T> &op, const T *uf, T *gf, cudaStream_t s) {
   using L = GfLay<N, E, T>;
-  auto kern = k_hex_gradface<N, E, BND, SQ, T, MINB>;
+  auto kern = k_hex_gradface<N, E, BND, T, MINB>;
   static DevFlags done;
   cudaError_t err = set_smem(kern, L::TOTAL, done, c.dev);
   if (err != cudaSuccess) return err;
-  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.J, m.Q, m.Jz, op, c.ph, jump, c.fp_n, c.fp_pe, c.face_need, c.bcs, gf,
-                                                                  c.ld,
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.Q, op, c.ph, uf, c.fp_poff, (const T *)c.fp_n, c.face_code, c.bcs, gf, c.ld,
                                                                   c.Nel);
   return cudaGetLastError();
 }
 
 template <int N, int E, typename T>
-cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, double *q,
-                            cudaStream_t s) {
+cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void *u, const void *uf, void *gf, void *q, cudaStream_t s) {
   using L = GfLay<N, E, T>;
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
-  constexpr int MINB = min_blocks(L::TOTAL, N * N * E);
-  Maps<N, E> m;
-  if (!make_maps<N, E, T>(c, u, jump, m, q)) return cudaErrorNotSupported;
-  const Ops1D<N> op = make_ops<N>(h_ops);
+  constexpr int MINB = min_blocks(L::TOTAL, N * N * E, sizeof(T) == 8 ? 128 : 96);  // single-precision arithmetic needs fewer registers
+  Maps m;
   if (!q) return cudaErrorInvalidValue;  // the z-face pass re-reads the stored Q slices
-  return c.nbnd ? launch_gradface_k<N, E, true, true, T, MINB>(c, m, op, jump, gf, s) : launch_gradface_k<N, E, false, true, T, MINB>(c, m, op, jump, gf, s);
+  if (!make_maps<N, E, T>(c, u, m, q)) return cudaErrorNotSupported;
+  const Ops1D<N, T> op = make_ops<N, T>(h_ops);
+  return c.nbnd ? launch_gradface_k<N, E, true, T, MINB>(c, m, op, (const T *)uf, (T *)gf, s)
+                : launch_gradface_k<N, E, false, T, MINB>(c, m, op, (const T *)uf, (T *)gf, s);
 }
 
 template <int N, typename T>
 constexpr bool fits() {
-  return GfLay<N, Cfg<N>::E, T>::TOTAL <= SMEM_MAX && N * N * Cfg<N>::E <= 1024;
+  return GfLay<N, Cfg<N, T>::E, T>::TOTAL <= SMEM_MAX && N * N * Cfg<N, T>::E <= 1024;
 }
 
 template <int N, typename T>
-cudaError_t gradface_n(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, double *q, cudaStream_t s) {
+cudaError_t gradface_n(const DevConsts &c, const double *h_ops, const void *u, const void *uf, void *gf, void *q, cudaStream_t s) {
   if constexpr (fits<N, T>()) {
-    return launch_gradface<N, Cfg<N>::E, T>(c, h_ops, u, jump, gf, q, s);
+    return launch_gradface<N, Cfg<N, T>::E, T>(c, h_ops, u, uf, gf, q, s);
   } else {
     return cudaErrorNotSupported;
   }
@@ -349,10 +499,9 @@ bool hex_tma_supported(int n, bool f64) {
   }
 }
 
-cudaError_t hex_tma_gradface(const DevConsts &c, const double *h_ops, const void *u, const double *jump, double *gf, double *q,
-                             cudaStream_t s) {
+cudaError_t hex_tma_gradface(const DevConsts &c, const double *h_ops, const void *u, const void *uf, void *gf, void *q, cudaStream_t s) {
   switch (c.n) {
-#define FR_CASE(NN) case NN: return c.f64 ? gradface_n<NN, double>(c, h_ops, u, jump, gf, q, s) : gradface_n<NN, float>(c, h_ops, u, jump, gf, q, s);
+#define FR_CASE(NN) case NN: return c.f64 ? gradface_n<NN, double>(c, h_ops, u, uf, gf, q, s) : gradface_n<NN, float>(c, h_ops, u, uf, gf, q, s);
     FR_CASE(2) FR_CASE(3) FR_CASE(4) FR_CASE(5) FR_CASE(6) FR_CASE(7)
 #undef FR_CASE
     default: return cudaErrorNotSupported;

@@ -95,19 +95,22 @@ __device__ __forceinline__ void inviscid_flux(const double *w, const Phys &ph, d
   }
 }
 
-// f_vis[n][a] of Eq 22-24 SUBTRACTED from f (f -= f_vis).  q[n][a] = d_n u_a.
-// d_i v_j by the quotient rule; Delta*dT = (mu*gamma/Pr) d e (A8); 2/3 kept in 2-D (A22).
+// f_vis[n][a] of Eq 22-24 SUBTRACTED from f (f -= f_vis), from the perturbation state w and ITS gradient qw[n][a] = d_n w_a
+// (T is constant, so grad w = T grad u; differentiating w instead of u keeps the O(E0) terms out of the second derivatives).
+// d_i v_j = (d_i w_mj - dv_j d_i rho) / rho with dv = w_m / rho = v - v0 (quotient rule, Galilean invariant);
+// Delta*dT = (mu*gamma/Pr) d e (A8) with  d_i E - (E/rho) d_i rho = d_i w_E - ((w_E - p0)/rho) d_i rho;  2/3 kept in 2-D (A22).
+// v: the full velocities.  With no reference state these are the plain formulas in conserved variables.
 template <int ND>
-__device__ __forceinline__ void subtract_viscous_flux(const double *u, const double (*q)[ND + 2], const double *v,
+__device__ __forceinline__ void subtract_viscous_flux(const double *w, const double (*qw)[ND + 2], const double *v,
                                                       const Phys &ph, double (*f)[ND + 2]) {
-  const double rrho = 1.0 / u[0];
-  const double E = u[ND + 1];
+  const double rrho = 1.0 / (w[0] + ph.rho0);
+  const double Es = (w[ND + 1] - ph.p0) * rrho;
   double dv[ND][ND];
   double div = 0;
 #pragma unroll
   for (int i = 0; i < ND; ++i) {
 #pragma unroll
-    for (int j = 0; j < ND; ++j) dv[i][j] = (q[i][1 + j] - v[j] * q[i][0]) * rrho;
+    for (int j = 0; j < ND; ++j) dv[i][j] = (qw[i][1 + j] - (w[1 + j] * rrho) * qw[i][0]) * rrho;
     div += dv[i][i];
   }
   const double lam = -2.0 / 3.0 * ph.mu * div;
@@ -119,7 +122,7 @@ __device__ __forceinline__ void subtract_viscous_flux(const double *u, const dou
   const double kap = ph.mu * ph.gamma / ph.Pr;
 #pragma unroll
   for (int n = 0; n < ND; ++n) {
-    double de = (q[n][ND + 1] - (E * rrho) * q[n][0]) * rrho;
+    double de = (qw[n][ND + 1] - Es * qw[n][0]) * rrho;
     double vt = 0;
 #pragma unroll
     for (int j = 0; j < ND; ++j) { de -= v[j] * dv[n][j]; vt += v[j] * T[j][n]; }
@@ -129,19 +132,19 @@ __device__ __forceinline__ void subtract_viscous_flux(const double *u, const dou
   }
 }
 
-// normal viscous flux n . f_vis(u, q)   (used by the LDG interface flux)
+// normal viscous flux n . f_vis(w, grad w)   (used by the LDG interface flux)
 template <int ND>
-__device__ __forceinline__ void normal_viscous_flux(const double *u, const double (*q)[ND + 2], const double *nrm,
+__device__ __forceinline__ void normal_viscous_flux(const double *w, const double (*qw)[ND + 2], const double *nrm,
                                                     const Phys &ph, double *fn) {
   double f[ND][ND + 2], v[ND];
-  const double rrho = 1.0 / u[0];
+  const double rrho = 1.0 / (w[0] + ph.rho0);
 #pragma unroll
-  for (int d = 0; d < ND; ++d) v[d] = u[1 + d] * rrho;
+  for (int d = 0; d < ND; ++d) v[d] = ph.v0[d] + w[1 + d] * rrho;
 #pragma unroll
   for (int n = 0; n < ND; ++n)
 #pragma unroll
     for (int a = 0; a < ND + 2; ++a) f[n][a] = 0.0;
-  subtract_viscous_flux<ND>(u, q, v, ph, f);
+  subtract_viscous_flux<ND>(w, qw, v, ph, f);
 #pragma unroll
   for (int a = 0; a < ND + 2; ++a) {
     double s = 0;
@@ -225,20 +228,18 @@ __device__ __forceinline__ double ghost_states(const BcDev &bc, const double *uL
   return 1.0;
 }
 
-// Common normal flux Eq 26 with the penalty in its dissipative sign (A7), on perturbation states w (the viscous part is
-// evaluated from the conserved variables; its mass row is zero, so it is the same in both sets of variables):
+// Common normal flux Eq 26 with the penalty in its dissipative sign (A7), on perturbation states w and their gradients
+// (the viscous flux has a zero mass row, so it is the same in both sets of variables):
 // F = F_inv(wL, wRinv) - n.{(1/2+beta) f_L^vis + (1/2-beta) f_R^vis} + tau (wL - wR)
 template <int ND, bool NS>
 __device__ __forceinline__ void common_flux(const double *wL, const double *wR, const double *wRinv, const double (*qL)[ND + 2],
                                             const double (*qR)[ND + 2], const double *nrm, const Phys &ph, double *F) {
   rusanov<ND>(wL, wRinv, nrm, ph, F);
   if (NS) {
-    double fvL[ND + 2], fvR[ND + 2], uL[ND + 2], uR[ND + 2];
+    double fvL[ND + 2], fvR[ND + 2];
     const double wl = 0.5 + ph.beta, wr = 0.5 - ph.beta;
-    from_pert<ND>(ph, wL, uL);
-    from_pert<ND>(ph, wR, uR);
-    if (wl != 0.0) normal_viscous_flux<ND>(uL, qL, nrm, ph, fvL);
-    if (wr != 0.0) normal_viscous_flux<ND>(uR, qR, nrm, ph, fvR);
+    if (wl != 0.0) normal_viscous_flux<ND>(wL, qL, nrm, ph, fvL);
+    if (wr != 0.0) normal_viscous_flux<ND>(wR, qR, nrm, ph, fvR);
 #pragma unroll
     for (int a = 0; a < ND + 2; ++a) {
       double fv = 0;

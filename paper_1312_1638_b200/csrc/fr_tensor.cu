@@ -149,21 +149,21 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
   double *uf = (double *)(work + tp.off_uf), *cf = (double *)(work + tp.off_cf), *qu = (double *)(work + tp.off_qu),
          *qf = (double *)(work + tp.off_qf);
   if constexpr (ND == 3) {
-    // hexahedra: sm_100a TMA path, 5 launches for Navier-Stokes (3 for Euler); neither Q^f nor F~ is stored
+    // hexahedra: sm_100a TMA path, 4 launches for Navier-Stokes (3 for Euler); C^f, Q^f and F~ are never stored; the
+    // flux-point arrays and Q are in the storage precision T
+    (void)cf;
     FR_MARK(prof, "hex_interp_tma");
     cudaError_t e = hex_tma_interp(c, tp.h_ops, u, uf, s);
     if (e != cudaSuccess) return e;
     if (c.ns) {
-      FR_MARK(prof, "common_sol");
-      launch_common_jump(c, uf, cf, s);
       FR_MARK(prof, "hex_gradface");
-      e = hex_tma_gradface(c, tp.h_ops, u, cf, qu, qf, s);
+      e = hex_tma_gradface(c, tp.h_ops, u, uf, qu, qf, s);
       if (e != cudaSuccess) return e;
       FR_MARK(prof, "common_flux_g");
-      launch_common_flux_g(c, uf, qu, s);
+      launch_common_flux_g(c, uf, qu, !c.f64, s);
     } else {
       FR_MARK(prof, "common_flux");
-      launch_common_flux(c, uf, qf, s);
+      launch_common_flux(c, uf, qf, !c.f64, s);
     }
     FR_MARK(prof, "hex_fluxdiv_tma");
     e = hex_tma_fluxdiv(c, tp.h_ops, u, qf, uf, rhs, s);
@@ -189,7 +189,7 @@ cudaError_t run(const DevConsts &c, const TensorPlan &tp, const T *u, T *rhs, ch
     FR_MARK(prof, "tflux");
     launch_tflux(c, u, qu, s);
     FR_MARK(prof, "common_flux");
-    launch_common_flux(c, uf, qf, s);
+    launch_common_flux(c, uf, qf, false, s);
     FR_MARK(prof, "tp_div");
     k_tp_div<N, ND, T><<<dim3(gx, 1, 1), bu, 0, s>>>(op, qu, uf, c.rcpj, rhs, ncols, c.ld, c.Nel);
     return cudaGetLastError();
@@ -230,13 +230,16 @@ cudaError_t tensor_plan(const DevConsts &c, const RefOps &o, const MeshConsts &,
   auto al = [](int64_t x) { return (x + 255) / 256 * 256; };
   const int64_t ncols = (int64_t)c.NV * c.ld;
   int64_t off = 0;
-  tp.off_uf = off; off = al(off + (int64_t)o.Nf * ncols * 8);
-  tp.off_cf = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
   tp.use_tma = c.blk;
-  if (tp.use_tma) {  // G^f (and Q, slice-major) besides U^f and the jumps
-    tp.off_qu = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
-    tp.off_qf = off; if (c.ns) off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
+  if (tp.use_tma) {  // U^f -> D~, G^f and Q (slice-major) in the storage precision
+    const int64_t esz = c.f64 ? 8 : 4;
+    tp.off_uf = off; off = al(off + (int64_t)o.Nf * ncols * esz);
+    tp.off_cf = off;
+    tp.off_qu = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * esz);
+    tp.off_qf = off; if (c.ns) off = al(off + (int64_t)o.nd * o.Nu * ncols * esz);
   } else {
+    tp.off_uf = off; off = al(off + (int64_t)o.Nf * ncols * 8);
+    tp.off_cf = off; if (c.ns) off = al(off + (int64_t)o.Nf * ncols * 8);
     tp.off_qu = off; off = al(off + (int64_t)o.nd * o.Nu * ncols * 8);
     tp.off_qf = off; if (c.ns) off = al(off + (int64_t)o.nd * o.Nf * ncols * 8);
   }
@@ -250,10 +253,11 @@ cudaError_t tensor_rhs(const DevConsts &c, const TensorPlan &tp, const void *u, 
 
 int tensor_rhs_launches(const DevConsts &c) {
   int n;
-  if (c.nd == 3) n = c.ns ? 5 : 3;  // interp, (common sol, gradface,) common flux, fluxdiv
+  if (c.nd == 3) n = c.ns ? 4 : 3;  // interp, (gradface,) common flux, fluxdiv
   else n = c.ns ? 7 : 4;            // interp, (common sol, grad, interp q,) tflux, common flux, div
-  if (c.nbnd) n += c.ns ? 2 : 1;
-  if (!c.npairs) n -= c.ns ? 2 : 1;
+  const int pair_groups = (c.nd == 3 || !c.ns) ? 1 : 2;  // launch groups that run over flux-point pairs / boundary points
+  if (c.nbnd) n += pair_groups;
+  if (!c.npairs) n -= pair_groups;
   return n;
 }
 

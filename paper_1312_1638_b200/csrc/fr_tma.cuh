@@ -80,11 +80,20 @@ __device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk
 __device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 
-// resident CTAs per SM the kernel is compiled for: limited by shared memory, by >= 128 registers per thread
-constexpr int min_blocks(size_t smem, int threads) {
+// per-thread asynchronous copies global -> shared (gathers): BYTES = 4 | 8 | 16
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void *dst, const void *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_addr(dst)), "l"(src), "n"(BYTES) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int PENDING>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(PENDING) : "memory"); }
+
+// resident CTAs per SM the kernel is compiled for: limited by shared memory, by >= `regs` registers per thread
+constexpr int min_blocks(size_t smem, int threads, int regs = 128) {
   int by_smem = (int)((SMEM_MAX + 1024) / (smem + 1024));
   int warps = (threads + 31) / 32;
-  int by_regs = 65536 / (128 * 32 * warps);
+  int by_regs = 65536 / (regs * 32 * warps);
   int by_thr = 2048 / (32 * warps);
   int m = by_smem < by_regs ? by_smem : by_regs;
   m = m < by_thr ? m : by_thr;
@@ -92,44 +101,47 @@ constexpr int min_blocks(size_t smem, int threads) {
 }
 
 // Q~ -> Q at one solution point for variable a:  q_n = (1/J) sum_i S[i][n] q~_i   (Eq 10 :206)
-__device__ __forceinline__ void to_physical(const double (*S)[3], double rj, double qx, double qy, double qz, double *q) {
+template <typename R>
+__device__ __forceinline__ void to_physical(const R (*S)[3], R rj, R qx, R qy, R qz, R *q) {
 #pragma unroll
   for (int n = 0; n < 3; ++n) q[n] = rj * fma(S[0][n], qx, fma(S[1][n], qy, S[2][n] * qz));
 }
 
-// n . f_vis(u, q) (Eq 22-24) with the gradient fed one conserved variable at a time (getg(a, g) -> d_n u_a), so that
-// at most the velocity-gradient tensor is live: d_i v_j by the quotient rule, Delta dT = (mu gamma / Pr) d e (A8).
-template <typename GetG>
-__device__ __forceinline__ void visc_normal_stream(const double *u, const double *nrm, const Phys &ph, GetG getg, double *G) {
-  const double rrho = 1.0 / u[0], En = u[4];
-  double v[3], g0[3], dv[3][3], de[3];
+// n . f_vis (Eq 22-24) from the perturbation state w and its gradient fed one variable at a time (getg(a, g) -> d_n w_a), so
+// that at most the velocity-gradient tensor is live: d_i v_j by the quotient rule with dv = w_m / rho, Delta dT = (mu gamma / Pr)
+// d e (A8); formulas of subtract_viscous_flux (fr_physics.cuh).
+template <typename R, typename GetG>
+__device__ __forceinline__ void visc_normal_stream(const R *w, const R *nrm, const Phys &ph, GetG getg, R *G) {
+  const R rrho = (R)1 / (w[0] + (R)ph.rho0), Es = (w[4] - (R)ph.p0) * rrho;
+  const R mu = (R)ph.mu;
+  R v[3], dvl[3], g0[3], dv[3][3], de[3];
 #pragma unroll
-  for (int d = 0; d < 3; ++d) v[d] = u[1 + d] * rrho;
+  for (int d = 0; d < 3; ++d) { dvl[d] = w[1 + d] * rrho; v[d] = (R)ph.v0[d] + dvl[d]; }
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
-    double g[3];
+    R g[3];
     getg(a, g);
 #pragma unroll
     for (int n = 0; n < 3; ++n) {
       if (a == 0) g0[n] = g[n];
-      else if (a < 4) dv[n][a - 1] = (g[n] - v[a - 1] * g0[n]) * rrho;
-      else de[n] = (g[n] - (En * rrho) * g0[n]) * rrho;
+      else if (a < 4) dv[n][a - 1] = (g[n] - dvl[a - 1] * g0[n]) * rrho;
+      else de[n] = (g[n] - Es * g0[n]) * rrho;
     }
   }
-  const double lam = -2.0 / 3.0 * ph.mu * (dv[0][0] + dv[1][1] + dv[2][2]);
-  const double kap = ph.mu * ph.gamma / ph.Pr;
-  double Tm[3][3];
+  const R lam = (R)(-2.0 / 3.0) * mu * (dv[0][0] + dv[1][1] + dv[2][2]);
+  const R kap = (R)(ph.mu * ph.gamma / ph.Pr);
+  R Tm[3][3];
 #pragma unroll
   for (int a = 0; a < 3; ++a)
 #pragma unroll
-    for (int b = 0; b < 3; ++b) Tm[a][b] = ph.mu * (dv[a][b] + dv[b][a]) + (a == b ? lam : 0.0);
-  G[0] = 0.0;
+    for (int b = 0; b < 3; ++b) Tm[a][b] = mu * (dv[a][b] + dv[b][a]) + (a == b ? lam : (R)0);
+  G[0] = 0;
 #pragma unroll
   for (int b = 0; b < 3; ++b) G[1 + b] = fma(nrm[0], Tm[0][b], fma(nrm[1], Tm[1][b], nrm[2] * Tm[2][b]));
-  double s = 0;
+  R s = 0;
 #pragma unroll
   for (int n = 0; n < 3; ++n) {
-    double d = de[n], vt = 0;
+    R d = de[n], vt = 0;
 #pragma unroll
     for (int b = 0; b < 3; ++b) { d -= v[b] * dv[n][b]; vt += v[b] * Tm[b][n]; }
     s = fma(nrm[n], vt + kap * d, s);
@@ -137,16 +149,18 @@ __device__ __forceinline__ void visc_normal_stream(const double *u, const double
   G[4] = s;
 }
 
-// G at one flux point from the interpolated state and gradient.  Interior: n . f_vis(u^f, q^f) with the
+// G at one flux point from the interpolated perturbation state and its gradient.  Interior: n . f_vis(w^f, q^f) with the
 // element's own outward normal (the pair kernel applies the LDG weights 1/2 +- beta, Eq 27).  Boundary:
 // the complete (1/2+beta) n.f_vis(u_L, q_L) + (1/2-beta) n.f_vis(B_ldg u_L, B_ldg q_L)  (App C, A20).
 template <bool BND>
-__device__ __forceinline__ void face_visc(const double *uf, const double (*qf)[NV], const double *nrm, const Phys &ph, int pe,
+__device__ __forceinline__ void face_visc(const double *wf, const double (*qf)[NV], const double *nrm, const Phys &ph, int pe,
                                           const BcDev *__restrict__ bcs, double *G) {
-  normal_viscous_flux<3>(uf, qf, nrm, ph, G);
+  normal_viscous_flux<3>(wf, qf, nrm, ph, G);
   if (BND && pe < 0) {
-    double gi[NV], gl[NV], qg[3][NV], GR[NV];
+    double uf[NV], gi[NV], gl[NV], qg[3][NV], GR[NV];
+    from_pert<3>(ph, wf, uf);
     const double keep = ghost_states<3>(bcs[-1 - pe], uf, ph.gamma, gi, gl);
+    to_pert<3>(ph, gl, gl);
 #pragma unroll
     for (int n = 0; n < 3; ++n)
 #pragma unroll
@@ -156,6 +170,24 @@ __device__ __forceinline__ void face_visc(const double *uf, const double (*qf)[N
 #pragma unroll
     for (int a = 0; a < NV; ++a) G[a] = (wl != 0.0 ? wl * G[a] : 0.0) + (wr != 0.0 ? wr * GR[a] : 0.0);
   }
+}
+
+// the same with operands in R (boundary instantiations of k_hex_gradface; the ghost-state algebra stays in double)
+template <bool BND, typename R>
+__device__ __forceinline__ void face_visc_r(const R *wf, const R (*qf)[NV], const R *nrm, const Phys &ph, int pe, const BcDev *__restrict__ bcs,
+                                            R *G) {
+  double w[NV], q[3][NV], n3[3], g[NV];
+#pragma unroll
+  for (int a = 0; a < NV; ++a) w[a] = (double)wf[a];
+#pragma unroll
+  for (int n = 0; n < 3; ++n) {
+    n3[n] = (double)nrm[n];
+#pragma unroll
+    for (int a = 0; a < NV; ++a) q[n][a] = (double)qf[n][a];
+  }
+  face_visc<BND>(w, q, n3, ph, pe, bcs, g);
+#pragma unroll
+  for (int a = 0; a < NV; ++a) G[a] = (R)g[a];
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -191,19 +223,20 @@ bool encode3(CUtensorMap *m, bool f64, const void *base, uint64_t d0, uint64_t d
 
 // Element-blocked internal array (fr_dev.hpp: fp_row) [ld / FR_BLK][r2][r1][FR_BLK] as a 4-D map (lane, r1, r2, block);
 // box (E, b1, b2, 1).  Coordinates of a CTA that starts at element e0: (e0 % FR_BLK, row, block of rows, e0 / FR_BLK).
-inline bool encode_blk(CUtensorMap *m, const void *base, uint64_t ld, uint64_t r1, uint64_t r2, uint32_t E, uint32_t b1, uint32_t b2,
+inline bool encode_blk(CUtensorMap *m, bool f64, const void *base, uint64_t ld, uint64_t r1, uint64_t r2, uint32_t E, uint32_t b1, uint32_t b2,
                        int bcast = 0) {
   EncodeTiledFn fn = encoder();
   if (!fn) return false;
+  const uint64_t esz = f64 ? 8 : 4;
   cuuint64_t dims[4] = {(cuuint64_t)FR_BLK, r1, r2, ld / FR_BLK};
-  cuuint64_t strides[3] = {(cuuint64_t)FR_BLK * 8, r1 * FR_BLK * 8, r1 * r2 * FR_BLK * 8};
+  cuuint64_t strides[3] = {(cuuint64_t)FR_BLK * esz, r1 * FR_BLK * esz, r1 * r2 * FR_BLK * esz};
   // affine meshes store one point per element: the point dimension(s) are broadcast through a zero stride, so the
   // kernels see the same [rows][E] boxes while DRAM holds (and serves) each value once
-  if (bcast == 1) { strides[0] = 0; strides[1] = FR_BLK * 8; strides[2] = r2 * FR_BLK * 8; }       // r1 broadcast: [block][r2][FR_BLK]
-  if (bcast == 2) { strides[0] = 0; strides[1] = 0; strides[2] = FR_BLK * 8; }                      // r1 and r2 broadcast: [block][FR_BLK]
+  if (bcast == 1) { strides[0] = 0; strides[1] = FR_BLK * esz; strides[2] = r2 * FR_BLK * esz; }   // r1 broadcast: [block][r2][FR_BLK]
+  if (bcast == 2) { strides[0] = 0; strides[1] = 0; strides[2] = FR_BLK * esz; }                    // r1 and r2 broadcast: [block][FR_BLK]
   cuuint32_t box[4] = {E, b1, b2, 1};
   cuuint32_t estr[4] = {1, 1, 1, 1};
-  return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+  return fn(m, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -217,10 +250,12 @@ cudaError_t set_smem(K kern, size_t smem, DevFlags &done, int dev) {
   return e;
 }
 
-// elements per CTA for each n = p + 1 (row segments of E*8 bytes)
-template <int N>
+// elements per CTA for each n = p + 1 (row segments of E*8 bytes; N = 7: only 4 elements fit the shared memory).  The same in
+// single precision: twice the elements (64-byte segments again) halves the resident CTAs of the register-bound kernels and
+// was slower (C3 fp32: gradient kernel 0.41 -> 0.47 ms, divergence kernel 0.19 -> 0.22 ms)
+template <int N, typename T>
 struct Cfg {
-  static constexpr int E = N <= 2 ? 32 : (N == 3 ? 16 : (N <= 6 ? 8 : 4));  // N = 7: only 4 elements fit the shared memory
+  static constexpr int E = N <= 2 ? 32 : (N == 3 ? 16 : (N <= 6 ? 8 : 4));
 };
 
 }  // namespace
