@@ -43,6 +43,12 @@ def parse():
     ap.add_argument("--system", default="")
     ap.add_argument("--generic", action="store_true", help="force the generic staged kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fill", type=float, default=0.0, help="size the mesh so that the device footprint is this fraction of 180 GB (C5)")
+    ap.add_argument("--sweep", action="store_true", help="C5 sweep: one JSON line per (p, system, precision) at --fill")
+    ap.add_argument("--sweep-p", default="1,2,3,4,5,6")
+    ap.add_argument("--sweep-systems", default="navier-stokes,euler")
+    ap.add_argument("--sweep-precisions", default="f64,f32")
+    ap.add_argument("--peaks", action="store_true", help="measure the FP64 / FP32 FMA peaks and the copy bandwidth of this GPU")
     return ap.parse_args()
 
 
@@ -217,45 +223,65 @@ def run_reference(args):
     print(json.dumps(out))
 
 
-def main():
-    args = parse()
-    if args.impl == "reference":
-        return run_reference(args)
+def fill_size(args, fraction, hbm_bytes=180e9):
+    """Elements per direction of the periodic cube whose device footprint (u, rhs, RHS scratch, RK4 registers, the library's own
+    tables) is `fraction` of the HBM, from the library's own size queries on a small probe mesh; capped so that the host-side
+    setup (mesh arrays, coordinates, lookup tables: measured ~ (600 + 170 N_f + 60 N_u) bytes per element at peak) stays inside
+    the box's free memory."""
+    from paper_1312_1638_b200 import Context
+    from paper_1312_1638_b200.binding import FLAG_HOST_ONLY
 
+    a2 = argparse.Namespace(**vars(args))
+    a2.n = 4
+    mesh, disc, _, _ = workload(a2)
+    ctx = Context(mesh).setup_operators(precision=args.precision, **disc)
+    ld = ctx.ld
+    sz = 8 if args.precision == "f64" else 4
+    tables = ctx.Nf / 2 * (16 + 5 * sz) + ctx.Nf * (3 * sz + 8) + 6 + 10 * sz
+    per_elem = (2 * ctx.state_bytes + ctx.workspace_bytes) / ld + tables
+    ctx.teardown()
+    n_dev = int((fraction * hbm_bytes / per_elem) ** (1.0 / 3.0))
+    host_per_elem = 600 + 170 * ctx.Nf + 60 * ctx.Nu + 2 * ctx.Nu * ctx.NV * sz
+    try:
+        avail = [int(l.split()[1]) * 1024 for l in open("/proc/meminfo") if l.startswith("MemAvailable")][0]
+    except Exception:
+        avail = 64e9
+    n_host = int((0.55 * avail / host_per_elem) ** (1.0 / 3.0))
+    return min(n_dev, n_host), per_elem, n_dev, n_host
+
+
+def measure(args, world, rank, local, barrier, light=False):
+    """One workload: device-resident timing, end to end with host buffers, per-kernel events, RK4 step; returns the JSON dict
+    (rank 0) or None.  light: no end-to-end leg and no CPU baseline (sweeps at 90 GB)."""
     import torch
-    import torch.distributed as dist
 
     from paper_1312_1638_b200 import Context
-    from paper_1312_1638_b200.binding import FLAG_FORCE_GENERIC
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the FR library has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+    from paper_1312_1638_b200.binding import FLAG_FORCE_GENERIC, FLAG_LEAN
 
     mesh, disc, over, desc = workload(args)
     t0 = time.time()
-    ctx = Context(mesh).setup_operators(precision=args.precision, flags=FLAG_FORCE_GENERIC if args.generic else 0, **disc)
+    flags = (FLAG_FORCE_GENERIC if args.generic else 0) | (FLAG_LEAN if light else 0)
+    ctx = Context(mesh).setup_operators(precision=args.precision, flags=flags, **disc)
     setup_s = time.time() - t0
+    n_el_mesh, p_g = int(mesh["nodes"].shape[0]), mesh["p_g"]
+    if light:
+        mesh = None  # release the host mesh
     X = ctx.solution_point_coords()
     U = ctx.pad(W.config_state(args.workload, X, **over))
+    del X
     dof = ctx.Nu * ctx.NV * ctx.n_elems
-    u_host = torch.from_numpy(U).pin_memory()
-    r_host = torch.empty_like(u_host).pin_memory()
+    u_host = torch.from_numpy(U)
+    if not light:
+        u_host = u_host.pin_memory()
+        r_host = torch.empty_like(u_host).pin_memory()
     u = u_host.cuda()
+    if light:
+        del u_host, U
     r = torch.zeros_like(u)
     work = torch.zeros(ctx.workspace_bytes, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream().cuda_stream
     up, rp, wp = u.data_ptr(), r.data_ptr(), work.data_ptr()
+    dev_bytes = int(torch.cuda.memory_allocated())
 
     # ---- device-resident timing ----
     for _ in range(max(args.warmup, 3)):
@@ -281,17 +307,20 @@ def main():
     value = aggregate_value(dof, ms_step, world)
 
     # ---- end to end through the C ABI with host buffers (H2D + RHS + D2H per step) ----
-    n_e2e = max(3, min(args.steps, 10))
-    for _ in range(2):
-        ctx.rhs_host(u_host.data_ptr(), r_host.data_ptr(), up, rp, wp, stream)
-    barrier()
-    ev0.record()
-    for _ in range(n_e2e):
-        ctx.rhs_host(u_host.data_ptr(), r_host.data_ptr(), up, rp, wp, stream)
-    ev1.record()
-    barrier()
-    e2e_ms = max_over_ranks(ev0.elapsed_time(ev1), world) / n_e2e
-    e2e_val = aggregate_value(dof, e2e_ms, world)
+    e2e = None
+    if not light:
+        n_e2e = max(3, min(args.steps, 10))
+        for _ in range(2):
+            ctx.rhs_host(u_host.data_ptr(), r_host.data_ptr(), up, rp, wp, stream)
+        barrier()
+        ev0.record()
+        for _ in range(n_e2e):
+            ctx.rhs_host(u_host.data_ptr(), r_host.data_ptr(), up, rp, wp, stream)
+        ev1.record()
+        barrier()
+        e2e_ms = max_over_ranks(ev0.elapsed_time(ev1), world) / n_e2e
+        e2e = {"value": aggregate_value(dof, e2e_ms, world), "unit": UNIT, "ms_per_step": e2e_ms,
+               "h2d_bytes_per_step": int(u_host.numel() * u_host.element_size()), "d2h_bytes_per_step": int(r_host.numel() * r_host.element_size())}
 
     # ---- per-kernel durations (events between kernels, same stream), dominant kernel roofline ----
     acc = {}
@@ -300,9 +329,7 @@ def main():
         for name, ms in ctx.rhs_profiled(up, rp, wp, stream):
             acc[name] = acc.get(name, 0.0) + ms / n_prof
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        return None
     peaks = {}
     pk_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(pk_path):
@@ -310,7 +337,7 @@ def main():
     peak_gbs = float(peaks.get("hbm_gbs", 6650.0))
     peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s"
     nd, NV, Nu, Nf, ns = ctx.ndims, ctx.NV, ctx.Nu, ctx.Nf, disc["system"] == "navier-stokes"
-    affine = mesh["p_g"] == 1
+    affine = p_g == 1
     sz = 8 if args.precision == "f64" else 4
     szi = sz if any(n.startswith("hex_") for n in acc) else 8  # the hexahedral TMA path stores its intermediates in the storage precision
     kern = []
@@ -322,26 +349,30 @@ def main():
     top = kern[0]
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    lib = os.path.join(ROOT, "paper_1312_1638_b200", "libfr_b200.so")
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(args.workload + "-" + args.precision, {}).get(top["name"])
+            t = json.load(open(tpath))
+            # the ncu figures belong to one build of the library: dropped when the sources have changed since
+            if t.get("source_sha16") == source_sha16():
+                traffic = t.get(args.workload + "-" + args.precision, {}).get(top["name"])
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "kernel": top["name"], "achieved": top["algorithmic_GBps"], "peak": peak_gbs, "unit": "GB/s",
                 "frac": (top["algorithmic_GBps"] / peak_gbs) if top["algorithmic_GBps"] else None, "traffic": traffic,
                 "peak_source": peak_src, "kernel_ms": top["ms"], "kernel_share_of_step": top["share"]}
     words = rhs_algorithmic_words(nd, NV, Nu, Nf, ns, affine)
-    rhs_gbs = words * (8 if args.precision == "f64" else 4) * ctx.n_elems / (ms_step * 1e-3) / 1e9
+    rhs_gbs = words * sz * ctx.n_elems / (ms_step * 1e-3) / 1e9
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": args.precision, "data": "synthetic", "config": dict(desc, parallelism="replicas only (%d)" % world, setup_s=round(setup_s, 2)),
+        "dtype": args.precision, "data": "synthetic",
+        "config": dict(desc, parallelism="replicas only (%d)" % world, setup_s=round(setup_s, 2), device_bytes=dev_bytes),
         "clocks": sampler.summary(),
-        "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(u_host.numel() * u_host.element_size()),
-                "d2h_bytes_per_step": int(r_host.numel() * r_host.element_size())},
+        "e2e": e2e,
         "gpu_launches": int(ctx.rhs_kernel_launches) * args.steps,
         "roofline": roofline,
-        "rhs_roofline": {"bound": "hbm", "algorithmic_bytes_per_point": words * (8 if args.precision == "f64" else 4) / Nu,
+        "rhs_roofline": {"bound": "hbm", "algorithmic_bytes_per_point": words * sz / Nu,
                          "achieved": rhs_gbs, "peak": peak_gbs, "unit": "GB/s", "frac": rhs_gbs / peak_gbs,
                          "note": "SURVEY 8(d) fused lower-bound bytes of the WHOLE RHS / measured RHS time"},
         "kernels": kern,
@@ -358,12 +389,95 @@ def main():
     ev1.record()
     torch.cuda.synchronize()
     out["s_per_rk4_step"] = ev0.elapsed_time(ev1) * 1e-3 / nrk
-    if not args.no_cpu_baseline and world == 1:
+    if not light and not args.no_cpu_baseline and world == 1:
         cdof, ts, cores, sample = time_oracle(args, sample_size(args), 5)
-        out["cpu_baseline"] = {"value": cdof / float(np.mean(ts)) / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        out["cpu_baseline"] = {"value": cdof / float(np.mean(ts)) / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                               "cpu": cpu_model()}
     else:
         out["cpu_baseline"] = None
+    ctx.teardown()
+    del u, r, work
+    torch.cuda.empty_cache()
+    return out
+
+
+def source_sha16():
+    """hash of the CUDA sources: profiles/traffic.json records the one its ncu figures were taken with"""
+    import hashlib
+
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1312_1638_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def cpu_model():
+    try:
+        return [l.split(":", 1)[1].strip() for l in open("/proc/cpuinfo") if l.startswith("model name")][0]
+    except Exception:
+        return "unknown"
+
+
+def run_peaks(args):
+    """Measured roofline denominators of this GPU: FP64 / FP32 FMA peaks (the library's microbenchmark) and copy bandwidth."""
+    import torch
+
+    from paper_1312_1638_b200.binding import measure_peaks
+
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    out = measure_peaks()
+    out["gpu"] = torch.cuda.get_device_name()
+    pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(pk):
+        out["driver_hbm_gbs"] = json.load(open(pk)).get("hbm_gbs")
     print(json.dumps(out))
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.peaks:
+        return run_peaks(args)
+
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the FR library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    if args.sweep:
+        # C5 of BASELINE.json: p = 1..6 x {Navier-Stokes, Euler} x {f64, f32} on meshes sized to --fill of the HBM
+        args.workload = "C5"
+        ps = [int(x) for x in args.sweep_p.split(",")]
+        for p in ps:
+            for system in args.sweep_systems.split(","):
+                for prec in args.sweep_precisions.split(","):
+                    a2 = argparse.Namespace(**vars(args))
+                    a2.p, a2.system, a2.precision = p, system, prec
+                    a2.n, per_elem, n_dev, n_host = fill_size(a2, args.fill)
+                    out = measure(a2, world, rank, local, barrier, light=True)
+                    if out is not None:
+                        out["config"].update(fill_target=args.fill, device_bytes_per_element=per_elem, n_for_fill=n_dev, n_host_cap=n_host)
+                        print(json.dumps(out), flush=True)
+    else:
+        if args.fill > 0:
+            args.n = fill_size(args, args.fill)[0]
+        out = measure(args, world, rank, local, barrier, light=args.fill > 0)
+        if out is not None:
+            print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
 

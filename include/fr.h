@@ -95,6 +95,9 @@ typedef struct {
 
 #define FR_FLAG_FORCE_GENERIC 1
 #define FR_FLAG_HOST_ONLY 2      /* build the host tables only (no CUDA call): queries work, fr_rhs fails */
+#define FR_FLAG_LEAN 4           /* release the host copies of the mesh and of the setup tables once they are uploaded (meshes of
+                                    10^7 elements): fr_get_pairs / fr_get_metrics and a second fr_setup_operators then return
+                                    FR_EINVAL; sizes, coordinates, operators, fr_rhs and the steppers are unaffected */
 
 /* Creates a context (owned by the library; release with fr_teardown).  Validates connectivity only;
  * geometric checks happen in fr_setup_operators once the point sets are known. */
@@ -163,6 +166,11 @@ int fr_dopri5_step(fr_ctx *ctx, void *u_dev, double dt, void *work_dev, void *st
  * u_dev / rhs_dev / work_dev are caller-allocated device staging buffers as in fr_rhs. */
 int fr_rhs_host(fr_ctx *ctx, const void *u_host, void *rhs_host, void *u_dev, void *rhs_dev, void *work_dev,
                 void *stream);
+
+/* Roofline denominators of the current CUDA device, measured: FP64 and FP32 FMA throughput (TFLOP/s, FMA-chain
+ * microbenchmark, 2 flops per FMA) and device-to-device copy bandwidth (GB/s, read + write bytes over 2 GiB).  Needs about
+ * 4 GiB of free device memory for a moment; synchronises the device.  Not part of the right-hand-side path. */
+int fr_measure_peaks(double *fp64_tflops_host, double *fp32_tflops_host, double *copy_gbs_host);
 
 /* Frees host objects and the library's own constant uploads.  NULL is allowed. */
 void fr_teardown(fr_ctx *ctx);

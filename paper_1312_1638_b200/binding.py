@@ -17,7 +17,7 @@ QUAD, TRI, HEX = 0, 1, 2
 EULER, NAVIER_STOKES = 0, 1
 F32, F64 = 0, 1
 BC_SUP_INFLOW, BC_SUB_OUTFLOW, BC_NOSLIP_WALL = 0, 1, 2
-FLAG_FORCE_GENERIC, FLAG_HOST_ONLY = 1, 2
+FLAG_FORCE_GENERIC, FLAG_HOST_ONLY, FLAG_LEAN = 1, 2, 4
 CORRECTIONS = {"dg": 0, "sd": 1, "hu": 2}
 STEPPERS = {"euler": 0, "rk4": 1, "dopri5": 2}
 ETYPES = {"quad": QUAD, "tri": TRI, "hex": HEX}
@@ -77,6 +77,7 @@ def _load():
         "fr_rhs_profiled": (C.c_int, [P, P, P, P, P, C.c_int, C.POINTER(C.c_int), P, P]),
         "fr_rk4_step": (C.c_int, [P, P, C.c_double, P, P]),
         "fr_rhs_host": (C.c_int, [P, P, P, P, P, P, P]),
+        "fr_measure_peaks": (C.c_int, [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]),
         "fr_teardown": (None, [P]),
         "fr_last_error": (C.c_char_p, [P]),
     }
@@ -91,7 +92,16 @@ EXPORTS = ["fr_setup_mesh", "fr_setup_operators", "fr_num_solution_points", "fr_
            "fr_leading_dim", "fr_state_bytes", "fr_workspace_bytes", "fr_stepper_workspace_bytes", "fr_rhs_kernel_launches",
            "fr_euler_step", "fr_dopri5_step", "fr_solution_point_coords",
            "fr_operator_dims", "fr_get_operator", "fr_get_pairs", "fr_get_metrics", "fr_rhs", "fr_rhs_profiled", "fr_rk4_step", "fr_rhs_host",
-           "fr_teardown", "fr_last_error"]
+           "fr_measure_peaks", "fr_teardown", "fr_last_error"]
+
+
+def measure_peaks():
+    """-> dict(fp64_tflops, fp32_tflops, copy_gbs) of the current CUDA device (fr_measure_peaks)."""
+    a, b, c = C.c_double(), C.c_double(), C.c_double()
+    rc = lib.fr_measure_peaks(C.byref(a), C.byref(b), C.byref(c))
+    if rc != 0:
+        raise FrError(rc, "fr_measure_peaks failed")
+    return {"fp64_tflops": a.value, "fp32_tflops": b.value, "copy_gbs": c.value}
 
 
 def _ptr(a):

@@ -23,6 +23,7 @@ struct fr_ctx {
   bool ready = false;
   bool use_tensor = false;
   bool host_only = false;
+  bool lean = false;  // FR_FLAG_LEAN: host tables released after upload
   DevConsts dc{};
   WorkLayout wl{};
   TensorPlan tp{};
@@ -105,6 +106,7 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
   if (d->precision != FR_F32 && d->precision != FR_F64) return fail(c, FR_EINVAL, "unknown precision");
   if (!(d->gamma > 1.0)) return fail(c, FR_EINVAL, "gamma must be > 1");
   if (d->system == FR_NAVIER_STOKES && (!(d->mu >= 0.0) || !(d->Pr > 0.0))) return fail(c, FR_EINVAL, "mu >= 0 and Pr > 0 required");
+  if (c->lean) return fail(c, FR_EINVAL, "fr_setup_operators: the context was set up with FR_FLAG_LEAN (host mesh released)");
   try {
     c->ready = false;
     free_dev(c);
@@ -233,6 +235,14 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     w.partials = take((int64_t)RK_MAX_PARTIALS * 8);
     w.reg0 = off; w.reg_stride = align_up(state, 256);
     w.total = w.reg0 + 3 * w.reg_stride;
+    if (d->flags & FR_FLAG_LEAN) {
+      auto drop = [](auto &v) { typename std::decay<decltype(v)>::type().swap(v); };
+      MeshConsts &m = c->mc;
+      drop(m.smat); drop(m.rcpj); drop(m.pLs); drop(m.pLe); drop(m.pRs); drop(m.pRe); drop(m.pn); drop(m.pJnL); drop(m.pJnR);
+      drop(m.bs); drop(m.be); drop(m.bbc); drop(m.bn); drop(m.bJn); drop(m.fp_pe); drop(m.fp_ps); drop(m.fp_n); drop(m.fp_Jn);
+      drop(c->mesh.nodes); drop(c->mesh.ifaces); drop(c->mesh.shifts); drop(c->mesh.bfaces);
+      c->lean = true;
+    }
     c->ready = true;
     return FR_OK;
   } catch (const std::bad_alloc &) {
@@ -287,6 +297,7 @@ int fr_get_operator(const fr_ctx *c, int id, double *buf) {
 
 int fr_get_pairs(const fr_ctx *c, int32_t *pairs, double *normals, double *jn) {
   FR_NEED_READY(c, FR_EINVAL)
+  if (c->lean) return fail(c, FR_EINVAL, "fr_get_pairs: host tables were released (FR_FLAG_LEAN)");
   const MeshConsts &m = c->mc;
   const int nd = c->ops.nd;
   for (int64_t i = 0; i < m.npairs; ++i) {
@@ -299,6 +310,7 @@ int fr_get_pairs(const fr_ctx *c, int32_t *pairs, double *normals, double *jn) {
 
 int fr_get_metrics(const fr_ctx *c, double *smat, double *rcpj) {
   FR_NEED_READY(c, FR_EINVAL)
+  if (c->lean) return fail(c, FR_EINVAL, "fr_get_metrics: host tables were released (FR_FLAG_LEAN)");
   if (smat) std::memcpy(smat, c->mc.smat.data(), c->mc.smat.size() * sizeof(double));
   if (rcpj) std::memcpy(rcpj, c->mc.rcpj.data(), c->mc.rcpj.size() * sizeof(double));
   return FR_OK;

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <numeric>
+#include <parallel/algorithm>
 
 #include "fr_host.hpp"
 
@@ -152,11 +153,12 @@ int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, int pa
     if (pair_block <= 0) return (int64_t)pr.Ls * Nel + pr.Le;
     return ((int64_t)(pr.Le / pair_block) * Nf + pr.Ls) * pair_block + pr.Le % pair_block;
   };
-  std::sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return key(pairs[a]) < key(pairs[b]); });
+  __gnu_parallel::sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return key(pairs[a]) < key(pairs[b]); });
   const int64_t np = (int64_t)pairs.size();
   out.npairs = np;
   out.pLs.resize(np); out.pLe.resize(np); out.pRs.resize(np); out.pRe.resize(np);
   out.pn.resize((size_t)nd * np); out.pJnL.resize(np); out.pJnR.resize(np);
+#pragma omp parallel for schedule(static)
   for (int64_t i = 0; i < np; ++i) {
     const Pair &pr = pairs[order[i]];
     out.pLs[i] = pr.Ls; out.pLe[i] = pr.Le; out.pRs[i] = pr.Rs; out.pRe[i] = pr.Re;
@@ -167,6 +169,7 @@ int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, int pa
     out.fp_pe[(size_t)pr.Ls * ld + pr.Le] = pr.Re; out.fp_ps[(size_t)pr.Ls * ld + pr.Le] = pr.Rs;
     out.fp_pe[(size_t)pr.Rs * ld + pr.Re] = pr.Le; out.fp_ps[(size_t)pr.Rs * ld + pr.Re] = pr.Ls;
   }
+#pragma omp parallel for schedule(static)
   for (int64_t i = 0; i < np; ++i) {  // R side flagged by a negative J*n
     const Pair &pr = pairs[order[i]];
     out.fp_Jn[(size_t)pr.Rs * ld + pr.Re] = -out.fp_Jn[(size_t)pr.Rs * ld + pr.Re];
