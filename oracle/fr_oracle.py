@@ -467,7 +467,7 @@ class FROracle:
     dtype: np.float64 or np.longdouble for the STATE arithmetic (operators and metrics are
     always built in long double and rounded once to dtype)."""
 
-    def __init__(self, mesh, prm, bcs=None, dtype=np.float64):
+    def __init__(self, mesh, prm, bcs=None, dtype=np.float64, pair=True):
         self.mesh, self.prm, self.bcs, self.dtype = mesh, dict(prm), bcs or {}, dtype
         self.ref = ref = RefElement(mesh["etype"], prm["p"])
         self.ops = Operators(ref, self.prm.get("correction", "dg"))
@@ -475,7 +475,8 @@ class FROracle:
         self.NV = ref.nd + 2
         self.Nel = mesh["nodes"].shape[0]
         self._geometry()
-        self._pair()
+        if pair:  # FRMixedOracle pairs the flux points of all element types itself
+            self._pair()
         c = lambda a: np.asarray(a, dtype=dtype)
         o = self.ops
         self.M0, self.M1, self.M2, self.M3, self.M4, self.M6 = c(o.M0), c(o.M1), c(o.M2), c(o.M3), c(o.M4), c(o.M6)
@@ -674,3 +675,133 @@ class FROracle:
     def l2_error(self, a, b):
         """sqrt( integral (a-b)^2 ) per variable (Eq 32 :557)."""
         return np.sqrt(self.integrate((a - b) ** 2))
+
+
+# =============================================================================
+# meshes of several element types (PAPER.md:141 element types; :603 "mixed unstructured mesh")
+# =============================================================================
+class FRMixedOracle:
+    """FR semi-discretisation on a mesh whose parts have different element types (workloads.mixed_mesh dictionary).
+    Every element-local step (O5, O7, O8, O10) is the single-type oracle's, part by part; the interface steps (O6, O9) run
+    over flux-point pairs whose two sides may lie in different parts -- "only the lookup table changes".
+    States, right-hand sides: lists of arrays [N_u(part), N_V, N_el(part)]."""
+
+    def __init__(self, mesh, prm, bcs=None, dtype=np.float64):
+        self.mesh, self.prm, self.bcs, self.dtype = mesh, dict(prm), bcs or {}, dtype
+        self.nd = mesh["ndims"]
+        self.parts = []
+        for part in mesh["parts"]:
+            sub = {"ndims": mesh["ndims"], "etype": part["etype"], "p_g": part["p_g"], "nodes": part["nodes"],
+                   "ifaces": np.zeros((0, 4), np.int32), "shifts": np.zeros((0, self.nd)), "bfaces": np.zeros((0, 3), np.int32)}
+            self.parts.append(FROracle(sub, prm, None, dtype, pair=False))
+        self._pair()
+
+    def _pair(self):
+        """Lookup table by brute-force matching of physical flux-point coordinates across parts (reading A11)."""
+        P = self.parts
+        pairs = []  # (partL, sigmaL, elemL, partR, sigmaR, elemR)
+        for (tL, eL, fL, tR, eR, fR), shift in zip(self.mesh["ifaces"], self.mesh["shifts"]):
+            nL, nR = P[tL].ref.nfp, P[tR].ref.nfp
+            if nL != nR:
+                raise ValueError("the two sides of an interface have different numbers of flux points")
+            sL, sR = fL * nL + np.arange(nL), fR * nR + np.arange(nR)
+            xL = np.asarray(P[tL].xf_phys, float)[sL, eL]
+            xR = np.asarray(P[tR].xf_phys, float)[sR, eR] + shift[None, :]
+            d2 = np.sum((xL[:, None, :] - xR[None, :, :]) ** 2, -1)
+            match = np.argmin(d2, axis=1)
+            h = np.sqrt(np.sum((xL[0] - xL[-1]) ** 2)) if nL > 1 else 1.0
+            if np.sqrt(np.max(np.min(d2, axis=1))) > 1e-9 * h + 1e-12 or sorted(match.tolist()) != list(range(nR)):
+                raise ValueError("unmatched flux-point pair on a mixed interface")
+            for k in range(nL):
+                pairs.append((tL, sL[k], eL, tR, sR[match[k]], eR))
+        self.pairs = np.array(pairs, dtype=np.int64).reshape(-1, 6)
+        bnd = []
+        for (t, e, f, bc) in self.mesh["bfaces"]:
+            nfp = P[t].ref.nfp
+            bnd += [(t, f * nfp + k, e, bc) for k in range(nfp)]
+        self.bnd = np.array(bnd, dtype=np.int64).reshape(-1, 4)
+        cnt = [np.zeros((q.Nf, q.Nel), dtype=np.int64) for q in P]
+        for (tL, sL, eL, tR, sR, eR) in self.pairs:
+            cnt[tL][sL, eL] += 1
+            cnt[tR][sR, eR] += 1
+        for (t, s_, e, _) in self.bnd:
+            cnt[t][s_, e] += 1
+        if any(np.any(c != 1) for c in cnt):
+            raise ValueError("flux points not covered exactly once by interfaces + boundaries")
+
+    def _side(self, arrs, side):
+        """values at the flux points of one side of every pair: [npairs, ...]"""
+        t, s_, e = self.pairs[:, 3 * side], self.pairs[:, 3 * side + 1], self.pairs[:, 3 * side + 2]
+        out = None
+        for k in range(len(self.parts)):
+            m = t == k
+            if not np.any(m):
+                continue
+            v = arrs[k][s_[m], ..., e[m]] if arrs[k].ndim == 3 else arrs[k][s_[m], e[m]]
+            if out is None:
+                out = np.zeros((len(t),) + v.shape[1:], dtype=v.dtype)
+            out[m] = v
+        return out
+
+    def _scatter(self, dst, side, vals):
+        t, s_, e = self.pairs[:, 3 * side], self.pairs[:, 3 * side + 1], self.pairs[:, 3 * side + 2]
+        for k in range(len(self.parts)):
+            m = t == k
+            if np.any(m):
+                dst[k][s_[m], :, e[m]] = vals[m]
+
+    def rhs(self, us):
+        P, prm, nd = self.parts, self.prm, self.nd
+        ns = prm["system"] == "navier-stokes"
+        us = [np.asarray(u, dtype=self.dtype) for u in us]
+        ufs = [q.interpolate(u) for q, u in zip(P, us)]                      # O5
+        qs, qfs = [None] * len(P), [None] * len(P)
+        bmask = [self.bnd[:, 0] == k for k in range(len(P))]
+        if ns:
+            b = prm["beta"]
+            uL, uR = self._side(ufs, 0), self._side(ufs, 1)                   # O6, Eq 7 + Eq 25
+            c = (0.5 - b) * uL + (0.5 + b) * uR
+            Cs = [np.empty_like(uf) for uf in ufs]
+            self._scatter(Cs, 0, c)
+            self._scatter(Cs, 1, c)
+            for k, q in enumerate(P):
+                for bc_id, (kind, par) in self.bcs.items():
+                    m = bmask[k] & (self.bnd[:, 3] == bc_id)
+                    if np.any(m):
+                        s_, e = self.bnd[m, 1], self.bnd[m, 2]
+                        ub = ufs[k][s_, :, e].T
+                        _, gl, _ = ghost_states(kind, par, ub, prm["gamma"])
+                        Cs[k][s_, :, e] = ((0.5 - b) * ub + (0.5 + b) * gl).T
+                qs[k], qfs[k] = q.gradient(us[k], ufs[k], Cs[k])              # O7
+        fts = [q.transformed_flux(u, qq) for q, u, qq in zip(P, us, qs)]      # O8
+        Ds = [np.empty_like(uf) for uf in ufs]                                # O9
+        uL, uR = self._side(ufs, 0).T, self._side(ufs, 1).T
+        qL = np.stack([self._side([qf[n] for qf in qfs], 0).T for n in range(nd)]) if ns else None
+        qR = np.stack([self._side([qf[n] for qf in qfs], 1).T for n in range(nd)]) if ns else None
+        nL = self._side([np.moveaxis(q.nhat_f, 2, 1) for q in P], 0).T  # [nd, npairs]
+        F = common_flux(uL, uR, qL, qR, nL, prm)
+        JL, JR = self._side([q.Jn_f for q in P], 0), self._side([q.Jn_f for q in P], 1)
+        self._scatter(Ds, 0, (JL[None, :] * F).T)
+        self._scatter(Ds, 1, (-JR[None, :] * F).T)
+        for k, q in enumerate(P):
+            for bc_id, (kind, par) in self.bcs.items():
+                m = bmask[k] & (self.bnd[:, 3] == bc_id)
+                if np.any(m):
+                    s_, e = self.bnd[m, 1], self.bnd[m, 2]
+                    ub = ufs[k][s_, :, e].T
+                    gi, gl, keep = ghost_states(kind, par, ub, prm["gamma"])
+                    qb = np.stack([qfs[k][n][s_, :, e].T for n in range(nd)]) if ns else None
+                    Fb = common_flux(ub, gl, qb, keep * qb if ns else None, q.nhat_f[s_, e].T, prm, uR_inv=gi)
+                    Ds[k][s_, :, e] = (q.Jn_f[s_, e][None, :] * Fb).T
+        return [q.divergence(ft, D) for q, ft, D in zip(P, fts, Ds)]          # O10
+
+    def rk4_step(self, us, dt):
+        add = lambda a, b, c: [x + c * y for x, y in zip(a, b)]
+        k1 = self.rhs(us)
+        k2 = self.rhs(add(us, k1, dt / 2))
+        k3 = self.rhs(add(us, k2, dt / 2))
+        k4 = self.rhs(add(us, k3, dt))
+        return [u + (dt / 6) * (a + 2 * b + 2 * c + d) for u, a, b, c, d in zip(us, k1, k2, k3, k4)]
+
+    def integrate(self, gs):
+        return sum(q.integrate(g) for q, g in zip(self.parts, gs))

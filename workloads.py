@@ -197,6 +197,108 @@ def tri_mesh(n, length=1.0, jitter=0.1, seed=4321, periodic=True):
     }
 
 
+def mixed_mesh(n, length=1.0, jitter=0.1, seed=2468, periodic=True, tri_from=None):
+    """Quadrilaterals and triangles sharing edges in one mesh (the paper's mixed unstructured workload): an n x n
+    grid on [0,length]^2 whose columns i < tri_from (default n // 2) stay quadrilaterals while the others are split into
+    triangles along alternating diagonals; interior vertices jittered by U(-jitter*h, jitter*h) (seeded), boundary vertices
+    unjittered so that periodic images match.  Straight-sided (p_g = 1; the jittered quadrilaterals are bilinear, not affine).
+
+    Mixed mesh dictionary:
+      ndims 2, parts: [ {etype, p_g, nodes [n_el, n_nodes, 2]} , ... ]   (part 0 = quads, part 1 = triangles)
+      ifaces  int32 [n_if, 6] = (partL, elemL, faceL, partR, elemR, faceR)   (order significant, A12)
+      shifts  float64 [n_if, 2]:  x_L = x_R + shift
+      bfaces  int32 [n_b, 4] = (part, elem, face, bc_id)      bc_id: 0 bottom, 1 right, 2 top, 3 left
+    Face numbering per type as in the single-type meshes (quad face = 2 d + s, triangle face k = edge v_k -> v_k+1)."""
+    tri_from = n // 2 if tri_from is None else tri_from
+    h = length / n
+    rng = np.random.default_rng(seed)
+    vx, vy = np.meshgrid(np.arange(n + 1) * h, np.arange(n + 1) * h, indexing="xy")
+    V = np.stack([vx, vy], -1)
+    jit = rng.uniform(-jitter * h, jitter * h, size=V.shape)
+    jit[0, :, :] = 0.0
+    jit[-1, :, :] = 0.0
+    jit[:, 0, :] = 0.0
+    jit[:, -1, :] = 0.0
+    Vf = (V + jit).reshape(-1, 2)
+
+    def vid(i, j):
+        return j * (n + 1) + i
+
+    def canon(v):
+        i, j = v % (n + 1), v // (n + 1)
+        if periodic:
+            i, j = i % n, j % n
+        return j * (n + 1) + i
+
+    quads, tris = [], []
+    edges = {}
+
+    def add_edge(v0, v1, part, elem, face):
+        edges.setdefault(tuple(sorted((canon(v0), canon(v1)))), []).append((part, elem, face, v0, v1))
+
+    for j in range(n):
+        for i in range(n):
+            a, b, c, d = vid(i, j), vid(i + 1, j), vid(i + 1, j + 1), vid(i, j + 1)
+            if i < tri_from:
+                e = len(quads)
+                quads.append((a, b, d, c))  # lattice order (0,0),(1,0),(0,1),(1,1)
+                for face, (v0, v1) in enumerate(((a, d), (b, c), (a, b), (d, c))):  # faces x-, x+, y-, y+
+                    add_edge(v0, v1, 0, e, face)
+            else:
+                pair = ((a, b, c), (a, c, d)) if (i + j) % 2 == 0 else ((a, b, d), (b, c, d))
+                for t in pair:
+                    e = len(tris)
+                    tris.append(t)
+                    for k in range(3):
+                        add_edge(t[k], t[(k + 1) % 3], 1, e, k)
+    ifaces, shifts, bfaces = [], [], []
+    tol = 1e-9 * length
+    for lst in edges.values():
+        if len(lst) == 2:
+            (pL, eL, fL, a0, a1), (pR, eR, fR, b0, b1) = lst
+            mL, mR = 0.5 * (Vf[a0] + Vf[a1]), 0.5 * (Vf[b0] + Vf[b1])
+            ifaces.append((pL, eL, fL, pR, eR, fR))
+            shifts.append(np.round((mL - mR) / length) * length)
+        elif len(lst) == 1:
+            (pt, e, f, a0, a1) = lst[0]
+            mid = 0.5 * (Vf[a0] + Vf[a1])
+            bc = 0 if mid[1] < tol else 1 if mid[0] > length - tol else 2 if mid[1] > length - tol else 3
+            bfaces.append((pt, e, f, bc))
+        else:
+            raise RuntimeError("non-manifold edge")
+    parts = []
+    if quads:
+        parts.append({"etype": "quad", "p_g": 1, "nodes": np.ascontiguousarray(Vf[np.array(quads)], dtype=np.float64)})
+    if tris:
+        parts.append({"etype": "tri", "p_g": 1, "nodes": np.ascontiguousarray(Vf[np.array(tris)], dtype=np.float64)})
+    if len(parts) == 1:  # degenerate splits keep the part numbering of the interface records consistent
+        only = 0 if quads else 1
+        ifaces = [(0, eL, fL, 0, eR, fR) for (_, eL, fL, _, eR, fR) in ifaces]
+        bfaces = [(0, e, f, bc) for (_, e, f, bc) in bfaces]
+        del only
+    return {
+        "ndims": 2,
+        "parts": parts,
+        "ifaces": np.array(ifaces, dtype=np.int32).reshape(-1, 6),
+        "shifts": np.array(shifts, dtype=np.float64).reshape(-1, 2),
+        "bfaces": np.array(bfaces, dtype=np.int32).reshape(-1, 4),
+        "lengths": (length, length),
+        "shape": (n, n),
+    }
+
+
+def part_mesh(mixed, t):
+    """Part t of a mixed mesh as a single-type mesh dictionary: the interfaces whose two sides lie in the part, and the part's
+    boundary faces (topology bookkeeping only)."""
+    ifc, bf = mixed["ifaces"], mixed["bfaces"]
+    own = (ifc[:, 0] == t) & (ifc[:, 3] == t)
+    return {
+        "ndims": mixed["ndims"], "etype": mixed["parts"][t]["etype"], "p_g": mixed["parts"][t]["p_g"], "nodes": mixed["parts"][t]["nodes"],
+        "ifaces": np.ascontiguousarray(ifc[own][:, [1, 2, 4, 5]]), "shifts": np.ascontiguousarray(mixed["shifts"][own]),
+        "bfaces": np.ascontiguousarray(bf[bf[:, 0] == t][:, 1:]), "lengths": mixed["lengths"], "shape": mixed["shape"],
+    }
+
+
 def curve_tri_mesh(mesh, p_g=2, amplitude=0.01):
     """Raises a straight-sided triangle mesh to geometry degree p_g: lattice nodes (rows j = 0..p_g, i = 0..p_g-j) of each
     straight triangle, displaced by amplitude*sin(2 pi x/L)*sin(2 pi y/L) in both coordinates (smooth, zero on the box
