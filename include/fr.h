@@ -71,6 +71,29 @@ typedef struct {
   const fr_bc_desc *bcs;   /* [n_bcs] */
 } fr_mesh_desc;
 
+/* Mesh of SEVERAL element types sharing faces (PAPER.md:141 "triangles, quadrilaterals"; :603 the mixed unstructured mesh of
+ * Table 2): parts of one element type each, and interface records that name the part of each side.  2-D (quadrilaterals and
+ * triangles).  All pointers: host, read during the call only. */
+typedef struct {
+  int32_t etype;           /* FR_QUAD | FR_TRI */
+  int32_t p_g;
+  int64_t n_elems;
+  const double *nodes;     /* [n_elems][n_nodes(p_g)][ndims] */
+} fr_mesh_part;
+
+typedef struct {
+  int32_t ndims;           /* 2 */
+  int32_t n_parts;
+  int32_t n_bcs;
+  int32_t reserved;
+  int64_t n_ifaces, n_bfaces;
+  const fr_mesh_part *parts;
+  const int32_t *ifaces;   /* [n_ifaces][6] = partL, elemL, faceL, partR, elemR, faceR; L/R order is significant (A12) */
+  const double *shifts;    /* [n_ifaces][ndims] */
+  const int32_t *bfaces;   /* [n_bfaces][4] = part, elem, face, bc_id */
+  const fr_bc_desc *bcs;
+} fr_mixed_mesh_desc;
+
 /* Discretisation: order p, system (§4), storage precision, gas constants gamma (Eq 21),
  * mu, Pr (Eq 22-23; mu constant, A9), LDG beta / tau (Eq 25-27 :506-516; tau enters with the dissipative
  * sign, A7).  Point sets are fixed (A6).  correction: FR_CORR_DG (A5; every element type), FR_CORR_SD / FR_CORR_HU
@@ -102,6 +125,20 @@ typedef struct {
 /* Creates a context (owned by the library; release with fr_teardown).  Validates connectivity only;
  * geometric checks happen in fr_setup_operators once the point sets are known. */
 int fr_setup_mesh(fr_ctx **out, const fr_mesh_desc *mesh);
+
+/* The same for a mesh of several element types.  State matrices of such a context are ONE buffer holding the parts one after
+ * the other: part t is a [N_u(t)][N_V][ld(t)] matrix at byte offset fr_part_info(...).state_offset (256-byte aligned);
+ * fr_state_bytes gives the total.  fr_rhs and the steppers take that buffer; the orders 1 <= p <= 4 (fused element kernels of
+ * both types) are supported, FR_EUNSUPPORTED otherwise.  Single-type size queries (fr_num_solution_points, fr_num_flux_points,
+ * fr_leading_dim, fr_solution_point_coords, fr_get_*) return FR_EINVAL on a mixed context: use the per-part queries. */
+int fr_setup_mesh_mixed(fr_ctx **out, const fr_mixed_mesh_desc *mesh);
+int64_t fr_num_parts(const fr_ctx *ctx);           /* 1 for a single-type context */
+typedef struct {
+  int32_t etype, reserved;
+  int64_t n_elems, n_solution_points, n_flux_points, leading_dim, state_offset /* bytes */;
+} fr_part_info_t;
+int fr_part_info(const fr_ctx *ctx, int part, fr_part_info_t *info_host);
+int fr_part_solution_point_coords(const fr_ctx *ctx, int part, double *xyz_host); /* [N_u][n_elems][ndims] of the part */
 
 /* Builds M0..M6 (App A :737-768) on the host in extended precision, the metric terms S = J*J^-1, 1/J
  * (Eq 10, 12, 19) at the solution points, the physical normals and J*n (Eq 14, 16) at the flux points,

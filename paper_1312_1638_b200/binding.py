@@ -43,6 +43,23 @@ class fr_mesh_desc(C.Structure):
     ]
 
 
+class fr_mesh_part(C.Structure):
+    _fields_ = [("etype", C.c_int32), ("p_g", C.c_int32), ("n_elems", C.c_int64), ("nodes", C.c_void_p)]
+
+
+class fr_mixed_mesh_desc(C.Structure):
+    _fields_ = [
+        ("ndims", C.c_int32), ("n_parts", C.c_int32), ("n_bcs", C.c_int32), ("reserved", C.c_int32),
+        ("n_ifaces", C.c_int64), ("n_bfaces", C.c_int64),
+        ("parts", C.c_void_p), ("ifaces", C.c_void_p), ("shifts", C.c_void_p), ("bfaces", C.c_void_p), ("bcs", C.c_void_p),
+    ]
+
+
+class fr_part_info_t(C.Structure):
+    _fields_ = [("etype", C.c_int32), ("reserved", C.c_int32), ("n_elems", C.c_int64), ("n_solution_points", C.c_int64),
+                ("n_flux_points", C.c_int64), ("leading_dim", C.c_int64), ("state_offset", C.c_int64)]
+
+
 class fr_disc_desc(C.Structure):
     _fields_ = [
         ("p", C.c_int32), ("system", C.c_int32), ("precision", C.c_int32), ("flags", C.c_int32),
@@ -61,6 +78,10 @@ def _load():
     P, I64 = C.c_void_p, C.c_int64
     sig = {
         "fr_setup_mesh": (C.c_int, [C.POINTER(P), C.POINTER(fr_mesh_desc)]),
+        "fr_setup_mesh_mixed": (C.c_int, [C.POINTER(P), C.POINTER(fr_mixed_mesh_desc)]),
+        "fr_num_parts": (I64, [P]),
+        "fr_part_info": (C.c_int, [P, C.c_int, C.POINTER(fr_part_info_t)]),
+        "fr_part_solution_point_coords": (C.c_int, [P, C.c_int, P]),
         "fr_setup_operators": (C.c_int, [P, C.POINTER(fr_disc_desc)]),
         "fr_num_solution_points": (I64, [P]), "fr_num_flux_points": (I64, [P]), "fr_num_vars": (I64, [P]),
         "fr_num_pairs": (I64, [P]), "fr_leading_dim": (I64, [P]), "fr_state_bytes": (I64, [P]),
@@ -88,7 +109,7 @@ def _load():
 
 
 lib = _load()
-EXPORTS = ["fr_setup_mesh", "fr_setup_operators", "fr_num_solution_points", "fr_num_flux_points", "fr_num_vars", "fr_num_pairs",
+EXPORTS = ["fr_setup_mesh", "fr_setup_mesh_mixed", "fr_num_parts", "fr_part_info", "fr_part_solution_point_coords", "fr_setup_operators", "fr_num_solution_points", "fr_num_flux_points", "fr_num_vars", "fr_num_pairs",
            "fr_leading_dim", "fr_state_bytes", "fr_workspace_bytes", "fr_stepper_workspace_bytes", "fr_rhs_kernel_launches",
            "fr_euler_step", "fr_dopri5_step", "fr_solution_point_coords",
            "fr_operator_dims", "fr_get_operator", "fr_get_pairs", "fr_get_metrics", "fr_rhs", "fr_rhs_profiled", "fr_rk4_step", "fr_rhs_host",
@@ -115,6 +136,9 @@ class Context:
         """mesh: workloads.py mesh dict; bcs: {bc_id: (kind, params)} as the oracle takes them."""
         self._h = C.c_void_p()
         self._keep = []
+        self.mixed = "parts" in mesh
+        if self.mixed:
+            return self._init_mixed(mesh, bcs)
         nodes = np.ascontiguousarray(mesh["nodes"], dtype=np.float64)
         ifaces = np.ascontiguousarray(mesh["ifaces"], dtype=np.int32)
         shifts = np.ascontiguousarray(mesh["shifts"], dtype=np.float64)
@@ -144,6 +168,39 @@ class Context:
             raise FrError(rc, (lib.fr_last_error(None) or b"").decode())
         self.ndims, self.n_elems = mesh["ndims"], nodes.shape[0]
 
+    @staticmethod
+    def _bc_array(bcs):
+        bcs = bcs or {}
+        nb = (max(bcs) + 1) if bcs else 0
+        arr = (fr_bc_desc * max(nb, 1))()
+        for i, (kind, par) in bcs.items():
+            arr[i].kind = BC_KINDS[kind]
+            arr[i].rho = float(par.get("rho", 0.0))
+            v = list(par.get("v", ())) + [0.0] * 3
+            for d in range(3):
+                arr[i].v[d] = float(v[d])
+            arr[i].p = float(par.get("p", 0.0))
+            arr[i].cpTw = float(par.get("cpTw", 0.0))
+        return arr, nb
+
+    def _init_mixed(self, mesh, bcs):
+        """mesh: workloads.mixed_mesh dictionary (parts of one element type each, 6-column interface records)."""
+        nodes = [np.ascontiguousarray(p["nodes"], dtype=np.float64) for p in mesh["parts"]]
+        parts = (fr_mesh_part * len(nodes))()
+        for t, (p, nd_) in enumerate(zip(mesh["parts"], nodes)):
+            parts[t].etype, parts[t].p_g, parts[t].n_elems, parts[t].nodes = ETYPES[p["etype"]], p["p_g"], nd_.shape[0], _ptr(nd_)
+        ifaces = np.ascontiguousarray(mesh["ifaces"], dtype=np.int32)
+        shifts = np.ascontiguousarray(mesh["shifts"], dtype=np.float64)
+        bfaces = np.ascontiguousarray(mesh["bfaces"], dtype=np.int32)
+        arr, nb = self._bc_array(bcs)
+        d = fr_mixed_mesh_desc(ndims=mesh["ndims"], n_parts=len(nodes), n_bcs=nb, n_ifaces=ifaces.shape[0], n_bfaces=bfaces.shape[0],
+                               parts=C.cast(parts, C.c_void_p), ifaces=_ptr(ifaces), shifts=_ptr(shifts), bfaces=_ptr(bfaces),
+                               bcs=C.cast(arr, C.c_void_p) if nb else None)
+        rc = lib.fr_setup_mesh_mixed(C.byref(self._h), C.byref(d))
+        if rc != 0:
+            raise FrError(rc, (lib.fr_last_error(None) or b"").decode())
+        self.ndims, self.n_elems = mesh["ndims"], sum(n.shape[0] for n in nodes)
+
     def _check(self, rc):
         if rc != 0:
             raise FrError(rc, (lib.fr_last_error(self._h) or b"").decode())
@@ -158,6 +215,16 @@ class Context:
             for i, v in enumerate(ref.get("v", ())):
                 d.v_ref[i] = float(v)
         self._check(lib.fr_setup_operators(self._h, C.byref(d)))
+        self.dtype = np.float64 if d.precision == F64 else np.float32
+        self.NV = lib.fr_num_vars(self._h)
+        if self.mixed:
+            self.parts = []
+            for t in range(lib.fr_num_parts(self._h)):
+                info = fr_part_info_t()
+                self._check(lib.fr_part_info(self._h, t, C.byref(info)))
+                self.parts.append(dict(etype=info.etype, n_elems=info.n_elems, Nu=info.n_solution_points, Nf=info.n_flux_points,
+                                       ld=info.leading_dim, offset=info.state_offset))
+            return self
         self.Nu = lib.fr_num_solution_points(self._h)
         self.Nf = lib.fr_num_flux_points(self._h)
         self.NV = lib.fr_num_vars(self._h)
@@ -171,6 +238,13 @@ class Context:
     rhs_kernel_launches = property(lambda self: lib.fr_rhs_kernel_launches(self._h))
 
     def solution_point_coords(self):
+        if self.mixed:
+            out = []
+            for t, p in enumerate(self.parts):
+                x = np.empty((p["Nu"], p["n_elems"], self.ndims), dtype=np.float64)
+                self._check(lib.fr_part_solution_point_coords(self._h, t, _ptr(x)))
+                out.append(x)
+            return out
         x = np.empty((self.Nu, self.n_elems, self.ndims), dtype=np.float64)
         self._check(lib.fr_solution_point_coords(self._h, _ptr(x)))
         return x
@@ -225,13 +299,27 @@ class Context:
 
     # --- layout helpers (host side, no arithmetic of the method) ---
     def pad(self, u):
-        """[Nu, NV, n_elems] -> padded [Nu, NV, ld] in the context precision (pad columns zero)."""
+        """[Nu, NV, n_elems] -> padded [Nu, NV, ld] in the context precision (pad columns zero).
+        Mixed meshes: list of such arrays, one per part -> ONE flat buffer with the parts at their state offsets."""
+        if self.mixed:
+            flat = np.zeros(self.state_bytes // np.dtype(self.dtype).itemsize, dtype=self.dtype)
+            for p, up in zip(self.parts, u):
+                o = p["offset"] // flat.itemsize
+                flat[o:o + p["Nu"] * self.NV * p["ld"]].reshape(p["Nu"], self.NV, p["ld"])[:, :, : p["n_elems"]] = up
+            return flat
         out = np.zeros((self.Nu, self.NV, self.ld), dtype=self.dtype)
         out[:, :, : self.n_elems] = u
         return out
 
     def unpad(self, u):
-        return np.asarray(u)[:, :, : self.n_elems]
+        u = np.asarray(u)
+        if self.mixed:
+            out = []
+            for p in self.parts:
+                o = p["offset"] // u.itemsize
+                out.append(np.array(u.reshape(-1)[o:o + p["Nu"] * self.NV * p["ld"]].reshape(p["Nu"], self.NV, p["ld"])[:, :, : p["n_elems"]]))
+            return out
+        return u.reshape(self.Nu, self.NV, self.ld)[:, :, : self.n_elems]
 
     def teardown(self):
         if self._h:

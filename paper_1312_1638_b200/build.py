@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfr_b200.so")
 CPP = ["fr_basis.cpp", "fr_mesh.cpp"]
-CU = ["fr_api.cu", "fr_generic.cu", "fr_tensor.cu", "fr_hex_tma.cu", "fr_hex_fluxdiv_tma.cu", "fr_hex_interp_tma.cu", "fr_element.cu", "fr_rk.cu", "fr_peaks.cu"]
+CU = ["fr_api.cu", "fr_generic.cu", "fr_tensor.cu", "fr_hex_tma.cu", "fr_hex_fluxdiv_tma.cu", "fr_hex_interp_tma.cu", "fr_element.cu", "fr_rk.cu", "fr_peaks.cu", "fr_mixed.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 

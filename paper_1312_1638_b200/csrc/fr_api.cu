@@ -1,4 +1,5 @@
 // C ABI of the FR library (include/fr.h): context management, constant uploads, RHS and RK4 drivers.
+#include <algorithm>
 #include <cstdio>
 #include <cstring>
 #include <exception>
@@ -11,6 +12,7 @@
 #include "fr_host.hpp"
 #include "fr_element.hpp"
 #include "fr_hex_tma.hpp"
+#include "fr_mixed.hpp"
 #include "fr_tensor.hpp"
 
 using namespace fr;
@@ -29,6 +31,17 @@ struct fr_ctx {
   TensorPlan tp{};
   std::vector<void *> dev_allocs;
   mutable std::string err;
+  // ---- mesh of several element types (fr_setup_mesh_mixed): one sub-context per part, cross-part tables here ----
+  bool sub = false;                  // this context is a part of a mixed mesh
+  std::vector<fr_ctx *> parts;       // owned
+  std::vector<int32_t> mx_ifaces;    // [n][6]
+  std::vector<double> mx_shifts;
+  MixedPairs mx{};
+  std::vector<int64_t> mx_soff;      // byte offset of every part in a state buffer
+  std::vector<int64_t> mx_fpo;       // offset (doubles) of every part inside a flux-point region
+  std::vector<int64_t> mx_qoff;      // byte offset of every part's Q array in the workspace
+  int64_t mx_state = 0, mx_region = 0, mx_uf = 0, mx_cf = 0, mx_gf = 0;  // total state bytes; region size (doubles); region byte offsets
+  ~fr_ctx() { for (fr_ctx *q : parts) delete q; }
 };
 
 static thread_local std::string g_setup_err;
@@ -99,8 +112,58 @@ int fr_setup_mesh(fr_ctx **out, const fr_mesh_desc *m) {
   }
 }
 
+int fr_setup_mesh_mixed(fr_ctx **out, const fr_mixed_mesh_desc *m) {
+  if (!out) return fail(nullptr, FR_EINVAL, "fr_setup_mesh_mixed: out is NULL");
+  *out = nullptr;
+  if (!m) return fail(nullptr, FR_EINVAL, "fr_setup_mesh_mixed: mesh is NULL");
+  if (m->ndims != 2) return fail(nullptr, FR_EUNSUPPORTED, "mixed meshes are two-dimensional (quadrilaterals and triangles)");
+  if (m->n_parts < 1 || m->n_parts > 8 || !m->parts) return fail(nullptr, FR_EINVAL, "n_parts out of range [1,8]");
+  if (m->n_ifaces < 0 || m->n_bfaces < 0 || (m->n_ifaces > 0 && (!m->ifaces || !m->shifts)) || (m->n_bfaces > 0 && (!m->bfaces || !m->bcs)))
+    return fail(nullptr, FR_EINVAL, "interface / boundary arrays missing");
+  fr_ctx *c = nullptr;
+  try {
+    c = new fr_ctx();
+    c->mesh.nd = 2;
+    for (int t = 0; t < m->n_parts; ++t) {
+      const fr_mesh_part &pt = m->parts[t];
+      if (pt.etype != FR_QUAD && pt.etype != FR_TRI) { delete c; return fail(nullptr, FR_EINVAL, "a part of a mixed mesh must hold quadrilaterals or triangles"); }
+      // boundary faces of this part as a single-type list
+      std::vector<int32_t> bf;
+      for (int64_t b = 0; b < m->n_bfaces; ++b)
+        if (m->bfaces[4 * b] == t) { bf.push_back(m->bfaces[4 * b + 1]); bf.push_back(m->bfaces[4 * b + 2]); bf.push_back(m->bfaces[4 * b + 3]); }
+      fr_mesh_desc d1{};
+      d1.ndims = 2; d1.etype = pt.etype; d1.p_g = pt.p_g; d1.n_bcs = m->n_bcs; d1.n_elems = pt.n_elems;
+      d1.n_ifaces = 0; d1.n_bfaces = (int64_t)bf.size() / 3; d1.nodes = pt.nodes; d1.bfaces = bf.data(); d1.bcs = m->bcs;
+      fr_ctx *q = nullptr;
+      const int rc = fr_setup_mesh(&q, &d1);
+      if (rc != FR_OK) { delete c; return rc; }  // text already in g_setup_err
+      q->sub = true;
+      c->parts.push_back(q);
+    }
+    for (int64_t f = 0; f < m->n_ifaces; ++f) {
+      const int32_t *r = m->ifaces + 6 * f;
+      if (r[0] < 0 || r[0] >= m->n_parts || r[3] < 0 || r[3] >= m->n_parts) { delete c; return fail(nullptr, FR_EINVAL, "interface record references a part out of range"); }
+    }
+    for (int64_t b = 0; b < m->n_bfaces; ++b)
+      if (m->bfaces[4 * b] < 0 || m->bfaces[4 * b] >= m->n_parts) { delete c; return fail(nullptr, FR_EINVAL, "boundary face references a part out of range"); }
+    c->mx_ifaces.assign(m->ifaces, m->ifaces + (size_t)m->n_ifaces * 6);
+    c->mx_shifts.assign(m->shifts, m->shifts + (size_t)m->n_ifaces * 2);
+    *out = c;
+    return FR_OK;
+  } catch (const std::bad_alloc &) {
+    delete c;
+    return fail(nullptr, FR_ENOMEM, "out of host memory");
+  } catch (const std::exception &ex) {
+    delete c;
+    return fail(nullptr, FR_EINVAL, ex.what());
+  }
+}
+
+static int setup_mixed(fr_ctx *c, const fr_disc_desc *d);
+
 int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
   if (!c) return fail(nullptr, FR_EINVAL, "fr_setup_operators: ctx is NULL");
+  if (!c->parts.empty()) return setup_mixed(c, d);
   if (!d) return fail(c, FR_EINVAL, "fr_setup_operators: disc is NULL");
   if (d->system != FR_EULER && d->system != FR_NAVIER_STOKES) return fail(c, FR_EINVAL, "unknown system");
   if (d->precision != FR_F32 && d->precision != FR_F64) return fail(c, FR_EINVAL, "unknown precision");
@@ -118,7 +181,7 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     // hexahedra on the TMA-pipelined kernels keep every internal array element-blocked (fr_dev.hpp: fp_row)
     const bool blk = !c->host_only && !(d->flags & FR_FLAG_FORCE_GENERIC) && c->ops.etype == FR_HEX &&
                      hex_tma_supported(c->ops.n, d->precision == FR_F64);
-    int rc = build_mesh_consts(c->mesh, c->ops, ld, blk ? FR_BLK : 0, c->mc, err);
+    int rc = build_mesh_consts(c->mesh, c->ops, ld, blk ? FR_BLK : 0, c->mc, err, !c->sub);
     if (rc != FR_OK) return fail(c, rc, err);
     c->disc = *d;
     const RefOps &o = c->ops;
@@ -252,16 +315,195 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
   }
 }
 
+// ---- mesh of several element types: parts set up one by one, then the cross-part lookup table ----
+static int setup_mixed(fr_ctx *c, const fr_disc_desc *d) {
+  if (!d) return fail(c, FR_EINVAL, "fr_setup_operators: disc is NULL");
+  if (d->flags & (FR_FLAG_FORCE_GENERIC | FR_FLAG_HOST_ONLY | FR_FLAG_LEAN)) return fail(c, FR_EUNSUPPORTED, "mixed meshes: flags are not supported");
+  if (d->p < 1 || d->p > 4) return fail(c, FR_EUNSUPPORTED, "mixed meshes run the fused element kernels: 1 <= p <= 4");
+  try {
+    c->ready = false;
+    free_dev(c);
+    const int np_ = (int)c->parts.size(), nd = 2, NV = 4;
+    for (fr_ctx *q : c->parts) {
+      const int rc = fr_setup_operators(q, d);
+      if (rc != FR_OK) return fail(c, rc, "part: " + q->err);
+      if (!element_fused_supported(q->dc)) return fail(c, FR_EUNSUPPORTED, "mixed meshes need the fused element kernels for every part");
+    }
+    c->disc = *d;
+    c->dc = c->parts[0]->dc;  // N_V, physics, precision, device
+    // layout of a state buffer and of the flux-point regions
+    const int64_t esz = c->dc.f64 ? 8 : 4;
+    c->mx_soff.assign(np_, 0); c->mx_fpo.assign(np_, 0); c->mx_qoff.assign(np_, 0);
+    int64_t so = 0, fo = 0;
+    for (int t = 0; t < np_; ++t) {
+      const DevConsts &q = c->parts[t]->dc;
+      c->mx_soff[t] = so; so = align_up(so + (int64_t)q.Nu * NV * q.ld * esz, 256);
+      c->mx_fpo[t] = fo; fo = align_up(fo + (int64_t)q.Nf * NV * q.ld, 32);
+    }
+    c->mx_state = so; c->mx_region = fo;
+    // cross-part pairing by physical coordinates (:182, A11)
+    struct Pr { int64_t oL, oR; int32_t vL, vR; double n0, n1, jL, jR; };
+    const int64_t nif = (int64_t)c->mx_ifaces.size() / 6;
+    std::vector<Pr> pairs;
+    std::vector<std::vector<int32_t>> cover(np_);
+    for (int t = 0; t < np_; ++t) cover[t].assign((size_t)c->parts[t]->ops.Nf * c->parts[t]->mc.Nel, 0);
+    int64_t unmatched = 0;
+    for (int64_t f = 0; f < nif; ++f) {
+      const int32_t *r = &c->mx_ifaces[6 * f];
+      const fr_ctx *L = c->parts[r[0]], *R = c->parts[r[3]];
+      const int nfp = L->ops.nfp;
+      if (R->ops.nfp != nfp) return fail(c, FR_EMESH, "the two sides of an interface have different numbers of flux points");
+      const int64_t eL = r[1], eR = r[4];
+      if (eL < 0 || eL >= L->mc.Nel || eR < 0 || eR >= R->mc.Nel || r[2] < 0 || r[2] >= L->ops.nfaces || r[5] < 0 || r[5] >= R->ops.nfaces)
+        return fail(c, FR_EINVAL, "interface list references an element or face out of range");
+      auto xL = [&](int s, int n) { return L->mc.xf[((size_t)s * L->mc.Nel + eL) * nd + n]; };
+      auto xR = [&](int s, int n) { return R->mc.xf[((size_t)s * R->mc.Nel + eR) * nd + n] + c->mx_shifts[(size_t)f * nd + n]; };
+      double h2 = 0;
+      for (int n = 0; n < nd; ++n) { const double dd = xL(r[2] * nfp, n) - xL(r[2] * nfp + nfp - 1, n); h2 += dd * dd; }
+      const double tol2 = 1e-18 * (h2 > 0 ? h2 : 1.0) + 1e-24;
+      unsigned long long used = 0;
+      for (int k = 0; k < nfp; ++k) {
+        const int sL = r[2] * nfp + k;
+        int best = -1;
+        double bd = 1e300;
+        for (int mm = 0; mm < nfp; ++mm) {
+          double d2 = 0;
+          for (int n = 0; n < nd; ++n) { const double dd = xL(sL, n) - xR(r[5] * nfp + mm, n); d2 += dd * dd; }
+          if (d2 < bd) { bd = d2; best = mm; }
+        }
+        if (!(bd <= tol2) || ((used >> best) & 1ull)) ++unmatched;
+        used |= 1ull << best;
+        const int sR = r[5] * nfp + best;
+        const int64_t ldL = L->dc.ld, ldR = R->dc.ld;
+        Pr pr;
+        pr.oL = c->mx_fpo[r[0]] + (int64_t)sL * NV * ldL + eL; pr.vL = (int32_t)ldL;
+        pr.oR = c->mx_fpo[r[3]] + (int64_t)sR * NV * ldR + eR; pr.vR = (int32_t)ldR;
+        pr.n0 = L->mc.fp_n[((size_t)0 * L->ops.Nf + sL) * ldL + eL]; pr.n1 = L->mc.fp_n[((size_t)1 * L->ops.Nf + sL) * ldL + eL];
+        pr.jL = L->mc.fp_Jn[(size_t)sL * ldL + eL]; pr.jR = R->mc.fp_Jn[(size_t)sR * ldR + eR];
+        pairs.push_back(pr);
+        cover[r[0]][(size_t)sL * L->mc.Nel + eL]++; cover[r[3]][(size_t)sR * R->mc.Nel + eR]++;
+      }
+    }
+    if (unmatched) return fail(c, FR_EMESH, "unmatched flux-point pairs: " + std::to_string(unmatched));
+    for (int t = 0; t < np_; ++t) {
+      const fr_ctx *q = c->parts[t];
+      for (int64_t i = 0; i < q->mc.nbnd; ++i) cover[t][(size_t)q->mc.bs[i] * q->mc.Nel + q->mc.be[i]]++;
+      for (auto v : cover[t]) if (v != 1) return fail(c, FR_EMESH, "flux points not covered exactly once by interfaces + boundary faces");
+    }
+    std::sort(pairs.begin(), pairs.end(), [](const Pr &a, const Pr &b) { return a.oL < b.oL; });  // coalesced L side (:693)
+    const int64_t n = (int64_t)pairs.size();
+    std::vector<int64_t> oL(n), oR(n);
+    std::vector<int32_t> vL(n), vR(n);
+    std::vector<double> nrm(2 * (size_t)n), jL(n), jR(n);
+    for (int64_t i = 0; i < n; ++i) {
+      oL[i] = pairs[i].oL; oR[i] = pairs[i].oR; vL[i] = pairs[i].vL; vR[i] = pairs[i].vR;
+      nrm[i] = pairs[i].n0; nrm[(size_t)n + i] = pairs[i].n1; jL[i] = pairs[i].jL; jR[i] = pairs[i].jR;
+    }
+    cudaError_t e = cudaSuccess;
+    c->mx = MixedPairs();
+    c->mx.n = n;
+    e = upload(c, oL, &c->mx.oL);
+    if (e == cudaSuccess) e = upload(c, oR, &c->mx.oR);
+    if (e == cudaSuccess) e = upload(c, vL, &c->mx.vL);
+    if (e == cudaSuccess) e = upload(c, vR, &c->mx.vR);
+    if (e == cudaSuccess) e = upload(c, nrm, &c->mx.nrm);
+    if (e == cudaSuccess) e = upload(c, jL, &c->mx.jL);
+    if (e == cudaSuccess) e = upload(c, jR, &c->mx.jR);
+    if (e != cudaSuccess) { free_dev(c); return fail(c, FR_ECUDA, std::string("constant upload: ") + cudaGetErrorString(e)); }
+    for (fr_ctx *q : c->parts) std::vector<double>().swap(q->mc.xf);
+    // workspace: U^f (-> D~), C^f, G^f regions, Q of every part, stepper registers
+    int64_t off = 0;
+    auto take = [&](int64_t bytes) { int64_t o2 = off; off = align_up(off + bytes, 256); return o2; };
+    c->mx_uf = take(c->mx_region * 8);
+    c->mx_cf = c->dc.ns ? take(c->mx_region * 8) : 0;
+    c->mx_gf = c->dc.ns ? take(c->mx_region * 8) : 0;
+    for (int t = 0; t < np_; ++t) {
+      const DevConsts &q = c->parts[t]->dc;
+      c->mx_qoff[t] = c->dc.ns ? take((int64_t)nd * q.Nu * NV * q.ld * 8) : 0;
+    }
+    WorkLayout &w = c->wl;
+    w = WorkLayout();
+    w.partials = take((int64_t)RK_MAX_PARTIALS * 8);
+    w.reg0 = off; w.reg_stride = align_up(c->mx_state, 256);
+    w.total = w.reg0 + 3 * w.reg_stride;
+    c->ready = true;
+    return FR_OK;
+  } catch (const std::bad_alloc &) {
+    return fail(c, FR_ENOMEM, "out of host memory");
+  } catch (const std::exception &ex) {
+    return fail(c, FR_EINVAL, ex.what());
+  }
+}
+
+// rhs of a mixed mesh: the fused element kernels part by part, the interface kernels over all flux-point pairs at once
+static cudaError_t mixed_rhs(fr_ctx *c, const void *u, void *rhs, char *work, cudaStream_t s, Prof *prof) {
+  const int np_ = (int)c->parts.size();
+  double *uf = (double *)(work + c->mx_uf), *cf = (double *)(work + c->mx_cf), *gf = (double *)(work + c->mx_gf);
+  const bool ns = c->dc.ns;
+  cudaError_t e = cudaSuccess;
+  auto up = [&](int t) { return (const void *)((const char *)u + c->mx_soff[t]); };
+  FR_MARK(prof, "el_interp");
+  for (int t = 0; t < np_ && e == cudaSuccess; ++t) e = element_interp(c->parts[t]->dc, up(t), uf + c->mx_fpo[t], s);
+  if (e != cudaSuccess) return e;
+  if (ns) {
+    FR_MARK(prof, "common_sol");
+    mixed_common_sol(c->mx, c->dc.ph, uf, cf, s);
+    for (int t = 0; t < np_; ++t)
+      if (c->parts[t]->dc.nbnd) launch_common_sol(c->parts[t]->dc, uf + c->mx_fpo[t], cf + c->mx_fpo[t], s);
+    FR_MARK(prof, "el_gradface");
+    for (int t = 0; t < np_ && e == cudaSuccess; ++t)
+      e = element_gradface(c->parts[t]->dc, up(t), cf + c->mx_fpo[t], uf + c->mx_fpo[t], (double *)(work + c->mx_qoff[t]), gf + c->mx_fpo[t], s);
+    if (e != cudaSuccess) return e;
+    FR_MARK(prof, "common_flux_g");
+    mixed_common_flux(c->mx, c->dc.ph, true, uf, gf, s);
+    for (int t = 0; t < np_; ++t)
+      if (c->parts[t]->dc.nbnd) launch_common_flux_g(c->parts[t]->dc, uf + c->mx_fpo[t], gf + c->mx_fpo[t], false, s);
+  } else {
+    FR_MARK(prof, "common_flux");
+    mixed_common_flux(c->mx, c->dc.ph, false, uf, nullptr, s);
+    for (int t = 0; t < np_; ++t)
+      if (c->parts[t]->dc.nbnd) launch_common_flux(c->parts[t]->dc, uf + c->mx_fpo[t], nullptr, false, s);
+  }
+  FR_MARK(prof, "el_fluxdiv");
+  for (int t = 0; t < np_ && e == cudaSuccess; ++t)
+    e = element_fluxdiv(c->parts[t]->dc, up(t), (const double *)(work + c->mx_qoff[t]), uf + c->mx_fpo[t], (char *)rhs + c->mx_soff[t], s);
+  return e != cudaSuccess ? e : cudaGetLastError();
+}
+
 #define FR_NEED_READY(c, ret) \
   if (!(c)) return ret;      \
   if (!(c)->ready) { (c)->err = "fr_setup_operators has not completed"; return ret; }
 
-int64_t fr_num_solution_points(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return c->ops.Nu; }
-int64_t fr_num_flux_points(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return c->ops.Nf; }
+#define FR_NOT_MIXED(c, what) \
+  if (!(c)->parts.empty()) return fail(c, FR_EINVAL, what ": single-type query on a mixed-mesh context (use fr_part_info)");
+
+int64_t fr_num_solution_points(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) FR_NOT_MIXED(c, "fr_num_solution_points") return c->ops.Nu; }
+int64_t fr_num_flux_points(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) FR_NOT_MIXED(c, "fr_num_flux_points") return c->ops.Nf; }
 int64_t fr_num_vars(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return c->dc.NV; }
-int64_t fr_num_pairs(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return c->mc.npairs; }
-int64_t fr_leading_dim(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return c->dc.ld; }
-int64_t fr_state_bytes(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return (int64_t)c->ops.Nu * c->dc.NV * c->dc.ld * (c->dc.f64 ? 8 : 4); }
+int64_t fr_num_pairs(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return c->parts.empty() ? c->mc.npairs : c->mx.n; }
+int64_t fr_leading_dim(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) FR_NOT_MIXED(c, "fr_leading_dim") return c->dc.ld; }
+int64_t fr_state_bytes(const fr_ctx *c) {
+  FR_NEED_READY(c, FR_EINVAL)
+  if (!c->parts.empty()) return c->mx_state;
+  return (int64_t)c->ops.Nu * c->dc.NV * c->dc.ld * (c->dc.f64 ? 8 : 4);
+}
+int64_t fr_num_parts(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return c->parts.empty() ? 1 : (int64_t)c->parts.size(); }
+int fr_part_info(const fr_ctx *c, int part, fr_part_info_t *info) {
+  FR_NEED_READY(c, FR_EINVAL)
+  if (!info || part < 0 || part >= (c->parts.empty() ? 1 : (int)c->parts.size())) return fail(c, FR_EINVAL, "fr_part_info: part out of range or NULL output");
+  const fr_ctx *q = c->parts.empty() ? c : c->parts[part];
+  info->etype = q->ops.etype; info->reserved = 0;
+  info->n_elems = q->mc.Nel; info->n_solution_points = q->ops.Nu; info->n_flux_points = q->ops.Nf; info->leading_dim = q->dc.ld;
+  info->state_offset = c->parts.empty() ? 0 : c->mx_soff[part];
+  return FR_OK;
+}
+int fr_part_solution_point_coords(const fr_ctx *c, int part, double *xyz) {
+  FR_NEED_READY(c, FR_EINVAL)
+  if (!xyz || part < 0 || part >= (c->parts.empty() ? 1 : (int)c->parts.size())) return fail(c, FR_EINVAL, "fr_part_solution_point_coords: part out of range or NULL buffer");
+  const fr_ctx *q = c->parts.empty() ? c : c->parts[part];
+  std::memcpy(xyz, q->mc.xu.data(), q->mc.xu.size() * sizeof(double));
+  return FR_OK;
+}
 int64_t fr_workspace_bytes(const fr_ctx *c) { FR_NEED_READY(c, FR_EINVAL) return c->wl.total; }
 int64_t fr_stepper_workspace_bytes(const fr_ctx *c, int stepper) {
   FR_NEED_READY(c, FR_EINVAL)
@@ -271,11 +513,17 @@ int64_t fr_stepper_workspace_bytes(const fr_ctx *c, int stepper) {
 }
 int64_t fr_rhs_kernel_launches(const fr_ctx *c) {
   FR_NEED_READY(c, FR_EINVAL)
+  if (!c->parts.empty()) {
+    int64_t n = (int64_t)c->parts.size() * (c->dc.ns ? 3 : 2) + (c->mx.n ? (c->dc.ns ? 2 : 1) : 0);
+    for (const fr_ctx *q : c->parts) if (q->dc.nbnd) n += c->dc.ns ? 2 : 1;
+    return n;
+  }
   return c->use_tensor ? tensor_rhs_launches(c->dc) : generic_rhs_launches(c->dc);
 }
 
 int fr_solution_point_coords(const fr_ctx *c, double *xyz) {
   FR_NEED_READY(c, FR_EINVAL)
+  FR_NOT_MIXED(c, "fr_solution_point_coords")
   if (!xyz) return fail(c, FR_EINVAL, "xyz_host is NULL");
   std::memcpy(xyz, c->mc.xu.data(), c->mc.xu.size() * sizeof(double));
   return FR_OK;
@@ -283,6 +531,7 @@ int fr_solution_point_coords(const fr_ctx *c, double *xyz) {
 
 int fr_operator_dims(const fr_ctx *c, int id, int64_t *rows, int64_t *cols) {
   FR_NEED_READY(c, FR_EINVAL)
+  FR_NOT_MIXED(c, "fr_operator_dims")
   if (id < 0 || id > 6 || !rows || !cols) return fail(c, FR_EINVAL, "operator id out of range or NULL output");
   *rows = c->ops.rows[id]; *cols = c->ops.cols[id];
   return FR_OK;
@@ -290,6 +539,7 @@ int fr_operator_dims(const fr_ctx *c, int id, int64_t *rows, int64_t *cols) {
 
 int fr_get_operator(const fr_ctx *c, int id, double *buf) {
   FR_NEED_READY(c, FR_EINVAL)
+  FR_NOT_MIXED(c, "fr_get_operator")
   if (id < 0 || id > 6 || !buf) return fail(c, FR_EINVAL, "operator id out of range or NULL buffer");
   std::memcpy(buf, c->ops.M[id].data(), c->ops.M[id].size() * sizeof(double));
   return FR_OK;
@@ -297,6 +547,7 @@ int fr_get_operator(const fr_ctx *c, int id, double *buf) {
 
 int fr_get_pairs(const fr_ctx *c, int32_t *pairs, double *normals, double *jn) {
   FR_NEED_READY(c, FR_EINVAL)
+  FR_NOT_MIXED(c, "fr_get_pairs")
   if (c->lean) return fail(c, FR_EINVAL, "fr_get_pairs: host tables were released (FR_FLAG_LEAN)");
   const MeshConsts &m = c->mc;
   const int nd = c->ops.nd;
@@ -310,6 +561,7 @@ int fr_get_pairs(const fr_ctx *c, int32_t *pairs, double *normals, double *jn) {
 
 int fr_get_metrics(const fr_ctx *c, double *smat, double *rcpj) {
   FR_NEED_READY(c, FR_EINVAL)
+  FR_NOT_MIXED(c, "fr_get_metrics")
   if (c->lean) return fail(c, FR_EINVAL, "fr_get_metrics: host tables were released (FR_FLAG_LEAN)");
   if (smat) std::memcpy(smat, c->mc.smat.data(), c->mc.smat.size() * sizeof(double));
   if (rcpj) std::memcpy(rcpj, c->mc.rcpj.data(), c->mc.rcpj.size() * sizeof(double));
@@ -325,6 +577,11 @@ static int rhs_impl(fr_ctx *c, const void *u, void *rhs, void *work, void *strea
   if (cudaGetDevice(&dev) != cudaSuccess || dev != c->dc.dev)
     return fail(c, FR_EINVAL, "fr_rhs: the current CUDA device is not the one fr_setup_operators uploaded the constants to");
   cudaStream_t s = (cudaStream_t)stream;
+  if (!c->parts.empty()) {
+    cudaError_t em = mixed_rhs(c, u, rhs, (char *)work, s, prof);
+    if (em != cudaSuccess) return fail(c, FR_ECUDA, std::string("fr_rhs launch: ") + cudaGetErrorString(em));
+    return FR_OK;
+  }
   cudaError_t e = c->use_tensor ? tensor_rhs(c->dc, c->tp, u, rhs, (char *)work + c->wl.uf, s, prof)
                                 : generic_rhs(c->dc, c->wl, u, rhs, (char *)work, s, prof);
   if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("fr_rhs launch: ") + cudaGetErrorString(e));
@@ -356,6 +613,22 @@ int fr_rhs_profiled(fr_ctx *c, const void *u, void *rhs, void *work, void *strea
 }
 
 // ---- time steppers (Table 1 :263).  Registers: work + reg0 + i * reg_stride ----
+// out1 = sum a_i in_i, out2 = sum b_i in_i over the state matrices of the context (every part of a mixed mesh)
+static cudaError_t ctx_lincomb(const fr_ctx *c, int nin, const void *const *in, const double *a, const double *b, void *out1, void *out2,
+                               cudaStream_t s) {
+  const bool f64 = c->dc.f64;
+  if (c->parts.empty()) return rk_lincomb(f64, (int64_t)c->ops.Nu * c->dc.NV, c->dc.ld, c->dc.Nel, nin, in, a, b, out1, out2, s);
+  cudaError_t e = cudaSuccess;
+  for (size_t t = 0; t < c->parts.size() && e == cudaSuccess; ++t) {
+    const fr_ctx *q = c->parts[t];
+    const void *inp[RK_MAX_IN];
+    for (int i = 0; i < nin; ++i) inp[i] = (const char *)in[i] + c->mx_soff[t];
+    e = rk_lincomb(f64, (int64_t)q->ops.Nu * q->dc.NV, q->dc.ld, q->dc.Nel, nin, inp, a, b, out1 ? (char *)out1 + c->mx_soff[t] : nullptr,
+                   out2 ? (char *)out2 + c->mx_soff[t] : nullptr, s);
+  }
+  return e;
+}
+
 #define FR_STEPPER_PROLOGUE(name)                                                                       \
   FR_NEED_READY(c, FR_EINVAL)                                                                           \
   if (c->host_only) return fail(c, FR_EINVAL, name ": context was set up with FR_FLAG_HOST_ONLY");       \
@@ -363,26 +636,25 @@ int fr_rhs_profiled(fr_ctx *c, const void *u, void *rhs, void *work, void *strea
   cudaStream_t s = (cudaStream_t)stream;                                                                \
   char *wk = (char *)work;                                                                              \
   auto reg = [&](int i) { return (void *)(wk + c->wl.reg0 + i * c->wl.reg_stride); };                   \
-  const int64_t rows = (int64_t)c->ops.Nu * c->dc.NV, ld = c->dc.ld, nel = c->dc.Nel;                   \
-  const bool f64 = c->dc.f64;                                                                           \
   int rc;                                                                                               \
   cudaError_t e = cudaSuccess;
 
 int fr_rk4_step(fr_ctx *c, void *u, double dt, void *work, void *stream) {
   FR_STEPPER_PROLOGUE("fr_rk4_step")
   void *k = reg(0), *tmp = reg(1), *acc = reg(2);
+  const void *in[3] = {u, k, acc};
   // k1; tmp = u + dt/2 k1; acc = u + dt/6 k1
   if ((rc = fr_rhs(c, u, k, work, stream)) != FR_OK) return rc;
-  e = rk_axpy2(f64, rows, ld, nel, u, k, dt / 2, tmp, dt / 6, acc, 0, s);
+  { const double a[2] = {1, dt / 2}, b[2] = {1, dt / 6}; e = ctx_lincomb(c, 2, in, a, b, tmp, acc, s); }
   // k2; tmp = u + dt/2 k2; acc += dt/3 k2
   if (e == cudaSuccess && (rc = fr_rhs(c, tmp, k, work, stream)) != FR_OK) return rc;
-  if (e == cudaSuccess) e = rk_axpy2(f64, rows, ld, nel, u, k, dt / 2, tmp, dt / 3, acc, 1, s);
+  if (e == cudaSuccess) { const double a[3] = {1, dt / 2, 0}, b[3] = {0, dt / 3, 1}; e = ctx_lincomb(c, 3, in, a, b, tmp, acc, s); }
   // k3; tmp = u + dt k3; acc += dt/3 k3
   if (e == cudaSuccess && (rc = fr_rhs(c, tmp, k, work, stream)) != FR_OK) return rc;
-  if (e == cudaSuccess) e = rk_axpy2(f64, rows, ld, nel, u, k, dt, tmp, dt / 3, acc, 1, s);
+  if (e == cudaSuccess) { const double a[3] = {1, dt, 0}, b[3] = {0, dt / 3, 1}; e = ctx_lincomb(c, 3, in, a, b, tmp, acc, s); }
   // k4; u = acc + dt/6 k4
   if (e == cudaSuccess && (rc = fr_rhs(c, tmp, k, work, stream)) != FR_OK) return rc;
-  if (e == cudaSuccess) e = rk_axpy2(f64, rows, ld, nel, u, k, 0.0, u, dt / 6, acc, 2, s);
+  if (e == cudaSuccess) { const double a[3] = {0, dt / 6, 1}; e = ctx_lincomb(c, 3, in, a, nullptr, u, nullptr, s); }
   if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("fr_rk4_step launch: ") + cudaGetErrorString(e));
   return FR_OK;
 }
@@ -393,13 +665,14 @@ int fr_euler_step(fr_ctx *c, void *u, double dt, void *work, void *stream) {
   if ((rc = fr_rhs(c, u, k, work, stream)) != FR_OK) return rc;
   const void *in[2] = {u, k};
   const double a[2] = {1.0, dt};
-  e = rk_lincomb(f64, rows, ld, nel, 2, in, a, nullptr, u, nullptr, s);
+  e = ctx_lincomb(c, 2, in, a, nullptr, u, nullptr, s);
   if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("fr_euler_step launch: ") + cudaGetErrorString(e));
   return FR_OK;
 }
 
 int fr_dopri5_step(fr_ctx *c, void *u, double dt, void *work, void *stream, double *err_dev) {
   FR_STEPPER_PROLOGUE("fr_dopri5_step")
+  if (err_dev && !c->parts.empty()) return fail(c, FR_EUNSUPPORTED, "fr_dopri5_step: the error norm is not available on mixed meshes (pass NULL)");
   // Dormand-Prince 5(4), reading A24.  Row i+1 of A gives the state of stage i+1; row 7 = the fifth-order weights (FSAL).
   static const double A[7][6] = {
       {0, 0, 0, 0, 0, 0},
@@ -416,23 +689,24 @@ int fr_dopri5_step(fr_ctx *c, void *u, double dt, void *work, void *stream, doub
     const void *in[7] = {u, reg(0), reg(1), reg(2), reg(3), reg(4), reg(5)};
     double a[7] = {1.0, 0, 0, 0, 0, 0, 0};
     for (int j = 0; j < i; ++j) a[1 + j] = dt * A[i][j];
-    e = rk_lincomb(f64, rows, ld, nel, 1 + i, in, a, nullptr, tmp, nullptr, s);
+    e = ctx_lincomb(c, 1 + i, in, a, nullptr, tmp, nullptr, s);
     if (e == cudaSuccess && (rc = fr_rhs(c, tmp, reg(i), work, stream)) != FR_OK) return rc;
   }
-  if (e == cudaSuccess) {  // u <- u + dt sum b5_i k_i ; tmp <- the fourth-order solution minus the same (without k7)
+  if (e == cudaSuccess) {  // u <- u + dt sum b5_i k_i ; tmp <- dt sum (b5_i - b4_i) k_i without k7
     const void *in[7] = {u, reg(0), reg(1), reg(2), reg(3), reg(4), reg(5)};
     double a[7] = {1.0, 0, 0, 0, 0, 0, 0}, b[7] = {0, 0, 0, 0, 0, 0, 0};
     for (int j = 0; j < 6; ++j) { a[1 + j] = dt * A[6][j]; b[1 + j] = dt * (A[6][j] - B4[j]); }
-    e = rk_lincomb(f64, rows, ld, nel, 7, in, a, err_dev ? b : nullptr, u, err_dev ? tmp : nullptr, s);
+    e = ctx_lincomb(c, 7, in, a, err_dev ? b : nullptr, u, err_dev ? tmp : nullptr, s);
   }
   if (err_dev && e == cudaSuccess) {
     if ((rc = fr_rhs(c, u, reg(1), work, stream)) != FR_OK) return rc;  // k7
     const void *in[2] = {tmp, reg(1)};
     const double a[2] = {1.0, -dt * B4[6]};  // + dt (b5_7 - b4_7) k7, b5_7 = 0
-    e = rk_lincomb(f64, rows, ld, nel, 2, in, a, nullptr, tmp, nullptr, s);
-    // RMS of the error estimate: distance of tmp from zero = rms_diff(tmp, 0 * tmp); reuse k7's register as the zero operand
-    if (e == cudaSuccess) { const void *z[1] = {tmp}; const double za[1] = {0.0}; e = rk_lincomb(f64, rows, ld, nel, 1, z, za, nullptr, reg(1), nullptr, s); }
-    if (e == cudaSuccess) e = rk_rms_diff(f64, rows, ld, nel, tmp, reg(1), (double *)(wk + c->wl.partials), err_dev, s);
+    e = ctx_lincomb(c, 2, in, a, nullptr, tmp, nullptr, s);
+    // RMS of the error estimate = distance of tmp from a zero register (k7's, no longer needed)
+    if (e == cudaSuccess) { const void *z[1] = {tmp}; const double za[1] = {0.0}; e = ctx_lincomb(c, 1, z, za, nullptr, reg(1), nullptr, s); }
+    if (e == cudaSuccess)
+      e = rk_rms_diff(c->dc.f64, (int64_t)c->ops.Nu * c->dc.NV, c->dc.ld, c->dc.Nel, tmp, reg(1), (double *)(wk + c->wl.partials), err_dev, s);
   }
   if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("fr_dopri5_step launch: ") + cudaGetErrorString(e));
   return FR_OK;
@@ -454,6 +728,7 @@ int fr_rhs_host(fr_ctx *c, const void *u_host, void *rhs_host, void *u_dev, void
 
 void fr_teardown(fr_ctx *c) {
   if (!c) return;
+  for (fr_ctx *q : c->parts) free_dev(q);
   free_dev(c);
   delete c;
 }

@@ -85,6 +85,7 @@ cudaError_t generic_rhs(const DevConsts &c, const WorkLayout &w, const void *u, 
 int generic_rhs_launches(const DevConsts &c);
 // point-wise / pair kernels of the generic path reused by the tensor-product path
 void launch_common_jump(const DevConsts &c, const double *uf, double *cf, cudaStream_t s);  // {C - u^f} of Eq 9
+void launch_common_sol(const DevConsts &c, const double *uf, double *cf, cudaStream_t s);   // C of Eq 7 (2-D element kernels)
 void launch_tflux(const DevConsts &c, const void *u, double *qu, cudaStream_t s);           // Eq 12, in place over Q^u
 void launch_common_flux(const DevConsts &c, void *uf, const void *qf, bool f32, cudaStream_t s);  // Eq 15-17, in place over U^f (f32: float arrays)
 
@@ -94,8 +95,6 @@ constexpr int RK_MAX_PARTIALS = 4096;
 // out1 = sum_i a[i] in[i], out2 = sum_i b[i] in[i]  (either output may be NULL or alias an input)
 cudaError_t rk_lincomb(bool f64, int64_t rows, int64_t ld, int64_t nel, int nin, const void *const *in, const double *a, const double *b,
                        void *out1, void *out2, cudaStream_t s);
-cudaError_t rk_axpy2(bool f64, int64_t rows, int64_t ld, int64_t nel, const void *u, const void *k, double a, void *out1, double b,
-                     void *out2, int mode, cudaStream_t s);
 // *out = sqrt(mean (x - y)^2) over the rows x nel values, deterministic; part: RK_MAX_PARTIALS doubles of scratch
 cudaError_t rk_rms_diff(bool f64, int64_t rows, int64_t ld, int64_t nel, const void *x, const void *y, double *part, double *out,
                         cudaStream_t s);

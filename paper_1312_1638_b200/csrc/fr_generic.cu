@@ -351,6 +351,12 @@ void launch_common_jump(const DevConsts &c, const double *uf, double *cf, cudaSt
   }
 }
 
+void launch_common_sol(const DevConsts &c, const double *uf, double *cf, cudaStream_t s) {  // 2-D, C itself (Eq 7)
+  const int TB = 128;
+  if (c.npairs) k_common_sol<2, false><<<(unsigned)((c.npairs + TB - 1) / TB), TB, 0, s>>>(c, uf, cf);
+  if (c.nbnd) k_common_sol_bnd<2, false><<<(unsigned)((c.nbnd + TB - 1) / TB), TB, 0, s>>>(c, uf, cf);
+}
+
 template <int ND, bool NS>
 static void launch_tflux_t(const DevConsts &c, const void *u, double *qu, cudaStream_t s) {
   const int TB = 128;

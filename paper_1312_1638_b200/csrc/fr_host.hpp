@@ -48,6 +48,7 @@ struct MeshConsts {
   std::vector<int32_t> fp_pe, fp_ps;  // [Nf][ld] partner element / flux point (-1-bc_id at boundaries)
   std::vector<double> fp_n;     // [nd][Nf][ld] OWN outward unit normal
   std::vector<double> fp_Jn;    // [Nf][ld]; sign bit set (negative) when this flux point is the R side
+  std::vector<double> xf;       // [Nf][Nel][nd] flux-point coordinates, kept only for the parts of a mixed mesh
   bool affine = false;          // every element has constant S (J) — metric arrays could be per element
 };
 
@@ -63,6 +64,9 @@ struct MeshInput {
 
 // fr_mesh.cpp; returns FR_OK or an error code with text in err
 // pair_block > 0: order the flux-point pairs element-block major (blocks of pair_block elements) instead of sigma major
-int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, int pair_block, MeshConsts &out, std::string &err);
+// standalone = false (part of a mixed mesh): the part's own interface list is empty, interior flux points are left for the
+// cross-part pairing of fr_api.cu (no coverage check here), and the flux-point coordinates are kept in out.xf
+int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, int pair_block, MeshConsts &out, std::string &err,
+                      bool standalone = true);
 
 }  // namespace fr

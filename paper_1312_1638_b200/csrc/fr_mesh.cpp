@@ -45,7 +45,8 @@ inline long double adjugate(int nd, const long double Jm[3][3], long double S[3]
 
 }  // namespace
 
-int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, int pair_block, MeshConsts &out, std::string &err) {
+int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, int pair_block, MeshConsts &out, std::string &err,
+                      bool standalone) {
   const int nd = in.nd, Nu = ops.Nu, Nf = ops.Nf, Nn = ops.Nn, nfp = ops.nfp;
   const int64_t Nel = in.Nel;
   out = MeshConsts();
@@ -142,7 +143,7 @@ int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, int pa
   }
   int64_t badcover = 0;
   for (auto c : cover) if (c != 1) ++badcover;
-  if (badcover) { err = "flux points not covered exactly once by interfaces + boundary faces: " + std::to_string(badcover); return FR_EMESH; }
+  if (badcover && standalone) { err = "flux points not covered exactly once by interfaces + boundary faces: " + std::to_string(badcover); return FR_EMESH; }
 
   // iteration order: sort by the L flux point (sigma major, element minor) so that consecutive threads
   // read consecutive elements of one row.  With element-blocked flux-point arrays (pair_block > 0
@@ -186,6 +187,7 @@ int build_mesh_consts(const MeshInput &in, const RefOps &ops, int64_t ld, int pa
       out.bJn[i] = out.fp_Jn[(size_t)s * ld + e];
       out.fp_pe[(size_t)s * ld + e] = -1 - in.bfaces[3 * b + 2]; out.fp_ps[(size_t)s * ld + e] = s;
     }
+  if (!standalone) out.xf.swap(xf);
   return FR_OK;
 }
 

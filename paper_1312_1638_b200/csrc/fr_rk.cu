@@ -87,18 +87,6 @@ cudaError_t rk_lincomb(bool f64, int64_t rows, int64_t ld, int64_t nel, int nin,
   return cudaGetLastError();
 }
 
-cudaError_t rk_axpy2(bool f64, int64_t rows, int64_t ld, int64_t nel, const void *u, const void *k, double a, void *out1, double b,
-                     void *out2, int mode, cudaStream_t s) {
-  // mode 0: out1 = u + a k ; out2 = u + b k          (RK4 stage 1: next stage state, accumulator)
-  // mode 1: out1 = u + a k ; out2 = out2 + b k       (stages 2, 3)
-  // mode 2: out1 = out2 + b k                        (stage 4: u <- acc + dt/6 k4; out1 == u)
-  const void *in[3] = {u, k, out2};
-  if (mode == 0) { const double ca[3] = {1, a, 0}, cb[3] = {1, b, 0}; return rk_lincomb(f64, rows, ld, nel, 2, in, ca, cb, out1, out2, s); }
-  if (mode == 1) { const double ca[3] = {1, a, 0}, cb[3] = {0, b, 1}; return rk_lincomb(f64, rows, ld, nel, 3, in, ca, cb, out1, out2, s); }
-  const double ca[3] = {0, b, 1};
-  return rk_lincomb(f64, rows, ld, nel, 3, in, ca, nullptr, out1, nullptr, s);
-}
-
 cudaError_t rk_rms_diff(bool f64, int64_t rows, int64_t ld, int64_t nel, const void *x, const void *y, double *part, double *out,
                         cudaStream_t s) {
   const int TB = 256;

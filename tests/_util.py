@@ -31,14 +31,14 @@ class GpuRunner:
         self.torch = torch
         self.ctx = ctx
         self.tdtype = torch.float64 if ctx.dtype == np.float64 else torch.float32
-        shape = (ctx.Nu, ctx.NV, ctx.ld)
-        self.u = torch.zeros(shape, dtype=self.tdtype, device="cuda")
-        self.r = torch.zeros(shape, dtype=self.tdtype, device="cuda")
+        n = ctx.state_bytes // np.dtype(ctx.dtype).itemsize  # flat buffers: one matrix, or the parts of a mixed mesh
+        self.u = torch.zeros(n, dtype=self.tdtype, device="cuda")
+        self.r = torch.zeros(n, dtype=self.tdtype, device="cuda")
         self.work = torch.zeros(max(ctx.stepper_workspace_bytes("dopri5"), 256), dtype=torch.uint8, device="cuda")
         self.stream = torch.cuda.current_stream().cuda_stream
 
     def set_state(self, U):
-        self.u.copy_(self.torch.from_numpy(self.ctx.pad(U)))
+        self.u.copy_(self.torch.from_numpy(np.ascontiguousarray(self.ctx.pad(U)).reshape(-1)))
 
     def rhs(self, U=None):
         if U is not None:

@@ -559,3 +559,77 @@ def test_euler_and_dopri5_steppers_parity(case):
         ref2, _ = o.dopri5_step(ref2, 3 * dt)
     got2 = run.rk4(U, 3 * dt, 3, stepper="dopri5")
     _check(case + "-dopri5-x3", got2, ref2, TOL64)
+
+
+# ------------------------------------------------------------------------------------------
+# quadrilaterals and triangles sharing edges in one mesh
+# ------------------------------------------------------------------------------------------
+def _mixed_check(name, got, ref, floor=None, tol=TOL64):
+    """parts compared together: per-field norms over the concatenation of all parts' points (columns padded per part)"""
+    cat = lambda parts: np.concatenate([np.asarray(a, dtype=np.longdouble).reshape(-1, a.shape[1], 1).transpose(2, 1, 0) for a in parts], axis=2)
+    g, r = cat(got), cat(ref)
+    bar = tol if floor is None else np.maximum(tol, 2 * rel_l2_per_field(cat(floor), r))
+    return _check(name, np.asarray(g, dtype=np.float64), r, bar, None if floor is None else rel_l2_per_field(cat(floor), r))
+
+
+@pytest.mark.parametrize("p", [1, 2, 3, 4])
+def test_mixed_quad_tri_mesh_parity(p):
+    from oracle.fr_oracle import FRMixedOracle
+
+    ref = dict(rho=1.0, v=(1.0, 1.0), p=1.0 / (1.4 * 0.2 ** 2))  # freestream of workloads.sinusoidal_2d
+    for label, mesh, bcs in (("mixed-periodic", W.mixed_mesh(6, 1.0, 0.1), None), ("mixed-bnd", W.mixed_mesh(5, 1.0, 0.1, periodic=False, tri_from=3), BC2_MIXED)):
+        for system in ("navier-stokes", "euler"):
+            disc = dict(NS, p=p, system=system, ref=ref)
+            o = FRMixedOracle(mesh, disc, bcs)
+            old = FRMixedOracle(mesh, disc, bcs, dtype=np.longdouble)
+            Us = [np.ascontiguousarray(np.moveaxis(W.add_relative_noise(W.sinusoidal_2d(np.asarray(q.xu_phys, float)), 1e-2, 21 + i), -1, 1))
+                  for i, q in enumerate(o.parts)]
+            R, R_ld = o.rhs(Us), old.rhs([np.asarray(u, dtype=np.longdouble) for u in Us])
+            ctx = _ctx(mesh, disc, bcs=bcs)
+            for x, q in zip(ctx.solution_point_coords(), o.parts):
+                assert np.allclose(x, np.asarray(q.xu_phys, float), atol=1e-13)
+            run = GpuRunner(ctx)
+            names = [n for n, _ in ctx.rhs_profiled(*_ptrs(run))]
+            assert "el_interp" in names and "el_fluxdiv" in names, names
+            _mixed_check("%s-p%d-%s-f64" % (label, p, system), run.rhs(Us), R_ld, floor=R)
+            U32 = [u.astype(np.float32) for u in Us]
+            R32 = o.rhs([u.astype(np.float64) for u in U32])
+            got32 = GpuRunner(_ctx(mesh, disc, precision="f32", bcs=bcs)).rhs(U32)
+            assert all(g.dtype == np.float32 for g in got32)
+            _mixed_check("%s-p%d-%s-f32" % (label, p, system), got32, R32, tol=TOL32)
+
+
+BC2_MIXED = {0: ("sup-inflow", dict(rho=1.0, v=(1.0, 1.0), p=17.8)), 1: ("sub-outflow", dict(p=17.5)),
+             2: ("noslip-wall", dict(cpTw=62.0, v=(0.2, 0.0))), 3: ("noslip-wall", dict(cpTw=61.0, v=(0.0, 0.0)))}
+
+
+def test_mixed_mesh_steppers_and_conservation():
+    from oracle.fr_oracle import FRMixedOracle
+
+    mesh = W.mixed_mesh(6, 1.0, 0.1)
+    disc = dict(NS, p=3, ref=dict(rho=1.0, v=(1.0, 1.0), p=1.0 / (1.4 * 0.2 ** 2)))
+    o = FRMixedOracle(mesh, disc)
+    Us = [np.ascontiguousarray(np.moveaxis(W.add_relative_noise(W.sinusoidal_2d(np.asarray(q.xu_phys, float)), 1e-2, 5 + i), -1, 1))
+          for i, q in enumerate(o.parts)]
+    run = GpuRunner(_ctx(mesh, disc))
+    R = run.rhs(Us)
+    tot, mag = o.integrate(R), o.integrate([np.abs(r) for r in R])
+    assert np.all(np.abs(tot) <= 1e-12 * mag), (tot, mag)
+    dt = 2e-5
+    ref = Us
+    for _ in range(3):
+        ref = o.rk4_step(ref, dt)
+    _mixed_check("mixed-rk4x3", run.rk4(Us, dt, 3), ref)
+    ref = [u + dt * r for u, r in zip(Us, o.rhs(Us))]
+    _mixed_check("mixed-euler", run.rk4(Us, dt, 1, stepper="euler"), ref)
+    assert max(np.max(np.abs(a - b)) for a, b in zip(ref, Us)) > 1e-7
+
+
+def test_mixed_mesh_error_paths():
+    from paper_1312_1638_b200 import Context, FrError
+
+    mesh = W.mixed_mesh(4)
+    with pytest.raises(FrError):  # an interface record is missing: flux points left uncovered
+        Context(dict(mesh, ifaces=mesh["ifaces"][1:], shifts=mesh["shifts"][1:])).setup_operators(**dict(NS, p=2))
+    with pytest.raises(FrError):  # orders outside the fused element kernels
+        Context(mesh).setup_operators(**dict(NS, p=5))
