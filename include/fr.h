@@ -198,6 +198,11 @@ int fr_euler_step(fr_ctx *ctx, void *u_dev, double dt, void *work_dev, void *str
  * (bit-reproducible).  Step-size control is the caller's.  work_dev: >= fr_stepper_workspace_bytes(FR_STEPPER_DOPRI5). */
 int fr_dopri5_step(fr_ctx *ctx, void *u_dev, double dt, void *work_dev, void *stream, double *err_dev);
 
+/* out = sum_i coef[i] * in[i] over state matrices (device, context precision; n_in <= 8; out may alias an input; pad columns
+ * untouched): the register update the steppers above are built from, for callers that write their own stepper -- e.g. one
+ * with a halo exchange between the stages (domain decomposition, partition.py). */
+int fr_state_lincomb(fr_ctx *ctx, int n_in, const void *const *in_dev, const double *coef_host, void *out_dev, void *stream);
+
 /* End-to-end variant with HOST buffers: copies u_host -> u_dev (H2D), evaluates fr_rhs, copies
  * rhs_dev -> rhs_host (D2H), all asynchronously on `stream` (pinned host memory recommended).
  * u_dev / rhs_dev / work_dev are caller-allocated device staging buffers as in fr_rhs. */

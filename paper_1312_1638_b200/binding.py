@@ -98,6 +98,7 @@ def _load():
         "fr_rhs_profiled": (C.c_int, [P, P, P, P, P, C.c_int, C.POINTER(C.c_int), P, P]),
         "fr_rk4_step": (C.c_int, [P, P, C.c_double, P, P]),
         "fr_rhs_host": (C.c_int, [P, P, P, P, P, P, P]),
+        "fr_state_lincomb": (C.c_int, [P, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_double), P, P]),
         "fr_measure_peaks": (C.c_int, [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]),
         "fr_teardown": (None, [P]),
         "fr_last_error": (C.c_char_p, [P]),
@@ -112,7 +113,7 @@ lib = _load()
 EXPORTS = ["fr_setup_mesh", "fr_setup_mesh_mixed", "fr_num_parts", "fr_part_info", "fr_part_solution_point_coords", "fr_setup_operators", "fr_num_solution_points", "fr_num_flux_points", "fr_num_vars", "fr_num_pairs",
            "fr_leading_dim", "fr_state_bytes", "fr_workspace_bytes", "fr_stepper_workspace_bytes", "fr_rhs_kernel_launches",
            "fr_euler_step", "fr_dopri5_step", "fr_solution_point_coords",
-           "fr_operator_dims", "fr_get_operator", "fr_get_pairs", "fr_get_metrics", "fr_rhs", "fr_rhs_profiled", "fr_rk4_step", "fr_rhs_host",
+           "fr_operator_dims", "fr_get_operator", "fr_get_pairs", "fr_get_metrics", "fr_rhs", "fr_rhs_profiled", "fr_rk4_step", "fr_rhs_host", "fr_state_lincomb",
            "fr_measure_peaks", "fr_teardown", "fr_last_error"]
 
 
@@ -293,6 +294,13 @@ class Context:
 
     def dopri5_step(self, u_ptr, dt, work_ptr, stream=0, err_ptr=None):
         self._check(lib.fr_dopri5_step(self._h, u_ptr, float(dt), work_ptr, stream, err_ptr))
+
+    def state_lincomb(self, in_ptrs, coefs, out_ptr, stream=0):
+        """out = sum coefs[i] * in[i] over state matrices (device pointers)."""
+        n = len(in_ptrs)
+        arr = (C.c_void_p * n)(*in_ptrs)
+        cf = (C.c_double * n)(*[float(x) for x in coefs])
+        self._check(lib.fr_state_lincomb(self._h, n, arr, cf, out_ptr, stream))
 
     def rhs_host(self, u_host_ptr, rhs_host_ptr, u_ptr, rhs_ptr, work_ptr, stream=0):
         self._check(lib.fr_rhs_host(self._h, u_host_ptr, rhs_host_ptr, u_ptr, rhs_ptr, work_ptr, stream))

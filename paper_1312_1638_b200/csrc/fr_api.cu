@@ -712,6 +712,16 @@ int fr_dopri5_step(fr_ctx *c, void *u, double dt, void *work, void *stream, doub
   return FR_OK;
 }
 
+int fr_state_lincomb(fr_ctx *c, int n_in, const void *const *in, const double *coef, void *out, void *stream) {
+  FR_NEED_READY(c, FR_EINVAL)
+  if (c->host_only) return fail(c, FR_EINVAL, "fr_state_lincomb: context was set up with FR_FLAG_HOST_ONLY");
+  if (n_in < 1 || n_in > RK_MAX_IN || !in || !coef || !out) return fail(c, FR_EINVAL, "fr_state_lincomb: bad arguments");
+  for (int i = 0; i < n_in; ++i) if (!in[i]) return fail(c, FR_EINVAL, "fr_state_lincomb: NULL operand");
+  cudaError_t e = ctx_lincomb(c, n_in, in, coef, nullptr, out, nullptr, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("fr_state_lincomb launch: ") + cudaGetErrorString(e));
+  return FR_OK;
+}
+
 int fr_rhs_host(fr_ctx *c, const void *u_host, void *rhs_host, void *u_dev, void *rhs_dev, void *work, void *stream) {
   FR_NEED_READY(c, FR_EINVAL)
   if (!u_host || !rhs_host || !u_dev || !rhs_dev || !work) return fail(c, FR_EINVAL, "fr_rhs_host: NULL pointer");

@@ -633,3 +633,35 @@ def test_mixed_mesh_error_paths():
         Context(dict(mesh, ifaces=mesh["ifaces"][1:], shifts=mesh["shifts"][1:])).setup_operators(**dict(NS, p=2))
     with pytest.raises(FrError):  # orders outside the fused element kernels
         Context(mesh).setup_operators(**dict(NS, p=5))
+
+
+# ------------------------------------------------------------------------------------------
+# domain decomposition, device side of paper_1312_1638_b200/partition.py
+# ------------------------------------------------------------------------------------------
+def test_domain_decomposition_submesh_rhs_on_gpu():
+    """The right-hand side of every rank's sub-mesh (owned elements + two ghost layers, cut faces with a dummy boundary) equals
+    the whole-mesh right-hand side on the owned elements, through the library on the GPU; the two ranks run one after the other
+    on this GPU and their ghost columns are filled from the full state (what the halo exchange delivers; the exchange itself is
+    covered on gloo in test_multirank_cpu.py)."""
+    import torch
+
+    from paper_1312_1638_b200.partition import DistributedContext
+
+    mesh, disc = W.config("C3", n=6, p=2)
+    o = FROracle(mesh, disc)
+    U = W.config_state("C3", np.asarray(o.xu_phys, float), n=6, p=2)
+    full = GpuRunner(_ctx(mesh, disc)).rhs(U)
+    for rank in (0, 1, 2):
+        dc = DistributedContext(mesh, disc, world=3, rank=rank)
+        assert dc.n_owned < dc.ids.size
+        u = torch.from_numpy(dc.ctx.pad(U[:, :, dc.ids])).cuda()
+        r = torch.zeros_like(u)
+        dc.world = 1  # no peers in this process: the ghost columns are already in place
+        dc.rhs(u, r)
+        torch.cuda.synchronize()
+        got = dc.ctx.unpad(r.cpu().numpy())[:, :, : dc.n_owned]
+        _check("dd-rank%d" % rank, got, full[:, :, dc.ids[: dc.n_owned]], 1e-13)
+        u0 = u.clone()
+        dc.rk4_step(u, 1e-4)
+        torch.cuda.synchronize()
+        assert torch.isfinite(u[:, :, : dc.n_owned]).all() and (u - u0).abs().max() > 0

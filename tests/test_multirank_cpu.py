@@ -34,3 +34,60 @@ def test_max_over_ranks_aggregation_gloo(tmp_path):
     d = json.loads(line)
     assert d["ms"] == 15.0  # the slower rank
     assert abs(d["val"] - 2 * 1000 / 15e-3 / 1e9) < 1e-12
+
+
+def test_domain_decomposition_halo_exchange_gloo(tmp_path):
+    """SURVEY 8(f) item 2, host side: the element partition with two ghost layers and one halo exchange of
+    state columns per right-hand side (paper_1312_1638_b200/partition.py) reproduces the single-rank right-hand side and RK4
+    state on the owned elements of every rank.  world_size 2 and 3 on gloo; the per-rank compute is the oracle (no GPU here),
+    the exchange code is the one the GPU path uses."""
+    script = tmp_path / "dd.py"
+    script.write_text(textwrap.dedent("""
+        import os, sys, json
+        sys.path.insert(0, %r)
+        import numpy as np, torch, torch.distributed as dist
+        import workloads as W
+        from oracle.fr_oracle import FROracle
+        from paper_1312_1638_b200.partition import decompose, exchange_halo
+        dist.init_process_group("gloo")
+        rank, world = dist.get_rank(), dist.get_world_size()
+        mesh = W.box_mesh((5, 12), (1.0, 2.4), p_g=2, warp=lambda X: 0.02 * np.stack([np.sin(2 * np.pi * X[..., 0]) * np.sin(2 * np.pi * X[..., 1] / 2.4)] * 2, -1))
+        disc = dict(p=3, system="navier-stokes", gamma=1.4, mu=0.02, Pr=0.71, beta=0.5, tau=0.1)
+        full = FROracle(mesh, disc)
+        X = np.asarray(full.xu_phys, float)
+        U = np.ascontiguousarray(np.moveaxis(W.add_relative_noise(W.sinusoidal_2d(X / 2.4), 1e-2, 3), -1, 1))
+        plan = decompose(mesh, world)
+        ids, n_own = plan.local[rank], plan.n_owned[rank]
+        assert n_own < ids.size < mesh["nodes"].shape[0]          # there are ghosts, and not the whole mesh
+        sub = FROracle(plan.sub_mesh(rank), disc, {plan.cut_bc: ("sup-inflow", dict(rho=1.0, v=(0.3, 0.1), p=9.0))})
+        def local_rhs(u_loc):
+            u_loc[:, :, n_own:] = np.nan                            # ghost columns are stale until the exchange
+            exchange_halo(plan, rank, u_loc, dist)
+            return sub.rhs(u_loc)
+        u = np.ascontiguousarray(U[:, :, ids])
+        R = local_rhs(u.copy())
+        R_ref = full.rhs(U)
+        err_rhs = float(np.max(np.abs(R[:, :, :n_own] - R_ref[:, :, ids[:n_own]])) / np.max(np.abs(R_ref)))
+        # two RK4 steps with a halo exchange in every stage
+        dt, ref = 1e-4, U
+        for _ in range(2):
+            ref = full.rk4_step(ref, dt)
+            k1 = local_rhs(u.copy()); k2 = local_rhs(u + dt / 2 * k1); k3 = local_rhs(u + dt / 2 * k2); k4 = local_rhs(u + dt * k3)
+            u = u + dt / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
+        err_rk = float(np.max(np.abs(u[:, :, :n_own] - ref[:, :, ids[:n_own]])))
+        out = torch.tensor([err_rhs, err_rk, float(plan.halo_bytes(rank, U.shape[0] * U.shape[1] * 8))], dtype=torch.float64)
+        dist.all_reduce(out, op=dist.ReduceOp.MAX)
+        if rank == 0:
+            print(json.dumps({"err_rhs": out[0].item(), "err_rk": out[1].item(), "halo_bytes": out[2].item(), "world": world}))
+        dist.destroy_process_group()
+    """ % ROOT))
+    import json
+
+    for world, port in ((2, 29531), (3, 29532)):
+        env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), OMP_NUM_THREADS="2")
+        out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=%d" % world, "--master-addr", "127.0.0.1",
+                              "--master-port", str(port), str(script)], capture_output=True, text=True, env=env, timeout=600)
+        assert out.returncode == 0, out.stderr[-3000:]
+        d = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+        assert d["world"] == world and d["halo_bytes"] > 0
+        assert d["err_rhs"] <= 1e-13 and d["err_rk"] <= 1e-13, d
