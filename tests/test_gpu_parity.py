@@ -660,8 +660,57 @@ def test_domain_decomposition_submesh_rhs_on_gpu():
         dc.rhs(u, r)
         torch.cuda.synchronize()
         got = dc.ctx.unpad(r.cpu().numpy())[:, :, : dc.n_owned]
-        _check("dd-rank%d" % rank, got, full[:, :, dc.ids[: dc.n_owned]], 1e-13)
+        _check("dd-rank%d" % rank, got, full[:, :, dc.ids[: dc.n_owned]], TOL64)
         u0 = u.clone()
         dc.rk4_step(u, 1e-4)
         torch.cuda.synchronize()
         assert torch.isfinite(u[:, :, : dc.n_owned]).all() and (u - u0).abs().max() > 0
+
+
+@pytest.mark.parametrize("nd", [2, 3])
+def test_couette_order_of_accuracy(nd):
+    """SURVEY 8(f) item 4, second half: the paper's Couette case (Eq 34-36, constants at :589, walls
+    Eq 51-53 :817-825) marched with fr_rk4_step from the analytic profile to the discrete steady state (t = 1.3: the residual
+    has fallen by four decades, calibrated with the oracle); the L2 energy error against the analytic solution (Eq 37-39)
+    converges at order ~ p + 1 under h-refinement (:601, Tables 2-4); the error measured is that of the total energy, as in the paper.  A short horizon is compared with the oracle state."""
+    cp, Tw, vw, Pr, mu = 1005.0, 300.0, 69.445, 0.72, 0.417
+    bcs = {2: ("noslip-wall", dict(cpTw=cp * Tw, v=(0.0,) * nd)), 3: ("noslip-wall", dict(cpTw=cp * Tw, v=(vw,) + (0.0,) * (nd - 1)))}
+    ref = dict(rho=1.16, v=(0.0,) * nd, p=1e5)
+    orders = {}
+    for p, ns_ in ((1, (2, 4, 8, 16) if nd == 2 else (2, 4, 8)), (2, (2, 4, 8)), (3, (2, 4) if nd == 3 else (2, 4, 8))):
+        errs = []
+        for n in ns_:
+            mesh = W.box_mesh((n, n) if nd == 2 else (n, n, 2), (1.0,) * nd, periodic=(True, False) if nd == 2 else (True, False, True))
+            disc = dict(p=p, system="navier-stokes", gamma=1.4, mu=mu, Pr=Pr, beta=0.5, tau=0.1, ref=ref)
+            o = FROracle(mesh, disc, bcs)
+            Uex = _couette(np.asarray(o.xu_phys, float))
+            dt = 0.4 * (1.0 / n) / ((2 * p + 1) * 420.0)
+            run = GpuRunner(_ctx(mesh, disc, bcs=bcs))
+            if n == 2:  # parity of the marching itself: 40 steps against the oracle from a perturbed profile
+                # (long-double oracle: R_rho_v and R_rho_w of this flow are ~1e-9 of the flux scale p0 = 1e5, so the double
+                # oracle's own rounding is what a comparison with it would measure)
+                U0 = Uex * (1 + 1e-3 * np.sin(7 * np.asarray(o.xu_phys, float)[..., 0])[:, None, :])
+                old = FROracle(mesh, disc, bcs, dtype=np.longdouble)
+                want = np.asarray(U0, dtype=np.longdouble)
+                for _ in range(40):
+                    want = old.rk4_step(want, np.longdouble(dt))
+                want = np.asarray(want, dtype=np.float64)
+                dbl = U0
+                for _ in range(40):
+                    dbl = o.rk4_step(dbl, dt)
+                got = run.rk4(U0, dt, 40)
+                sc = np.max(np.abs(want), axis=(0, 2))
+                sc[1:-1] = np.max(sc[1:-1])
+                e_gpu, e_dbl = np.max(np.abs(got - want) / sc[None, :, None]), np.max(np.abs(dbl - want) / sc[None, :, None])
+                print("couette marching nd=%d p=%d: gpu vs long double %.2e, double oracle vs long double %.2e" % (nd, p, e_gpu, e_dbl))
+                # rounding differences are amplified ~1e3 over these steps at p = 3 on 2-element periodic directions: the bar is
+                # the tolerance or the double oracle's own distance from the long-double one, whichever is larger
+                assert e_gpu <= max(1e-12, e_dbl), (nd, p, e_gpu, e_dbl)
+            U = run.rk4(Uex, dt, int(np.ceil(1.3 / dt)))
+            assert np.all(np.isfinite(U))
+            errs.append(float(o.l2_error(U, Uex)[-1]))  # L2 error of the total energy, the paper's measure (Eq 37-39 :593-597)
+        h = np.log(1.0 / np.array(ns_))
+        orders[p] = float(np.polyfit(h, np.log(errs), 1)[0])
+        print("couette nd=%d p=%d errors %s order %.2f" % (nd, p, ["%.3e" % e for e in errs], orders[p]))
+    for p, q in orders.items():
+        assert q > p + 0.5, orders
