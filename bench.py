@@ -174,7 +174,8 @@ def time_oracle(args, sample_n, reps):
     from oracle.fr_oracle import FROracle
 
     a2 = argparse.Namespace(**vars(args))
-    a2.n = sample_n
+    if sample_n:
+        a2.n = sample_n
     mesh, disc, over, _ = workload(a2)
     o = FROracle(mesh, disc)
     U = W.config_state(args.workload, np.asarray(o.xu_phys, float), **over)
@@ -195,11 +196,9 @@ def time_oracle(args, sample_n, reps):
 
 
 def sample_size(args):
-    if args.workload in ("C3", "C2", "C5"):
-        return 8
-    if args.workload == "C4":
-        return 64
-    return 0
+    """Elements per direction of the oracle's timed sample: C1, C2 and C4 at full size, C3 on its 16^3
+    version (1/8 of the elements, same shape), C5 on the 8^3 sub-problem; scaled per DOF."""
+    return {"C3": 16, "C5": 8}.get(args.workload, 0)
 
 
 def run_reference(args):

@@ -56,6 +56,7 @@ int fail(const fr_ctx *c, int code, const std::string &msg) {
 void free_dev(fr_ctx *c) {
   for (void *p : c->dev_allocs) cudaFree(p);
   c->dev_allocs.clear();
+  if (c->dc.map_cache) { hex_tma_cache_destroy(c->dc.map_cache); c->dc.map_cache = nullptr; }
 }
 
 template <typename T>
@@ -202,6 +203,7 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     cudaError_t e = cudaGetDevice(&dc.dev);
     if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
     dc.blk = blk;
+    dc.map_cache = blk ? hex_tma_cache_create() : nullptr;
     auto reblock = [&](const auto &src, int rows) {  // [rows][ld] -> [ld / FR_BLK][rows][FR_BLK]
       typename std::decay<decltype(src)>::type dst(src.size());
       for (int64_t b = 0; b < ld / FR_BLK; ++b)

@@ -42,6 +42,7 @@ struct DevConsts {
   int nbcs;
   // element-centric tables (tensor-product kernels)
   const int32_t *fp_pe, *fp_ps;
+  void *map_cache;           // host object owned by the context (fr_tma.cuh: MapCache): encoded tensor maps keyed on the caller's pointers
   const int64_t *fp_poff;    // hexahedral TMA path, [block][Nf][FR_BLK]: offset of the partner's first variable in U^f, or -1 - bc_id
   const uint8_t *face_code;  // [6][ld] (hexahedra): 0 = face without LDG weight, 1 = L side, 2 = R side, 3 = boundary (fr_hex_tma.cu)
   const double *fp_n, *fp_Jn;

@@ -258,17 +258,22 @@ cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
   constexpr int MINB = min_blocks(L::TOTAL, N * N * E);
   const uint64_t ld = (uint64_t)c.ld;
-  CUtensorMap mS, mU, mQ, mD4, mD2, mR;
   static_assert(FR_BLK % E == 0, "a CTA's elements must lie in one element block");
   constexpr bool F64 = sizeof(T) == 8;
-  bool ok = encode_blk(&mS, F64, c.smat, ld, NU, 9, E, NFP, 9, c.aff ? 1 : 0);  // metric terms in T on this path (fr_api.cu)
+  bool fresh = true;
+  MapCache::Ent *ent = ((MapCache *)c.map_cache)->get(NS ? 2 : 3, u, q, dt, fresh);
+  CUtensorMap &mS = ent->m[0], &mU = ent->m[1], &mQ = ent->m[2], &mD4 = ent->m[3], &mD2 = ent->m[4], &mR = ent->m[5];
+  bool ok = !fresh;
+  if (fresh) {
+  ok = encode_blk(&mS, F64, c.smat, ld, NU, 9, E, NFP, 9, c.aff ? 1 : 0);  // metric terms in T on this path (fr_api.cu)
   ok = ok && encode3(&mU, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, 1);  // caller layout
   if (NS) ok = ok && encode_blk(&mQ, F64, q, ld, NV * NFP, 3 * N, E, NV * NFP, 3);
   else mQ = mS;
   ok = ok && encode_blk(&mD4, F64, dt, ld, NFP * NV, 6, E, NFP * NV, 4);
   ok = ok && encode_blk(&mD2, F64, dt, ld, NFP * NV, 6, E, NFP * NV, 2);
   ok = ok && encode_blk(&mR, F64, c.rcpj, ld, NFP, N, E, NFP, N, c.aff ? 2 : 0);
-  if (!ok) return cudaErrorNotSupported;
+  }
+  if (!ok) { ent->id = -1; return cudaErrorNotSupported; }
   auto kern = k_hex_fluxdiv_tma<N, E, NS, T, NB, MINB>;
   static DevFlags done;
   cudaError_t err = set_smem(kern, L::TOTAL, done, c.dev);

@@ -88,8 +88,10 @@ cudaError_t launch_interp(const DevConsts &c, const double *h_ops, const void *u
   constexpr size_t SMEM = 128 + al128(2 * N * 8) + al128(NU * NV * E * sizeof(T)) + 128;
   static_assert(SMEM <= SMEM_MAX && FR_BLK % E == 0, "configuration");
   const uint64_t ld = (uint64_t)c.ld;
-  CUtensorMap mU;
-  if (!encode3(&mU, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, N)) return cudaErrorNotSupported;
+  bool fresh = true;
+  MapCache::Ent *ent = ((MapCache *)c.map_cache)->get(0, u, nullptr, nullptr, fresh);
+  CUtensorMap &mU = ent->m[0];
+  if (fresh && !encode3(&mU, sizeof(T) == 8, u, ld, NFP * NV, N, ld, (uint64_t)NFP * NV * ld, E, NFP * NV, N)) { ent->id = -1; return cudaErrorNotSupported; }
   auto kern = k_hex_interp_tma<N, E, T>;
   static DevFlags done;
   cudaError_t err = set_smem(kern, SMEM, done, c.dev);

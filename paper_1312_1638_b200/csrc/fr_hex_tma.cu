@@ -465,9 +465,12 @@ cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void 
   using L = GfLay<N, E, T>;
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
   constexpr int MINB = min_blocks(L::TOTAL, N * N * E, sizeof(T) == 8 ? 128 : 96);  // single-precision arithmetic needs fewer registers
-  Maps m;
   if (!q) return cudaErrorInvalidValue;  // the z-face pass re-reads the stored Q slices
-  if (!make_maps<N, E, T>(c, u, m, q)) return cudaErrorNotSupported;
+  bool fresh = true;
+  MapCache::Ent *ent = ((MapCache *)c.map_cache)->get(1, u, q, nullptr, fresh);
+  Maps &m = *reinterpret_cast<Maps *>(ent->m);
+  static_assert(sizeof(Maps) <= sizeof(ent->m), "map cache entry");
+  if (fresh && !make_maps<N, E, T>(c, u, m, q)) { ent->id = -1; return cudaErrorNotSupported; }
   const Ops1D<N, T> op = make_ops<N, T>(h_ops);
   return c.nbnd ? launch_gradface_k<N, E, true, T, MINB>(c, m, op, (const T *)uf, (T *)gf, s)
                 : launch_gradface_k<N, E, false, T, MINB>(c, m, op, (const T *)uf, (T *)gf, s);
@@ -488,6 +491,9 @@ cudaError_t gradface_n(const DevConsts &c, const double *h_ops, const void *u, c
 }
 
 }  // namespace
+
+void *hex_tma_cache_create() { return new MapCache(); }
+void hex_tma_cache_destroy(void *cache) { delete (MapCache *)cache; }
 
 bool hex_tma_supported(int n, bool f64) {
   if (!encoder() || !hex_tma_fluxdiv_supported(n, f64)) return false;

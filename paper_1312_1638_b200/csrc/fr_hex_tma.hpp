@@ -7,6 +7,9 @@ namespace fr {
 // true when the sm_100a TMA kernels (both of them) can run this n = p+1 / precision: shared memory fits, the driver exposes
 // the tensor-map encoder.  The internal arrays are then element-blocked (fr_dev.hpp: fp_row).
 bool hex_tma_supported(int n, bool f64);
+// cache of encoded tensor maps (one per context; keyed on the u / workspace pointers of a call, which rarely change)
+void *hex_tma_cache_create();
+void hex_tma_cache_destroy(void *cache);
 
 // Flux-point arrays of this path (U^f -> D~, G^f) and Q are stored in the context's storage precision (double | float),
 // element-blocked; all arithmetic is double.

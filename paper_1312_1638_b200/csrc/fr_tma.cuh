@@ -241,6 +241,26 @@ inline bool encode_blk(CUtensorMap *m, bool f64, const void *base, uint64_t ld, 
 }
 
 // function attributes are per device: one flag per (kernel instantiation, device ordinal)
+// Encoded tensor maps of one context, keyed on (kernel, the pointers a call passes): cuTensorMapEncodeTiled costs about a
+// microsecond per map and an RHS needs 11 of them, which matters for the launch-bound small cases; RK steppers alternate
+// between two or three pointer sets.
+struct MapCache {
+  struct Ent { int id = -1; const void *p[3] = {nullptr, nullptr, nullptr}; CUtensorMap m[6]; };
+  static const int CAP = 16;
+  Ent e[CAP];
+  int next = 0;
+  // returns the entry and whether it has to be filled
+  Ent *get(int id, const void *a, const void *b, const void *c, bool &fresh) {
+    for (int i = 0; i < CAP; ++i)
+      if (e[i].id == id && e[i].p[0] == a && e[i].p[1] == b && e[i].p[2] == c) { fresh = false; return &e[i]; }
+    Ent *x = &e[next];
+    next = (next + 1) % CAP;
+    x->id = id; x->p[0] = a; x->p[1] = b; x->p[2] = c;
+    fresh = true;
+    return x;
+  }
+};
+
 template <typename K>
 cudaError_t set_smem(K kern, size_t smem, DevFlags &done, int dev) {
   if (done.test(dev)) return cudaSuccess;

@@ -208,3 +208,40 @@ def test_M6_single_element_gradient_with_exact_trace(etype, p):
         lhs = ref.wu @ qt[d]  # integral of q_d over the element
         rhs = np.sum(ref.wf * ref.nf[:, d] * C)  # boundary integral of C n_d
         assert abs(float(lhs - rhs)) < 1e-13
+
+
+@pytest.mark.parametrize("etype,p", [("tri", 1), ("tri", 2), ("tri", 3), ("tri", 4), ("quad", 3)])
+def test_M3_is_the_DG_lifting_weak_form(etype, p):
+    """What tells the DG correction from every other admissible one (reading A5; VERDICT r1 soft spot i): the divergence of the
+    correction field of flux point sigma, h_sigma = sum_rho M3[rho, sigma] l_rho, is the L2 representer of the weighted point
+    evaluation on the face:  int_Omega phi h_sigma = w_sigma phi(x_sigma)  for EVERY phi of degree <= p (an SD- or HU-like
+    correction satisfies it for degree <= p - 1 only).  Checked with the test's own quadrature (numpy Gauss-Legendre, Duffy
+    map on the triangle) against all monomials -- the strong-form DG equivalence M3 D~ + (M1 - M3 M2) F~ follows from it by
+    integration by parts (Eq 8)."""
+    from numpy.polynomial.legendre import leggauss
+
+    ref = RefElement(etype, p)
+    M3 = np.asarray(Operators(ref).M3, dtype=np.float64)
+    g, w = leggauss(p + 4)
+    a, b = np.meshgrid(g, g, indexing="ij")
+    wa, wb = np.meshgrid(w, w, indexing="ij")
+    if etype == "tri":
+        xq = np.stack([((1 + a) * (1 - b) / 2 - 1).ravel(), b.ravel()], -1)
+        wq = (wa * wb * (1 - b) / 2).ravel()
+    else:
+        xq, wq = np.stack([a.ravel(), b.ravel()], -1), (wa * wb).ravel()
+    Lq = np.asarray(ref.basis(xq)[0], dtype=np.float64)          # l_rho at the quadrature points
+    h = Lq @ M3                                                   # h_sigma at the quadrature points
+    xf, wf = np.asarray(ref.xf, float), np.asarray(ref.wf, float)
+    worst_p, worst_p1 = 0.0, 0.0
+    for ea in range(p + 2):
+        for eb in range(p + 2 - ea):
+            phi_q, phi_f = xq[:, 0] ** ea * xq[:, 1] ** eb, xf[:, 0] ** ea * xf[:, 1] ** eb
+            res = np.max(np.abs((wq * phi_q) @ h - wf * phi_f))
+            if ea + eb <= p:
+                worst_p = max(worst_p, res)
+            elif etype == "tri":
+                worst_p1 = max(worst_p1, res)
+    assert worst_p < 1e-12, worst_p
+    if etype == "tri":
+        assert worst_p1 > 1e-3  # and not beyond degree p: the identity is sharp
