@@ -87,12 +87,15 @@ def rhs_algorithmic_words(nd, NV, Nu, Nf, ns, affine):
     return w
 
 
-def kernel_bytes(name, nd, NV, Nu, Nf, ns, gfrac=1.0, sz=8, szi=8):
+def kernel_bytes(name, nd, NV, Nu, Nf, ns, gfrac=1.0, sz=8, szi=8, affine=False):
     """compulsory bytes per element for one launch group (inputs once + outputs once).
     sz: bytes of a state / metric word (8 | 4: the algorithmic size in the context's precision); szi: bytes of a flux-point /
     gradient intermediate as the path stores it (= sz on the hexahedral TMA path, 8 elsewhere); index words are 4 bytes,
     gather offsets 8.  gfrac: fraction of the faces that carry an LDG weight (1/2 when |beta| = 1/2)."""
+    # NOTE: fp_n (own normals, read by the gradient kernels) is counted at nd * N_f words whatever the mesh
     met = (nd * nd + 1) * Nu * sz
+    if affine and (name.startswith("hex_") or name.startswith("el_")):
+        met = (nd * nd + 1) * sz  # straight-sided elements: the fused kernels read the metric terms of ONE point per element
     pair_tab = (4 * 4 + (nd + 2) * sz) * Nf // 2  # per flux-point pair: 4 indices, unit normal, two J n
     U, R = Nu * NV * sz, Nu * NV * sz
     t = {
@@ -118,7 +121,8 @@ def kernel_bytes(name, nd, NV, Nu, Nf, ns, gfrac=1.0, sz=8, szi=8):
         "hex_fluxdiv_tma": U + R + Nf * NV * szi + (nd * Nu * NV * szi if ns else 0) + met,
         # fused triangle / quadrilateral kernels (fr_element.cu)
         "el_interp": U + Nf * NV * szi,
-        "el_gradface": U + 3 * Nf * NV * szi + met + nd * Nf * sz + nd * Nu * NV * szi,   # U, C, U^f, S, 1/J, normals -> Q, G^f
+        # U, own and partner U^f (+ 8-byte offsets, side codes), S, 1/J, normals -> Q, G^f
+        "el_gradface": U + 3 * Nf * NV * szi + Nf * 9 + met + nd * Nf * sz + nd * Nu * NV * szi,
         "el_fluxdiv": U + R + Nf * NV * szi + (nd * Nu * NV * szi if ns else 0) + met,
     }
     return t.get(name)
@@ -341,7 +345,7 @@ def measure(args, world, rank, local, barrier, light=False):
     szi = sz if any(n.startswith("hex_") for n in acc) else 8  # the hexahedral TMA path stores its intermediates in the storage precision
     kern = []
     for name, ms in acc.items():
-        byt = kernel_bytes(name, nd, NV, Nu, Nf, ns, 0.5 if abs(abs(disc.get("beta", 0.5)) - 0.5) < 1e-15 else 1.0, sz, szi)
+        byt = kernel_bytes(name, nd, NV, Nu, Nf, ns, 0.5 if abs(abs(disc.get("beta", 0.5)) - 0.5) < 1e-15 else 1.0, sz, szi, affine)
         gbs = (byt * ctx.n_elems / (ms * 1e-3) / 1e9) if (byt and ms > 0) else None
         kern.append({"name": name, "ms": ms, "share": ms / sum(acc.values()), "algorithmic_GBps": gbs})
     kern.sort(key=lambda k: -k["ms"])

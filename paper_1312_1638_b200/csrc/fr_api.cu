@@ -255,6 +255,21 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     }
     const bool want_el = dc.ns && element_fused_supported(dc);  // fused triangle kernels
     if (want_el) { UP(mc.fp_n, fp_n); if (mc.nbnd) { UP(mc.fp_pe, fp_pe); } }
+    if (want_el && !c->sub) {
+      // the fused 2-D gradient kernel forms the common solution itself (Eq 7, 25): partner of every flux point as an offset
+      // into U^f [N_f][N_V][ld], and on which side of its interface the flux point lies (1 = L, 2 = R, 3 = boundary)
+      std::vector<int64_t> poff((size_t)o.Nf * ld, 0);
+      std::vector<uint8_t> code((size_t)o.Nf * ld, 0);
+      for (int sg = 0; sg < o.Nf; ++sg)
+        for (int64_t el = 0; el < mc.Nel; ++el) {
+          const size_t i0 = (size_t)sg * ld + el;
+          const int32_t pe = mc.fp_pe[i0];
+          poff[i0] = pe < 0 ? 0 : (int64_t)mc.fp_ps[i0] * dc.NV * ld + pe;
+          code[i0] = pe < 0 ? 3 : (mc.fp_Jn[i0] < 0 ? 2 : 1);
+        }
+      UP(poff, fp_poff);
+      UP(code, face_code);
+    }
     if (want_tma) {
       // faces that carry an LDG weight (jump of Eq 9 and G^f of Eq 27): L sides weigh 1/2 + beta, R sides 1/2 - beta
       std::vector<uint8_t> code((size_t)o.nfaces * ld, 0);

@@ -108,7 +108,10 @@ __global__ void __launch_bounds__(TPB) k_el_interp(const __grid_constant__ OpsIn
 }
 
 // u [NU][NV][ld] (T), cf = common solution C [NF][NV][ld], uf = U^f [NF][NV][ld]; out: q [ND][NU][NV][ld], gf [NF][NV][ld]
-template <int NU, int NF, bool BND, typename T>
+// GATHER: the common solution C (Eq 7, 25) is formed here from the own and the partner's U^f (c.fp_poff / c.face_code, set up by
+// fr_api.cu for single-type meshes); cf then holds C at boundary flux points only (k_common_sol_bnd).  Otherwise (parts of a
+// mixed mesh) cf holds C everywhere.
+template <int NU, int NF, bool BND, bool GATHER, typename T>
 __global__ void __launch_bounds__(TPB) k_el_gradface(const __grid_constant__ OpsGrad<NU, NF> op, DevConsts c, const T *__restrict__ u,
                                                       const double *__restrict__ cf, const double *__restrict__ uf,
                                                       double *__restrict__ q, double *__restrict__ gf) {
@@ -123,8 +126,22 @@ __global__ void __launch_bounds__(TPB) k_el_gradface(const __grid_constant__ Ops
 #pragma unroll
     for (int r = 0; r < NU; ++r) uu[r] = (double)u[((size_t)r * NV + a) * ld + e];
     pert_rows<NU, T>(c.ph, a, u, ld, e, uu);  // the gradient is taken of the perturbation variables (fr_physics.cuh)
+    if (GATHER) {
+      const double wL = 0.5 - c.ph.beta, wR = 0.5 + c.ph.beta;  // C = wL u_L + wR u_R
 #pragma unroll
-    for (int s = 0; s < NF; ++s) cc[s] = cf[((size_t)s * NV + a) * ld + e];
+      for (int s = 0; s < NF; ++s) {
+        const int code = c.face_code[(size_t)s * ld + e];
+        if (BND && code == 3) {
+          cc[s] = cf[((size_t)s * NV + a) * ld + e];
+        } else {
+          const double own = uf[((size_t)s * NV + a) * ld + e], oth = uf[c.fp_poff[(size_t)s * ld + e] + (size_t)a * ld];
+          cc[s] = code == 1 ? wL * own + wR * oth : wL * oth + wR * own;
+        }
+      }
+    } else {
+#pragma unroll
+      for (int s = 0; s < NF; ++s) cc[s] = cf[((size_t)s * NV + a) * ld + e];
+    }
     // affine elements: the metric terms of point 0 serve every point (one load instead of N_u)
     double Sa[ND][ND], rja = 0;
     if (c.affine) {
@@ -276,12 +293,20 @@ cudaError_t gradface_t(const DevConsts &c, const void *u, const double *cf, cons
   const unsigned grid = (unsigned)((c.Nel + EB - 1) / EB);
   static DevFlags done;  // function attributes are per device
   if (!done.test(c.dev) && smem > 48 * 1024) {
-    cudaFuncSetAttribute(k_el_gradface<NU, NF, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(k_el_gradface<NU, NF, false, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_el_gradface<NU, NF, true, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_el_gradface<NU, NF, false, true, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_el_gradface<NU, NF, true, false, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_el_gradface<NU, NF, false, false, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   done.set(c.dev);
-  if (c.nbnd) k_el_gradface<NU, NF, true, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
-  else k_el_gradface<NU, NF, false, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
+  const bool gather = c.fp_poff != nullptr;
+  if (gather) {
+    if (c.nbnd) k_el_gradface<NU, NF, true, true, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
+    else k_el_gradface<NU, NF, false, true, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
+  } else {
+    if (c.nbnd) k_el_gradface<NU, NF, true, false, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
+    else k_el_gradface<NU, NF, false, false, T><<<grid, TPB, smem, s>>>(op, c, (const T *)u, cf, uf, q, gf);
+  }
   return cudaGetLastError();
 }
 

@@ -291,10 +291,10 @@ cudaError_t run(const DevConsts &c, const WorkLayout &w, const T *u, T *rhs, cha
     cudaError_t e = element_interp(c, u, uf, s);
     if (e != cudaSuccess) return e;
     if (NS) {
-      FR_MARK(prof, "common_sol");
-      if (c.npairs) k_common_sol<ND, false><<<blocks(c.npairs), TB, 0, s>>>(c, uf, cf);
-      if (c.nbnd) k_common_sol_bnd<ND, false><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, cf);
+      // the gradient kernel forms the common solution of interior flux points itself (c.fp_poff); boundaries keep their kernel
       FR_MARK(prof, "el_gradface");
+      if (!c.fp_poff && c.npairs) k_common_sol<ND, false><<<blocks(c.npairs), TB, 0, s>>>(c, uf, cf);
+      if (c.nbnd) k_common_sol_bnd<ND, false><<<blocks(c.nbnd), TB, 0, s>>>(c, uf, cf);
       if ((e = element_gradface(c, u, cf, uf, qu, qf, s)) != cudaSuccess) return e;
       FR_MARK(prof, "common_flux_g");
       launch_common_flux_g(c, uf, qf, false, s);
@@ -401,9 +401,9 @@ void launch_common_flux_g(const DevConsts &c, void *uf, const void *gf, bool f32
 
 int generic_rhs_launches(const DevConsts &c) {
   if (c.nd == 2 && element_fused_supported(c)) {
-    int n = c.ns ? 5 : 3;  // interp, (common sol, gradface,) common flux, fluxdiv
+    int n = c.ns ? 4 : 3;  // interp, (gradface with the common solution,) common flux, fluxdiv
     if (c.nbnd) n += c.ns ? 2 : 1;
-    if (!c.npairs) n -= c.ns ? 2 : 1;
+    if (!c.npairs) n -= 1;
     return n;
   }
   int n = 4;  // interp, tflux, common flux, divergence

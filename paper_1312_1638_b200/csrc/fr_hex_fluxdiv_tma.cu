@@ -14,7 +14,7 @@ struct FdLay {
   static constexpr int NFP = N * N, NU = N * NFP;
   static constexpr size_t BAR = 0;
   static constexpr size_t OPS = 128;  // sDh [N*N], sGm [N], sGp [N]
-  static constexpr size_t ST = OPS + al128((N * N + 2 * N) * 8);
+  static constexpr size_t ST = OPS + al128((N * N + 2 * N) * 8);  // (sized for double operators)
   static constexpr uint32_t S_TX = 9 * NFP * E * sizeof(T), U_TX = NFP * NV * E * sizeof(T), Q_TX = NS ? 3 * NV * NFP * E * sizeof(T) : 0;
   static constexpr size_t ST_U = al128(S_TX);
   static constexpr size_t ST_Q = ST_U + al128(U_TX);
@@ -29,7 +29,7 @@ struct FdLay {
   static constexpr bool EPI_ST = N >= 2 && EP_RJ + RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
   static constexpr bool EPI_DED = N >= 2 && !EPI_ST && RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
   static constexpr bool EPI_TMA = EPI_ST || EPI_DED;
-  static constexpr size_t DED = F + NB * F_BYTES;
+  static constexpr size_t DED = F + al128(NB * F_BYTES);  // TMA destination: 128-byte aligned
   static constexpr size_t TOTAL = DED + (EPI_DED ? al128(DXY_TX) : 0) + 128;  // + slack for the manual 128-byte alignment
 };
 
@@ -49,10 +49,13 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char *sm = smem_raw + ((128u - (smem_addr(smem_raw) & 127u)) & 127u);  // stays in the shared address space
   uint64_t *bar = (uint64_t *)(sm + L::BAR);
-  double *sDh = (double *)(sm + L::OPS), *sGm = sDh + N * N, *sGp = sGm + N;
+  // Arithmetic in double in both storage precisions (the inviscid flux and its divergence are where cancellation happens).
+  // Contractions in float were measured in single precision: no gain (0.192 ms either way on C3) and twice the freestream residual.
+  using R = double;
+  R *sDh = (R *)(sm + L::OPS), *sGm = sDh + N * N, *sGp = sGm + N;
   unsigned char *sSt = sm + L::ST;
-  double *sF = (double *)(sm + L::F);  // [NB][2][NV][NFP][E]
-  const int tid = threadIdx.x, el = tid % E, ij = tid / E, i = ij % N, j = ij / N;
+  R *sF = (R *)(sm + L::F);  // [NB][2][NV][NFP][E]
+  const int tid = threadIdx.x, el = tid % E, ij = patch_ij<N>(tid / E), i = ij % N, j = ij / N;  // 2 x 2 patches per warp (fr_tma.cuh)
   const int e0 = blockIdx.x * E, l0 = e0 % FR_BLK, eb = e0 / FR_BLK;  // first element: lane and element block (fp_row)
   const int64_t e = (int64_t)e0 + el;
   const bool act = e < Nel;
@@ -76,11 +79,11 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     if (N > 1) issue_stage(1, 1);
     if (L::EPI_DED) { mbar_expect_tx(&bar[2], L::DXY_TX); tma_load_4d(sm + L::DED, &tmD4, l0, 0, 0, eb, &bar[2]); }
   }
-  double acc[N][NV];
+  R acc[N][NV];
 #pragma unroll
   for (int k = 0; k < N; ++k)
 #pragma unroll
-    for (int a = 0; a < NV; ++a) acc[k][a] = 0.0;
+    for (int a = 0; a < NV; ++a) acc[k][a] = 0;
 
 #pragma unroll
   for (int k = 0; k < N; ++k) {
@@ -88,7 +91,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     const T *stS = (const T *)(sSt + (k & 1) * L::ST_BYTES);
     const T *stU = (const T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_U);
     const T *stQ = (const T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_Q);
-    double *buf = sF + (NB == 2 ? (k & 1) : 0) * (2 * NV * NFP * E);
+    R *buf = sF + (NB == 2 ? (k & 1) : 0) * (2 * NV * NFP * E);
     {
       double S[3][3], uu[NV];
 #pragma unroll
@@ -150,9 +153,9 @@ __global__ void __launch_bounds__(N *N *E, MINB)
           else if (a < 4) { f[n] = v[n] * ww[a] + (a - 1 == n ? pp : 0.0); if (NS) f[n] -= Tm[n][a - 1]; }
           else { f[n] = v[n] * (ww[4] + pp); if (NS) f[n] -= w[n]; }
         }
-        buf[((0 * NV + a) * NFP + ij) * E + el] = fma(S[0][0], f[0], fma(S[0][1], f[1], S[0][2] * f[2]));
-        buf[((1 * NV + a) * NFP + ij) * E + el] = fma(S[1][0], f[0], fma(S[1][1], f[1], S[1][2] * f[2]));
-        const double fz = fma(S[2][0], f[0], fma(S[2][1], f[1], S[2][2] * f[2]));
+        buf[((0 * NV + a) * NFP + ij) * E + el] = (R)fma(S[0][0], f[0], fma(S[0][1], f[1], S[0][2] * f[2]));
+        buf[((1 * NV + a) * NFP + ij) * E + el] = (R)fma(S[1][0], f[0], fma(S[1][1], f[1], S[1][2] * f[2]));
+        const R fz = (R)fma(S[2][0], f[0], fma(S[2][1], f[1], S[2][2] * f[2]));
 #pragma unroll
         for (int kk = 0; kk < N; ++kk) acc[kk][a] = fma(op.Dh[kk * N + k], fz, acc[kk][a]);
       }
@@ -177,7 +180,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     // x and y contractions within the slice
 #pragma unroll
     for (int m = 0; m < N; ++m) {
-      const double dx = sDh[i * N + m], dy = sDh[j * N + m];
+      const R dx = sDh[i * N + m], dy = sDh[j * N + m];
 #pragma unroll
       for (int a = 0; a < NV; ++a) {
         acc[k][a] = fma(dx, buf[((0 * NV + a) * NFP + j * N + m) * E + el], acc[k][a]);
@@ -186,7 +189,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     }
   }
   // lifting M3 D~ and the -1/J scale (Eq 19); faces: 0,1 = x-,x+ (idx j + N k); 2,3 = y (i + N k); 4,5 = z (i + N j)
-  const double gmi = sGm[i], gpi = sGp[i], gmj = sGm[j], gpj = sGp[j];
+  const double gmi = (double)sGm[i], gpi = (double)sGp[i], gmj = (double)sGm[j], gpj = (double)sGp[j];
   if (L::EPI_TMA) {
     const T *sDxy = (const T *)(L::EPI_DED ? sm + L::DED : sSt + ((N - 2) & 1) * L::ST_BYTES);  // [4][NFP*NV][E]
     const T *sRJ = (const T *)(sSt + ((N - 2) & 1) * L::ST_BYTES + (L::EPI_DED ? 0 : L::EP_RJ));  // [NU][E]
@@ -203,9 +206,9 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       double r0 = 0;  // R~ of the mass equation: R_mj = R_wmj + v0_j R_wrho, R_E = R_wE + h0 R_wrho (fr_physics.cuh)
 #pragma unroll
       for (int a = 0; a < NV; ++a) {
-        double v = acc[k][a];
-        v = fma(op.gm[k], (double)sDz[((0 * NFP + ij) * NV + a) * E + el], v);
-        v = fma(op.gp[k], (double)sDz[((1 * NFP + ij) * NV + a) * E + el], v);
+        double v = (double)acc[k][a];
+        v = fma((double)op.gm[k], (double)sDz[((0 * NFP + ij) * NV + a) * E + el], v);
+        v = fma((double)op.gp[k], (double)sDz[((1 * NFP + ij) * NV + a) * E + el], v);
         v = fma(gmi, (double)sDxy[((0 * NFP + fx) * NV + a) * E + el], v);
         v = fma(gpi, (double)sDxy[((1 * NFP + fx) * NV + a) * E + el], v);
         v = fma(gmj, (double)sDxy[((2 * NFP + fy) * NV + a) * E + el], v);
@@ -232,9 +235,9 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     double r0 = 0;
 #pragma unroll
     for (int a = 0; a < NV; ++a) {
-      double v = acc[k][a];
-      v = fma(op.gm[k], dzm[a], v);
-      v = fma(op.gp[k], dzp[a], v);
+      double v = (double)acc[k][a];
+      v = fma((double)op.gm[k], dzm[a], v);
+      v = fma((double)op.gp[k], dzp[a], v);
       v = fma(gmi, (double)dt[fp_row(true, ld, 6 * NFP * NV, (0 * NFP + fx) * NV + a, e)], v);
       v = fma(gpi, (double)dt[fp_row(true, ld, 6 * NFP * NV, (1 * NFP + fx) * NV + a, e)], v);
       v = fma(gmj, (double)dt[fp_row(true, ld, 6 * NFP * NV, (2 * NFP + fy) * NV + a, e)], v);
@@ -253,10 +256,11 @@ cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *
   using L2 = FdLay<N, E, NS, T, 2>;
   using L1 = FdLay<N, E, NS, T, 1>;
   // double-buffer F~ when that does not cost a resident CTA
-  constexpr int NB = (L2::TOTAL <= SMEM_MAX && min_blocks(L2::TOTAL, N * N * E) == min_blocks(L1::TOTAL, N * N * E)) ? 2 : 1;
+  constexpr int REGS = 128;
+  constexpr int NB = (L2::TOTAL <= SMEM_MAX && min_blocks(L2::TOTAL, N * N * E, REGS) == min_blocks(L1::TOTAL, N * N * E, REGS)) ? 2 : 1;
   using L = FdLay<N, E, NS, T, NB>;
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
-  constexpr int MINB = min_blocks(L::TOTAL, N * N * E);
+  constexpr int MINB = min_blocks(L::TOTAL, N * N * E, REGS);
   const uint64_t ld = (uint64_t)c.ld;
   static_assert(FR_BLK % E == 0, "a CTA's elements must lie in one element block");
   constexpr bool F64 = sizeof(T) == 8;

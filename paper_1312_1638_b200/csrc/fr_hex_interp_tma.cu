@@ -100,12 +100,18 @@ cudaError_t launch_interp(const DevConsts &c, const double *h_ops, const void *u
   return cudaGetLastError();
 }
 
+// elements per CTA of this kernel: as the other kernels, except N = 7 where its small footprint allows 64-byte rows
+template <int N>
+struct EI {
+  static constexpr int E = N == 7 ? 8 : Cfg<N, double>::E;
+};
+
 }  // namespace
 
 cudaError_t hex_tma_interp(const DevConsts &c, const double *h_ops, const void *u, void *uf, cudaStream_t s) {
   switch (c.n) {
 #define FR_CASE(NN) \
-  case NN: return c.f64 ? launch_interp<NN, Cfg<NN, double>::E, double>(c, h_ops, u, uf, s) : launch_interp<NN, Cfg<NN, float>::E, float>(c, h_ops, u, uf, s);
+  case NN: return c.f64 ? launch_interp<NN, EI<NN>::E, double>(c, h_ops, u, uf, s) : launch_interp<NN, EI<NN>::E, float>(c, h_ops, u, uf, s);
     FR_CASE(2) FR_CASE(3) FR_CASE(4) FR_CASE(5) FR_CASE(6) FR_CASE(7)
 #undef FR_CASE
     default: return cudaErrorNotSupported;

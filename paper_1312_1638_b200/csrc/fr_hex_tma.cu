@@ -80,7 +80,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   const T *stS = (const T *)(sm + L::SS);
   unsigned char *sSt = sm + L::ST;
   T *sQ = (T *)(sm + L::Q);  // [3][NFP][NV][E]
-  const int tid = threadIdx.x, el = tid % E, ij = tid / E, i = ij % N, j = ij / N;
+  const int tid = threadIdx.x, el = tid % E, ij = patch_ij<N>(tid / E), i = ij % N, j = ij / N;  // 2 x 2 patches per warp (fr_tma.cuh)
   const int e0 = blockIdx.x * E, l0 = e0 % FR_BLK, eb = e0 / FR_BLK;  // first element: lane and element block (fp_row)
   const int64_t e = (int64_t)e0 + el;
   const bool act = e < Nel;
@@ -209,6 +209,9 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       for (int a = 0; a < NV; ++a) uo[a] = fma(l, (R)sU[((size_t)(base + mm * stride) * NV + a) * E + el], uo[a]);
     }
   };
+  // own state at the task's flux point, kept from phase A (jump) to phase C (G^f) of the same slice when a thread has one task
+  constexpr bool KEEP = TPT == 1;
+  R uo_keep[KEEP ? NV : 1];
   auto phase_A = [&](int k) {  // jumps of the x/y faces of slice k, in place over the gathered partner values
     T *sP = (T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_P);
 #pragma unroll
@@ -217,6 +220,10 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       if (t >= 4 * N) continue;
       R uo[NV];
       if (code_xy[q] != 0) own_xy(t, k, uo);
+      if constexpr (KEEP) {
+#pragma unroll
+        for (int a = 0; a < NV; ++a) uo_keep[a] = uo[a];
+      }
       int64_t bc = 0;
       if (BND && code_xy[q] == 3) bc = poff(face_of(t) * NFP + t % N + N * k);
       jump_of(code_xy[q], bc, uo, sP + (size_t)t * NV * E + el);
@@ -324,7 +331,12 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       R nrm[3], uo[NV], G[NV];
 #pragma unroll
       for (int n = 0; n < 3; ++n) nrm[n] = (R)fp_n[fp_row(true, ld, 3 * NF, n * NF + fp, e)];
-      own_xy(t, k, uo);
+      if constexpr (KEEP) {
+#pragma unroll
+        for (int a = 0; a < NV; ++a) uo[a] = uo_keep[a];
+      } else {
+        own_xy(t, k, uo);
+      }
       if constexpr (BND) {
         const int pe = code_xy[q] == 3 ? (int)poff(fp) : 0;
         R qf[3][NV];

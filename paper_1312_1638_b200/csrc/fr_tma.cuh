@@ -270,6 +270,19 @@ cudaError_t set_smem(K kern, size_t smem, DevFlags &done, int dev) {
   return e;
 }
 
+// Thread slot -> point (i, j) of a slice, grouping the points in 2 x 2 patches: the four slots that share a warp with E = 8
+// elements then touch two x-lines and two y-lines instead of (up to) four distinct lines in one direction, so a line read in
+// either direction is one 128-byte shared-memory wavefront.  A bijection of 0 .. N*N-1 that maps slots < k*N onto points < k*N
+// only loosely; the kernels use it for nothing but the choice of (i, j).
+template <int N>
+__device__ __forceinline__ int patch_ij(int slot) {
+  constexpr int M = N / 2;  // full 2 x 2 patches per patch row; a patch row holds 2 N points
+  if (slot >= 2 * N * M) return (N - 1) * N + (slot - 2 * N * M);  // last point row of an odd N
+  const int br = slot / (2 * N), s2 = slot % (2 * N);
+  if (s2 < 4 * M) return (2 * br + ((s2 >> 1) & 1)) * N + 2 * (s2 >> 2) + (s2 & 1);
+  return (2 * br + (s2 - 4 * M)) * N + N - 1;  // last point column of an odd N
+}
+
 // elements per CTA for each n = p + 1 (row segments of E*8 bytes; N = 7: only 4 elements fit the shared memory).  The same in
 // single precision: twice the elements (64-byte segments again) halves the resident CTAs of the register-bound kernels and
 // was slower (C3 fp32: gradient kernel 0.41 -> 0.47 ms, divergence kernel 0.19 -> 0.22 ms)
