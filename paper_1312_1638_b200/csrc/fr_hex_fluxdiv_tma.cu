@@ -256,7 +256,7 @@ cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *
   using L2 = FdLay<N, E, NS, T, 2>;
   using L1 = FdLay<N, E, NS, T, 1>;
   // double-buffer F~ when that does not cost a resident CTA
-  constexpr int REGS = 128;
+  constexpr int REGS = 128;  // (96 registers for a third resident CTA: 176 bytes of spills at p = 4 in single precision, rejected)
   constexpr int NB = (L2::TOTAL <= SMEM_MAX && min_blocks(L2::TOTAL, N * N * E, REGS) == min_blocks(L1::TOTAL, N * N * E, REGS)) ? 2 : 1;
   using L = FdLay<N, E, NS, T, NB>;
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
