@@ -712,5 +712,5 @@ def test_couette_order_of_accuracy(nd):
         h = np.log(1.0 / np.array(ns_))
         orders[p] = float(np.polyfit(h, np.log(errs), 1)[0])
         print("couette nd=%d p=%d errors %s order %.2f" % (nd, p, ["%.3e" % e for e in errs], orders[p]))
-    for p, q in orders.items():
-        assert q > p + 0.5, orders
+    for p, q in orders.items():  # the paper: 2.21 / 2.99 / 3.97 (Table 2), 2.06 / 2.87 / 3.99 (Table 3); measured here: profiles/r02_couette.md
+        assert p + 0.7 < q < p + 1.8, orders
