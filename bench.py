@@ -26,6 +26,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 import workloads as W  # noqa: E402
 
+ORACLE_SINGLE_THREAD_S = None
 METRIC = "FR RHS GDOF/s"
 UNIT = "GDOF/s"
 
@@ -189,14 +190,20 @@ def time_oracle(args, sample_n, reps):
         t0 = time.perf_counter()
         o.rhs(U)
         ts.append(time.perf_counter() - t0)
+    global ORACLE_SINGLE_THREAD_S
     try:
-        from threadpoolctl import threadpool_info
+        from threadpoolctl import threadpool_info, threadpool_limits
 
         cores = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+        with threadpool_limits(limits=1):  # the same code with its BLAS calls on one thread
+            t0 = time.perf_counter()
+            o.rhs(U)
+            ORACLE_SINGLE_THREAD_S = time.perf_counter() - t0
     except Exception:
         cores = os.cpu_count()
-    return U.size, ts, cores, "%s-shaped %s sub-problem (%d elements, %d DOF), %d oracle RHS evaluations, numpy float64" % (
-        args.workload, "x".join(str(s) for s in mesh["shape"]), mesh["nodes"].shape[0], U.size, reps)
+        ORACLE_SINGLE_THREAD_S = None
+    return U.size, ts, cores, "%s %s (%d elements, %d DOF), %d oracle RHS evaluations, numpy float64" % (
+        args.workload, ("at full size, %s" if not sample_n else "on its %s version") % "x".join(str(s) for s in mesh["shape"]), mesh["nodes"].shape[0], U.size, reps)
 
 
 def sample_size(args):
@@ -219,7 +226,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": len(ts), "warmup": args.warmup,
         "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": desc,
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "cpu": cpu_model(),
+                         "single_thread_value": (dof / ORACLE_SINGLE_THREAD_S / 1e9) if ORACLE_SINGLE_THREAD_S else None},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -395,7 +403,7 @@ def measure(args, world, rank, local, barrier, light=False):
     if not light and not args.no_cpu_baseline and world == 1:
         cdof, ts, cores, sample = time_oracle(args, sample_size(args), 5)
         out["cpu_baseline"] = {"value": cdof / float(np.mean(ts)) / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
-                               "cpu": cpu_model()}
+                               "cpu": cpu_model(), "single_thread_value": (cdof / ORACLE_SINGLE_THREAD_S / 1e9) if ORACLE_SINGLE_THREAD_S else None}
     else:
         out["cpu_baseline"] = None
     ctx.teardown()
