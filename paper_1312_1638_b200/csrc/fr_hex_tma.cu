@@ -33,7 +33,8 @@ namespace {
 // ---------------------------------------------------------------------------------------------
 // shared-memory layout (byte offsets from a 128-byte aligned base)
 // ---------------------------------------------------------------------------------------------
-template <int N, int E, typename T>
+// NST: depth of the {1/J, x/y partner values} ring (2; 1 where the second stage would cost the second resident CTA: p = 6 in double)
+template <int N, int E, typename T, int NST = 2>
 struct GfLay {
   static constexpr int NFP = N * N, NU = N * NFP;
   static constexpr size_t BAR = 0;
@@ -48,7 +49,7 @@ struct GfLay {
   static constexpr size_t ST_P = al128(R_TX);
   static constexpr size_t P_BYTES = 4 * N * NV * E * sizeof(T);   // [slot 0..3 = faces 1, 3, 0, 2][N][NV][E]
   static constexpr size_t ST_BYTES = ST_P + al128(P_BYTES);
-  static constexpr size_t Q = ST + 2 * ST_BYTES;
+  static constexpr size_t Q = ST + NST * ST_BYTES;
   static constexpr size_t Q_BYTES = 3 * NV * NFP * E * sizeof(T);
   static constexpr size_t TOTAL = Q + al128(Q_BYTES) + 128;
 };
@@ -61,13 +62,13 @@ struct GfLay {
 // uf: U^f of all elements in perturbation variables (k_hex_interp_tma), element-blocked; fp_poff: for every flux point the
 // offset of its partner's first variable in uf, or -1 - bc_id on a boundary; face_code [6][ld]: 0 = no LDG weight (skip),
 // 1 = L side (1/2 + beta), 2 = R side (1/2 - beta), 3 = boundary.
-template <int N, int E, bool BND, typename T, int MINB>
+template <int N, int E, bool BND, typename T, int MINB, int NST>
 __global__ void __launch_bounds__(N *N *E, MINB)
     k_hex_gradface(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS,
                    const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmQ, Ops1D<N, T> op, Phys ph,
                    const T *__restrict__ uf, const int64_t *__restrict__ fp_poff, const T *__restrict__ fp_n,
                    const uint8_t *__restrict__ face_code, const BcDev *__restrict__ bcs, T *__restrict__ gf, int64_t ld, int64_t Nel) {
-  using L = GfLay<N, E, T>;
+  using L = GfLay<N, E, T, NST>;
   using R = T;  // arithmetic type of this kernel: the gradient feeds the viscous flux only (see the header comment)
   constexpr int NFP = N * N, NF = 6 * NFP;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -108,7 +109,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     tma_load_3d(sm + L::U, &tmU, e0, 0, 0, &bar[0]);
     issue_S(0);
     issue_R(0, 0);
-    if (N > 1) issue_R(1, 1);
+    if (NST > 1 && N > 1) issue_R(1, 1);
   }
   // x/y-face tasks of a thread per slice: task t = ij + q NFP < 4 N handles flux point (slot t / N, line m = t % N) of the
   // thread's element; slots 0..3 = faces 1, 3 (+x, +y: the L sides of structured meshes, so that skipped tasks fall into the
@@ -133,8 +134,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
     for (int a = 0; a < NV; ++a) cp_async<sizeof(T)>(dst + a * E, uf + off + (int64_t)a * FR_BLK);
   };
-  auto gather_xy = [&](int k, int64_t *off) {  // slice k into stage k & 1
-    T *sP = (T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_P);
+  auto gather_xy = [&](int k, int64_t *off) {  // slice k into stage k % NST
+    T *sP = (T *)(sSt + (k % NST) * L::ST_BYTES + L::ST_P);
 #pragma unroll
     for (int q = 0; q < TPT; ++q) {
       const int t = ij + q * NFP;
@@ -154,20 +155,24 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     }
     gather_xy(0, off);
     cp_async_commit();
-    if (N > 1) {
+    // slices 1 .. NST - 1 (one group each), then the offsets of slice NST wait in registers
 #pragma unroll
-      for (int q = 0; q < TPT; ++q) {
-        const int t = ij + q * NFP;
-        off[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N + N) : 0;
+    for (int k1 = 1; k1 < NST; ++k1) {
+      if (k1 < N) {
+#pragma unroll
+        for (int q = 0; q < TPT; ++q) {
+          const int t = ij + q * NFP;
+          off[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N + N * k1) : 0;
+        }
+        gather_xy(k1, off);
       }
-      gather_xy(1, off);
+      cp_async_commit();
     }
-    cp_async_commit();
-    if (N > 2) {
+    if (N > NST) {
 #pragma unroll
       for (int q = 0; q < TPT; ++q) {
         const int t = ij + q * NFP;
-        off_nx[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N + 2 * N) : 0;
+        off_nx[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N + N * NST) : 0;
       }
     }
   }
@@ -213,7 +218,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   constexpr bool KEEP = TPT == 1;
   R uo_keep[KEEP ? NV : 1];
   auto phase_A = [&](int k) {  // jumps of the x/y faces of slice k, in place over the gathered partner values
-    T *sP = (T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_P);
+    T *sP = (T *)(sSt + (k % NST) * L::ST_BYTES + L::ST_P);
 #pragma unroll
     for (int q = 0; q < TPT; ++q) {
       const int t = ij + q * NFP;
@@ -244,7 +249,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     }
     __syncthreads();
   }
-  cp_async_wait<1>();  // z faces and slice 0 have arrived (this thread's own copies)
+  cp_async_wait<NST - 1>();  // z faces and slice 0 have arrived (this thread's own copies)
   {
     R uz[2][NV];
 #pragma unroll
@@ -271,10 +276,10 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 
 #pragma unroll
   for (int k = 0; k < N; ++k) {
-    mbar_wait(&bar[1 + (k & 1)], (k >> 1) & 1);
+    mbar_wait(&bar[1 + (k % NST)], (k / NST) & 1);
     mbar_wait(&bar[3], k & 1);
-    const T *stR = (const T *)(sSt + (k & 1) * L::ST_BYTES);
-    const T *stJ = (const T *)(sSt + (k & 1) * L::ST_BYTES + L::ST_P);  // [slot][line][NV][E]: slots 0, 1 = +x, +y; 2, 3 = -x, -y
+    const T *stR = (const T *)(sSt + (k % NST) * L::ST_BYTES);
+    const T *stJ = (const T *)(sSt + (k % NST) * L::ST_BYTES + L::ST_P);  // [slot][line][NV][E]: slots 0, 1 = +x, +y; 2, 3 = -x, -y
     const T *su = sU + (size_t)(NFP * k) * NV * E + el;  // slice k
     {
       R S[3][3];
@@ -306,15 +311,15 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     fence_proxy_async();  // make the sQ writes visible to the bulk store
     __syncthreads();      // Q of the slice is complete; S, 1/J and the jumps of stage k&1 have been consumed
     if (tid == 0 && k + 1 < N) issue_S(k + 1);
-    if (tid == 0 && k + 2 < N) issue_R(k & 1, k + 2);
+    if (tid == 0 && k + NST < N) issue_R(k % NST, k + NST);
     if (tid == 0) { tma_store_4d(&tmQ, l0, 0, 3 * k, eb, sQ); tma_store_commit(); }
-    if (k + 2 < N) {  // partner values of slice k + 2 into the freed stage; the offsets of slice k + 3 start their way
-      gather_xy(k + 2, off_nx);
-      if (k + 3 < N) {
+    if (k + NST < N) {  // partner values of slice k + NST into the freed stage; the offsets of the slice after it start their way
+      gather_xy(k + NST, off_nx);
+      if (k + NST + 1 < N) {
 #pragma unroll
         for (int q = 0; q < TPT; ++q) {
           const int t = ij + q * NFP;
-          off_nx[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N + N * (k + 3)) : 0;
+          off_nx[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N + N * (k + NST + 1)) : 0;
         }
       }
     }
@@ -365,7 +370,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       for (int a = 0; a < NV; ++a) gf[fp_row(true, ld, NF * NV, fp * NV + a, e)] = (T)G[a];
     }
     if (k + 1 < N) {
-      cp_async_wait<1>();  // slice k + 1 has arrived (slice k + 2 may still be in flight)
+      cp_async_wait<NST - 1>();  // slice k + 1 has arrived (with two stages slice k + 2 may still be in flight)
       phase_A(k + 1);
     }
     if (tid == 0) tma_store_wait_read();  // the bulk store has read sQ
@@ -374,7 +379,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   // ---- z faces.  Q^f on them is sum_k l(+-1)_k Q(i, j, k): instead of carrying 2 x 15 accumulators through the slice
   // loop, the Q slices just stored are streamed once more (TMA loads, L2 hits) through two buffers that the slice loop
   // no longer needs: [SS .. Q) (S, 1/J, x/y jumps) and [U .. SS) (U block, z jumps).  The last slice is still in sQ.
-  static_assert(L::Q - L::SS >= L::Q_BYTES && L::SS - L::U >= L::Q_BYTES, "Q slice does not fit the reused buffers");
+  constexpr bool ZB_IN_U = L::SS - L::U >= 2 * al128(L::Q_BYTES);  // both reload buffers inside the U block + z jumps
+  static_assert(ZB_IN_U || (L::Q - L::SS >= L::Q_BYTES && L::SS - L::U >= L::Q_BYTES), "Q slice does not fit the reused buffers");
   R ufz[2][NV];
 #pragma unroll
   for (int s = 0; s < 2; ++s)
@@ -389,7 +395,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       ufz[1][a] = fma(op.lp[m], v, ufz[1][a]);
     }
   __syncthreads();  // U block, z jumps and the stages are dead from here on
-  unsigned char *zb[2] = {sm + L::SS, sm + L::U};
+  unsigned char *zb[2] = {ZB_IN_U ? sm + L::U : sm + L::SS, ZB_IN_U ? sm + L::U + al128(L::Q_BYTES) : sm + L::U};
   if (tid == 0) {
     tma_store_wait_all();  // every Q slice of this CTA has reached global memory
 #pragma unroll
@@ -460,10 +466,10 @@ bool make_maps(const DevConsts &c, const void *u, Maps &m, const void *q) {
   return ok;
 }
 
-template <int N, int E, bool BND, typename T, int MINB>
+template <int N, int E, bool BND, typename T, int MINB, int NST>
 cudaError_t launch_gradface_k(const DevConsts &c, const Maps &m, const Ops1D<N, T> &op, const T *uf, T *gf, cudaStream_t s) {
-  using L = GfLay<N, E, T>;
-  auto kern = k_hex_gradface<N, E, BND, T, MINB>;
+  using L = GfLay<N, E, T, NST>;
+  auto kern = k_hex_gradface<N, E, BND, T, MINB, NST>;
   static DevFlags done;
   cudaError_t err = set_smem(kern, L::TOTAL, done, c.dev);
   if (err != cudaSuccess) return err;
@@ -474,9 +480,12 @@ cudaError_t launch_gradface_k(const DevConsts &c, const Maps &m, const Ops1D<N, 
 
 template <int N, int E, typename T>
 cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void *u, const void *uf, void *gf, void *q, cudaStream_t s) {
-  using L = GfLay<N, E, T>;
+  // one ring stage instead of two where that is what lets a second CTA reside on the SM (p = 6 in double precision: 121.6 -> 115.5 KB)
+  constexpr int REGS = sizeof(T) == 8 ? 128 : 96;
+  constexpr int NST = (min_blocks(GfLay<N, E, T, 2>::TOTAL, N * N * E, REGS) < 2 && min_blocks(GfLay<N, E, T, 1>::TOTAL, N * N * E, REGS) >= 2) ? 1 : 2;
+  using L = GfLay<N, E, T, NST>;
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
-  constexpr int MINB = min_blocks(L::TOTAL, N * N * E, sizeof(T) == 8 ? 128 : 96);  // single-precision arithmetic needs fewer registers
+  constexpr int MINB = min_blocks(L::TOTAL, N * N * E, REGS);  // single-precision arithmetic needs fewer registers
   if (!q) return cudaErrorInvalidValue;  // the z-face pass re-reads the stored Q slices
   bool fresh = true;
   MapCache::Ent *ent = ((MapCache *)c.map_cache)->get(1, u, q, nullptr, fresh);
@@ -484,8 +493,8 @@ cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void 
   static_assert(sizeof(Maps) <= sizeof(ent->m), "map cache entry");
   if (fresh && !make_maps<N, E, T>(c, u, m, q)) { ent->id = -1; return cudaErrorNotSupported; }
   const Ops1D<N, T> op = make_ops<N, T>(h_ops);
-  return c.nbnd ? launch_gradface_k<N, E, true, T, MINB>(c, m, op, (const T *)uf, (T *)gf, s)
-                : launch_gradface_k<N, E, false, T, MINB>(c, m, op, (const T *)uf, (T *)gf, s);
+  return c.nbnd ? launch_gradface_k<N, E, true, T, MINB, NST>(c, m, op, (const T *)uf, (T *)gf, s)
+                : launch_gradface_k<N, E, false, T, MINB, NST>(c, m, op, (const T *)uf, (T *)gf, s);
 }
 
 template <int N, typename T>
