@@ -195,7 +195,7 @@ int fr_euler_step(fr_ctx *ctx, void *u_dev, double dt, void *work_dev, void *str
 /* One step of the Dormand-Prince 5(4) pair (Table 1 :263 "DOPRI5"; the published tableau, reading A24): seven fr_rhs
  * evaluations; u advanced in place with the fifth-order weights.  err_dev (device, may be NULL): receives the RMS over
  * all n_elems*N_u*N_V values of the embedded error estimate dt * sum_i (b5_i - b4_i) k_i, reduced in a fixed order
- * (bit-reproducible).  Step-size control is the caller's.  work_dev: >= fr_stepper_workspace_bytes(FR_STEPPER_DOPRI5). */
+ * (bit-reproducible; FR_EUNSUPPORTED with a non-NULL err_dev on a mixed-mesh context).  Step-size control is the caller's.  work_dev: >= fr_stepper_workspace_bytes(FR_STEPPER_DOPRI5). */
 int fr_dopri5_step(fr_ctx *ctx, void *u_dev, double dt, void *work_dev, void *stream, double *err_dev);
 
 /* out = sum_i coef[i] * in[i] over state matrices (device, context precision; n_in <= 8; out may alias an input; pad columns

@@ -91,3 +91,41 @@ def test_domain_decomposition_halo_exchange_gloo(tmp_path):
         d = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
         assert d["world"] == world and d["halo_bytes"] > 0
         assert d["err_rhs"] <= 1e-13 and d["err_rk"] <= 1e-13, d
+
+
+def test_partition_plan_invariants():
+    """Index bookkeeping of the domain decomposition (no communication): every element is owned once; ghosts are exactly the
+    elements within two face-neighbour steps; send and receive tables of every pair of ranks list the same global elements in
+    the same order; a sub-mesh covers each of its flux-point faces once (interfaces kept + cut faces + original boundaries)."""
+    import numpy as np
+
+    import workloads as W
+    from paper_1312_1638_b200.partition import decompose
+
+    for mesh, world in ((W.box_mesh((4, 4, 9), (1.0, 1.0, 2.0), periodic=(True, False, True)), 3), (W.tri_mesh(8, 1.0, 0.1, 3), 4)):
+        n_el = mesh["nodes"].shape[0]
+        plan = decompose(mesh, world)
+        owned = np.concatenate([plan.local[r][: plan.n_owned[r]] for r in range(world)])
+        assert np.array_equal(np.sort(owned), np.arange(n_el))
+        nfaces = {"hex": 6, "tri": 3, "quad": 4}[mesh["etype"]]
+        for r in range(world):
+            ids = plan.local[r]
+            for peer, idx in plan.recv[r].items():
+                assert np.array_equal(ids[idx], plan.local[peer][plan.send[peer][r]])
+                assert np.all(plan.owner[ids[idx]] == peer) and np.all(idx >= plan.n_owned[r])
+            got = np.sort(np.concatenate([v for v in plan.recv[r].values()])) if plan.recv[r] else np.zeros(0, int)
+            assert np.array_equal(got, np.arange(plan.n_owned[r], ids.size))  # every ghost is received exactly once
+            sub = plan.sub_mesh(r)
+            cover = np.zeros((ids.size, nfaces), dtype=int)
+            np.add.at(cover, (sub["ifaces"][:, 0], sub["ifaces"][:, 1]), 1)
+            np.add.at(cover, (sub["ifaces"][:, 2], sub["ifaces"][:, 3]), 1)
+            np.add.at(cover, (sub["bfaces"][:, 0], sub["bfaces"][:, 1]), 1)
+            assert np.all(cover == 1)
+            # the owned elements and their neighbours' neighbours are all present: no cut face within one step of an owned element
+            cut = sub["bfaces"][sub["bfaces"][:, 2] == plan.cut_bc][:, 0]
+            near = np.zeros(ids.size, dtype=bool)
+            near[: plan.n_owned[r]] = True
+            touch = near[sub["ifaces"][:, 0]] | near[sub["ifaces"][:, 2]]
+            near[sub["ifaces"][touch, 0]] = True
+            near[sub["ifaces"][touch, 2]] = True
+            assert not np.any(near[cut])
