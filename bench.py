@@ -6,7 +6,7 @@ over the whole synthetic mesh.  Default workload: C3 of BASELINE.json — 32^3 p
 p=4, 3-D Navier-Stokes, fp64, Taylor-Green + seeded noise (the configuration the metric's target
 "p=4 hexahedral Navier-Stokes FP64 RHS" is quoted on).  Inputs exceed L2 (state 164 MB, working set >1 GB).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C2|C1|C4|C5] [--precision f64|f32]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C2|C1|C4|C5|Q] [--precision f64|f32]
   python bench.py --impl reference ...      # the oracle on the host cores, bounded sample
 
 Multi-GPU: the path is single-GPU by the north_star ("no sharding or collectives") => replicas only:
@@ -209,7 +209,7 @@ def time_oracle(args, sample_n, reps):
 def sample_size(args):
     """Elements per direction of the oracle's timed sample: C1, C2 and C4 at full size, C3 on its 16^3
     version (1/8 of the elements, same shape), C5 on the 8^3 sub-problem; scaled per DOF."""
-    return {"C3": 16, "C5": 8}.get(args.workload, 0)
+    return {"C3": 16, "C5": 8, "Q": 64}.get(args.workload, 0)
 
 
 def run_reference(args):

@@ -193,9 +193,10 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     dc.Nel = mc.Nel; dc.ld = ld; dc.npairs = mc.npairs; dc.nbnd = mc.nbnd;
     dc.ns = d->system == FR_NAVIER_STOKES; dc.f64 = d->precision == FR_F64;
     dc.staged = (d->flags & FR_FLAG_FORCE_GENERIC) != 0;
+    dc.force_el = c->sub;
     // the reference state (perturbation form, fr_physics.cuh) serves the fused kernel families; the staged sequence and the
     // line kernels of high-order quadrilaterals evaluate the plain formulas
-    const bool fused = !dc.staged && (o.etype == FR_HEX ? blk : (o.n >= 2 && o.n <= (o.etype == FR_TRI ? 6 : 5)));
+    const bool fused = !dc.staged && (o.etype == FR_HEX ? blk : element_fused_supported(dc));
     const double zero3[3] = {0, 0, 0};
     dc.ph = make_phys(d->gamma, d->mu, d->Pr, d->ldg_beta, d->ldg_tau, fused ? d->rho_ref : 0.0, fused ? d->v_ref : zero3, fused ? d->p_ref : 0.0);
     dc.dev = -1;
@@ -253,7 +254,7 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
         }
       UP(reblock(poff, o.Nf), fp_poff);
     }
-    const bool want_el = dc.ns && element_fused_supported(dc);  // fused triangle kernels
+    const bool want_el = dc.ns && element_fused_supported(dc);  // fused triangle / quadrilateral kernels
     if (want_el) { UP(mc.fp_n, fp_n); if (mc.nbnd) { UP(mc.fp_pe, fp_pe); } }
     if (want_el && !c->sub) {
       // the fused 2-D gradient kernel forms the common solution itself (Eq 7, 25): partner of every flux point as an offset

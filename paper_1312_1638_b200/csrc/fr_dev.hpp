@@ -22,6 +22,7 @@ struct DevConsts {
   bool ns;       // Navier-Stokes (gradients, LDG) or Euler
   bool f64;      // storage precision of u / rhs
   bool staged;   // FR_FLAG_FORCE_GENERIC: the paper's staged kernel sequence, no fused kernels
+  bool force_el; // part of a mixed mesh: always the fused element kernels (quadrilaterals p = 4 too)
   bool affine;   // every element has constant metric terms (straight-sided simplices, parallelepipeds): one point serves all
   bool aff;      // blk and every element affine: smat / rcpj hold ONE point per element ([block][9][FR_BLK], [block][1][FR_BLK])
   bool blk;      // library-internal arrays are element-blocked (FR_BLK elements per block), see fp_row()

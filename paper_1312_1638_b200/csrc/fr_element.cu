@@ -339,11 +339,14 @@ cudaError_t interp_t(const DevConsts &c, const void *u, double *uf, cudaStream_t
 }  // namespace
 
 // triangles p = 1 .. 5 (N_u = (p+1)(p+2)/2, N_f = 3 (p+1)) and quadrilaterals p = 1 .. 4 (N_u = (p+1)^2, N_f = 4 (p+1)): at these
-// sizes the dense operators cost less than the extra launches and HBM round trips of the staged / sum-factorised sequences
+// sizes the dense operators cost less than the extra launches and HBM round trips of the staged / sum-factorised sequences.
+// Quadrilaterals at p = 4 with Navier-Stokes are the exception: the fused gradient kernel needs 254 registers there and the
+// sum-factorised line kernels are faster (16.6 against 14.5 GDOF/s on 768^2 elements); Euler at p = 4 stays fused (51 against
+// 31 GDOF/s).  Parts of a mixed mesh always take the fused kernels (force_el): the cross-part pair kernels expect their layout.
 bool element_fused_supported(const DevConsts &c) {
   if (c.staged) return false;
   if (c.etype == FR_TRI) return c.n >= 2 && c.n <= 6;
-  if (c.etype == FR_QUAD) return c.n >= 2 && c.n <= 5;
+  if (c.etype == FR_QUAD) return c.n >= 2 && c.n <= ((c.force_el || !c.ns) ? 5 : 4);
   return false;
 }
 

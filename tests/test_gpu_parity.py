@@ -203,8 +203,9 @@ def _sweep(label, mesh, p, bcs=None, systems=("navier-stokes", "euler"), precisi
             run = GpuRunner(ctx)
             name = "%s-p%d-%s-%s" % (label, p, system, precision)
             if expect is not None:
+                want = expect(system) if callable(expect) else expect
                 names = [n for n, _ in ctx.rhs_profiled(*_ptrs(run))]
-                assert any(expect in n for n in names), (name, names)
+                assert any(want in n for n in names), (name, names)
                 if not bcs:  # boundary kernels are extra launches inside the same profiled groups
                     assert len(names) == ctx.rhs_kernel_launches, (name, names, ctx.rhs_kernel_launches)
             if precision == "f64":
@@ -239,10 +240,13 @@ def test_hex_orders_outside_the_tma_kernels(p):
 
 @pytest.mark.parametrize("p", [0, 1, 2, 3, 4, 5, 6])
 def test_quads_every_order_curved_affine_boundary(p):
-    """Quadrilaterals: fused element kernels (fr_element.cu, 1 <= p <= 4) and the line kernels of fr_tensor.cu (p = 0, p >= 5),
-    affine and curved (p_g = 2), periodic and with walls / inflow / outflow."""
+    """Quadrilaterals: fused element kernels (fr_element.cu; Navier-Stokes 1 <= p <= 3, Euler 1 <= p <= 4) and the line kernels
+    of fr_tensor.cu otherwise, affine and curved (p_g = 2), periodic and with walls / inflow / outflow."""
     L = (2 * np.pi,) * 2
-    expect = "el_" if 1 <= p <= 4 else "tp_"
+
+    def expect(system):
+        return "el_" if 1 <= p <= (3 if system == "navier-stokes" else 4) else "tp_"
+
     _sweep("quad-affine", W.box_mesh((5, 7), L), p, expect=expect)
     _sweep("quad-curved", W.box_mesh((7, 5), L, p_g=2, warp=W.sine_warp(0.08)), p, expect=expect)
     _sweep("quad-bnd", W.box_mesh((3, 4), L, p_g=2, warp=W.sine_warp(0.05), periodic=(False, False)), p, bcs=BC2,

@@ -409,13 +409,14 @@ def fourier_state(X, seed, gamma=1.4, mach=0.3, n_modes=8, amp=0.02):
 # the BASELINE.json configs
 # ----------------------------------------------------------------------------
 def config(name, **over):
-    """Returns (mesh, disc) for C1..C5 (C5 takes p=, n=, system=).  disc["ref"] is the freestream the state generator of the
+    """Returns (mesh, disc) for C1..C5 (C5 takes p=, n=, system=) and for Q (768^2 periodic affine quadrilaterals, p=, n=,
+    system=: the 2-D tensor-product throughput case of SURVEY 8(f); not a BASELINE.json config).  disc["ref"] is the freestream the state generator of the
     config perturbs (density, velocity, pressure): the library takes it as its constant reference state (a conditioning
     hint, include/fr.h); the oracle ignores it."""
     mesh, disc = _config(name, **over)
     nd = mesh["ndims"]
-    p0 = {"C1": 1.0, "C2": 1.0 / (1.4 * 0.1 ** 2), "C3": 1.0 / (1.4 * 0.1 ** 2), "C4": 1.0 / (1.4 * 0.2 ** 2), "C5": 1.0 / (1.4 * 0.3 ** 2)}[name]
-    v0 = {"C1": (1.0, 1.0), "C2": (0.0,) * 3, "C3": (0.0,) * 3, "C4": (1.0, 1.0), "C5": (1.0, 0.5, 0.25)}[name]
+    p0 = {"C1": 1.0, "C2": 1.0 / (1.4 * 0.1 ** 2), "C3": 1.0 / (1.4 * 0.1 ** 2), "C4": 1.0 / (1.4 * 0.2 ** 2), "C5": 1.0 / (1.4 * 0.3 ** 2), "Q": 1.0 / (1.4 * 0.2 ** 2)}[name]
+    v0 = {"C1": (1.0, 1.0), "C2": (0.0,) * 3, "C3": (0.0,) * 3, "C4": (1.0, 1.0), "C5": (1.0, 0.5, 0.25), "Q": (1.0, 1.0)}[name]
     disc["ref"] = dict(rho=1.0, v=v0[:nd], p=p0)
     return mesh, disc
 
@@ -443,6 +444,10 @@ def _config(name, **over):
         p = over.get("p", 3)
         mesh = box_mesh((n,) * 3, (2 * np.pi,) * 3)
         disc = dict(p=p, system=over.get("system", "navier-stokes"), gamma=g, mu=tgv_viscosity(1600.0), Pr=0.71, beta=0.5, tau=0.1, dt=1e-3, steps=1)
+    elif name == "Q":
+        n = over.get("n", 768)
+        mesh = box_mesh((n, n), (1.0, 1.0))
+        disc = dict(p=over.get("p", 3), system=over.get("system", "navier-stokes"), gamma=g, mu=1.0 / 100.0, Pr=0.71, beta=0.5, tau=0.1, dt=1e-5, steps=1)
     else:
         raise KeyError(name)
     return mesh, disc
@@ -457,7 +462,7 @@ def config_state(name, X, **over):
         U = taylor_green(X)
     elif name == "C3":
         U = add_relative_noise(taylor_green(X), 1e-3, 1234)
-    elif name == "C4":
+    elif name in ("C4", "Q"):
         U = sinusoidal_2d(X)
     elif name == "C5":
         U = fourier_state(X, seed=2025 + over.get("p", 3))
