@@ -179,6 +179,19 @@ int fr_get_metrics(const fr_ctx *ctx, double *smat_host, double *rcpj_host);
  * (element index >= n_elems) of rhs are left untouched.  Non-finite states are not detected (A19). */
 int fr_rhs(fr_ctx *ctx, const void *u_dev, void *rhs_dev, void *work_dev, void *stream);
 
+/* fr_rhs for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the scratch of the kernel sequence lives in a static device array of FR_STATIC_WORK_BYTES inside the library
+ * instead of a caller-owned work_dev.  Same arguments, layouts and result (bit for bit) as fr_rhs.  Calls no cudaMalloc /
+ * cudaFree / allocating library routine; the address of the array is resolved once per device (cudaGetSymbolAddress on the
+ * first call with that device current -- make that first call outside graph capture).  Contexts whose right-hand-side scratch
+ * (fr_stepper_workspace_bytes(ctx, FR_STEPPER_EULER) minus one state register) exceeds FR_STATIC_WORK_BYTES are rejected with
+ * FR_ENOMEM and a message naming both sizes.  Every GPU that loads the library holds the array until the process exits.  ALL
+ * calls on a device share it, whatever the context or stream: two calls that overlap on the GPU race; serialise them (one
+ * stream, or events).  The array keeps the previous call's contents; the kernels write every scratch value before reading it,
+ * so nothing needs clearing between calls. */
+#define FR_STATIC_WORK_BYTES (32 * 1024 * 1024)
+int fr_rhs_static(fr_ctx *ctx, const void *u_dev, void *rhs_dev, void *stream);
+
 /* fr_rhs with a CUDA event recorded on `stream` before each kernel and after the last; synchronises the
  * stream and returns, for each of the *n_kernels launch groups, its duration ms[i] and a name
  * (names_host: max_kernels x 32 chars).  For measurement only. */

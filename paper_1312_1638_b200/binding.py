@@ -18,6 +18,7 @@ EULER, NAVIER_STOKES = 0, 1
 F32, F64 = 0, 1
 BC_SUP_INFLOW, BC_SUB_OUTFLOW, BC_NOSLIP_WALL = 0, 1, 2
 FLAG_FORCE_GENERIC, FLAG_HOST_ONLY, FLAG_LEAN = 1, 2, 4
+STATIC_WORK_BYTES = 32 * 1024 * 1024  # FR_STATIC_WORK_BYTES: scratch of fr_rhs_static, held inside the library
 CORRECTIONS = {"dg": 0, "sd": 1, "hu": 2}
 STEPPERS = {"euler": 0, "rk4": 1, "dopri5": 2}
 ETYPES = {"quad": QUAD, "tri": TRI, "hex": HEX}
@@ -95,6 +96,7 @@ def _load():
         "fr_get_pairs": (C.c_int, [P, P, P, P]),
         "fr_get_metrics": (C.c_int, [P, P, P]),
         "fr_rhs": (C.c_int, [P, P, P, P, P]),
+        "fr_rhs_static": (C.c_int, [P, P, P, P]),
         "fr_rhs_profiled": (C.c_int, [P, P, P, P, P, C.c_int, C.POINTER(C.c_int), P, P]),
         "fr_rk4_step": (C.c_int, [P, P, C.c_double, P, P]),
         "fr_rhs_host": (C.c_int, [P, P, P, P, P, P, P]),
@@ -113,7 +115,7 @@ lib = _load()
 EXPORTS = ["fr_setup_mesh", "fr_setup_mesh_mixed", "fr_num_parts", "fr_part_info", "fr_part_solution_point_coords", "fr_setup_operators", "fr_num_solution_points", "fr_num_flux_points", "fr_num_vars", "fr_num_pairs",
            "fr_leading_dim", "fr_state_bytes", "fr_workspace_bytes", "fr_stepper_workspace_bytes", "fr_rhs_kernel_launches",
            "fr_euler_step", "fr_dopri5_step", "fr_solution_point_coords",
-           "fr_operator_dims", "fr_get_operator", "fr_get_pairs", "fr_get_metrics", "fr_rhs", "fr_rhs_profiled", "fr_rk4_step", "fr_rhs_host", "fr_state_lincomb",
+           "fr_operator_dims", "fr_get_operator", "fr_get_pairs", "fr_get_metrics", "fr_rhs", "fr_rhs_static", "fr_rhs_profiled", "fr_rk4_step", "fr_rhs_host", "fr_state_lincomb",
            "fr_measure_peaks", "fr_teardown", "fr_last_error"]
 
 
@@ -274,6 +276,11 @@ class Context:
     # --- the hot path: raw device pointers (ints) in, nothing out ---
     def rhs(self, u_ptr, rhs_ptr, work_ptr, stream=0):
         self._check(lib.fr_rhs(self._h, u_ptr, rhs_ptr, work_ptr, stream))
+
+    def rhs_static(self, u_ptr, rhs_ptr, stream=0):
+        """fr_rhs with the scratch in the library's static device array (no allocation; at most STATIC_WORK_BYTES; calls that
+        overlap on the GPU race, include/fr.h)."""
+        self._check(lib.fr_rhs_static(self._h, u_ptr, rhs_ptr, stream))
 
     def rhs_profiled(self, u_ptr, rhs_ptr, work_ptr, stream=0):
         """-> [(kernel name, ms)] for one RHS (events between kernels; synchronises)."""

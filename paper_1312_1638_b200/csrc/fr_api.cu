@@ -2,7 +2,9 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
+#include <cstdint>
 #include <exception>
+#include <mutex>
 #include <new>
 #include <string>
 #include <type_traits>
@@ -607,6 +609,42 @@ static int rhs_impl(fr_ctx *c, const void *u, void *rhs, void *work, void *strea
 }
 
 int fr_rhs(fr_ctx *c, const void *u, void *rhs, void *work, void *stream) { return rhs_impl(c, u, rhs, work, stream, nullptr); }
+
+// ---- fr_rhs without a caller-owned workspace (include/fr.h): scratch in a static device array ----
+// In host code `g_static_work` is a host-side stand-in of the device array, not a device address: the address is asked of the
+// runtime once per device, with that device current, and cached.
+static __device__ __align__(256) unsigned char g_static_work[FR_STATIC_WORK_BYTES];
+
+static cudaError_t static_work_address(int dev, void **out) {
+  static std::mutex mtx;
+  static void *ptr[256] = {};
+  if (dev < 0 || dev >= 256) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(mtx);
+  if (!ptr[dev]) {
+    void *p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_static_work);  // the current device is `dev` (checked by the caller)
+    if (e != cudaSuccess) return e;
+    if (!p || ((uintptr_t)p & 255)) return cudaErrorInvalidSymbol;
+    ptr[dev] = p;
+  }
+  *out = ptr[dev];
+  return cudaSuccess;
+}
+
+int fr_rhs_static(fr_ctx *c, const void *u, void *rhs, void *stream) {
+  FR_NEED_READY(c, FR_EINVAL)
+  if (c->host_only) return fail(c, FR_EINVAL, "fr_rhs_static: context was set up with FR_FLAG_HOST_ONLY");
+  if (c->wl.reg0 > (int64_t)FR_STATIC_WORK_BYTES)
+    return fail(c, FR_ENOMEM, "fr_rhs_static: the right-hand side needs " + std::to_string(c->wl.reg0) + " bytes of scratch, the static array holds " +
+                                  std::to_string((int64_t)FR_STATIC_WORK_BYTES) + " (FR_STATIC_WORK_BYTES): use fr_rhs with a caller-owned workspace");
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != c->dc.dev)
+    return fail(c, FR_EINVAL, "fr_rhs_static: the current CUDA device is not the one fr_setup_operators uploaded the constants to");
+  void *work = nullptr;
+  cudaError_t e = static_work_address(dev, &work);
+  if (e != cudaSuccess) return fail(c, FR_ECUDA, std::string("fr_rhs_static: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+  return rhs_impl(c, u, rhs, work, stream, nullptr);
+}
 
 int fr_rhs_profiled(fr_ctx *c, const void *u, void *rhs, void *work, void *stream, int max_kernels, int *n_kernels,
                     float *ms, char *names) {
