@@ -143,37 +143,36 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     }
   };
   {
-    // z faces and slice 0 (group 0), slice 1 (group 1); the offsets of slice 2 wait in registers
-    int64_t off[TPT];
+    // Every table entry the prologue needs is loaded first, independent of the face codes (the table holds an offset for every
+    // flux point), so that the codes and the offsets of the z faces and of slices 0 .. NST come back in ONE round trip instead
+    // of four dependent ones (the cp.async statements below are ordering points for the compiler).
+    int64_t offz[2], offk[NST][TPT];
 #pragma unroll
-    for (int s = 0; s < 2; ++s)
-      if (code_z[s] == 1 || code_z[s] == 2) gather(sPz + (size_t)(s * NFP + ij) * NV * E + el, poff((4 + s) * NFP + ij));
+    for (int s = 0; s < 2; ++s) offz[s] = poff((4 + s) * NFP + ij);
 #pragma unroll
-    for (int q = 0; q < TPT; ++q) {
-      const int t = ij + q * NFP;
-      off[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N) : 0;
-    }
-    gather_xy(0, off);
-    cp_async_commit();
-    // slices 1 .. NST - 1 (one group each), then the offsets of slice NST wait in registers
+    for (int k1 = 0; k1 < NST; ++k1)
 #pragma unroll
-    for (int k1 = 1; k1 < NST; ++k1) {
-      if (k1 < N) {
-#pragma unroll
-        for (int q = 0; q < TPT; ++q) {
-          const int t = ij + q * NFP;
-          off[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N + N * k1) : 0;
-        }
-        gather_xy(k1, off);
+      for (int q = 0; q < TPT; ++q) {
+        const int t = ij + q * NFP;
+        offk[k1][q] = (t < 4 * N && k1 < N) ? poff(face_of(t) * NFP + t % N + N * k1) : 0;
       }
-      cp_async_commit();
-    }
     if (N > NST) {
 #pragma unroll
       for (int q = 0; q < TPT; ++q) {
         const int t = ij + q * NFP;
-        off_nx[q] = (code_xy[q] == 1 || code_xy[q] == 2) ? poff(face_of(t) * NFP + t % N + N * NST) : 0;
+        off_nx[q] = t < 4 * N ? poff(face_of(t) * NFP + t % N + N * NST) : 0;
       }
+    }
+    // z faces and slice 0 (group 0), slices 1 .. NST - 1 (one group each); the offsets of slice NST wait in registers
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+      if (code_z[s] == 1 || code_z[s] == 2) gather(sPz + (size_t)(s * NFP + ij) * NV * E + el, offz[s]);
+    gather_xy(0, offk[0]);
+    cp_async_commit();
+#pragma unroll
+    for (int k1 = 1; k1 < NST; ++k1) {
+      if (k1 < N) gather_xy(k1, offk[k1]);
+      cp_async_commit();
     }
   }
   // jump C - U^f (Eq 9) from the partner's U^f and the own interpolated state, both in the perturbation variables w (whose
