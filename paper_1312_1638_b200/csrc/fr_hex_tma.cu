@@ -275,6 +275,15 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 
 #pragma unroll
   for (int k = 0; k < N; ++k) {
+    // own outward normals of the slice's x/y flux points (global, element-blocked): requested here, consumed in the face phase
+    T nrm_pf[TPT][3];
+#pragma unroll
+    for (int q = 0; q < TPT; ++q) {
+      const int t = ij + q * NFP;
+#pragma unroll
+      for (int n = 0; n < 3; ++n)
+        nrm_pf[q][n] = code_xy[q] != 0 ? fp_n[fp_row(true, ld, 3 * NF, n * NF + face_of(t) * NFP + t % N + N * k, e)] : (T)0;
+    }
     mbar_wait(&bar[1 + (k % NST)], (k / NST) & 1);
     mbar_wait(&bar[3], k & 1);
     const T *stR = (const T *)(sSt + (k % NST) * L::ST_BYTES);
@@ -334,7 +343,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       const int fp = f * NFP + m + N * k;
       R nrm[3], uo[NV], G[NV];
 #pragma unroll
-      for (int n = 0; n < 3; ++n) nrm[n] = (R)fp_n[fp_row(true, ld, 3 * NF, n * NF + fp, e)];
+      for (int n = 0; n < 3; ++n) nrm[n] = (R)nrm_pf[q][n];
       if constexpr (KEEP) {
 #pragma unroll
         for (int a = 0; a < NV; ++a) uo[a] = uo_keep[a];
@@ -401,6 +410,14 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     for (int k = 0; k < 2; ++k)
       if (k < N - 1) { mbar_expect_tx(&bar[4 + k], (uint32_t)L::Q_BYTES); tma_load_4d(zb[k], &tmQ, l0, 0, 3 * k, eb, &bar[4 + k]); }
   }
+  T nrm_z[2][3];  // own normals of the z flux points: requested before the reload loop
+  int pe_z[2];
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+#pragma unroll
+    for (int n = 0; n < 3; ++n) nrm_z[s][n] = code_z[s] != 0 ? fp_n[fp_row(true, ld, 3 * NF, n * NF + (4 + s) * NFP + ij, e)] : (T)0;
+    pe_z[s] = (BND && code_z[s] == 3) ? (int)poff((4 + s) * NFP + ij) : 0;
+  }
   R zq[2][3][NV];
 #pragma unroll
   for (int s = 0; s < 2; ++s)
@@ -434,8 +451,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     const int fp = (4 + s) * NFP + ij;
     R nrm[3], G[NV];
 #pragma unroll
-    for (int n = 0; n < 3; ++n) nrm[n] = (R)fp_n[fp_row(true, ld, 3 * NF, n * NF + fp, e)];
-    const int pe = (BND && code_z[s] == 3) ? (int)poff(fp) : 0;
+    for (int n = 0; n < 3; ++n) nrm[n] = (R)nrm_z[s][n];
+    const int pe = pe_z[s];
     if constexpr (BND) face_visc_r<BND, R>(ufz[s], zq[s], nrm, ph, pe, bcs, G);
     else visc_normal_stream<R>(ufz[s], nrm, ph, [&](int a, R *g) {
 #pragma unroll
