@@ -128,7 +128,13 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
   for (int s = 0; s < 2; ++s) code_z[s] = act ? face_code[(size_t)(4 + s) * ld + e] : 0;
 
-  auto poff = [&](int fp) { return fp_poff[fp_row(true, ld, NF, fp, e)]; };
+  // element-blocked tables (fp_row): all elements of a CTA lie in one element block, so a row of the CTA's elements starts at
+  // (block base, CTA-uniform 64-bit) + row * FR_BLK + lane (32-bit per-thread index)
+  const int lane = l0 + el;
+  const int64_t *poff_blk = fp_poff + (size_t)eb * NF * FR_BLK;
+  const T *fpn_blk = fp_n + (size_t)eb * (3 * NF) * FR_BLK;
+  T *gf_blk = gf + (size_t)eb * (NF * NV) * FR_BLK;
+  auto poff = [&](int fp) { return poff_blk[fp * FR_BLK + lane]; };
   // gather of the partner's U^f (N_V values) of one flux point: per-thread asynchronous copies, consumed by the same thread
   auto gather = [&](T *dst, int64_t off) {
 #pragma unroll
@@ -282,7 +288,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       const int t = ij + q * NFP;
 #pragma unroll
       for (int n = 0; n < 3; ++n)
-        nrm_pf[q][n] = code_xy[q] != 0 ? fp_n[fp_row(true, ld, 3 * NF, n * NF + face_of(t) * NFP + t % N + N * k, e)] : (T)0;
+        nrm_pf[q][n] = code_xy[q] != 0 ? fpn_blk[(n * NF + face_of(t) * NFP + t % N + N * k) * FR_BLK + lane] : (T)0;
     }
     mbar_wait(&bar[1 + (k % NST)], (k / NST) & 1);
     mbar_wait(&bar[3], k & 1);
@@ -375,7 +381,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
         }, G);
       }
 #pragma unroll
-      for (int a = 0; a < NV; ++a) gf[fp_row(true, ld, NF * NV, fp * NV + a, e)] = (T)G[a];
+      for (int a = 0; a < NV; ++a) gf_blk[(fp * NV + a) * FR_BLK + lane] = (T)G[a];
     }
     if (k + 1 < N) {
       cp_async_wait<NST - 1>();  // slice k + 1 has arrived (with two stages slice k + 2 may still be in flight)
@@ -415,7 +421,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
   for (int s = 0; s < 2; ++s) {
 #pragma unroll
-    for (int n = 0; n < 3; ++n) nrm_z[s][n] = code_z[s] != 0 ? fp_n[fp_row(true, ld, 3 * NF, n * NF + (4 + s) * NFP + ij, e)] : (T)0;
+    for (int n = 0; n < 3; ++n) nrm_z[s][n] = code_z[s] != 0 ? fpn_blk[(n * NF + (4 + s) * NFP + ij) * FR_BLK + lane] : (T)0;
     pe_z[s] = (BND && code_z[s] == 3) ? (int)poff((4 + s) * NFP + ij) : 0;
   }
   R zq[2][3][NV];
@@ -459,7 +465,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       for (int n = 0; n < 3; ++n) g[n] = zq[s][n][a];
     }, G);
 #pragma unroll
-    for (int a = 0; a < NV; ++a) gf[fp_row(true, ld, NF * NV, fp * NV + a, e)] = (T)G[a];
+    for (int a = 0; a < NV; ++a) gf_blk[(fp * NV + a) * FR_BLK + lane] = (T)G[a];
   }
 }
 
