@@ -254,6 +254,21 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     }
     __syncthreads();
   }
+  // the thread's own column (i, j, .) of w for the contractions along z: in registers in single precision (25 registers; 1.6 %
+  // off the kernel on C3), read from the U block in double precision (50 registers more than the 128 that two resident CTAs
+  // of 7 warps allow: 0.35 -> 0.42 ms with the spills)
+  constexpr bool ZREG = sizeof(T) == 4 && !BND && N <= 6;  // (the boundary instantiations and p = 6 would spill)
+  R wcol[ZREG ? N : 1][NV];
+  if constexpr (ZREG) {
+#pragma unroll
+    for (int m = 0; m < N; ++m)
+#pragma unroll
+      for (int a = 0; a < NV; ++a) wcol[m][a] = (R)sU[((size_t)(NFP * m + ij) * NV + a) * E + el];
+  }
+  auto wz = [&](int m, int a) -> R {
+    if constexpr (ZREG) return wcol[m][a];
+    else return (R)sU[((size_t)(NFP * m + ij) * NV + a) * E + el];
+  };
   cp_async_wait<NST - 1>();  // z faces and slice 0 have arrived (this thread's own copies)
   {
     R uz[2][NV];
@@ -265,7 +280,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     for (int m = 0; m < N; ++m)
 #pragma unroll
       for (int a = 0; a < NV; ++a) {
-        const R v = (R)sU[((size_t)(NFP * m + ij) * NV + a) * E + el];
+        const R v = wz(m, a);
         uz[0][a] = fma(op.lm[m], v, uz[0][a]);
         uz[1][a] = fma(op.lp[m], v, uz[1][a]);
       }
@@ -314,7 +329,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
         for (int m = 0; m < N; ++m) {
           qx = fma(sD[i * N + m], (R)su[((j * N + m) * NV + a) * E], qx);
           qy = fma(sD[j * N + m], (R)su[((m * N + i) * NV + a) * E], qy);
-          qz = fma(op.D[k * N + m], (R)sU[((size_t)(NFP * m + ij) * NV + a) * E + el], qz);
+          qz = fma(op.D[k * N + m], wz(m, a), qz);
         }
         R q3[3];
         to_physical(S, rj, qx, qy, qz, q3);
@@ -404,7 +419,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   for (int m = 0; m < N; ++m)
 #pragma unroll
     for (int a = 0; a < NV; ++a) {
-      const R v = (R)sU[((size_t)(NFP * m + ij) * NV + a) * E + el];
+      const R v = wz(m, a);
       ufz[0][a] = fma(op.lm[m], v, ufz[0][a]);
       ufz[1][a] = fma(op.lp[m], v, ufz[1][a]);
     }
