@@ -290,13 +290,13 @@ cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *
 
 template <int N, typename T>
 constexpr bool fd_fits() {
-  return FdLay<N, Cfg<N, T>::E, true, T, 1>::TOTAL <= SMEM_MAX && N * N * Cfg<N, T>::E <= 1024 && N * N * NV <= 256;
+  return FdLay<N, Cfg<N, T>::E_SLAB, true, T, 1>::TOTAL <= SMEM_MAX && N * N * Cfg<N, T>::E_SLAB <= 1024 && N * N * NV <= 256;
 }
 
 template <int N, typename T>
 cudaError_t fluxdiv_n(const DevConsts &c, const double *h_ops, const void *u, const void *q, const void *dt, void *rhs, cudaStream_t s) {
   if constexpr (fd_fits<N, T>()) {
-    constexpr int E = Cfg<N, T>::E;
+    constexpr int E = Cfg<N, T>::E_SLAB;
     return c.ns ? launch_fluxdiv<N, E, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, E, false, T>(c, h_ops, u, q, dt, rhs, s);
   } else {
     return cudaErrorNotSupported;

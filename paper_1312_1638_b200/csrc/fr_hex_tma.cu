@@ -536,13 +536,13 @@ cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void 
 
 template <int N, typename T>
 constexpr bool fits() {
-  return GfLay<N, Cfg<N, T>::E, T>::TOTAL <= SMEM_MAX && N * N * Cfg<N, T>::E <= 1024;
+  return GfLay<N, Cfg<N, T>::E_SLAB, T>::TOTAL <= SMEM_MAX && N * N * Cfg<N, T>::E_SLAB <= 1024;
 }
 
 template <int N, typename T>
 cudaError_t gradface_n(const DevConsts &c, const double *h_ops, const void *u, const void *uf, void *gf, void *q, cudaStream_t s) {
   if constexpr (fits<N, T>()) {
-    return launch_gradface<N, Cfg<N, T>::E, T>(c, h_ops, u, uf, gf, q, s);
+    return launch_gradface<N, Cfg<N, T>::E_SLAB, T>(c, h_ops, u, uf, gf, q, s);
   } else {
     return cudaErrorNotSupported;
   }

@@ -289,6 +289,9 @@ __device__ __forceinline__ int patch_ij(int slot) {
 template <int N, typename T>
 struct Cfg {
   static constexpr int E = N <= 2 ? 32 : (N == 3 ? 16 : (N <= 6 ? 8 : 4));
+  // the two z-slab kernels at p = 5 in double precision: 8 elements leave room for ONE resident CTA of 9 warps, 4 elements for
+  // two of 5 (48^3 elements: gradient kernel 2.41 -> 2.34 ms, divergence kernel 1.41 -> 1.31 ms)
+  static constexpr int E_SLAB = (N == 6 && sizeof(T) == 8) ? 4 : E;
 };
 
 }  // namespace
