@@ -9,13 +9,15 @@
 namespace fr {
 namespace {
 
-template <int N, int E, bool NS, typename T, int NB>
+// AFF: Euler on an affine mesh (one set of metric terms per element, fr_api.cu): S and 1/J are read once per thread from the
+// per-element tables, the ring carries the U slice only, and ALL of D~ has a buffer of its own that is loaded at kernel start.
+template <int N, int E, bool NS, typename T, int NB, bool AFF = false>
 struct FdLay {
   static constexpr int NFP = N * N, NU = N * NFP;
   static constexpr size_t BAR = 0;
   static constexpr size_t OPS = 128;  // sDh [N*N], sGm [N], sGp [N]
   static constexpr size_t ST = OPS + al128((N * N + 2 * N) * 8);  // (sized for double operators)
-  static constexpr uint32_t S_TX = 9 * NFP * E * sizeof(T), U_TX = NFP * NV * E * sizeof(T), Q_TX = NS ? 3 * NV * NFP * E * sizeof(T) : 0;
+  static constexpr uint32_t S_TX = AFF ? 0 : 9 * NFP * E * sizeof(T), U_TX = NFP * NV * E * sizeof(T), Q_TX = NS ? 3 * NV * NFP * E * sizeof(T) : 0;
   static constexpr size_t ST_U = al128(S_TX);
   static constexpr size_t ST_Q = ST_U + al128(U_TX);
   static constexpr size_t ST_BYTES = ST_Q + al128(Q_TX);
@@ -26,25 +28,27 @@ struct FdLay {
   // gets a buffer of its own, loaded at kernel start; 1/J and the z faces still reuse the freed stages.
   static constexpr uint32_t DXY_TX = 4 * NFP * NV * E * sizeof(T), RJ_TX = NU * E * sizeof(T), DZ_TX = 2 * NFP * NV * E * sizeof(T);
   static constexpr size_t EP_RJ = al128(DXY_TX);
-  static constexpr bool EPI_ST = N >= 2 && EP_RJ + RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
-  static constexpr bool EPI_DED = N >= 2 && !EPI_ST && RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
+  static constexpr bool EPI_ALL = AFF && !NS && N >= 2;
+  static constexpr bool EPI_ST = !EPI_ALL && N >= 2 && EP_RJ + RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
+  static constexpr bool EPI_DED = !EPI_ALL && N >= 2 && !EPI_ST && RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
   static constexpr bool EPI_TMA = EPI_ST || EPI_DED;
   static constexpr size_t DED = F + al128(NB * F_BYTES);  // TMA destination: 128-byte aligned
-  static constexpr size_t TOTAL = DED + (EPI_DED ? al128(DXY_TX) : 0) + 128;  // + slack for the manual 128-byte alignment
+  static constexpr size_t DED_Z = DED + al128(DXY_TX);     // EPI_ALL: D~ of the z faces behind D~ of the x/y faces
+  static constexpr size_t TOTAL = DED + (EPI_DED ? al128(DXY_TX) : 0) + (EPI_ALL ? al128(DXY_TX) + al128(DZ_TX) : 0) + 128;  // + slack for the manual 128-byte alignment
 };
 
 // tmS: smat as (ld, NU, 9), box (E, NFP, 9);  tmU: u as (ld, NFP*NV, N), box (E, NFP*NV, 1);
 // tmQ: Q workspace as (ld, NV*NFP, 3N), box (E, NV*NFP, 3)  (slice-major layout written by k_hex_gradface).
 // Epilogue operands (when they fit the stage buffers): tmD4 / tmD2: D~ as (ld, NFP*NV, 6), boxes (E, NFP*NV, 4) / (E, NFP*NV, 2);
 // tmR: rcpj as (ld, NFP, N), box (E, NFP, N).
-template <int N, int E, bool NS, typename T, int NB, int MINB>
+template <int N, int E, bool NS, typename T, int NB, int MINB, bool AFF>
 __global__ void __launch_bounds__(N *N *E, MINB)
     k_hex_fluxdiv_tma(const __grid_constant__ CUtensorMap tmS, const __grid_constant__ CUtensorMap tmU,
                       const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmD4,
                       const __grid_constant__ CUtensorMap tmD2, const __grid_constant__ CUtensorMap tmR, Ops1D<N> op, Phys ph,
-                      const T *__restrict__ rcpj, bool aff, const T *__restrict__ dt, T *__restrict__ rhs, int64_t ld,
-                      int64_t Nel) {
-  using L = FdLay<N, E, NS, T, NB>;
+                      const T *__restrict__ rcpj, const T *__restrict__ smat, bool aff, const T *__restrict__ dt, T *__restrict__ rhs,
+                      int64_t ld, int64_t Nel) {
+  using L = FdLay<N, E, NS, T, NB, AFF>;
   constexpr int NFP = N * N;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char *sm = smem_raw + ((128u - (smem_addr(smem_raw) & 127u)) & 127u);  // stays in the shared address space
@@ -70,14 +74,22 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   __syncthreads();
   auto issue_stage = [&](int s, int k) {
     mbar_expect_tx(&bar[s], L::S_TX + L::U_TX + L::Q_TX);
-    tma_load_4d(sSt + s * L::ST_BYTES, &tmS, l0, NFP * k, 0, eb, &bar[s]);
+    if (!AFF) tma_load_4d(sSt + s * L::ST_BYTES, &tmS, l0, NFP * k, 0, eb, &bar[s]);
     tma_load_3d(sSt + s * L::ST_BYTES + L::ST_U, &tmU, e0, 0, k, &bar[s]);
     if (NS) tma_load_4d(sSt + s * L::ST_BYTES + L::ST_Q, &tmQ, l0, 0, 3 * k, eb, &bar[s]);
   };
   if (tid == 0) {
     issue_stage(0, 0);
     if (N > 1) issue_stage(1, 1);
-    if (L::EPI_DED) { mbar_expect_tx(&bar[2], L::DXY_TX); tma_load_4d(sm + L::DED, &tmD4, l0, 0, 0, eb, &bar[2]); }
+    if (L::EPI_DED || L::EPI_ALL) { mbar_expect_tx(&bar[2], L::DXY_TX); tma_load_4d(sm + L::DED, &tmD4, l0, 0, 0, eb, &bar[2]); }
+    if (L::EPI_ALL) { mbar_expect_tx(&bar[3], L::DZ_TX); tma_load_4d(sm + L::DED_Z, &tmD2, l0, 0, 4, eb, &bar[3]); }
+  }
+  double Sr[3][3];  // AFF: the element's metric terms, [block][9][FR_BLK] (fr_api.cu)
+  if (AFF) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+      for (int b = 0; b < 3; ++b) Sr[a][b] = (double)smat[((size_t)eb * 9 + a * 3 + b) * FR_BLK + l0 + el];
   }
   R acc[N][NV];
 #pragma unroll
@@ -97,7 +109,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
       for (int a = 0; a < 3; ++a)
 #pragma unroll
-        for (int b = 0; b < 3; ++b) S[a][b] = (double)stS[((a * 3 + b) * NFP + ij) * E + el];
+        for (int b = 0; b < 3; ++b) S[a][b] = AFF ? Sr[a][b] : (double)stS[((a * 3 + b) * NFP + ij) * E + el];
 #pragma unroll
       for (int a = 0; a < NV; ++a) uu[a] = (double)stU[(ij * NV + a) * E + el];
       // primitive variables (Eq 20-21) through the perturbation variables w about the reference state (fr_physics.cuh):
@@ -190,18 +202,19 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   }
   // lifting M3 D~ and the -1/J scale (Eq 19); faces: 0,1 = x-,x+ (idx j + N k); 2,3 = y (i + N k); 4,5 = z (i + N j)
   const double gmi = (double)sGm[i], gpi = (double)sGp[i], gmj = (double)sGm[j], gpj = (double)sGp[j];
-  if (L::EPI_TMA) {
-    const T *sDxy = (const T *)(L::EPI_DED ? sm + L::DED : sSt + ((N - 2) & 1) * L::ST_BYTES);  // [4][NFP*NV][E]
+  if (L::EPI_TMA || L::EPI_ALL) {
+    const T *sDxy = (const T *)((L::EPI_DED || L::EPI_ALL) ? sm + L::DED : sSt + ((N - 2) & 1) * L::ST_BYTES);  // [4][NFP*NV][E]
     const T *sRJ = (const T *)(sSt + ((N - 2) & 1) * L::ST_BYTES + (L::EPI_DED ? 0 : L::EP_RJ));  // [NU][E]
-    const T *sDz = (const T *)(sSt + ((N - 1) & 1) * L::ST_BYTES);                                         // [2][NFP*NV][E]
+    const T *sDz = (const T *)(L::EPI_ALL ? sm + L::DED_Z : sSt + ((N - 1) & 1) * L::ST_BYTES);                // [2][NFP*NV][E]
+    const double rj_el = L::EPI_ALL ? (double)rcpj[(size_t)eb * FR_BLK + l0 + el] : 0.0;  // [block][1][FR_BLK]
     mbar_wait(&bar[2], 0);
     mbar_wait(&bar[3], 0);
-    mbar_wait(&bar[4], 0);
+    if (!L::EPI_ALL) mbar_wait(&bar[4], 0);
     if (!act) return;
 #pragma unroll
     for (int k = 0; k < N; ++k) {
       const int r = ij + NFP * k;
-      const double rj = (double)sRJ[r * E + el];
+      const double rj = L::EPI_ALL ? rj_el : (double)sRJ[r * E + el];
       const int fx = j + N * k, fy = i + N * k;
       double r0 = 0;  // R~ of the mass equation: R_mj = R_wmj + v0_j R_wrho, R_E = R_wE + h0 R_wrho (fr_physics.cuh)
 #pragma unroll
@@ -249,16 +262,16 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   }
 }
 
-template <int N, int E, bool NS, typename T>
+template <int N, int E, bool NS, typename T, bool AFF>
 cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *u, const void *q, const void *dt, void *rhs,
                            cudaStream_t s) {
   constexpr int NFP = N * N, NU = N * NFP;
-  using L2 = FdLay<N, E, NS, T, 2>;
-  using L1 = FdLay<N, E, NS, T, 1>;
+  using L2 = FdLay<N, E, NS, T, 2, AFF>;
+  using L1 = FdLay<N, E, NS, T, 1, AFF>;
   // double-buffer F~ when that does not cost a resident CTA
   constexpr int REGS = 128;  // (96 registers for a third resident CTA: 176 bytes of spills at p = 4 in single precision, rejected)
   constexpr int NB = (L2::TOTAL <= SMEM_MAX && min_blocks(L2::TOTAL, N * N * E, REGS) == min_blocks(L1::TOTAL, N * N * E, REGS)) ? 2 : 1;
-  using L = FdLay<N, E, NS, T, NB>;
+  using L = FdLay<N, E, NS, T, NB, AFF>;
   static_assert(L::TOTAL <= SMEM_MAX, "shared memory");
   constexpr int MINB = min_blocks(L::TOTAL, N * N * E, REGS);
   const uint64_t ld = (uint64_t)c.ld;
@@ -278,12 +291,12 @@ cudaError_t launch_fluxdiv(const DevConsts &c, const double *h_ops, const void *
   ok = ok && encode_blk(&mR, F64, c.rcpj, ld, NFP, N, E, NFP, N, c.aff ? 2 : 0);
   }
   if (!ok) { ent->id = -1; return cudaErrorNotSupported; }
-  auto kern = k_hex_fluxdiv_tma<N, E, NS, T, NB, MINB>;
+  auto kern = k_hex_fluxdiv_tma<N, E, NS, T, NB, MINB, AFF>;
   static DevFlags done;
   cudaError_t err = set_smem(kern, L::TOTAL, done, c.dev);
   if (err != cudaSuccess) return err;
   const Ops1D<N> op = make_ops<N>(h_ops);
-  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(mS, mU, mQ, mD4, mD2, mR, op, c.ph, (const T *)c.rcpj, c.aff, (const T *)dt, (T *)rhs, c.ld,
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(mS, mU, mQ, mD4, mD2, mR, op, c.ph, (const T *)c.rcpj, (const T *)c.smat, c.aff, (const T *)dt, (T *)rhs, c.ld,
                                                                   c.Nel);
   return cudaGetLastError();
 }
@@ -297,7 +310,11 @@ template <int N, typename T>
 cudaError_t fluxdiv_n(const DevConsts &c, const double *h_ops, const void *u, const void *q, const void *dt, void *rhs, cudaStream_t s) {
   if constexpr (fd_fits<N, T>()) {
     constexpr int E = Cfg<N, T>::E_SLAB;
-    return c.ns ? launch_fluxdiv<N, E, true, T>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, E, false, T>(c, h_ops, u, q, dt, rhs, s);
+    if (c.ns) return launch_fluxdiv<N, E, true, T, false>(c, h_ops, u, q, dt, rhs, s);
+    if constexpr (FdLay<N, E, false, T, 1, true>::TOTAL <= SMEM_MAX) {
+      if (c.aff) return launch_fluxdiv<N, E, false, T, true>(c, h_ops, u, q, dt, rhs, s);
+    }
+    return launch_fluxdiv<N, E, false, T, false>(c, h_ops, u, q, dt, rhs, s);
   } else {
     return cudaErrorNotSupported;
   }
