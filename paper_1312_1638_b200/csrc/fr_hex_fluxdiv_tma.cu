@@ -9,8 +9,9 @@
 namespace fr {
 namespace {
 
-// AFF: Euler on an affine mesh (one set of metric terms per element, fr_api.cu): S and 1/J are read once per thread from the
-// per-element tables, the ring carries the U slice only, and ALL of D~ has a buffer of its own that is loaded at kernel start.
+// AFF: affine mesh (one set of metric terms per element, fr_api.cu): S and 1/J are read once per thread from the per-element
+// tables and the ring carries no metric slice.  Euler: the ring holds the U slice only and ALL of D~ has a buffer of its own
+// that is loaded at kernel start (EPI_ALL).
 template <int N, int E, bool NS, typename T, int NB, bool AFF = false>
 struct FdLay {
   static constexpr int NFP = N * N, NU = N * NFP;
@@ -29,8 +30,9 @@ struct FdLay {
   static constexpr uint32_t DXY_TX = 4 * NFP * NV * E * sizeof(T), RJ_TX = NU * E * sizeof(T), DZ_TX = 2 * NFP * NV * E * sizeof(T);
   static constexpr size_t EP_RJ = al128(DXY_TX);
   static constexpr bool EPI_ALL = AFF && !NS && N >= 2;
-  static constexpr bool EPI_ST = !EPI_ALL && N >= 2 && EP_RJ + RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
-  static constexpr bool EPI_DED = !EPI_ALL && N >= 2 && !EPI_ST && RJ_TX <= ST_BYTES && DZ_TX <= ST_BYTES;
+  static constexpr uint32_t RJ_NEED = AFF ? 0 : RJ_TX;  // AFF: 1/J is one value per element, read from its table
+  static constexpr bool EPI_ST = !EPI_ALL && N >= 2 && EP_RJ + RJ_NEED <= ST_BYTES && DZ_TX <= ST_BYTES;
+  static constexpr bool EPI_DED = !EPI_ALL && N >= 2 && !EPI_ST && RJ_NEED <= ST_BYTES && DZ_TX <= ST_BYTES;
   static constexpr bool EPI_TMA = EPI_ST || EPI_DED;
   static constexpr size_t DED = F + al128(NB * F_BYTES);  // TMA destination: 128-byte aligned
   static constexpr size_t DED_Z = DED + al128(DXY_TX);     // EPI_ALL: D~ of the z faces behind D~ of the x/y faces
@@ -178,10 +180,12 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     if (L::EPI_ST && tid == 0 && k == N - 2) {  // this stage is not refilled any more: bring D~ (x/y faces) and 1/J
       mbar_expect_tx(&bar[2], L::DXY_TX);
       tma_load_4d(sSt + (k & 1) * L::ST_BYTES, &tmD4, l0, 0, 0, eb, &bar[2]);
-      mbar_expect_tx(&bar[4], L::RJ_TX);
-      tma_load_4d(sSt + (k & 1) * L::ST_BYTES + L::EP_RJ, &tmR, l0, 0, 0, eb, &bar[4]);
+      if (!AFF) {
+        mbar_expect_tx(&bar[4], L::RJ_TX);
+        tma_load_4d(sSt + (k & 1) * L::ST_BYTES + L::EP_RJ, &tmR, l0, 0, 0, eb, &bar[4]);
+      }
     }
-    if (L::EPI_DED && tid == 0 && k == N - 2) {
+    if (L::EPI_DED && !AFF && tid == 0 && k == N - 2) {
       mbar_expect_tx(&bar[4], L::RJ_TX);
       tma_load_4d(sSt + (k & 1) * L::ST_BYTES, &tmR, l0, 0, 0, eb, &bar[4]);
     }
@@ -206,15 +210,15 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     const T *sDxy = (const T *)((L::EPI_DED || L::EPI_ALL) ? sm + L::DED : sSt + ((N - 2) & 1) * L::ST_BYTES);  // [4][NFP*NV][E]
     const T *sRJ = (const T *)(sSt + ((N - 2) & 1) * L::ST_BYTES + (L::EPI_DED ? 0 : L::EP_RJ));  // [NU][E]
     const T *sDz = (const T *)(L::EPI_ALL ? sm + L::DED_Z : sSt + ((N - 1) & 1) * L::ST_BYTES);                // [2][NFP*NV][E]
-    const double rj_el = L::EPI_ALL ? (double)rcpj[(size_t)eb * FR_BLK + l0 + el] : 0.0;  // [block][1][FR_BLK]
+    const double rj_el = AFF ? (double)rcpj[(size_t)eb * FR_BLK + l0 + el] : 0.0;  // [block][1][FR_BLK]
     mbar_wait(&bar[2], 0);
     mbar_wait(&bar[3], 0);
-    if (!L::EPI_ALL) mbar_wait(&bar[4], 0);
+    if (!AFF) mbar_wait(&bar[4], 0);
     if (!act) return;
 #pragma unroll
     for (int k = 0; k < N; ++k) {
       const int r = ij + NFP * k;
-      const double rj = L::EPI_ALL ? rj_el : (double)sRJ[r * E + el];
+      const double rj = AFF ? rj_el : (double)sRJ[r * E + el];
       const int fx = j + N * k, fy = i + N * k;
       double r0 = 0;  // R~ of the mass equation: R_mj = R_wmj + v0_j R_wrho, R_E = R_wE + h0 R_wrho (fr_physics.cuh)
 #pragma unroll
@@ -310,11 +314,10 @@ template <int N, typename T>
 cudaError_t fluxdiv_n(const DevConsts &c, const double *h_ops, const void *u, const void *q, const void *dt, void *rhs, cudaStream_t s) {
   if constexpr (fd_fits<N, T>()) {
     constexpr int E = Cfg<N, T>::E_SLAB;
-    if (c.ns) return launch_fluxdiv<N, E, true, T, false>(c, h_ops, u, q, dt, rhs, s);
-    if constexpr (FdLay<N, E, false, T, 1, true>::TOTAL <= SMEM_MAX) {
-      if (c.aff) return launch_fluxdiv<N, E, false, T, true>(c, h_ops, u, q, dt, rhs, s);
+    if constexpr (FdLay<N, E, false, T, 1, true>::TOTAL <= SMEM_MAX && FdLay<N, E, true, T, 1, true>::EPI_TMA) {
+      if (c.aff) return c.ns ? launch_fluxdiv<N, E, true, T, true>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, E, false, T, true>(c, h_ops, u, q, dt, rhs, s);
     }
-    return launch_fluxdiv<N, E, false, T, false>(c, h_ops, u, q, dt, rhs, s);
+    return c.ns ? launch_fluxdiv<N, E, true, T, false>(c, h_ops, u, q, dt, rhs, s) : launch_fluxdiv<N, E, false, T, false>(c, h_ops, u, q, dt, rhs, s);
   } else {
     return cudaErrorNotSupported;
   }
