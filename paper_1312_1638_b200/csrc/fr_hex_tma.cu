@@ -62,12 +62,15 @@ struct GfLay {
 // uf: U^f of all elements in perturbation variables (k_hex_interp_tma), element-blocked; fp_poff: for every flux point the
 // offset of its partner's first variable in uf, or -1 - bc_id on a boundary; face_code [6][ld]: 0 = no LDG weight (skip),
 // 1 = L side (1/2 + beta), 2 = R side (1/2 - beta), 3 = boundary.
-template <int N, int E, bool BND, typename T, int MINB, int NST>
+// AFF: affine mesh (one set of metric terms per element): S and 1/J are read once per thread from the per-element tables
+// ([block][9][FR_BLK], [block][1][FR_BLK], fr_api.cu) instead of streaming through the ring.
+template <int N, int E, bool BND, typename T, int MINB, int NST, bool AFF>
 __global__ void __launch_bounds__(N *N *E, MINB)
     k_hex_gradface(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS,
                    const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmQ, Ops1D<N, T> op, Phys ph,
                    const T *__restrict__ uf, const int64_t *__restrict__ fp_poff, const T *__restrict__ fp_n,
-                   const uint8_t *__restrict__ face_code, const BcDev *__restrict__ bcs, T *__restrict__ gf, int64_t ld, int64_t Nel) {
+                   const uint8_t *__restrict__ face_code, const BcDev *__restrict__ bcs, T *__restrict__ gf, const T *__restrict__ smat,
+                   const T *__restrict__ rcpj, int64_t ld, int64_t Nel) {
   using L = GfLay<N, E, T, NST>;
   using R = T;  // arithmetic type of this kernel: the gradient feeds the viscous flux only (see the header comment)
   constexpr int NFP = N * N, NF = 6 * NFP;
@@ -107,9 +110,11 @@ __global__ void __launch_bounds__(N *N *E, MINB)
   if (tid == 0) {
     mbar_expect_tx(&bar[0], L::U_TX);
     tma_load_3d(sm + L::U, &tmU, e0, 0, 0, &bar[0]);
-    issue_S(0);
-    issue_R(0, 0);
-    if (NST > 1 && N > 1) issue_R(1, 1);
+    if (!AFF) {
+      issue_S(0);
+      issue_R(0, 0);
+      if (NST > 1 && N > 1) issue_R(1, 1);
+    }
   }
   // x/y-face tasks of a thread per slice: task t = ij + q NFP < 4 N handles flux point (slot t / N, line m = t % N) of the
   // thread's element; slots 0..3 = faces 1, 3 (+x, +y: the L sides of structured meshes, so that skipped tasks fall into the
@@ -239,6 +244,14 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       jump_of(code_xy[q], bc, uo, sP + (size_t)t * NV * E + el);
     }
   };
+  R S_el[3][3], rj_el = 0;
+  if (AFF) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+      for (int b = 0; b < 3; ++b) S_el[a][b] = (R)smat[((size_t)eb * 9 + a * 3 + b) * FR_BLK + lane];
+    rj_el = (R)rcpj[(size_t)eb * FR_BLK + lane];
+  }
   mbar_wait(&bar[0], 0);
   if (ph.rho0 != 0.0) {
     // the U block becomes w = T (u - u_ref) in place (fr_physics.cuh): every thread converts its own column
@@ -305,8 +318,10 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       for (int n = 0; n < 3; ++n)
         nrm_pf[q][n] = code_xy[q] != 0 ? fpn_blk[(n * NF + face_of(t) * NFP + t % N + N * k) * FR_BLK + lane] : (T)0;
     }
-    mbar_wait(&bar[1 + (k % NST)], (k / NST) & 1);
-    mbar_wait(&bar[3], k & 1);
+    if (!AFF) {
+      mbar_wait(&bar[1 + (k % NST)], (k / NST) & 1);
+      mbar_wait(&bar[3], k & 1);
+    }
     const T *stR = (const T *)(sSt + (k % NST) * L::ST_BYTES);
     const T *stJ = (const T *)(sSt + (k % NST) * L::ST_BYTES + L::ST_P);  // [slot][line][NV][E]: slots 0, 1 = +x, +y; 2, 3 = -x, -y
     const T *su = sU + (size_t)(NFP * k) * NV * E + el;  // slice k
@@ -315,8 +330,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
 #pragma unroll
       for (int a = 0; a < 3; ++a)
 #pragma unroll
-        for (int b = 0; b < 3; ++b) S[a][b] = (R)stS[((a * 3 + b) * NFP + ij) * E + el];
-      const R rj = (R)stR[ij * E + el];
+        for (int b = 0; b < 3; ++b) S[a][b] = AFF ? S_el[a][b] : (R)stS[((a * 3 + b) * NFP + ij) * E + el];
+      const R rj = AFF ? rj_el : (R)stR[ij * E + el];
       const R gmi = sGm[i], gpi = sGp[i], gmj = sGm[j], gpj = sGp[j];
 #pragma unroll
       for (int a = 0; a < NV; ++a) {
@@ -339,8 +354,8 @@ __global__ void __launch_bounds__(N *N *E, MINB)
     }
     fence_proxy_async();  // make the sQ writes visible to the bulk store
     __syncthreads();      // Q of the slice is complete; S, 1/J and the jumps of stage k&1 have been consumed
-    if (tid == 0 && k + 1 < N) issue_S(k + 1);
-    if (tid == 0 && k + NST < N) issue_R(k % NST, k + NST);
+    if (!AFF && tid == 0 && k + 1 < N) issue_S(k + 1);
+    if (!AFF && tid == 0 && k + NST < N) issue_R(k % NST, k + NST);
     if (tid == 0) { tma_store_4d(&tmQ, l0, 0, 3 * k, eb, sQ); tma_store_commit(); }
     if (k + NST < N) {  // partner values of slice k + NST into the freed stage; the offsets of the slice after it start their way
       gather_xy(k + NST, off_nx);
@@ -503,15 +518,15 @@ bool make_maps(const DevConsts &c, const void *u, Maps &m, const void *q) {
   return ok;
 }
 
-template <int N, int E, bool BND, typename T, int MINB, int NST>
+template <int N, int E, bool BND, typename T, int MINB, int NST, bool AFF>
 cudaError_t launch_gradface_k(const DevConsts &c, const Maps &m, const Ops1D<N, T> &op, const T *uf, T *gf, cudaStream_t s) {
   using L = GfLay<N, E, T, NST>;
-  auto kern = k_hex_gradface<N, E, BND, T, MINB, NST>;
+  auto kern = k_hex_gradface<N, E, BND, T, MINB, NST, AFF>;
   static DevFlags done;
   cudaError_t err = set_smem(kern, L::TOTAL, done, c.dev);
   if (err != cudaSuccess) return err;
-  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.Q, op, c.ph, uf, c.fp_poff, (const T *)c.fp_n, c.face_code, c.bcs, gf, c.ld,
-                                                                  c.Nel);
+  kern<<<(unsigned)((c.Nel + E - 1) / E), N * N * E, L::TOTAL, s>>>(m.U, m.S, m.R1, m.Q, op, c.ph, uf, c.fp_poff, (const T *)c.fp_n, c.face_code, c.bcs, gf,
+                                                                  (const T *)c.smat, (const T *)c.rcpj, c.ld, c.Nel);
   return cudaGetLastError();
 }
 
@@ -530,8 +545,14 @@ cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void 
   static_assert(sizeof(Maps) <= sizeof(ent->m), "map cache entry");
   if (fresh && !make_maps<N, E, T>(c, u, m, q)) { ent->id = -1; return cudaErrorNotSupported; }
   const Ops1D<N, T> op = make_ops<N, T>(h_ops);
-  return c.nbnd ? launch_gradface_k<N, E, true, T, MINB, NST>(c, m, op, (const T *)uf, (T *)gf, s)
-                : launch_gradface_k<N, E, false, T, MINB, NST>(c, m, op, (const T *)uf, (T *)gf, s);
+  // the affine specialisation where it was measured to win (C5-shaped meshes: p = 6 3.07 -> 2.39 ms, p = 5 -4.9 %, p = 3, 4 -1 % in
+  // double; p = 6 -4.5 % in single precision; p = 2 in double and p = 4, 5 in single precision lose 1 - 8 % with it)
+  constexpr bool AFF_WINS = sizeof(T) == 8 ? N >= 4 : N == 7;
+  if (AFF_WINS && c.aff)
+    return c.nbnd ? launch_gradface_k<N, E, true, T, MINB, NST, true>(c, m, op, (const T *)uf, (T *)gf, s)
+                  : launch_gradface_k<N, E, false, T, MINB, NST, true>(c, m, op, (const T *)uf, (T *)gf, s);
+  return c.nbnd ? launch_gradface_k<N, E, true, T, MINB, NST, false>(c, m, op, (const T *)uf, (T *)gf, s)
+                : launch_gradface_k<N, E, false, T, MINB, NST, false>(c, m, op, (const T *)uf, (T *)gf, s);
 }
 
 template <int N, typename T>
