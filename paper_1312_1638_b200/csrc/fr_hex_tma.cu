@@ -548,9 +548,11 @@ cudaError_t launch_gradface(const DevConsts &c, const double *h_ops, const void 
   // the affine specialisation where it was measured to win (C5-shaped meshes: p = 6 3.07 -> 2.39 ms, p = 5 -4.9 %, p = 3, 4 -1 % in
   // double; p = 6 -4.5 % in single precision; p = 2 in double and p = 4, 5 in single precision lose 1 - 8 % with it)
   constexpr bool AFF_WINS = sizeof(T) == 8 ? N >= 4 : N == 7;
-  if (AFF_WINS && c.aff)
-    return c.nbnd ? launch_gradface_k<N, E, true, T, MINB, NST, true>(c, m, op, (const T *)uf, (T *)gf, s)
-                  : launch_gradface_k<N, E, false, T, MINB, NST, true>(c, m, op, (const T *)uf, (T *)gf, s);
+  if constexpr (AFF_WINS) {
+    if (c.aff)
+      return c.nbnd ? launch_gradface_k<N, E, true, T, MINB, NST, true>(c, m, op, (const T *)uf, (T *)gf, s)
+                    : launch_gradface_k<N, E, false, T, MINB, NST, true>(c, m, op, (const T *)uf, (T *)gf, s);
+  }
   return c.nbnd ? launch_gradface_k<N, E, true, T, MINB, NST, false>(c, m, op, (const T *)uf, (T *)gf, s)
                 : launch_gradface_k<N, E, false, T, MINB, NST, false>(c, m, op, (const T *)uf, (T *)gf, s);
 }
