@@ -88,7 +88,7 @@ def rhs_algorithmic_words(nd, NV, Nu, Nf, ns, affine):
     return w
 
 
-def kernel_bytes(name, nd, NV, Nu, Nf, ns, gfrac=1.0, sz=8, szi=8, affine=False):
+def kernel_bytes(name, nd, NV, Nu, Nf, ns, gfrac=1.0, sz=8, szi=8, affine=False, hex_tma=False):
     """compulsory bytes per element for one launch group (inputs once + outputs once).
     sz: bytes of a state / metric word (8 | 4: the algorithmic size in the context's precision); szi: bytes of a flux-point /
     gradient intermediate as the path stores it (= sz on the hexahedral TMA path, 8 elsewhere); index words are 4 bytes,
@@ -98,6 +98,8 @@ def kernel_bytes(name, nd, NV, Nu, Nf, ns, gfrac=1.0, sz=8, szi=8, affine=False)
     if affine and (name.startswith("hex_") or name.startswith("el_")):
         met = (nd * nd + 1) * sz  # straight-sided elements: the fused kernels read the metric terms of ONE point per element
     pair_tab = (4 * 4 + (nd + 2) * sz) * Nf // 2  # per flux-point pair: 4 indices, unit normal, two J n
+    if affine and hex_tma:  # affine hexahedra on the TMA path: normal and J n per FACE (fr_dev.hpp: pf_n), indices per pair
+        pair_tab = 4 * 4 * Nf // 2 + 2 * nd * (nd + 1) * sz
     U, R = Nu * NV * sz, Nu * NV * sz
     t = {
         # generic staged path (App A sequence)
@@ -353,7 +355,8 @@ def measure(args, world, rank, local, barrier, light=False):
     szi = sz if any(n.startswith("hex_") for n in acc) else 8  # the hexahedral TMA path stores its intermediates in the storage precision
     kern = []
     for name, ms in acc.items():
-        byt = kernel_bytes(name, nd, NV, Nu, Nf, ns, 0.5 if abs(abs(disc.get("beta", 0.5)) - 0.5) < 1e-15 else 1.0, sz, szi, affine)
+        byt = kernel_bytes(name, nd, NV, Nu, Nf, ns, 0.5 if abs(abs(disc.get("beta", 0.5)) - 0.5) < 1e-15 else 1.0, sz, szi, affine,
+                           hex_tma=any(n.startswith("hex_") for n in acc))
         gbs = (byt * ctx.n_elems / (ms * 1e-3) / 1e9) if (byt and ms > 0) else None
         kern.append({"name": name, "ms": ms, "share": ms / sum(acc.values()), "algorithmic_GBps": gbs})
     kern.sort(key=lambda k: -k["ms"])

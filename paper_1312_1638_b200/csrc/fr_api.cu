@@ -1,5 +1,6 @@
 // C ABI of the FR library (include/fr.h): context management, constant uploads, RHS and RK4 drivers.
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <cstdint>
@@ -240,7 +241,21 @@ int fr_setup_operators(fr_ctx *c, const fr_disc_desc *d) {
     } else if (dc.blk) { UPT(reblock(mc.smat, o.nd * o.nd * o.Nu), smat); UPT(reblock(mc.rcpj, o.Nu), rcpj); }
     else { UP(mc.smat, smat); UP(mc.rcpj, rcpj); }
     UP(mc.pLs, pLs); UP(mc.pLe, pLe); UP(mc.pRs, pRs); UP(mc.pRe, pRe);
-    UPT(mc.pn, pn); UPT(mc.pJnL, pJnL); UPT(mc.pJnR, pJnR);
+    if (dc.aff) {
+      // affine hexahedra: normal and J n of a flux point are those of its face (first flux point of the face); per-face tables
+      // replace the per-pair ones (fr_dev.hpp: pf_n): 4 nd (nd + 1) words per element instead of (nd + 2) N_f / 2
+      const int nf = o.nfaces;
+      std::vector<double> fn((size_t)o.nd * nf * ld, 0.0), fj((size_t)nf * ld, 0.0);
+      for (int f = 0; f < nf; ++f)
+        for (int64_t el = 0; el < mc.Nel; ++el) {
+          const int sg = f * o.nfp;
+          for (int n = 0; n < o.nd; ++n) fn[((size_t)n * nf + f) * ld + el] = mc.fp_n[((size_t)n * o.Nf + sg) * ld + el];
+          fj[(size_t)f * ld + el] = std::fabs(mc.fp_Jn[(size_t)sg * ld + el]);  // (the sign bit marks R sides)
+        }
+      UPT(fn, pf_n); UPT(fj, pf_Jn);
+    } else {
+      UPT(mc.pn, pn); UPT(mc.pJnL, pJnL); UPT(mc.pJnR, pJnR);
+    }
     UP(mc.bs, bs); UP(mc.be, be); UP(mc.bbc, bbc); UP(mc.bn, bn); UP(mc.bJn, bJn);
     // element-centric flux-point tables of the fused hexahedral gradient kernel (own normals, boundary ids)
     const bool want_tma = !(d->flags & FR_FLAG_FORCE_GENERIC) && o.etype == FR_HEX && dc.ns && hex_tma_supported(o.n, dc.f64);

@@ -47,6 +47,10 @@ struct DevConsts {
   const int64_t *fp_poff;    // hexahedral TMA path, [block][Nf][FR_BLK]: offset of the partner's first variable in U^f, or -1 - bc_id
   const uint8_t *face_code;  // [6][ld] (hexahedra): 0 = face without LDG weight, 1 = L side, 2 = R side, 3 = boundary (fr_hex_tma.cu)
   const double *fp_n, *fp_Jn;
+  // affine hexahedral meshes on the TMA path (aff): the unit normal and J n of a flux point are those of its face, so the pair
+  // kernels read them from per-face tables [nd][2 nd][ld] / [2 nd][ld] (storage precision; re-read from cache by the N^2 flux
+  // points of a face) instead of the per-pair tables pn / pJnL / pJnR.  NULL: per-pair tables.
+  const double *pf_n, *pf_Jn;
 };
 
 // Element-blocked layout of library-internal arrays (flux-point arrays U^f / D~, jumps, G^f, Q, and the metric / normal

@@ -158,6 +158,25 @@ __global__ void k_tflux(DevConsts c, const T *__restrict__ u, double *__restrict
     }
 }
 
+// unit normal of the L side and J n of both sides of pair i (Eq 14-16): per-pair tables in iteration order, or the per-face
+// tables of an affine hexahedral mesh (fr_dev.hpp: pf_n)
+template <int ND, typename TI>
+__device__ __forceinline__ void pair_normals(const DevConsts &c, int64_t i, double *nrm, double &jl, double &jr) {
+  if (c.pf_n) {
+    const int fL = c.pLs[i] / c.nfp, fR = c.pRs[i] / c.nfp;
+    const size_t eL = (size_t)c.pLe[i], eR = (size_t)c.pRe[i];
+#pragma unroll
+    for (int n = 0; n < ND; ++n) nrm[n] = (double)((const TI *)c.pf_n)[((size_t)n * 2 * ND + fL) * c.ld + eL];
+    jl = (double)((const TI *)c.pf_Jn)[(size_t)fL * c.ld + eL];
+    jr = (double)((const TI *)c.pf_Jn)[(size_t)fR * c.ld + eR];
+    return;
+  }
+#pragma unroll
+  for (int n = 0; n < ND; ++n) nrm[n] = (double)((const TI *)c.pn)[(size_t)n * c.npairs + i];  // tables in TI (fr_api.cu)
+  jl = (double)((const TI *)c.pJnL)[i];
+  jr = (double)((const TI *)c.pJnR)[i];
+}
+
 // Common normal flux over flux-point pairs, Eq 15-17 (:227-235); in place over U^f -> D~ (:300)
 // TI: storage type of the flux-point arrays (double; float on the hexahedral TMA path in single precision)
 template <int ND, bool NS, typename TI>
@@ -177,10 +196,9 @@ __global__ void __launch_bounds__(128, NS ? 2 : FLUXG_MINB) k_common_flux(DevCon
 #pragma unroll
       for (int a = 0; a < NV; ++a) { qL[n][a] = (double)qf[n * blk + oL + (size_t)a * vs]; qR[n][a] = (double)qf[n * blk + oR + (size_t)a * vs]; }
   }
-#pragma unroll
-  for (int n = 0; n < ND; ++n) nrm[n] = (double)((const TI *)c.pn)[(size_t)n * c.npairs + i];  // tables in TI (fr_api.cu)
+  double jl, jr;
+  pair_normals<ND, TI>(c, i, nrm, jl, jr);
   common_flux<ND, NS>(uL, uR, uR, qL, qR, nrm, c.ph, F);
-  const double jl = (double)((const TI *)c.pJnL)[i], jr = (double)((const TI *)c.pJnR)[i];
 #pragma unroll
   for (int a = 0; a < NV; ++a) { uf[oL + (size_t)a * vs] = (TI)(jl * F[a]); uf[oR + (size_t)a * vs] = (TI)(-jr * F[a]); }
 }
@@ -231,10 +249,9 @@ __global__ void __launch_bounds__(128, FLUXG_MINB) k_common_flux_g(DevConsts c, 
   for (int a = 0; a < NV; ++a) { uL[a] = (double)uf[oL + (size_t)a * vs]; uR[a] = (double)uf[oR + (size_t)a * vs]; }
 #pragma unroll
   for (int a = 0; a < NV; ++a) { gL[a] = wl != 0.0 ? (double)gf[oL + (size_t)a * vs] : 0.0; gR[a] = wr != 0.0 ? (double)gf[oR + (size_t)a * vs] : 0.0; }
-#pragma unroll
-  for (int n = 0; n < ND; ++n) nrm[n] = (double)((const TI *)c.pn)[(size_t)n * c.npairs + i];
+  double jl, jr;
+  pair_normals<ND, TI>(c, i, nrm, jl, jr);
   rusanov<ND>(uL, uR, nrm, c.ph, F);
-  const double jl = (double)((const TI *)c.pJnL)[i], jr = (double)((const TI *)c.pJnR)[i];
 #pragma unroll
   for (int a = 0; a < NV; ++a) {
     const double f = F[a] + c.ph.tau * (uL[a] - uR[a]) - (wl * gL[a] - wr * gR[a]);
