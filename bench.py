@@ -250,7 +250,8 @@ def fill_size(args, fraction, hbm_bytes=180e9):
     ctx = Context(mesh).setup_operators(precision=args.precision, **disc)
     ld = ctx.ld
     sz = 8 if args.precision == "f64" else 4
-    tables = ctx.Nf / 2 * (16 + 5 * sz) + ctx.Nf * (3 * sz + 8) + 6 + 10 * sz
+    # pair indices, per-face normals / J n (affine hexahedra), own normals + partner offsets, face codes, metric terms of one point
+    tables = ctx.Nf / 2 * 16 + 24 * sz + ctx.Nf * (3 * sz + 8) + 6 + 10 * sz
     per_elem = (2 * ctx.state_bytes + ctx.workspace_bytes) / ld + tables
     ctx.teardown()
     n_dev = int((fraction * hbm_bytes / per_elem) ** (1.0 / 3.0))
