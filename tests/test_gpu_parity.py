@@ -228,6 +228,8 @@ def test_hex_tma_every_order_curved_affine_boundary(p):
     L = (2 * np.pi,) * 3
     _sweep("hex-curved", W.box_mesh(shape, L, p_g=min(p, 3), warp=W.sine_warp(0.05)), p, expect="tma")
     _sweep("hex-affine", W.box_mesh(shape[::-1], L), p, expect="tma")
+    # affine elements of DIFFERENT sizes (per-element metric terms in registers, per-face normal tables indexed by element)
+    _sweep("hex-graded", W.box_mesh((3, 2, 3), L, warp=W.graded_warp(0.25)), p, expect="tma")
     _sweep("hex-bnd", W.box_mesh((2, 1, 3), L, p_g=2, warp=W.sine_warp(0.03), periodic=(True, True, False)), p, bcs=BC3,
            precisions=("f64",), expect="tma")
 

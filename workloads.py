@@ -118,6 +118,16 @@ def sine_warp(amplitude=0.05):
     return w
 
 
+def graded_warp(amplitude=0.25):
+    """Grading of a periodic box [0, 2 pi]^d with p_g = 1: every coordinate is displaced by amplitude * sin of ITSELF, so the
+    elements stay axis-aligned boxes (affine) of different sizes and the periodic images keep matching."""
+
+    def w(X):
+        return amplitude * np.sin(X)
+
+    return w
+
+
 # ----------------------------------------------------------------------------
 # unstructured-looking triangle mesh (C4)
 # ----------------------------------------------------------------------------
