@@ -174,6 +174,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
         for (int kk = 0; kk < N; ++kk) acc[kk][a] = fma(op.Dh[kk * N + k], fz, acc[kk][a]);
       }
     }
+    fence_proxy_async();  // generic-proxy reads of the stage are ordered before the bulk copies that refill it (fr_hex_tma.cu, z faces)
     __syncthreads();
     // every thread has consumed stage k&1: refill it with slice k+2
     if (tid == 0 && k + 2 < N) issue_stage(k & 1, k + 2);

@@ -438,6 +438,11 @@ __global__ void __launch_bounds__(N *N *E, MINB)
       ufz[0][a] = fma(op.lm[m], v, ufz[0][a]);
       ufz[1][a] = fma(op.lp[m], v, ufz[1][a]);
     }
+  // The reload buffers are written by the async proxy (TMA) after they were read through the generic proxy: the proxy fence
+  // before each barrier orders those reads before the bulk copy that the barrier releases.  Without it a shared-memory load
+  // issued before the barrier, whose value only feeds register accumulators, may still be in flight when the copy lands
+  // (seen in single precision: G^f of a z face differed from run to run in a few warps per launch).
+  fence_proxy_async();
   __syncthreads();  // U block, z jumps and the stages are dead from here on
   unsigned char *zb[2] = {ZB_IN_U ? sm + L::U : sm + L::SS, ZB_IN_U ? sm + L::U + al128(L::Q_BYTES) : sm + L::U};
   if (tid == 0) {
@@ -477,6 +482,7 @@ __global__ void __launch_bounds__(N *N *E, MINB)
         zq[1][n][a] = fma(op.lp[k], q, zq[1][n][a]);
       }
     if (k + 2 < N - 1) {  // refill this buffer with slice k + 2
+      fence_proxy_async();  // this thread's reads of the buffer are ordered before the refill (see above)
       __syncthreads();
       if (tid == 0) { mbar_expect_tx(&bar[4 + (k & 1)], (uint32_t)L::Q_BYTES); tma_load_4d(zb[k & 1], &tmQ, l0, 0, 3 * (k + 2), eb, &bar[4 + (k & 1)]); }
     }

@@ -341,6 +341,22 @@ def test_full_size_C3_fp32_sampled():
 
 
 @pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_full_size_C3_rhs_is_bitwise_reproducible(precision):
+    """The same right-hand side eight times on the 32^3 mesh: every result identical to the first, bit for bit.  (The path has
+    no atomics; a difference is a race.  Found one: the z-face pass of k_hex_gradface refilled a shared-memory buffer by TMA
+    while loads of it that fed only register accumulators were still in flight - a few warps per launch in single precision,
+    which a parity sample could hit or miss.)"""
+    mesh, disc = W.config("C3")
+    ctx = _ctx(mesh, disc, precision=precision)
+    U = W.config_state("C3", ctx.solution_point_coords()).astype(ctx.dtype)
+    run = GpuRunner(ctx)
+    first = run.rhs(U).copy()
+    for it in range(7):
+        again = run.rhs(U)
+        assert np.array_equal(first, again), (precision, it, int(np.count_nonzero(first != again)))
+
+
+@pytest.mark.parametrize("precision", ["f64", "f32"])
 def test_full_size_C3_freestream_and_conservation(precision):
     """Freestream preservation (PAPER.md:151-160, :216 metrics) and the conservation sum on the 32^3 curved mesh itself: the
     GPU result of the whole mesh, weighted with the oracle's quadrature weights and Jacobians (geometry only)."""
